@@ -1,0 +1,215 @@
+"""Workload recipes for BASELINE.json configs 1..5.
+
+Random numbers: numpy's counter-based Philox4x64 (np.random.Philox(key=...)), keyed by
+(SEED_BASE + config index, stream id); uniforms are numpy's 53-bit doubles, normals numpy's ziggurat.
+Every array is a pure function of (config index, sizes), so oracle and GPU always see the same inputs.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+TOBS = 31457280.0          # 1 "year" of the configs = 3 * 2^21 * 5 s
+DT = 5.0
+C_LIGHT = 299792458.0
+ARMLENGTH = 2.5e9
+SEED_BASE = 0x2405_0469_0000
+ADD, REMOVE, SWAP = 0, 1, 2
+
+# stream ids within one config's key space
+_S_PARAMS, _S_WALKER, _S_MOVE, _S_JITTER, _S_ACCEPT, _S_PSD, _S_NOISE0 = 1, 2, 3, 4, 5, 6, 1000
+
+
+def _rng(config: int, stream: int) -> np.random.Generator:
+    return np.random.Generator(np.random.Philox(key=[SEED_BASE + config, stream]))
+
+
+def band_bins(f_lo: float, f_hi: float, T: float = TOBS):
+    """Global rfft bin range [k_lo, k_lo + n_f) covering f_lo..f_hi inclusive (bin k <-> f = k/T)."""
+    k_lo = int(np.ceil(f_lo * T - 1e-9))
+    k_hi = int(np.floor(f_hi * T + 1e-9))
+    return k_lo, k_hi - k_lo + 1
+
+
+def n_bins_for_f0(f0):
+    """Window length by f0 (BASELINE.json config 3/5): 128 (<1 mHz), 256 (1-4), 512 (4-10), 1024 above."""
+    f0 = np.asarray(f0)
+    return np.where(f0 < 1e-3, 128, np.where(f0 < 4e-3, 256, np.where(f0 < 10e-3, 512, 1024))).astype(np.int32)
+
+
+def instrument_psd(f, sqrt_S_acc: float = 3e-15, sqrt_S_oms: float = 15e-12, L: float = ARMLENGTH):
+    """A/E instrument noise PSD, Eq. 7-9, fractional-frequency TDI-1.5 units [1/Hz]."""
+    f = np.asarray(f, dtype=np.float64)
+    x = 2.0 * np.pi * f * L / C_LIGHT
+    S_pm = sqrt_S_acc ** 2 * (2.0 * np.pi * C_LIGHT * f) ** -2 * (1.0 + (0.4e-3 / f) ** 2) * (1.0 + (f / 8e-3) ** 4)
+    S_op = sqrt_S_oms ** 2 * (2.0 * np.pi * f / C_LIGHT) ** 2 * (1.0 + (2e-3 / f) ** 4)
+    return 8.0 * np.sin(x) ** 2 * (2.0 * S_pm * (3.0 + 2.0 * np.cos(x) + np.cos(2.0 * x)) + S_op * (2.0 + np.cos(x)))
+
+
+def _draw_params(g: np.random.Generator, B: int, f_lo: float, f_hi: float):
+    """[amp, f0, fdot, phi0, cos_iota, psi, lambda, sin_beta] per BASELINE.json config 1."""
+    p = np.empty((B, 8), np.float64)
+    u = g.random((B, 8))
+    p[:, 0] = 10.0 ** (-23.0 + 2.0 * u[:, 0])                       # amp log-U[1e-23, 1e-21]
+    p[:, 1] = f_lo * (f_hi / f_lo) ** u[:, 1]                       # f0 log-U
+    p[:, 2] = (2.0 * u[:, 2] - 1.0) * 1e-16                         # fdot U[-1e-16, 1e-16]
+    p[:, 3] = 2.0 * np.pi * u[:, 3]                                 # phi0
+    p[:, 4] = 2.0 * u[:, 4] - 1.0                                   # cos iota
+    p[:, 5] = np.pi * u[:, 5]                                       # psi
+    p[:, 6] = 2.0 * np.pi * u[:, 6]                                 # lambda
+    p[:, 7] = 2.0 * u[:, 7] - 1.0                                   # sin beta
+    return p
+
+
+# calibration constant of the config-5 amplitude recipe: rho0^2 = T (amp0 * _RESP_C0 * x |sin x|)^2 / S(f0)
+# approximates the orientation-averaged optimal SNR of a source of amplitude amp0 (value immaterial to parity)
+_RESP_C0 = 4.74
+
+
+@dataclass
+class Workload:
+    config: int
+    name: str
+    Tobs: float
+    dt: float
+    k_lo: int
+    n_f: int
+    n_walkers: int
+    psd: np.ndarray                      # [n_psd, 2, n_f] f64, S_n
+    walker_psd: Optional[np.ndarray]     # [n_walkers] int32 or None
+    params_new: Optional[np.ndarray]     # [B, 8]
+    params_old: Optional[np.ndarray]     # [B, 8]
+    walker_index: np.ndarray             # [B] int32
+    move: Optional[np.ndarray]           # [B] int8 or None
+    move_all: int
+    N: int                               # used when n_bins is None
+    n_bins: Optional[np.ndarray]         # [B] int32 or None
+    accepted: Optional[np.ndarray]       # [B] uint8 or None
+    _psd_scale: np.ndarray = field(default=None, repr=False)
+
+    @property
+    def B(self) -> int:
+        return int(self.walker_index.shape[0])
+
+    def psd_row_of(self, w: int) -> int:
+        if self.walker_psd is not None:
+            return int(self.walker_psd[w])
+        return 0 if self.psd.shape[0] == 1 else w
+
+    def resid_row(self, w: int) -> np.ndarray:
+        """Residual of walker w: complex128 [2, n_f], Re and Im ~ N(0, S T / 4) (P7 normalisation)."""
+        g = _rng(self.config, _S_NOISE0 + w)
+        z = g.standard_normal((2, self.n_f, 2))
+        sig = np.sqrt(self.psd[self.psd_row_of(w)] * (self.Tobs / 4.0))
+        out = np.empty((2, self.n_f), np.complex128)
+        out.real = z[..., 0] * sig
+        out.imag = z[..., 1] * sig
+        return out
+
+    def resid(self) -> np.ndarray:
+        """All residuals: complex128 [n_walkers, 2, n_f] (config 5 full size: 10.8 GB -- use resid_row)."""
+        out = np.empty((self.n_walkers, 2, self.n_f), np.complex128)
+        for w in range(self.n_walkers):
+            out[w] = self.resid_row(w)
+        return out
+
+    def subset(self, idx) -> "Workload":
+        """Same data, a subset of the proposal rows (for sampled parity / bounded CPU baselines)."""
+        idx = np.asarray(idx)
+        pick = lambda a: None if a is None else np.ascontiguousarray(a[idx])
+        return Workload(self.config, self.name, self.Tobs, self.dt, self.k_lo, self.n_f, self.n_walkers,
+                        self.psd, self.walker_psd, pick(self.params_new), pick(self.params_old),
+                        pick(self.walker_index), pick(self.move), self.move_all, self.N, pick(self.n_bins),
+                        pick(self.accepted), self._psd_scale)
+
+
+def _psd_rows(config: int, n_rows: int, k_lo: int, n_f: int, jitter: bool):
+    f = (k_lo + np.arange(n_f, dtype=np.float64)) / TOBS
+    psd = np.empty((n_rows, 2, n_f), np.float64)
+    g = _rng(config, _S_PSD)
+    scale = 1.0 + 0.05 * (2.0 * g.random((n_rows, 2)) - 1.0) if jitter else np.ones((n_rows, 2))
+    for r in range(n_rows):
+        S = instrument_psd(f, 3e-15 * scale[r, 0], 15e-12 * scale[r, 1])
+        psd[r, 0] = S
+        psd[r, 1] = S                                               # same S for A and E
+    return psd, scale
+
+
+def make_workload(config: int, B: Optional[int] = None, n_walkers: Optional[int] = None,
+                  per_walker: Optional[int] = None) -> Workload:
+    """Build config 1..5.  B / n_walkers / per_walker shrink the case for tests; the draws for a
+    smaller B are a prefix of the draws for a larger one (same Philox streams)."""
+    if config == 1:
+        B = 64 if B is None else B
+        k_lo, n_f = band_bins(1e-3, 4e-3)
+        psd, sc = _psd_rows(1, 1, k_lo, n_f, False)
+        p = _draw_params(_rng(1, _S_PARAMS), B, 1e-3, 4e-3)
+        return Workload(1, "cfg1_tiny_add", TOBS, DT, k_lo, n_f, 1, psd, None, p, None,
+                        np.zeros(B, np.int32), None, ADD, 128, None, None, sc)
+    if config == 2:
+        B = 4096 if B is None else B
+        k_lo, n_f = band_bins(0.1e-3, 30e-3)
+        psd, sc = _psd_rows(2, 1, k_lo, n_f, False)
+        p = _draw_params(_rng(2, _S_PARAMS), B, 0.1e-3, 15e-3)
+        return Workload(2, "cfg2_add4096", TOBS, DT, k_lo, n_f, 1, psd, None, p, None,
+                        np.zeros(B, np.int32), None, ADD, 256, None, None, sc)
+    if config == 3:
+        B = 65536 if B is None else B
+        nw = 36 if n_walkers is None else n_walkers
+        k_lo, n_f = band_bins(0.1e-3, 30e-3)
+        psd, sc = _psd_rows(3, nw, k_lo, n_f, True)
+        p = _draw_params(_rng(3, _S_PARAMS), B, 0.1e-3, 15e-3)
+        w = _rng(3, _S_WALKER).integers(0, nw, B).astype(np.int32)
+        mv = (_rng(3, _S_MOVE).random(B) < 0.5).astype(np.int8)      # 0 = ADD, 1 = REMOVE
+        # ADD rows read params_new, REMOVE rows read params_old: hand the same draw to both
+        return Workload(3, "cfg3_mixed_add_remove", TOBS, DT, k_lo, n_f, nw, psd, None, p, p.copy(),
+                        w, mv, ADD, 0, n_bins_for_f0(p[:, 1]), None, sc)
+    if config == 4:
+        B = 32768 if B is None else B
+        nw = 36 if n_walkers is None else n_walkers
+        k_lo, n_f = band_bins(0.1e-3, 30e-3)
+        psd, sc = _psd_rows(4, nw, k_lo, n_f, True)
+        old = _draw_params(_rng(4, _S_PARAMS), B, 4e-3, 10e-3)
+        g = _rng(4, _S_JITTER).standard_normal((B, 8))
+        new = old.copy()
+        new[:, 0] = old[:, 0] * (1.0 + 0.01 * g[:, 0])
+        new[:, 1] = old[:, 1] + 1e-9 * g[:, 1]
+        new[:, 3] = old[:, 3] + 0.05 * g[:, 3]
+        new[:, 5] = old[:, 5] + 0.05 * g[:, 5]
+        new[:, 6] = old[:, 6] + 0.05 * g[:, 6]
+        iota = np.arccos(old[:, 4]) + 0.05 * g[:, 4]                 # reflect into [0, pi]
+        iota = np.abs(iota); iota = np.where(iota > np.pi, 2.0 * np.pi - iota, iota)
+        new[:, 4] = np.cos(iota)
+        beta = np.arcsin(old[:, 7]) + 0.05 * g[:, 7]                 # reflect into [-pi/2, pi/2]
+        beta = np.where(beta > np.pi / 2, np.pi - beta, beta); beta = np.where(beta < -np.pi / 2, -np.pi - beta, beta)
+        new[:, 7] = np.sin(beta)
+        w = _rng(4, _S_WALKER).integers(0, nw, B).astype(np.int32)
+        return Workload(4, "cfg4_swap", TOBS, DT, k_lo, n_f, nw, psd, None, new, old,
+                        w, None, SWAP, 512, None, None, sc)
+    if config == 5:
+        n_t, n_w36 = 10, 36
+        nw = n_t * n_w36 if n_walkers is None else n_walkers
+        per = 12000 if per_walker is None else per_walker
+        B = nw * per if B is None else B
+        k_lo, n_f = band_bins(0.1e-3, 30e-3)
+        n_rows = min(n_w36, nw)
+        psd, sc = _psd_rows(5, n_rows, k_lo, n_f, True)
+        walker_psd = (np.arange(nw) % n_rows).astype(np.int32)       # "vertical" PSD sharing across temps
+        p = _draw_params(_rng(5, _S_PARAMS), B, 0.1e-3, 15e-3)
+        # SNR-weighted amplitude: rho ~ p(rho) ∝ rho^-4 on [7, 500] (inverse CDF), amp = amp0 rho / rho0(f0)
+        u = p[:, 0].copy(); u = (np.log10(u) + 23.0) / 2.0            # recover the uniform behind column 0
+        lo, hi = 7.0, 500.0
+        rho = (lo ** -3 - u * (lo ** -3 - hi ** -3)) ** (-1.0 / 3.0)
+        f0 = p[:, 1]
+        x = 2.0 * np.pi * f0 * ARMLENGTH / C_LIGHT
+        amp0 = 1e-22
+        rho0 = np.sqrt(TOBS / instrument_psd(f0)) * amp0 * _RESP_C0 * x * np.abs(np.sin(x))
+        p[:, 0] = amp0 * rho / rho0
+        w = (np.arange(B) // per).astype(np.int32) if B == nw * per else \
+            _rng(5, _S_WALKER).integers(0, nw, B).astype(np.int32)
+        acc = (_rng(5, _S_ACCEPT).random(B) < 0.25).astype(np.uint8)
+        return Workload(5, "cfg5_ensemble_sweep", TOBS, DT, k_lo, n_f, nw, psd, walker_psd, p, None,
+                        w, None, ADD, 0, n_bins_for_f0(p[:, 1]), acc, sc)
+    raise ValueError(f"unknown config {config}")

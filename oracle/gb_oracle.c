@@ -1,0 +1,419 @@
+/*
+ * gb_oracle.c -- CPU ORACLE for the Galactic-binary (GB) waveform + delta-log-likelihood hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call it.  The CUDA product
+ * path (paper_2405_04690_b200/) shares no code, header, table or constant generator with this file
+ * and never calls it.
+ *
+ * What it computes (plain, slow, fp64, in the paper's order and notation):
+ *   the GB frequency-domain TDI A/E waveform by the fast/slow decomposition (sec. II.A,
+ *   PAPER.md:696-704 App. F), TDI generation 1.5 with equal constant arms, A/E channels
+ *   (Eq. 6), the noise-weighted inner product (Eq. 2), the add / swap
+ *   delta log-likelihoods (Eq. 4, 5) and the residual refresh of Algorithm 1
+ *   (PAPER.md:599-613).  The paper does not print the waveform equations; the reading
+ *   followed here is SURVEY.md sec. 8(c) steps O1..O9 (restated in DESIGN.md "Readings").
+ *
+ * Style rules: one function per step O1..O9, C99 complex arithmetic so each line reads like the
+ * formula, no blocking, no fusion, no reordering, no tables shared between sources.  Compile with
+ * -ffp-contract=off so that q = floor(fl(f0*T)+0.5) is rounded as written (reading S4).
+ * The only parallelism is an OpenMP "parallel for" over independent proposals / walkers, which does
+ * not change any result bit.
+ *
+ * Pins (tests/test_oracle_pins.py, all -m "not gpu"): frozen-geometry time-domain TDI + DFT (P1),
+ * decimation identity (P1'), full-rate dt*rfft (P2), moving geometry (P3), Parseval (P4),
+ * monochromatic closed form (P5), delta-lnL invariants (P6), tiny-T brute force (P8).
+ * "parity unpinned": physical fidelity to the LDC Sangria generator / GBGPU (neither is in this
+ * container); the oracle, not those codes, defines the result.
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define GBO_C_LIGHT 299792458.0
+#define GBO_PI 3.14159265358979323846264338327950288
+
+typedef struct {
+    double Tobs;      /* observation time T [s]                    (31457280)            */
+    double dt;        /* sampling cadence of the data [s]          (5); not used by O1-O6 */
+    double armlength; /* L [m]                                     (2.5e9)               */
+    double au;        /* AU [m]                                    (1.495978707e11)      */
+    double year;      /* sidereal year [s]                         (31558149.763545603)  */
+    double kappa;     /* initial orbital phase of the guiding centre                     */
+    double lambda0;   /* initial orientation of the constellation                        */
+} gbo_config;
+
+typedef struct {          /* host-resident data view; mirrors the product's gb_data but is its own type */
+    double *resid;        /* [n_walkers][2][n_f] complex128 interleaved (r = d - H)                     */
+    const double *psd;    /* [n_psd][2][n_f] f64; S_n, or 1/S_n if psd_is_inverse                       */
+    const int32_t *walker_psd; /* [n_walkers] -> psd row; NULL = identity (or row 0 if n_psd == 1)      */
+    int64_t k_lo, n_f;    /* residual element i <-> global bin k_lo + i                                  */
+    int32_t n_walkers, n_psd, psd_is_inverse;
+} gbo_data;
+
+enum { GBO_ADD = 0, GBO_REMOVE = 1, GBO_SWAP = 2 };
+enum { GBO_OK = 0, GBO_ERR_INVALID = -1 };
+
+void gbo_default_config(gbo_config *c) {
+    c->Tobs = 31457280.0;
+    c->dt = 5.0;
+    c->armlength = 2.5e9;
+    c->au = 1.495978707e11;
+    c->year = 31558149.763545603;
+    c->kappa = 0.0;
+    c->lambda0 = 0.0;
+}
+
+/* params row = [amp, f0, fdot, phi0, cos_iota, psi, lambda, sin_beta]  (reading S3) */
+enum { P_AMP = 0, P_F0, P_FDOT, P_PHI0, P_COSI, P_PSI, P_LAM, P_SINB };
+
+typedef struct {
+    double u[3], v[3], k[3]; /* polarisation basis and propagation direction */
+    double complex DP, DC;   /* polarisation constants                        */
+    int64_t q;               /* carrier bin                                   */
+    double delta;            /* f0*T - q, cycles                              */
+} gbo_source;
+
+/* ---- O1  source constants ---------------------------------------------------- */
+static void o1_source_constants(const gbo_config *c, const double *p, gbo_source *s) {
+    double sinb = p[P_SINB];
+    double cosb = sqrt(1.0 - sinb * sinb);     /* cos(beta) >= 0                                */
+    /* theta_c = pi/2 - beta  =>  cos(theta_c) = sin(beta), sin(theta_c) = cos(beta); phi = lambda */
+    double costh = sinb, sinth = cosb;
+    double cosph = cos(p[P_LAM]), sinph = sin(p[P_LAM]);
+    s->u[0] = costh * cosph;  s->u[1] = costh * sinph;  s->u[2] = -sinth;
+    s->v[0] = sinph;          s->v[1] = -cosph;         s->v[2] = 0.0;
+    s->k[0] = -sinth * cosph; s->k[1] = -sinth * sinph; s->k[2] = -costh;
+    double amp = p[P_AMP], ci = p[P_COSI];
+    double Ap = amp * (1.0 + ci * ci);         /* A_plus  */
+    double Ac = -2.0 * amp * ci;               /* A_cross */
+    double c2p = cos(2.0 * p[P_PSI]), s2p = sin(2.0 * p[P_PSI]);
+    s->DP = Ap * c2p - I * (Ac * s2p);
+    s->DC = -Ap * s2p - I * (Ac * c2p);
+    double prod = p[P_F0] * c->Tobs;           /* rounded product (no FMA contraction)          */
+    s->q = (int64_t)floor(prod + 0.5);
+    s->delta = fma(p[P_F0], c->Tobs, -(double)s->q);
+}
+
+/* ---- O2  analytic equal-arm orbits, first order in eccentricity -------------- */
+static void o2_orbits(const gbo_config *c, double t, double x[3][3]) {
+    double fm = 1.0 / c->year;
+    double ecc = c->armlength / (2.0 * sqrt(3.0) * c->au);
+    double alpha = 2.0 * GBO_PI * fm * t + c->kappa;
+    double sa = sin(alpha), ca = cos(alpha);
+    for (int i = 0; i < 3; i++) {              /* spacecraft i+1 */
+        double beta = 2.0 * GBO_PI * i / 3.0 + c->lambda0;
+        double sb = sin(beta), cb = cos(beta);
+        x[i][0] = c->au * ca + c->au * ecc * (sa * ca * sb - (1.0 + sa * sa) * cb);
+        x[i][1] = c->au * sa + c->au * ecc * (sa * ca * cb - (1.0 + ca * ca) * sb);
+        x[i][2] = -sqrt(3.0) * c->au * ecc * cos(alpha - beta);
+    }
+}
+
+static double dot3(const double a[3], const double b[3]) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+static double sinc(double th) {
+    if (fabs(th) < 1e-8) return 1.0 - th * th / 6.0;
+    return sin(th) / th;
+}
+
+/* ---- O3 + O4 + O5  slow envelope of A and E at time sample n of N ---- */
+static void slow_envelope(const gbo_config *c, const double *p, const gbo_source *src, int N, int n,
+                          double *As_out, double *Es_out) {
+    const gbo_source s = *src;
+    double T = c->Tobs, L = c->armlength;
+    double f0 = p[P_F0], fdot = p[P_FDOT], phi0 = p[P_PHI0];
+    double t = (double)n * T / (double)N;
+    double x[3][3];
+    o2_orbits(c, t, x);
+
+    double xarg = 2.0 * GBO_PI * (f0 + fdot * t) * L / GBO_C_LIGHT;  /* x(t_n), common to all links */
+    double complex Y[3][3];                                            /* Y[r][s], receiver r, sender s */
+    for (int r = 0; r < 3; r++) {
+        double kx = dot3(s.k, x[r]) / GBO_C_LIGHT;                     /* k.x_r / c            */
+        double xi = t - kx;                                            /* xi_r                 */
+        double a_r = 1.0 + (2.0 / 3.0) * (fdot / f0) * xi;
+        double phi = 2.0 * GBO_PI * (s.delta * ((double)n / (double)N) - f0 * kx)
+                   + GBO_PI * fdot * xi * xi + phi0;                   /* Phi(xi_r) - 2 pi q t_n / T */
+        for (int sd = 0; sd < 3; sd++) {
+            if (sd == r) { Y[r][sd] = 0.0; continue; }
+            double nrs[3];                                             /* O3 link vector       */
+            for (int d = 0; d < 3; d++) nrs[d] = (x[r][d] - x[sd][d]) / L;
+            double nu_u = dot3(s.u, nrs), nu_v = dot3(s.v, nrs), kap = dot3(s.k, nrs);
+            double dplus = nu_u * nu_u - nu_v * nu_v;
+            double dcross = 2.0 * nu_u * nu_v;
+            double complex D = dplus * s.DP + dcross * s.DC;
+            double th = 0.5 * xarg * (1.0 - kap);
+            Y[r][sd] = -(0.5 * I) * xarg * sinc(th) * cexp(-I * th) * D * a_r * cexp(I * phi);
+        }
+    }
+    /* O5  first-generation Michelson with delay phasor E1 = exp(-i x); indices receiver,sender */
+    double complex E1 = cexp(-I * xarg);
+    double complex XYZ[3];
+    for (int a = 0; a < 3; a++) {              /* a = 0: X (1,2,3), 1: Y (2,3,1), 2: Z (3,1,2) */
+        int i1 = a, i2 = (a + 1) % 3, i3 = (a + 2) % 3;
+        XYZ[a] = (1.0 - E1 * E1) * ((Y[i1][i3] - Y[i1][i2]) + E1 * (Y[i3][i1] - Y[i2][i1]));
+    }
+    double complex As = (XYZ[2] - XYZ[0]) / sqrt(2.0);                 /* Eq. 6a */
+    double complex Es = (XYZ[0] - 2.0 * XYZ[1] + XYZ[2]) / sqrt(6.0);  /* Eq. 6b */
+    As_out[0] = creal(As); As_out[1] = cimag(As);
+    Es_out[0] = creal(Es); Es_out[1] = cimag(Es);
+}
+
+/* public form: O1 then O3-O5 for one sample (exposed for pins P4, P5) */
+void gbo_slow_envelope(const gbo_config *c, const double *p, int N, int n, double *As_out, double *Es_out) {
+    gbo_source s;
+    o1_source_constants(c, p, &s);
+    slow_envelope(c, p, &s, N, n, As_out, Es_out);
+}
+
+/* ---- plain O(N^2) DFT, numpy-forward sign:  F[j] = sum_n x[n] exp(-2 pi i j n / N) ------------- */
+void gbo_dft(const double *x, int N, double *F) {
+    for (int j = 0; j < N; j++) {
+        double complex acc = 0.0;
+        for (int n = 0; n < N; n++) {
+            int m = (int)(((int64_t)j * n) % N);                       /* exact phase reduction */
+            double ang = -2.0 * GBO_PI * (double)m / (double)N;
+            acc += (x[2 * n] + I * x[2 * n + 1]) * (cos(ang) + I * sin(ang));
+        }
+        F[2 * j] = creal(acc); F[2 * j + 1] = cimag(acc);
+    }
+}
+
+/* ---- textbook iterative radix-2 decimation-in-time FFT, same sign; N a power of two ------------ */
+int gbo_fft(const double *x, int N, double *F) {
+    if (N < 1 || (N & (N - 1))) return GBO_ERR_INVALID;
+    int bits = 0; while ((1 << bits) < N) bits++;
+    double complex *a = (double complex *)malloc(sizeof(double complex) * (size_t)N);
+    for (int n = 0; n < N; n++) {
+        int rev = 0;
+        for (int b = 0; b < bits; b++) if (n & (1 << b)) rev |= 1 << (bits - 1 - b);
+        a[rev] = x[2 * n] + I * x[2 * n + 1];
+    }
+    for (int len = 2; len <= N; len <<= 1) {
+        for (int start = 0; start < N; start += len) {
+            for (int m = 0; m < len / 2; m++) {
+                double ang = -2.0 * GBO_PI * (double)m / (double)len;
+                double complex w = cos(ang) + I * sin(ang);
+                double complex e = a[start + m], o = w * a[start + m + len / 2];
+                a[start + m] = e + o;
+                a[start + m + len / 2] = e - o;
+            }
+        }
+    }
+    for (int j = 0; j < N; j++) { F[2 * j] = creal(a[j]); F[2 * j + 1] = cimag(a[j]); }
+    free(a);
+    return GBO_OK;
+}
+
+static int valid_N(int N) { return N >= 2 && N <= (1 << 20) && !(N & (N - 1)); }
+
+/* ---- O6  FFT of the slow part and mapping to bins ------------------------------
+ * A[kmin + j] = (T / (2N)) * F[j - N/2],  j = 0..N-1,  kmin = q - N/2,  F indexed modulo N.
+ * use_dft != 0 uses the O(N^2) definition instead of the radix-2 FFT (for pins).                  */
+int gbo_waveform_ex(const gbo_config *c, const double *p, int N, int use_dft,
+                    double *A, double *E, int64_t *kmin) {
+    if (!valid_N(N)) return GBO_ERR_INVALID;
+    gbo_source s;
+    o1_source_constants(c, p, &s);
+    double *as = (double *)malloc(sizeof(double) * 2 * (size_t)N * 4);
+    double *es = as + 2 * (size_t)N, *Fa = es + 2 * (size_t)N, *Fe = Fa + 2 * (size_t)N;
+    for (int n = 0; n < N; n++) slow_envelope(c, p, &s, N, n, as + 2 * n, es + 2 * n);
+    if (use_dft) { gbo_dft(as, N, Fa); gbo_dft(es, N, Fe); }
+    else         { gbo_fft(as, N, Fa); gbo_fft(es, N, Fe); }
+    double scale = c->Tobs / (2.0 * (double)N);
+    for (int j = 0; j < N; j++) {
+        int jj = (j - N / 2 + N) % N;          /* F[j - N/2] with negative indices wrapped */
+        A[2 * j] = scale * Fa[2 * jj]; A[2 * j + 1] = scale * Fa[2 * jj + 1];
+        E[2 * j] = scale * Fe[2 * jj]; E[2 * j + 1] = scale * Fe[2 * jj + 1];
+    }
+    *kmin = s.q - N / 2;
+    free(as);
+    return GBO_OK;
+}
+
+int gbo_waveform(const gbo_config *c, const double *p, int N, double *A, double *E, int64_t *kmin) {
+    return gbo_waveform_ex(c, p, N, 0, A, E, kmin);
+}
+
+/* batched form of the product's gb_waveform: AE_out [B][2][Nmax] complex128, kmin_out [B] */
+int gbo_waveform_batch(const gbo_config *c, const double *params, int64_t B, int N, const int32_t *n_bins,
+                       int Nmax, double *AE_out, int64_t *kmin_out, int nthreads) {
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads > 0 ? nthreads : 1)
+    for (int64_t b = 0; b < B; b++) {
+        int Nb = n_bins ? n_bins[b] : N;
+        if (!valid_N(Nb) || Nb > Nmax) { bad = 1; continue; }
+        double *A = (double *)malloc(sizeof(double) * 4 * (size_t)Nb), *E = A + 2 * (size_t)Nb;
+        gbo_waveform(c, params + 8 * b, Nb, A, E, &kmin_out[b]);
+        double *outA = AE_out + (size_t)b * 2 * 2 * (size_t)Nmax, *outE = outA + 2 * (size_t)Nmax;
+        memcpy(outA, A, sizeof(double) * 2 * (size_t)Nb);
+        memcpy(outE, E, sizeof(double) * 2 * (size_t)Nb);
+        free(A);
+    }
+    return bad ? GBO_ERR_INVALID : GBO_OK;
+}
+
+/* ---- O7  noise-weighted inner product on aligned windows (Eq. 2) --------------------
+ * <b|c> = (4/T) sum_ch sum_k Re[conj(b_ch[k]) c_ch[k]] / S_ch[k] over global bins k that lie in both
+ * windows and in the stored band [k_lo, k_lo + n_f)  (reading S13).
+ * b: window starting at global bin kb with nb bins, channel arrays bA,bE (interleaved complex);
+ * c likewise.  S given by psd row pointers (S or 1/S).                                              */
+static double o7_inner(const gbo_config *cfg, const gbo_data *d, int psd_row,
+                       const double *bA, const double *bE, int64_t kb, int nb,
+                       const double *cA, const double *cE, int64_t kc, int nc) {
+    int64_t lo = kb > kc ? kb : kc;
+    int64_t hi = (kb + nb) < (kc + nc) ? (kb + nb) : (kc + nc);
+    if (lo < d->k_lo) lo = d->k_lo;
+    if (hi > d->k_lo + d->n_f) hi = d->k_lo + d->n_f;
+    const double *SA = d->psd + ((size_t)psd_row * 2 + 0) * (size_t)d->n_f;
+    const double *SE = d->psd + ((size_t)psd_row * 2 + 1) * (size_t)d->n_f;
+    double sum = 0.0;
+    for (int64_t k = lo; k < hi; k++) {
+        int64_t ib = k - kb, ic = k - kc, i = k - d->k_lo;
+        double complex ba = bA[2 * ib] + I * bA[2 * ib + 1], ca = cA[2 * ic] + I * cA[2 * ic + 1];
+        double complex be = bE[2 * ib] + I * bE[2 * ib + 1], ce = cE[2 * ic] + I * cE[2 * ic + 1];
+        double ta = creal(conj(ba) * ca), te = creal(conj(be) * ce);
+        if (d->psd_is_inverse) sum += ta * SA[i] + te * SE[i];
+        else                   sum += ta / SA[i] + te / SE[i];
+    }
+    return 4.0 / cfg->Tobs * sum;
+}
+
+static int psd_row_of(const gbo_data *d, int w) {
+    if (d->walker_psd) return d->walker_psd[w];
+    return d->n_psd == 1 ? 0 : w;
+}
+
+/* residual of walker w viewed as a window over the whole stored band */
+static const double *resid_ch(const gbo_data *d, int w, int ch) {
+    return d->resid + (((size_t)w * 2 + (size_t)ch) * (size_t)d->n_f) * 2;
+}
+
+/* ---- O8  delta log-likelihood of one proposal row (Eq. 4, Eq. 5) ------- */
+static int o8_row(const gbo_config *c, const gbo_data *d, const double *pnew, const double *pold,
+                  int w, int mv, int N, double *dlnL, double *aux) {
+    if (w < 0 || w >= d->n_walkers) return GBO_ERR_INVALID;
+    int row = psd_row_of(d, w);
+    const double *rA = resid_ch(d, w, 0), *rE = resid_ch(d, w, 1);
+    double *buf = (double *)malloc(sizeof(double) * 8 * (size_t)N);
+    double *aA = buf, *aE = buf + 2 * (size_t)N, *oA = buf + 4 * (size_t)N, *oE = buf + 6 * (size_t)N;
+    int64_t ka = 0, ko = 0;
+    int rc = GBO_OK;
+    if (mv == GBO_ADD) {
+        gbo_waveform(c, pnew, N, aA, aE, &ka);
+        double aa = o7_inner(c, d, row, aA, aE, ka, N, aA, aE, ka, N);
+        double ra = o7_inner(c, d, row, rA, rE, d->k_lo, (int)d->n_f, aA, aE, ka, N);
+        *dlnL = ra - 0.5 * aa;                                  /* Eq. 4 with r = d - H */
+        if (aux) { aux[0] = aa; aux[1] = ra; }
+    } else if (mv == GBO_REMOVE) {
+        gbo_waveform(c, pold, N, oA, oE, &ko);
+        double oo = o7_inner(c, d, row, oA, oE, ko, N, oA, oE, ko, N);
+        double ro = o7_inner(c, d, row, rA, rE, d->k_lo, (int)d->n_f, oA, oE, ko, N);
+        *dlnL = -ro - 0.5 * oo;                                 /* Eq. 5 with a == 0     */
+        if (aux) { aux[0] = oo; aux[1] = ro; }
+    } else if (mv == GBO_SWAP) {
+        gbo_waveform(c, pnew, N, aA, aE, &ka);
+        gbo_waveform(c, pold, N, oA, oE, &ko);
+        double aa = o7_inner(c, d, row, aA, aE, ka, N, aA, aE, ka, N);
+        double oo = o7_inner(c, d, row, oA, oE, ko, N, oA, oE, ko, N);
+        double ao = o7_inner(c, d, row, aA, aE, ka, N, oA, oE, ko, N);
+        double ra = o7_inner(c, d, row, rA, rE, d->k_lo, (int)d->n_f, aA, aE, ka, N);
+        double ro = o7_inner(c, d, row, rA, rE, d->k_lo, (int)d->n_f, oA, oE, ko, N);
+        *dlnL = -0.5 * (aa + oo - 2.0 * ao - 2.0 * ra + 2.0 * ro);   /* Eq. 5 */
+        if (aux) { aux[0] = aa; aux[1] = ra; }
+    } else {
+        rc = GBO_ERR_INVALID;
+    }
+    free(buf);
+    return rc;
+}
+
+/* batched O8; proposals are evaluated independently against the same residual snapshot */
+int gbo_delta_loglike(const gbo_config *c, const gbo_data *d, const double *params_new,
+                      const double *params_old, const int32_t *walker_index, const int8_t *move,
+                      int move_all, int N, const int32_t *n_bins, int64_t B,
+                      double *dlnL_out, double *aux_out, int nthreads) {
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads > 0 ? nthreads : 1)
+    for (int64_t b = 0; b < B; b++) {
+        int mv = move ? move[b] : move_all;
+        int Nb = n_bins ? n_bins[b] : N;
+        if (!valid_N(Nb)) { bad = 1; continue; }
+        const double *pn = params_new ? params_new + 8 * b : NULL;
+        const double *po = params_old ? params_old + 8 * b : NULL;
+        if ((mv != GBO_REMOVE && !pn) || (mv != GBO_ADD && !po)) { bad = 1; continue; }
+        if (o8_row(c, d, pn, po, walker_index[b], mv, Nb, &dlnL_out[b], aux_out ? aux_out + 2 * b : NULL))
+            bad = 1;
+    }
+    return bad ? GBO_ERR_INVALID : GBO_OK;
+}
+
+/* r[k] += sign * h[k] on the part of the window inside the stored band */
+static void add_window(const gbo_data *d, int w, const double *hA, const double *hE, int64_t kh, int N, double sign) {
+    double *rA = (double *)resid_ch(d, w, 0), *rE = (double *)resid_ch(d, w, 1);
+    for (int j = 0; j < N; j++) {
+        int64_t i = kh + j - d->k_lo;
+        if (i < 0 || i >= d->n_f) continue;
+        rA[2 * i] += sign * hA[2 * j]; rA[2 * i + 1] += sign * hA[2 * j + 1];
+        rE[2 * i] += sign * hE[2 * j]; rE[2 * i + 1] += sign * hE[2 * j + 1];
+    }
+}
+
+/* ---- O9  residual update (Alg. 1): rows applied in order b = 0..B-1 ------------
+ * ADD: r -= a.  REMOVE: r += h.  SWAP: r += o, r -= a.  Rows of different walkers touch disjoint
+ * memory, so handing whole walkers to different threads leaves every bit as in the sequential loop. */
+int gbo_residual_update(const gbo_config *c, gbo_data *d, const double *params_new, const double *params_old,
+                        const int32_t *walker_index, const int8_t *move, int move_all,
+                        const uint8_t *accepted, int N, const int32_t *n_bins, int64_t B, int nthreads) {
+    int bad = 0;
+    for (int64_t b = 0; b < B; b++)
+        if (walker_index[b] < 0 || walker_index[b] >= d->n_walkers) return GBO_ERR_INVALID;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads > 0 ? nthreads : 1)
+    for (int w = 0; w < d->n_walkers; w++) {
+        for (int64_t b = 0; b < B; b++) {
+            if (walker_index[b] != w || (accepted && !accepted[b])) continue;
+            int mv = move ? move[b] : move_all;
+            int Nb = n_bins ? n_bins[b] : N;
+            if (!valid_N(Nb)) { bad = 1; continue; }
+            double *h = (double *)malloc(sizeof(double) * 4 * (size_t)Nb), *hE = h + 2 * (size_t)Nb;
+            int64_t kh;
+            if (mv == GBO_REMOVE || mv == GBO_SWAP) {
+                gbo_waveform(c, params_old + 8 * b, Nb, h, hE, &kh);
+                add_window(d, w, h, hE, kh, Nb, +1.0);
+            }
+            if (mv == GBO_ADD || mv == GBO_SWAP) {
+                gbo_waveform(c, params_new + 8 * b, Nb, h, hE, &kh);
+                add_window(d, w, h, hE, kh, Nb, -1.0);
+            }
+            if (mv != GBO_ADD && mv != GBO_REMOVE && mv != GBO_SWAP) bad = 1;
+            free(h);
+        }
+    }
+    return bad ? GBO_ERR_INVALID : GBO_OK;
+}
+
+/* <b|c> of two explicit windows against PSD row `psd_row` (exposed for pins P4-P6) */
+double gbo_inner_windows(const gbo_config *c, const gbo_data *d, int psd_row,
+                         const double *bA, const double *bE, int64_t kb, int nb,
+                         const double *cA, const double *cE, int64_t kc, int nc) {
+    return o7_inner(c, d, psd_row, bA, bE, kb, nb, cA, cE, kc, nc);
+}
+
+/* orbit positions at time t, row-major [3][3] (exposed for the orbit pin) */
+void gbo_orbits(const gbo_config *c, double t, double *x_out) {
+    double x[3][3];
+    o2_orbits(c, t, x);
+    memcpy(x_out, x, sizeof(x));
+}
+
+int gbo_max_threads(void) {
+#ifdef _OPENMP
+    extern int omp_get_max_threads(void);
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,211 @@
+"""ctypes wrapper around oracle/gb_oracle.c (the CPU oracle).
+
+TEST INFRASTRUCTURE ONLY: importable from tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs.  The product package never imports this module.
+
+All arithmetic of the method lives in gb_oracle.c; this file only marshals numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gb_oracle.c")
+_LIB = os.path.join(_HERE, "libgb_oracle.so")
+
+ADD, REMOVE, SWAP = 0, 1, 2
+
+
+def build(force: bool = False) -> str:
+    """Compile gb_oracle.c -> libgb_oracle.so (gcc, -O2, no FMA contraction, OpenMP)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fopenmp", "-Wall", "-Wextra",
+               "-shared", "-fPIC", _SRC, "-o", _LIB, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Config(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("Tobs", "dt", "armlength", "au", "year", "kappa", "lambda0")]
+
+
+class _Data(C.Structure):
+    _fields_ = [("resid", C.c_void_p), ("psd", C.c_void_p), ("walker_psd", C.c_void_p),
+                ("k_lo", C.c_int64), ("n_f", C.c_int64),
+                ("n_walkers", C.c_int32), ("n_psd", C.c_int32), ("psd_is_inverse", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.gbo_inner_windows.restype = C.c_double
+    return _lib
+
+
+@dataclass
+class Config:
+    Tobs: float = 31457280.0
+    dt: float = 5.0
+    armlength: float = 2.5e9
+    au: float = 1.495978707e11
+    year: float = 31558149.763545603
+    kappa: float = 0.0
+    lambda0: float = 0.0
+
+    def c(self) -> _Config:
+        return _Config(self.Tobs, self.dt, self.armlength, self.au, self.year, self.kappa, self.lambda0)
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def max_threads() -> int:
+    return int(lib().gbo_max_threads())
+
+
+class Data:
+    """Host residual / PSD view.  resid: complex128 [n_walkers, 2, n_f] (modified in place by
+    residual_update); psd: float64 [n_psd, 2, n_f]."""
+
+    def __init__(self, resid, psd, k_lo, walker_psd=None, psd_is_inverse=False):
+        assert resid.dtype == np.complex128 and resid.ndim == 3 and resid.shape[1] == 2
+        assert resid.flags.c_contiguous
+        self.resid = resid
+        self.psd = np.ascontiguousarray(psd, dtype=np.float64)
+        assert self.psd.ndim == 3 and self.psd.shape[1] == 2 and self.psd.shape[2] == resid.shape[2]
+        self.walker_psd = None if walker_psd is None else np.ascontiguousarray(walker_psd, dtype=np.int32)
+        self.k_lo = int(k_lo)
+        self.psd_is_inverse = bool(psd_is_inverse)
+
+    def c(self) -> _Data:
+        return _Data(_ptr(self.resid), _ptr(self.psd), _ptr(self.walker_psd), self.k_lo,
+                     self.resid.shape[2], self.resid.shape[0], self.psd.shape[0], int(self.psd_is_inverse))
+
+
+def slow_envelope(cfg: Config, params, N: int):
+    """A_s(t_n), E_s(t_n), n = 0..N-1 (steps O1-O5).  Returns two complex128 arrays [N]."""
+    p = _f64(params)
+    cc = cfg.c()
+    a = np.empty(2, np.float64)
+    e = np.empty(2, np.float64)
+    As = np.empty(N, np.complex128)
+    Es = np.empty(N, np.complex128)
+    for n in range(N):
+        lib().gbo_slow_envelope(C.byref(cc), _ptr(p), C.c_int(N), C.c_int(n), _ptr(a), _ptr(e))
+        As[n] = a[0] + 1j * a[1]
+        Es[n] = e[0] + 1j * e[1]
+    return As, Es
+
+
+def waveform(cfg: Config, params, N: int, use_dft: bool = False):
+    """One source: returns (A[N], E[N], kmin) (steps O1-O6)."""
+    p = _f64(params)
+    A = np.empty(N, np.complex128)
+    E = np.empty(N, np.complex128)
+    kmin = C.c_int64(0)
+    cc = cfg.c()
+    rc = lib().gbo_waveform_ex(C.byref(cc), _ptr(p), C.c_int(N), C.c_int(int(use_dft)), _ptr(A), _ptr(E),
+                               C.byref(kmin))
+    if rc != 0:
+        raise ValueError(f"gbo_waveform_ex rc={rc}")
+    return A, E, int(kmin.value)
+
+
+def waveform_batch(cfg: Config, params, N: int = 0, n_bins=None, nthreads: int = 1):
+    """Batched: returns (AE[B,2,Nmax] complex128, kmin[B] int64); rows shorter than Nmax are zero padded."""
+    p = _f64(params).reshape(-1, 8)
+    B = p.shape[0]
+    nb = None if n_bins is None else np.ascontiguousarray(n_bins, dtype=np.int32)
+    Nmax = int(N if nb is None else (nb.max() if B else N))
+    AE = np.zeros((B, 2, Nmax), np.complex128)
+    kmin = np.zeros(B, np.int64)
+    cc = cfg.c()
+    rc = lib().gbo_waveform_batch(C.byref(cc), _ptr(p), C.c_int64(B), C.c_int(N), _ptr(nb), C.c_int(Nmax),
+                                  _ptr(AE), _ptr(kmin), C.c_int(nthreads))
+    if rc != 0:
+        raise ValueError(f"gbo_waveform_batch rc={rc}")
+    return AE, kmin
+
+
+def delta_loglike(cfg: Config, data: Data, params_new, params_old, walker_index, move=None, move_all=ADD,
+                  N: int = 0, n_bins=None, want_aux: bool = False, nthreads: int = 1):
+    """Batched step O8.  Returns dlnL[B] (and aux[B,2] = (<h|h>, <r|h>) if want_aux)."""
+    pn = None if params_new is None else _f64(params_new).reshape(-1, 8)
+    po = None if params_old is None else _f64(params_old).reshape(-1, 8)
+    w = np.ascontiguousarray(walker_index, dtype=np.int32)
+    B = w.shape[0]
+    mv = None if move is None else np.ascontiguousarray(move, dtype=np.int8)
+    nb = None if n_bins is None else np.ascontiguousarray(n_bins, dtype=np.int32)
+    out = np.zeros(B, np.float64)
+    aux = np.zeros((B, 2), np.float64) if want_aux else None
+    cc, dd = cfg.c(), data.c()
+    rc = lib().gbo_delta_loglike(C.byref(cc), C.byref(dd), _ptr(pn), _ptr(po), _ptr(w), _ptr(mv),
+                                 C.c_int(move_all), C.c_int(N), _ptr(nb), C.c_int64(B), _ptr(out), _ptr(aux),
+                                 C.c_int(nthreads))
+    if rc != 0:
+        raise ValueError(f"gbo_delta_loglike rc={rc}")
+    return (out, aux) if want_aux else out
+
+
+def residual_update(cfg: Config, data: Data, params_new, params_old, walker_index, move=None, move_all=ADD,
+                    accepted=None, N: int = 0, n_bins=None, nthreads: int = 1):
+    """Step O9, in place on data.resid."""
+    pn = None if params_new is None else _f64(params_new).reshape(-1, 8)
+    po = None if params_old is None else _f64(params_old).reshape(-1, 8)
+    w = np.ascontiguousarray(walker_index, dtype=np.int32)
+    B = w.shape[0]
+    mv = None if move is None else np.ascontiguousarray(move, dtype=np.int8)
+    nb = None if n_bins is None else np.ascontiguousarray(n_bins, dtype=np.int32)
+    acc = None if accepted is None else np.ascontiguousarray(accepted, dtype=np.uint8)
+    cc, dd = cfg.c(), data.c()
+    rc = lib().gbo_residual_update(C.byref(cc), C.byref(dd), _ptr(pn), _ptr(po), _ptr(w), _ptr(mv),
+                                   C.c_int(move_all), _ptr(acc), C.c_int(N), _ptr(nb), C.c_int64(B),
+                                   C.c_int(nthreads))
+    if rc != 0:
+        raise ValueError(f"gbo_residual_update rc={rc}")
+
+
+def inner_windows(cfg: Config, data: Data, psd_row: int, bA, bE, kb: int, cA, cE, kc: int) -> float:
+    """<b|c> of two explicit windows (step O7)."""
+    bA, bE, cA, cE = (np.ascontiguousarray(z, dtype=np.complex128) for z in (bA, bE, cA, cE))
+    cc, dd = cfg.c(), data.c()
+    return float(lib().gbo_inner_windows(C.byref(cc), C.byref(dd), C.c_int(psd_row),
+                                         _ptr(bA), _ptr(bE), C.c_int64(kb), C.c_int(len(bA)),
+                                         _ptr(cA), _ptr(cE), C.c_int64(kc), C.c_int(len(cA))))
+
+
+def dft(x):
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    F = np.empty_like(x)
+    lib().gbo_dft(_ptr(x), C.c_int(len(x)), _ptr(F))
+    return F
+
+
+def fft(x):
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    F = np.empty_like(x)
+    rc = lib().gbo_fft(_ptr(x), C.c_int(len(x)), _ptr(F))
+    if rc != 0:
+        raise ValueError("gbo_fft: N must be a power of two")
+    return F
+
+
+def orbits(cfg: Config, t: float):
+    x = np.empty((3, 3), np.float64)
+    cc = cfg.c()
+    lib().gbo_orbits(C.byref(cc), C.c_double(t), _ptr(x))
+    return x
