@@ -1,0 +1,162 @@
+/*
+ * gbfit.h -- C ABI of the B200-native Galactic-binary (GB) waveform + delta-log-likelihood hot path
+ *            of the "Erebor" LISA global fit (arxiv 2405.04690; citations are PAPER.md:<line>).
+ *
+ * What the library computes
+ *   gb_waveform         frequency-domain TDI A/E waveform of each GB on its own N-bin window around f0,
+ *                       by the fast/slow decomposition (sec. II.A; App. F):
+ *                       the slow LISA response at N time samples (TDI generation 1.5, equal constant arms,
+ *                       PAPER.md:105; A,E of Eq. 6) followed by a length-N FFT.
+ *   gb_delta_loglike    the change of the Gaussian log-likelihood (Eq. 1-2) when one source
+ *                       is added (Eq. 4), removed, or swapped for another (Eq. 5,
+ *                       PAPER.md:96-103), against the walker's residual r = d - H and that walker's PSD;
+ *                       sums run only over the bins where the source lives.
+ *   gb_residual_update  the residual refresh of Algorithm 1: accepted waveforms are
+ *                       scatter-added into the per-walker residuals.
+ * The paper does not print the GB waveform equations; the exact definition implemented is
+ * written out in DESIGN.md ("The path", steps O1-O9) together with every reading of a silent point.
+ *
+ * General conventions
+ *   - Every pointer is a DEVICE pointer on the context's device unless the parameter comment says HOST.
+ *     The caller owns every buffer; the library allocates only inside gb_ctx (tables and scratch).
+ *   - All calls return an int status (GB_OK = 0, negative = error), never throw, never abort.
+ *   - Device work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream) and is asynchronous with respect to the host, except the *_host entry points, which
+ *     synchronise `stream` before returning.  Errors detectable at launch are returned at once; per-row
+ *     errors (walker index out of range, N not in {128,256,512,1024}) set a sticky device flag that the next
+ *     call to gb_check() reports, and give NaN in that row of the output.
+ *   - Complex arrays are complex128, interleaved (re, im) doubles.  Real arrays are f64.
+ *   - params row (8 f64): [amp, f0 (Hz), fdot (Hz/s), phi0, cos(iota), psi, lambda (ecl. lon.), sin(beta)].
+ *   - Frequency bins: global bin k  <->  f = k / Tobs  (the rfft grid of the data).
+ *     A source's window is bins kmin .. kmin+N-1 with kmin = floor(f0*Tobs + 0.5) - N/2.
+ *   - Residual semantic r = d - H: ADD subtracts the waveform, REMOVE adds it, SWAP adds old, subtracts new.
+ *   - Window bins outside the stored band [k_lo, k_lo + n_f) contribute nothing to any inner product and
+ *     are not scattered.
+ *   - Tempering, priors and proposal densities (Eq. 13) are not applied: the caller does
+ *     accept/reject.  Rows of one call are evaluated independently against the same residual snapshot.
+ *   - A gb_ctx may be used from one host thread at a time.
+ */
+#ifndef GBFIT_H
+#define GBFIT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gb_ctx gb_ctx; /* opaque; owns orbit tables, FFT twiddles and scratch on one device */
+
+typedef struct {      /* HOST POD, copied by gb_create */
+    double Tobs;      /* observation time [s]; the FFT grid is k / Tobs                 (31457280)           */
+    double dt;        /* cadence of the data [s]; only used to validate kmin+N-1 <= Tobs/(2 dt)   (5)         */
+    double armlength; /* L [m]                                                          (2.5e9)              */
+    double au;        /* astronomical unit [m]                                          (1.495978707e11)     */
+    double year;      /* orbital period of the constellation [s]                        (31558149.763545603) */
+    double kappa;     /* initial orbital phase of the guiding centre [rad]              (0)                  */
+    double lambda0;   /* initial orientation of the constellation [rad]                 (0)                  */
+    int32_t device;   /* CUDA device ordinal                                                                 */
+    int32_t reserved; /* set to 0                                                                            */
+} gb_config;
+
+typedef struct {      /* HOST POD describing DEVICE-resident data, caller-owned */
+    double *resid;              /* [n_walkers][2][n_f] complex128; ch 0 = A, ch 1 = E; r = d - H; 16-byte aligned */
+    const double *psd;          /* [n_psd][2][n_f] f64; S_n(f) per channel, or 1/S_n if psd_is_inverse           */
+    const int32_t *walker_psd;  /* [n_walkers] -> psd row; NULL = identity, or row 0 when n_psd == 1             */
+    int64_t k_lo, n_f;          /* residual element i  <->  global bin k_lo + i                                  */
+    int32_t n_walkers, n_psd, psd_is_inverse, reserved;
+} gb_data;
+
+enum { GB_ADD = 0, GB_REMOVE = 1, GB_SWAP = 2 };
+
+enum {
+    GB_OK = 0,
+    GB_ERR_INVALID = -1,   /* NULL required pointer, B < 0, bad N, bad config                    */
+    GB_ERR_CUDA = -2,      /* a CUDA runtime call failed; see gb_last_error                      */
+    GB_ERR_NOMEM = -3,     /* scratch allocation failed                                          */
+    GB_ERR_ROW = -4        /* gb_check: some row of an earlier call had a bad walker index or N  */
+};
+
+/* Fill *cfg with the defaults listed above (device 0).  cfg: HOST. */
+void gb_default_config(gb_config *cfg);
+
+/* Create a context on cfg->device: builds the orbit tables (analytic equal-arm orbits, O2) for
+ * N = 128, 256, 512, 1024 and the FFT twiddles.  cfg, out: HOST.  Returns GB_OK or an error. */
+int gb_create(const gb_config *cfg, gb_ctx **out);
+
+/* Free the context and its device memory (synchronises the device).  NULL is allowed. */
+void gb_destroy(gb_ctx *ctx);
+
+/* Last error message of this context (HOST string owned by ctx, valid until the next call). */
+const char *gb_last_error(const gb_ctx *ctx);
+
+/* Synchronise `stream`, then report and clear the sticky per-row error flag: GB_OK, GB_ERR_ROW or GB_ERR_CUDA. */
+int gb_check(gb_ctx *ctx, void *stream);
+
+/* Library version string "gbfit-b200 x.y" (HOST, static). */
+const char *gb_version(void);
+
+/* Number of kernels launched by this context since creation (bench.py's gpu_launches counter). */
+int64_t gb_launch_count(const gb_ctx *ctx);
+
+/*
+ * gb_waveform -- A/E windows of B sources.
+ *   params   [B][8] f64
+ *   N        window length used for every row when n_bins == NULL; one of 128, 256, 512, 1024
+ *   n_bins   [B] int32 per-row window length, or NULL
+ *   Nmax     row pitch of AE_out in complex elements (>= every row's N)
+ *   AE_out   [B][2][Nmax] complex128: element (b, ch, j) is the waveform at global bin kmin[b] + j, j < N_b;
+ *            elements j >= N_b are left untouched
+ *   kmin_out [B] int64, may be NULL
+ */
+int gb_waveform(gb_ctx *ctx, const double *params, int64_t B, int N, const int32_t *n_bins,
+                int Nmax, double *AE_out, int64_t *kmin_out, void *stream);
+
+/*
+ * gb_delta_loglike -- delta lnL of B proposals (Eq. 4, Eq. 5).
+ *   params_new   [B][8]; ADD: the proposed source; SWAP: the new source; REMOVE: ignored (may be NULL)
+ *   params_old   [B][8]; REMOVE / SWAP: the source currently in the model; ADD: ignored (may be NULL)
+ *   walker_index [B] int32 in [0, n_walkers)
+ *   move         [B] int8 GB_ADD / GB_REMOVE / GB_SWAP, or NULL to use move_all for every row
+ *   N, n_bins    as in gb_waveform (a SWAP row uses the same N for both sources)
+ *   dlnL_out     [B] f64:  ADD <r|a> - <a|a>/2;  REMOVE -<r|h> - <h|h>/2;
+ *                SWAP -( <a|a> + <o|o> - 2<a|o> - 2<r|a> + 2<r|o> ) / 2, <a|o> over the bins common to both windows
+ *   aux_out      optional [B][2] f64: (<h|h>, <r|h>) of the new source (ADD, SWAP) or of the removed one
+ */
+int gb_delta_loglike(gb_ctx *ctx, const gb_data *data, const double *params_new, const double *params_old,
+                     const int32_t *walker_index, const int8_t *move, int move_all, int N,
+                     const int32_t *n_bins, int64_t B, double *dlnL_out, double *aux_out, void *stream);
+
+/*
+ * gb_residual_update -- scatter accepted moves into data->resid in place (Alg. 1) with
+ * fp64 atomic adds: ADD r -= a; REMOVE r += h; SWAP r += o, r -= a.  accepted: [B] uint8 0/1, or NULL = all.
+ * Rows that overlap in frequency within one walker are summed in an unspecified order (results differ from
+ * a sequential sum by rounding only).
+ */
+int gb_residual_update(gb_ctx *ctx, const gb_data *data, const double *params_new, const double *params_old,
+                       const int32_t *walker_index, const int8_t *move, int move_all, const uint8_t *accepted,
+                       int N, const int32_t *n_bins, int64_t B, void *stream);
+
+/*
+ * Host-buffer forms (the end-to-end path): proposal arrays and outputs are HOST pointers (pinned memory
+ * gives the best copy rate); `data` still describes DEVICE-resident residuals and PSDs, which are the state
+ * that lives on the GPU across MCMC steps.  Each call copies its inputs to the device,
+ * runs the device form on `stream`, copies the result back and synchronises `stream`.
+ */
+int gb_waveform_host(gb_ctx *ctx, const double *params /*HOST*/, int64_t B, int N, const int32_t *n_bins /*HOST*/,
+                     int Nmax, double *AE_out /*HOST*/, int64_t *kmin_out /*HOST*/, void *stream);
+
+int gb_delta_loglike_host(gb_ctx *ctx, const gb_data *data, const double *params_new /*HOST*/,
+                          const double *params_old /*HOST*/, const int32_t *walker_index /*HOST*/,
+                          const int8_t *move /*HOST*/, int move_all, int N, const int32_t *n_bins /*HOST*/,
+                          int64_t B, double *dlnL_out /*HOST*/, double *aux_out /*HOST*/, void *stream);
+
+int gb_residual_update_host(gb_ctx *ctx, const gb_data *data, const double *params_new /*HOST*/,
+                            const double *params_old /*HOST*/, const int32_t *walker_index /*HOST*/,
+                            const int8_t *move /*HOST*/, int move_all, const uint8_t *accepted /*HOST*/,
+                            int N, const int32_t *n_bins /*HOST*/, int64_t B, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GBFIT_H */

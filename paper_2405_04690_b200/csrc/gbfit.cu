@@ -1,0 +1,859 @@
+// gbfit.cu -- kernels and C ABI of the GB waveform + delta-lnL hot path for sm_100a (B200).
+//
+// Launch structure of one call (all on the caller's stream, no host synchronisation):
+//   1. cudaMemsetAsync of the work counters
+//   2. gb_prep_kernel      one thread per proposal row: per-source constants (step O1) for the new and/or
+//                          old source, classification by (window length N, swap?) and warp-aggregated append
+//                          to that class's work list
+//   3. gb_main_kernel<N,SWAP>  one persistent launch per class that can occur: a group of G threads (one
+//                          CTA) takes a row from the class's list, evaluates the slow part at N time samples
+//                          (O2-O5), runs the length-N FFT of A and E in shared memory (O6), and finishes in
+//                          the same kernel with either the waveform store, the inner products + delta lnL
+//                          (O7, O8) or the atomic scatter into the residual (O9).  Waveforms never touch
+//                          global memory on the delta-lnL / update paths.
+#include <cuda_runtime.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "../../include/gbfit.h"
+#include "gb_fft.cuh"
+#include "gb_math.cuh"
+#include "gb_tables.hpp"
+
+using namespace gbk;
+
+namespace {
+
+enum Mode { MODE_WAVEFORM = 0, MODE_DLNL = 1, MODE_UPDATE = 2 };
+constexpr int kNumClasses = 8;   // class = 2 * log2(N / 128) + swap
+
+// ------------------------------------------------------------------------------------------------ args
+struct PrepArgs {
+    const double* params_new;
+    const double* params_old;
+    const int32_t* walker_index;
+    const int8_t* move;
+    const uint8_t* accepted;
+    const int32_t* n_bins;
+    int move_all, N, mode, n_walkers;
+    int64_t B;
+    double Tobs, tau;
+    int64_t kmax;            // largest valid global bin (Nyquist)
+    SrcConst* src_new;
+    SrcConst* src_old;
+    int32_t* lists;          // [kNumClasses][B]
+    int32_t* counts;         // [kNumClasses]
+    int32_t* errflag;
+    double* dlnL_out;
+};
+
+struct MainArgs {
+    const SrcConst* src_new;
+    const SrcConst* src_old;
+    const int32_t* lists;
+    const int32_t* counts;
+    int32_t* counters;       // [kNumClasses] next-item tickets
+    const double* orbit;     // [11][N] for this class's N
+    const cx* tw;            // [1024]
+    int64_t B;
+    int mode;
+    // data view
+    double* resid;
+    const double* psd;
+    const int32_t* walker_psd;
+    int64_t k_lo, n_f;
+    int32_t n_walkers, n_psd, psd_is_inverse;
+    // proposals
+    const int32_t* walker_index;
+    const int8_t* move;
+    int move_all;
+    // outputs
+    double* dlnL_out;
+    double* aux_out;
+    double* AE_out;
+    int64_t* kmin_out;
+    int Nmax;
+    double Tobs, tau;
+};
+
+// ------------------------------------------------------------------------------------------------ prep
+__device__ __forceinline__ int class_of_N(int N) {
+    return N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : N == 1024 ? 3 : -1;
+}
+
+__global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int cls = -1;
+    if (b < a.B) {
+        const int mv = a.mode == MODE_WAVEFORM ? GB_ADD : (a.move ? (int)a.move[b] : a.move_all);
+        const int N = a.n_bins ? a.n_bins[b] : a.N;
+        const int cN = class_of_N(N);
+        bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP;
+        if (a.mode != MODE_WAVEFORM) {
+            const int w = a.walker_index[b];
+            ok = ok && w >= 0 && w < a.n_walkers;
+        }
+        const bool active = a.accepted ? a.accepted[b] != 0 : true;
+        if (!ok) {
+            atomicOr(a.errflag, 1);
+            if (a.dlnL_out) a.dlnL_out[b] = __longlong_as_double(0x7ff8000000000000LL);
+        } else if (active) {
+            if (mv != GB_REMOVE) {
+                SrcConst s;
+                source_constants(a.params_new + 8 * b, a.Tobs, a.tau, N, s);
+                if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                a.src_new[b] = s;
+            }
+            if (mv != GB_ADD) {
+                SrcConst s;
+                source_constants(a.params_old + 8 * b, a.Tobs, a.tau, N, s);
+                if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                a.src_old[b] = s;
+            }
+            cls = 2 * cN + (mv == GB_SWAP ? 1 : 0);
+        }
+    }
+    // warp-aggregated append: one atomic per (warp, class)
+    const unsigned lane = threadIdx.x & 31;
+#pragma unroll
+    for (int c = 0; c < kNumClasses; c++) {
+        const unsigned m = __ballot_sync(0xffffffffu, cls == c);
+        if (m == 0) continue;
+        const int leader = __ffs(m) - 1;
+        int base = 0;
+        if ((int)lane == leader) base = atomicAdd(a.counts + c, __popc(m));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (cls == c) a.lists[(int64_t)c * a.B + base + __popc(m & ((1u << lane) - 1))] = (int32_t)b;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ main
+template <int N, int G>
+__device__ __forceinline__ void fft_all(cx* bA, cx* bE, const cx* tw, int tid);
+
+#define GB_STAGE(N_, G_, R_, Ns_)                                    \
+    {                                                                \
+        StageRegs<N_, G_, R_> rg;                                    \
+        fft_stage_read<N_, G_, R_>(bA, bE, tid, rg);                 \
+        __syncthreads();                                             \
+        fft_stage_write<N_, G_, R_, Ns_>(bA, bE, tw, tid, rg);       \
+        __syncthreads();                                             \
+    }
+
+template <>
+__device__ __forceinline__ void fft_all<128, 32>(cx* bA, cx* bE, const cx* tw, int tid) {
+    GB_STAGE(128, 32, 4, 1) GB_STAGE(128, 32, 4, 4) GB_STAGE(128, 32, 4, 16) GB_STAGE(128, 32, 2, 64)
+}
+template <>
+__device__ __forceinline__ void fft_all<256, 32>(cx* bA, cx* bE, const cx* tw, int tid) {
+    GB_STAGE(256, 32, 8, 1) GB_STAGE(256, 32, 8, 8) GB_STAGE(256, 32, 4, 64)
+}
+template <>
+__device__ __forceinline__ void fft_all<512, 64>(cx* bA, cx* bE, const cx* tw, int tid) {
+    GB_STAGE(512, 64, 8, 1) GB_STAGE(512, 64, 8, 8) GB_STAGE(512, 64, 8, 64)
+}
+template <>
+__device__ __forceinline__ void fft_all<1024, 128>(cx* bA, cx* bE, const cx* tw, int tid) {
+    GB_STAGE(1024, 128, 8, 1) GB_STAGE(1024, 128, 8, 8) GB_STAGE(1024, 128, 4, 64) GB_STAGE(1024, 128, 4, 256)
+}
+
+// slow part at this thread's samples n = tid + G j, then the FFT: bA, bE end up holding the window,
+// element j <-> global bin kmin + j.  s_src is the group's shared copy of the source constants.
+template <int N, int G>
+__device__ __forceinline__ void generate_waveform(const SrcConst* __restrict__ gsrc, SrcConst* s_src,
+                                                  const double* __restrict__ orbit, const cx* __restrict__ tw,
+                                                  cx* bA, cx* bE, double Tobs, double tau, int tid) {
+    constexpr int S = N / G;
+    // stage the 24 doubles of the source constants in shared memory (one broadcast read per use)
+    if (tid < 24) reinterpret_cast<double*>(s_src)[tid] = __ldg(reinterpret_cast<const double*>(gsrc) + tid);
+    __syncthreads();
+    const double dtN = Tobs / (double)N;
+    const double scale = (tid & 1) ? -Tobs / (2.0 * N) : Tobs / (2.0 * N);   // G is even: parity of n = parity of tid
+#pragma unroll 1
+    for (int j = 0; j < S; j++) {
+        const int n = tid + G * j;
+        OrbitSample o;
+        o.Rx = __ldg(orbit + 0 * N + n);
+        o.Ry = __ldg(orbit + 1 * N + n);
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            o.a[d] = __ldg(orbit + (2 + d) * N + n);
+            o.b[d] = __ldg(orbit + (5 + d) * N + n);
+            o.c[d] = __ldg(orbit + (8 + d) * N + n);
+        }
+        cd As, Es;
+        slow_sample(*s_src, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
+        bA[pad_idx(n)] = {As.re, As.im};
+        bE[pad_idx(n)] = {Es.re, Es.im};
+    }
+    __syncthreads();
+    fft_all<N, G>(bA, bE, tw, tid);
+}
+
+// sum NV per-thread values over the group; result valid in thread 0
+template <int G, int NV>
+__device__ __forceinline__ void group_reduce(double* v, double* s_red, int tid) {
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], off);
+    }
+    if (G > 32) {
+        const int warp = tid >> 5;
+        if ((tid & 31) == 0) {
+#pragma unroll
+            for (int i = 0; i < NV; i++) s_red[warp * NV + i] = v[i];
+        }
+        __syncthreads();
+        if (tid == 0) {
+#pragma unroll
+            for (int w = 1; w < G / 32; w++) {
+#pragma unroll
+                for (int i = 0; i < NV; i++) v[i] += s_red[w * NV + i];
+            }
+        }
+        __syncthreads();
+    }
+}
+
+__device__ __forceinline__ cx ld_cx(const double* p) {
+    const double2 v = *reinterpret_cast<const double2*>(p);
+    return {v.x, v.y};
+}
+
+template <int N, bool SWAP>
+__global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(MainArgs a) {
+    constexpr int G = Plan<N>::G;
+    constexpr int S = N / G;
+    constexpr int PN = padded_len(N);
+    constexpr int cls = 2 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (SWAP ? 1 : 0);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx* bufA0 = reinterpret_cast<cx*>(smem_raw);      // first (or only) waveform
+    cx* bufE0 = bufA0 + PN;
+    cx* bufA1 = bufE0 + PN;                           // SWAP: the new source; first = old
+    cx* bufE1 = bufA1 + PN;
+    __shared__ SrcConst s_src[SWAP ? 2 : 1];
+    __shared__ double s_red[(G / 32) * 5 + 1];
+    __shared__ int s_item;
+
+    const int tid = threadIdx.x;
+    const int count = a.counts[cls];
+    const int32_t* __restrict__ list = a.lists + (int64_t)cls * a.B;
+
+    for (;;) {
+        if (tid == 0) s_item = atomicAdd(a.counters + cls, 1);
+        __syncthreads();
+        const int item = s_item;
+        __syncthreads();
+        if (item >= count) break;
+        const int64_t b = list[item];
+        const int mv = a.mode == MODE_WAVEFORM ? GB_ADD : (a.move ? (int)a.move[b] : a.move_all);
+
+        // ---- waveform(s)
+        if (SWAP) {
+            generate_waveform<N, G>(a.src_old + b, &s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
+            generate_waveform<N, G>(a.src_new + b, &s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
+        } else {
+            generate_waveform<N, G>((mv == GB_REMOVE ? a.src_old : a.src_new) + b, &s_src[0], a.orbit, a.tw,
+                                    bufA0, bufE0, a.Tobs, a.tau, tid);
+        }
+        const int64_t kmin0 = s_src[0].kmin;
+
+        // ---- epilogue
+        if (a.mode == MODE_WAVEFORM) {
+            double2* outA = reinterpret_cast<double2*>(a.AE_out) + ((size_t)b * 2 + 0) * (size_t)a.Nmax;
+            double2* outE = reinterpret_cast<double2*>(a.AE_out) + ((size_t)b * 2 + 1) * (size_t)a.Nmax;
+#pragma unroll
+            for (int m = 0; m < S; m++) {
+                const int j = tid + G * m;
+                const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
+                outA[j] = make_double2(ha.re, ha.im);
+                outE[j] = make_double2(he.re, he.im);
+            }
+            if (tid == 0 && a.kmin_out) a.kmin_out[b] = kmin0;
+        } else {
+            const int w = a.walker_index[b];
+            const size_t nf = (size_t)a.n_f;
+            double* rA = a.resid + ((size_t)w * 2 + 0) * nf * 2;
+            double* rE = a.resid + ((size_t)w * 2 + 1) * nf * 2;
+            if (a.mode == MODE_DLNL) {
+                const int prow = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
+                const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
+                const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
+                const bool inv = a.psd_is_inverse != 0;
+                const double norm = 4.0 / a.Tobs;
+                if (!SWAP) {
+                    double v[2] = {0.0, 0.0};   // <h|h>, <r|h>
+#pragma unroll
+                    for (int m = 0; m < S; m++) {
+                        const int j = tid + G * m;
+                        const int64_t i = kmin0 + j - a.k_lo;
+                        if (i >= 0 && i < a.n_f) {
+                            const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
+                            const cx ra = ld_cx(rA + 2 * i), re = ld_cx(rE + 2 * i);
+                            const double wa = inv ? SA[i] : 1.0 / SA[i];
+                            const double we = inv ? SE[i] : 1.0 / SE[i];
+                            v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
+                            v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
+                        }
+                    }
+                    group_reduce<G, 2>(v, s_red, tid);
+                    if (tid == 0) {
+                        const double hh = norm * v[0], rh = norm * v[1];
+                        a.dlnL_out[b] = (mv == GB_REMOVE ? -rh : rh) - 0.5 * hh;
+                        if (a.aux_out) {
+                            a.aux_out[2 * b] = hh;
+                            a.aux_out[2 * b + 1] = rh;
+                        }
+                    }
+                } else {
+                    // buffers: 0 = old (o), 1 = new (a)
+                    const int64_t kmin1 = s_src[1].kmin;
+                    const int64_t shift = kmin1 - kmin0;   // o index of a's bin j is j + shift
+                    double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // aa, ra, ao, oo, ro
+#pragma unroll
+                    for (int m = 0; m < S; m++) {
+                        const int j = tid + G * m;
+                        int64_t i = kmin1 + j - a.k_lo;
+                        if (i >= 0 && i < a.n_f) {
+                            const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
+                            const cx ra = ld_cx(rA + 2 * i), re = ld_cx(rE + 2 * i);
+                            const double wa = inv ? SA[i] : 1.0 / SA[i];
+                            const double we = inv ? SE[i] : 1.0 / SE[i];
+                            v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
+                            v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
+                            const int64_t jo = j + shift;
+                            if (jo >= 0 && jo < N) {
+                                const cx oa = bufA0[pad_idx((int)jo)], oe = bufE0[pad_idx((int)jo)];
+                                v[2] += wa * (ha.re * oa.re + ha.im * oa.im) + we * (he.re * oe.re + he.im * oe.im);
+                            }
+                        }
+                        i = kmin0 + j - a.k_lo;
+                        if (i >= 0 && i < a.n_f) {
+                            const cx oa = bufA0[pad_idx(j)], oe = bufE0[pad_idx(j)];
+                            const cx ra = ld_cx(rA + 2 * i), re = ld_cx(rE + 2 * i);
+                            const double wa = inv ? SA[i] : 1.0 / SA[i];
+                            const double we = inv ? SE[i] : 1.0 / SE[i];
+                            v[3] += wa * (oa.re * oa.re + oa.im * oa.im) + we * (oe.re * oe.re + oe.im * oe.im);
+                            v[4] += wa * (ra.re * oa.re + ra.im * oa.im) + we * (re.re * oe.re + re.im * oe.im);
+                        }
+                    }
+                    group_reduce<G, 5>(v, s_red, tid);
+                    if (tid == 0) {
+                        const double aa = norm * v[0], ra = norm * v[1], ao = norm * v[2], oo = norm * v[3],
+                                     ro = norm * v[4];
+                        a.dlnL_out[b] = -0.5 * (aa + oo - 2.0 * ao - 2.0 * ra + 2.0 * ro);
+                        if (a.aux_out) {
+                            a.aux_out[2 * b] = aa;
+                            a.aux_out[2 * b + 1] = ra;
+                        }
+                    }
+                }
+            } else {   // MODE_UPDATE: r -= a (ADD), r += h (REMOVE), r += o - a (SWAP)
+                const double sgn0 = SWAP ? 1.0 : (mv == GB_REMOVE ? 1.0 : -1.0);
+#pragma unroll
+                for (int m = 0; m < S; m++) {
+                    const int j = tid + G * m;
+                    int64_t i = kmin0 + j - a.k_lo;
+                    if (i >= 0 && i < a.n_f) {
+                        const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
+                        atomicAdd(rA + 2 * i, sgn0 * ha.re);
+                        atomicAdd(rA + 2 * i + 1, sgn0 * ha.im);
+                        atomicAdd(rE + 2 * i, sgn0 * he.re);
+                        atomicAdd(rE + 2 * i + 1, sgn0 * he.im);
+                    }
+                    if (SWAP) {
+                        i = s_src[1].kmin + j - a.k_lo;
+                        if (i >= 0 && i < a.n_f) {
+                            const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
+                            atomicAdd(rA + 2 * i, -ha.re);
+                            atomicAdd(rA + 2 * i + 1, -ha.im);
+                            atomicAdd(rE + 2 * i, -he.re);
+                            atomicAdd(rE + 2 * i + 1, -he.im);
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();   // buffers and s_src are reused by the next item
+    }
+}
+
+template <int N, bool SWAP>
+constexpr size_t main_smem_bytes() {
+    return (size_t)padded_len(N) * sizeof(cx) * 2 * (SWAP ? 2 : 1);
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ context
+struct gb_ctx {
+    gb_config cfg;
+    int num_sms;
+    double* d_orbit[4];
+    cx* d_tw;
+    int32_t* d_counts;      // [kNumClasses] counts, [kNumClasses] counters, [1] errflag
+    SrcConst* d_src_new;
+    SrcConst* d_src_old;
+    int32_t* d_lists;
+    int64_t cap_new, cap_old, cap_lists;
+    int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
+    // staging for the *_host entry points
+    void* d_stage;
+    size_t cap_stage;
+    int64_t launches;
+    char err[512];
+};
+
+namespace {
+
+int set_err(gb_ctx* ctx, int code, const char* fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define GB_CUDA(ctx, call)                                                                              \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess)                                                                          \
+            return set_err(ctx, GB_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),    \
+                           __FILE__, __LINE__);                                                         \
+    } while (0)
+
+template <typename T>
+int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
+    if (need <= *cap) return GB_OK;
+    if (*ptr) {
+        GB_CUDA(ctx, cudaDeviceSynchronize());
+        GB_CUDA(ctx, cudaFree(*ptr));
+        *ptr = nullptr;
+        *cap = 0;
+    }
+    const int64_t want = need + need / 8;
+    if (cudaMalloc(reinterpret_cast<void**>(ptr), (size_t)want * sizeof(T)) != cudaSuccess) {
+        cudaGetLastError();
+        return set_err(ctx, GB_ERR_NOMEM, "scratch allocation of %lld bytes failed", (long long)(want * sizeof(T)));
+    }
+    *cap = want;
+    return GB_OK;
+}
+
+template <int N, bool SWAP>
+int setup_kernel(gb_ctx* ctx, int cls) {
+    const size_t smem = main_smem_bytes<N, SWAP>();
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int nb = 0;
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP>, Plan<N>::G, smem));
+    if (nb < 1) return set_err(ctx, GB_ERR_CUDA, "kernel class %d does not fit on an SM", cls);
+    ctx->grid_blocks[cls] = nb * ctx->num_sms;
+    return GB_OK;
+}
+
+template <int N, bool SWAP>
+int launch_main(gb_ctx* ctx, MainArgs& a, int cls, int64_t B, cudaStream_t st) {
+    a.orbit = ctx->d_orbit[cls >> 1];
+    int64_t grid = ctx->grid_blocks[cls];
+    if (grid > B) grid = B;
+    gb_main_kernel<N, SWAP><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP>(), st>>>(a);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+    return GB_OK;
+}
+
+struct Call {
+    int mode;
+    const gb_data* data;
+    const double* params_new;
+    const double* params_old;
+    const int32_t* walker_index;
+    const int8_t* move;
+    int move_all;
+    const uint8_t* accepted;
+    int N;
+    const int32_t* n_bins;
+    int64_t B;
+    double* dlnL_out;
+    double* aux_out;
+    double* AE_out;
+    int64_t* kmin_out;
+    int Nmax;
+};
+
+int run_call(gb_ctx* ctx, const Call& c, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (c.B < 0 || c.B > 0x7fffffff) return set_err(ctx, GB_ERR_INVALID, "B out of range");
+    if (c.B == 0) return GB_OK;
+    const bool need_new = c.mode == MODE_WAVEFORM || c.move != nullptr || c.move_all != GB_REMOVE;
+    const bool need_old = c.mode != MODE_WAVEFORM && (c.move != nullptr || c.move_all != GB_ADD);
+    if (c.mode != MODE_WAVEFORM) {
+        if (!c.data || !c.data->resid || !c.walker_index) return set_err(ctx, GB_ERR_INVALID, "NULL data / walker_index");
+        if (c.mode == MODE_DLNL && (!c.data->psd || !c.dlnL_out)) return set_err(ctx, GB_ERR_INVALID, "NULL psd / dlnL_out");
+        if (c.data->n_f <= 0 || c.data->n_walkers <= 0) return set_err(ctx, GB_ERR_INVALID, "empty data view");
+        if (!c.move && (c.move_all < GB_ADD || c.move_all > GB_SWAP)) return set_err(ctx, GB_ERR_INVALID, "bad move_all");
+        if (c.move == nullptr) {
+            if (need_new && !c.params_new) return set_err(ctx, GB_ERR_INVALID, "params_new is NULL");
+            if (need_old && !c.params_old) return set_err(ctx, GB_ERR_INVALID, "params_old is NULL");
+        } else if (!c.params_new && !c.params_old) {
+            return set_err(ctx, GB_ERR_INVALID, "params_new and params_old are NULL");
+        }
+    } else {
+        if (!c.params_new || !c.AE_out) return set_err(ctx, GB_ERR_INVALID, "NULL params / AE_out");
+    }
+    if (!c.n_bins && !(c.N == 128 || c.N == 256 || c.N == 512 || c.N == 1024))
+        return set_err(ctx, GB_ERR_INVALID, "N must be 128, 256, 512 or 1024");
+    if (c.mode == MODE_WAVEFORM && c.Nmax < (c.n_bins ? 128 : c.N)) return set_err(ctx, GB_ERR_INVALID, "Nmax too small");
+
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    int rc;
+    if (need_new && (rc = ensure_cap(ctx, &ctx->d_src_new, &ctx->cap_new, c.B))) return rc;
+    if (need_old && (rc = ensure_cap(ctx, &ctx->d_src_old, &ctx->cap_old, c.B))) return rc;
+    if ((rc = ensure_cap(ctx, &ctx->d_lists, &ctx->cap_lists, c.B * kNumClasses))) return rc;
+
+    GB_CUDA(ctx, cudaMemsetAsync(ctx->d_counts, 0, sizeof(int32_t) * 2 * kNumClasses, st));
+
+    PrepArgs p{};
+    p.params_new = c.params_new;
+    p.params_old = c.params_old;
+    p.walker_index = c.walker_index;
+    p.move = c.mode == MODE_WAVEFORM ? nullptr : c.move;
+    p.accepted = c.accepted;
+    p.n_bins = c.n_bins;
+    p.move_all = c.mode == MODE_WAVEFORM ? GB_ADD : c.move_all;
+    p.N = c.N;
+    p.mode = c.mode;
+    p.n_walkers = c.data ? c.data->n_walkers : 0;
+    p.B = c.B;
+    p.Tobs = ctx->cfg.Tobs;
+    p.tau = ctx->cfg.armlength / kCLight;
+    p.kmax = (int64_t)floor(ctx->cfg.Tobs / (2.0 * ctx->cfg.dt));
+    p.src_new = ctx->d_src_new;
+    p.src_old = ctx->d_src_old;
+    p.lists = ctx->d_lists;
+    p.counts = ctx->d_counts;
+    p.errflag = ctx->d_counts + 2 * kNumClasses;
+    p.dlnL_out = c.mode == MODE_DLNL ? c.dlnL_out : nullptr;
+    const unsigned pgrid = (unsigned)((c.B + 255) / 256);
+    gb_prep_kernel<<<pgrid, 256, 0, st>>>(p);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+
+    MainArgs a{};
+    a.src_new = ctx->d_src_new;
+    a.src_old = ctx->d_src_old;
+    a.lists = ctx->d_lists;
+    a.counts = ctx->d_counts;
+    a.counters = ctx->d_counts + kNumClasses;
+    a.tw = ctx->d_tw;
+    a.B = c.B;
+    a.mode = c.mode;
+    if (c.data) {
+        a.resid = c.data->resid;
+        a.psd = c.data->psd;
+        a.walker_psd = c.data->walker_psd;
+        a.k_lo = c.data->k_lo;
+        a.n_f = c.data->n_f;
+        a.n_walkers = c.data->n_walkers;
+        a.n_psd = c.data->n_psd;
+        a.psd_is_inverse = c.data->psd_is_inverse;
+    }
+    a.walker_index = c.walker_index;
+    a.move = p.move;
+    a.move_all = p.move_all;
+    a.dlnL_out = c.dlnL_out;
+    a.aux_out = c.aux_out;
+    a.AE_out = c.AE_out;
+    a.kmin_out = c.kmin_out;
+    a.Nmax = c.Nmax;
+    a.Tobs = ctx->cfg.Tobs;
+    a.tau = p.tau;
+
+    // launch only the classes that can occur; largest windows first
+    const bool may_swap = c.mode != MODE_WAVEFORM && (c.move ? true : c.move_all == GB_SWAP);
+    const bool may_single = c.mode == MODE_WAVEFORM || (c.move ? true : c.move_all != GB_SWAP);
+    for (int cN = 3; cN >= 0; cN--) {
+        const int Nc = 128 << cN;
+        if (!c.n_bins && Nc != c.N) continue;
+        if (may_swap) {
+            switch (Nc) {
+                case 128: rc = launch_main<128, true>(ctx, a, 2 * cN + 1, c.B, st); break;
+                case 256: rc = launch_main<256, true>(ctx, a, 2 * cN + 1, c.B, st); break;
+                case 512: rc = launch_main<512, true>(ctx, a, 2 * cN + 1, c.B, st); break;
+                default: rc = launch_main<1024, true>(ctx, a, 2 * cN + 1, c.B, st); break;
+            }
+            if (rc) return rc;
+        }
+        if (may_single) {
+            switch (Nc) {
+                case 128: rc = launch_main<128, false>(ctx, a, 2 * cN, c.B, st); break;
+                case 256: rc = launch_main<256, false>(ctx, a, 2 * cN, c.B, st); break;
+                case 512: rc = launch_main<512, false>(ctx, a, 2 * cN, c.B, st); break;
+                default: rc = launch_main<1024, false>(ctx, a, 2 * cN, c.B, st); break;
+            }
+            if (rc) return rc;
+        }
+    }
+    return GB_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ C ABI
+extern "C" {
+
+void gb_default_config(gb_config* cfg) {
+    if (!cfg) return;
+    cfg->Tobs = 31457280.0;
+    cfg->dt = 5.0;
+    cfg->armlength = 2.5e9;
+    cfg->au = 1.495978707e11;
+    cfg->year = 31558149.763545603;
+    cfg->kappa = 0.0;
+    cfg->lambda0 = 0.0;
+    cfg->device = 0;
+    cfg->reserved = 0;
+}
+
+const char* gb_version(void) { return "gbfit-b200 0.1"; }
+
+int gb_create(const gb_config* cfg, gb_ctx** out) {
+    if (!cfg || !out) return GB_ERR_INVALID;
+    *out = nullptr;
+    if (!(cfg->Tobs > 0) || !(cfg->dt > 0) || !(cfg->armlength > 0) || !(cfg->au > 0) || !(cfg->year > 0))
+        return GB_ERR_INVALID;
+    gb_ctx* ctx = new gb_ctx();
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->cfg = *cfg;
+    *out = ctx;   // returned even on failure so that gb_last_error can be read; caller destroys it
+    GB_CUDA(ctx, cudaSetDevice(cfg->device));
+    cudaDeviceProp prop;
+    GB_CUDA(ctx, cudaGetDeviceProperties(&prop, cfg->device));
+    if (prop.major < 10)
+        return set_err(ctx, GB_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", cfg->device,
+                       prop.major, prop.minor);
+    ctx->num_sms = prop.multiProcessorCount;
+    OrbitParams op{cfg->Tobs, cfg->armlength, cfg->au, cfg->year, cfg->kappa, cfg->lambda0};
+    for (int i = 0; i < 4; i++) {
+        const int N = 128 << i;
+        std::vector<double> tab((size_t)kOrbitRows * N);
+        build_orbit_table(op, N, tab.data());
+        GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->d_orbit[i]), tab.size() * sizeof(double)));
+        GB_CUDA(ctx, cudaMemcpy(ctx->d_orbit[i], tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    }
+    std::vector<double> tw(2 * kTwiddleN);
+    build_twiddles(tw.data());
+    GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->d_tw), tw.size() * sizeof(double)));
+    GB_CUDA(ctx, cudaMemcpy(ctx->d_tw, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice));
+    GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->d_counts), sizeof(int32_t) * (2 * kNumClasses + 1)));
+    GB_CUDA(ctx, cudaMemset(ctx->d_counts, 0, sizeof(int32_t) * (2 * kNumClasses + 1)));
+    int rc;
+    if ((rc = setup_kernel<128, false>(ctx, 0))) return rc;
+    if ((rc = setup_kernel<128, true>(ctx, 1))) return rc;
+    if ((rc = setup_kernel<256, false>(ctx, 2))) return rc;
+    if ((rc = setup_kernel<256, true>(ctx, 3))) return rc;
+    if ((rc = setup_kernel<512, false>(ctx, 4))) return rc;
+    if ((rc = setup_kernel<512, true>(ctx, 5))) return rc;
+    if ((rc = setup_kernel<1024, false>(ctx, 6))) return rc;
+    if ((rc = setup_kernel<1024, true>(ctx, 7))) return rc;
+    return GB_OK;
+}
+
+void gb_destroy(gb_ctx* ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->cfg.device);
+    cudaDeviceSynchronize();
+    for (int i = 0; i < 4; i++) cudaFree(ctx->d_orbit[i]);
+    cudaFree(ctx->d_tw);
+    cudaFree(ctx->d_counts);
+    cudaFree(ctx->d_src_new);
+    cudaFree(ctx->d_src_old);
+    cudaFree(ctx->d_lists);
+    cudaFree(ctx->d_stage);
+    delete ctx;
+}
+
+const char* gb_last_error(const gb_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
+
+int64_t gb_launch_count(const gb_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int gb_check(gb_ctx* ctx, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    int32_t flag = 0;
+    GB_CUDA(ctx, cudaMemcpyAsync(&flag, ctx->d_counts + 2 * kNumClasses, sizeof(flag), cudaMemcpyDeviceToHost, st));
+    GB_CUDA(ctx, cudaStreamSynchronize(st));
+    if (flag) {
+        GB_CUDA(ctx, cudaMemsetAsync(ctx->d_counts + 2 * kNumClasses, 0, sizeof(int32_t), st));
+        return set_err(ctx, GB_ERR_ROW, "row error flags 0x%x (1: bad N / move / walker index, 2: window beyond Nyquist)", flag);
+    }
+    return GB_OK;
+}
+
+int gb_waveform(gb_ctx* ctx, const double* params, int64_t B, int N, const int32_t* n_bins, int Nmax, double* AE_out,
+                int64_t* kmin_out, void* stream) {
+    Call c{};
+    c.mode = MODE_WAVEFORM;
+    c.params_new = params;
+    c.N = N;
+    c.n_bins = n_bins;
+    c.B = B;
+    c.AE_out = AE_out;
+    c.kmin_out = kmin_out;
+    c.Nmax = Nmax;
+    return run_call(ctx, c, stream);
+}
+
+int gb_delta_loglike(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                     const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                     int64_t B, double* dlnL_out, double* aux_out, void* stream) {
+    Call c{};
+    c.mode = MODE_DLNL;
+    c.data = data;
+    c.params_new = params_new;
+    c.params_old = params_old;
+    c.walker_index = walker_index;
+    c.move = move;
+    c.move_all = move_all;
+    c.N = N;
+    c.n_bins = n_bins;
+    c.B = B;
+    c.dlnL_out = dlnL_out;
+    c.aux_out = aux_out;
+    return run_call(ctx, c, stream);
+}
+
+int gb_residual_update(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                       const int32_t* walker_index, const int8_t* move, int move_all, const uint8_t* accepted, int N,
+                       const int32_t* n_bins, int64_t B, void* stream) {
+    Call c{};
+    c.mode = MODE_UPDATE;
+    c.data = data;
+    c.params_new = params_new;
+    c.params_old = params_old;
+    c.walker_index = walker_index;
+    c.move = move;
+    c.move_all = move_all;
+    c.accepted = accepted;
+    c.N = N;
+    c.n_bins = n_bins;
+    c.B = B;
+    return run_call(ctx, c, stream);
+}
+
+}  // extern "C"
+
+// ---- host-buffer forms: one staging buffer, carved per call ----------------------------------------
+namespace {
+struct Stager {
+    gb_ctx* ctx;
+    cudaStream_t st;
+    char* base;
+    size_t off;
+    template <typename T>
+    T* put(const T* host, size_t count) {   // reserve (and copy in if host != NULL)
+        off = (off + 255) & ~(size_t)255;
+        T* d = reinterpret_cast<T*>(base + off);
+        off += count * sizeof(T);
+        if (host) cudaMemcpyAsync(d, host, count * sizeof(T), cudaMemcpyHostToDevice, st);
+        return d;
+    }
+};
+int stage_reserve(gb_ctx* ctx, size_t bytes) {
+    if (bytes <= ctx->cap_stage) return GB_OK;
+    if (ctx->d_stage) {
+        GB_CUDA(ctx, cudaDeviceSynchronize());
+        GB_CUDA(ctx, cudaFree(ctx->d_stage));
+        ctx->d_stage = nullptr;
+        ctx->cap_stage = 0;
+    }
+    if (cudaMalloc(&ctx->d_stage, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return set_err(ctx, GB_ERR_NOMEM, "staging allocation of %zu bytes failed", bytes);
+    }
+    ctx->cap_stage = bytes;
+    return GB_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gb_waveform_host(gb_ctx* ctx, const double* params, int64_t B, int N, const int32_t* n_bins, int Nmax,
+                     double* AE_out, int64_t* kmin_out, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (B < 0 || !params || !AE_out || Nmax <= 0) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
+    if (B == 0) return GB_OK;
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    const size_t nAE = (size_t)B * 2 * (size_t)Nmax * 2;
+    int rc = stage_reserve(ctx, (size_t)B * (64 + 4 + 8) + nAE * 8 + 4096);
+    if (rc) return rc;
+    Stager s{ctx, reinterpret_cast<cudaStream_t>(stream), static_cast<char*>(ctx->d_stage), 0};
+    double* d_p = s.put(params, (size_t)B * 8);
+    int32_t* d_nb = n_bins ? s.put(n_bins, (size_t)B) : nullptr;
+    int64_t* d_k = s.put<int64_t>(nullptr, (size_t)B);
+    double* d_AE = s.put<double>(nullptr, nAE);
+    GB_CUDA(ctx, cudaMemsetAsync(d_AE, 0, nAE * 8, s.st));
+    rc = gb_waveform(ctx, d_p, B, N, d_nb, Nmax, d_AE, d_k, stream);
+    if (rc) return rc;
+    GB_CUDA(ctx, cudaMemcpyAsync(AE_out, d_AE, nAE * 8, cudaMemcpyDeviceToHost, s.st));
+    if (kmin_out) GB_CUDA(ctx, cudaMemcpyAsync(kmin_out, d_k, (size_t)B * 8, cudaMemcpyDeviceToHost, s.st));
+    GB_CUDA(ctx, cudaStreamSynchronize(s.st));
+    return GB_OK;
+}
+
+int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                          const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                          int64_t B, double* dlnL_out, double* aux_out, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (B < 0 || !walker_index || !dlnL_out) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
+    if (B == 0) return GB_OK;
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc = stage_reserve(ctx, (size_t)B * (64 + 64 + 4 + 1 + 4 + 8 + 16) + 8192);
+    if (rc) return rc;
+    Stager s{ctx, reinterpret_cast<cudaStream_t>(stream), static_cast<char*>(ctx->d_stage), 0};
+    double* d_pn = params_new ? s.put(params_new, (size_t)B * 8) : nullptr;
+    double* d_po = params_old ? s.put(params_old, (size_t)B * 8) : nullptr;
+    int32_t* d_w = s.put(walker_index, (size_t)B);
+    int8_t* d_mv = move ? s.put(move, (size_t)B) : nullptr;
+    int32_t* d_nb = n_bins ? s.put(n_bins, (size_t)B) : nullptr;
+    double* d_out = s.put<double>(nullptr, (size_t)B);
+    double* d_aux = aux_out ? s.put<double>(nullptr, (size_t)B * 2) : nullptr;
+    rc = gb_delta_loglike(ctx, data, d_pn, d_po, d_w, d_mv, move_all, N, d_nb, B, d_out, d_aux, stream);
+    if (rc) return rc;
+    GB_CUDA(ctx, cudaMemcpyAsync(dlnL_out, d_out, (size_t)B * 8, cudaMemcpyDeviceToHost, s.st));
+    if (aux_out) GB_CUDA(ctx, cudaMemcpyAsync(aux_out, d_aux, (size_t)B * 16, cudaMemcpyDeviceToHost, s.st));
+    GB_CUDA(ctx, cudaStreamSynchronize(s.st));
+    return GB_OK;
+}
+
+int gb_residual_update_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                            const int32_t* walker_index, const int8_t* move, int move_all, const uint8_t* accepted,
+                            int N, const int32_t* n_bins, int64_t B, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (B < 0 || !walker_index) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
+    if (B == 0) return GB_OK;
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc = stage_reserve(ctx, (size_t)B * (64 + 64 + 4 + 1 + 1 + 4) + 8192);
+    if (rc) return rc;
+    Stager s{ctx, reinterpret_cast<cudaStream_t>(stream), static_cast<char*>(ctx->d_stage), 0};
+    double* d_pn = params_new ? s.put(params_new, (size_t)B * 8) : nullptr;
+    double* d_po = params_old ? s.put(params_old, (size_t)B * 8) : nullptr;
+    int32_t* d_w = s.put(walker_index, (size_t)B);
+    int8_t* d_mv = move ? s.put(move, (size_t)B) : nullptr;
+    uint8_t* d_acc = accepted ? s.put(accepted, (size_t)B) : nullptr;
+    int32_t* d_nb = n_bins ? s.put(n_bins, (size_t)B) : nullptr;
+    rc = gb_residual_update(ctx, data, d_pn, d_po, d_w, d_mv, move_all, d_acc, N, d_nb, B, stream);
+    if (rc) return rc;
+    GB_CUDA(ctx, cudaStreamSynchronize(s.st));
+    return GB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,326 @@
+"""Thin Python binding of the C ABI in include/gbfit.h (argument marshalling only).
+
+Every step of the path (per-source constants, slow part, FFT, window gather, inner products, delta lnL,
+scatter-add) runs inside libgbfit.so's CUDA kernels.  torch is used for device memory and streams only;
+there is no CPU fallback: if libgbfit.so is missing or does not load, importing this module's `lib()`
+raises.  Function names and argument order follow include/gbfit.h (PAPER.md citations are there).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+ADD, REMOVE, SWAP = 0, 1, 2
+GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
+
+EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
+           "gb_launch_count", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
+           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host")
+
+
+class GbConfig(C.Structure):
+    _fields_ = [("Tobs", C.c_double), ("dt", C.c_double), ("armlength", C.c_double), ("au", C.c_double),
+                ("year", C.c_double), ("kappa", C.c_double), ("lambda0", C.c_double),
+                ("device", C.c_int32), ("reserved", C.c_int32)]
+
+
+class GbData(C.Structure):
+    _fields_ = [("resid", C.c_void_p), ("psd", C.c_void_p), ("walker_psd", C.c_void_p),
+                ("k_lo", C.c_int64), ("n_f", C.c_int64),
+                ("n_walkers", C.c_int32), ("n_psd", C.c_int32), ("psd_is_inverse", C.c_int32),
+                ("reserved", C.c_int32)]
+
+
+class GbError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"gbfit error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib() -> C.CDLL:
+    """Load libgbfit.so (built in-tree by paper_2405_04690_b200.build).  Fails loudly when absent."""
+    global _lib
+    if _lib is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise ImportError(f"{path} is missing: run `python -m paper_2405_04690_b200.build` "
+                              "(the GB hot path has no CPU or PyTorch fallback)")
+        L = C.CDLL(path)
+        vp, i64, i32, ci = C.c_void_p, C.c_int64, C.c_int32, C.c_int
+        L.gb_default_config.argtypes = [C.POINTER(GbConfig)]
+        L.gb_default_config.restype = None
+        L.gb_create.argtypes = [C.POINTER(GbConfig), C.POINTER(vp)]
+        L.gb_create.restype = ci
+        L.gb_destroy.argtypes = [vp]
+        L.gb_destroy.restype = None
+        L.gb_last_error.argtypes = [vp]
+        L.gb_last_error.restype = C.c_char_p
+        L.gb_check.argtypes = [vp, vp]
+        L.gb_check.restype = ci
+        L.gb_version.argtypes = []
+        L.gb_version.restype = C.c_char_p
+        L.gb_launch_count.argtypes = [vp]
+        L.gb_launch_count.restype = i64
+        wf = [vp, vp, i64, ci, vp, ci, vp, vp, vp]
+        dl = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, vp, vp, vp]
+        ru = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, vp, ci, vp, i64, vp]
+        for name, sig in (("gb_waveform", wf), ("gb_waveform_host", wf), ("gb_delta_loglike", dl),
+                          ("gb_delta_loglike_host", dl), ("gb_residual_update", ru),
+                          ("gb_residual_update_host", ru)):
+            fn = getattr(L, name)
+            fn.argtypes = sig
+            fn.restype = ci
+        _lib = L
+    return _lib
+
+
+def version() -> str:
+    return lib().gb_version().decode()
+
+
+# ----------------------------------------------------------------------------------------- marshalling
+def _dev_ptr(t: Optional[torch.Tensor], dtype, device, name: str):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.device != device:
+        raise ValueError(f"{name} is on {t.device}, context is on {device}")
+    dts = dtype if isinstance(dtype, tuple) else (dtype,)
+    if t.dtype not in dts:
+        raise TypeError(f"{name} must have dtype {dts}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_ptr(a, dtype, name: str):
+    """numpy array or CPU torch tensor (pinned or not) -> (void*, keepalive)."""
+    if a is None:
+        return None, None
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda:
+            raise TypeError(f"{name} must be a HOST buffer")
+        if not a.is_contiguous():
+            raise ValueError(f"{name} must be contiguous")
+        want = {np.float64: torch.float64, np.int32: torch.int32, np.int8: torch.int8, np.uint8: torch.uint8,
+                np.int64: torch.int64, np.complex128: torch.complex128}[dtype]
+        if a.dtype != want:
+            raise TypeError(f"{name} must have dtype {want}, got {a.dtype}")
+        return C.c_void_p(a.data_ptr()), a
+    arr = np.ascontiguousarray(a, dtype=dtype)
+    return C.c_void_p(arr.ctypes.data), arr
+
+
+def _stream_ptr(stream, device):
+    if stream is None:
+        stream = torch.cuda.current_stream(device)
+    if isinstance(stream, torch.cuda.Stream):
+        return C.c_void_p(stream.cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+class Data:
+    """Device-resident residuals and PSDs of the walkers (gb_data of include/gbfit.h).
+
+    resid: CUDA complex128 [n_walkers, 2, n_f] (or float64 [n_walkers, 2, n_f, 2]); modified in place by
+    residual_update.  psd: CUDA float64 [n_psd, 2, n_f].  walker_psd: CUDA int32 [n_walkers] or None.
+    """
+
+    def __init__(self, resid: torch.Tensor, psd: torch.Tensor, k_lo: int,
+                 walker_psd: Optional[torch.Tensor] = None, psd_is_inverse: bool = False):
+        if resid.dtype == torch.complex128:
+            if resid.dim() != 3 or resid.shape[1] != 2:
+                raise ValueError("resid must be [n_walkers, 2, n_f] complex128")
+        elif resid.dtype == torch.float64:
+            if resid.dim() != 4 or resid.shape[1] != 2 or resid.shape[3] != 2:
+                raise ValueError("resid must be [n_walkers, 2, n_f, 2] float64")
+        else:
+            raise TypeError("resid must be complex128 or float64")
+        if psd.dim() != 3 or psd.shape[1] != 2 or psd.shape[2] != resid.shape[2]:
+            raise ValueError("psd must be [n_psd, 2, n_f] float64")
+        dev = resid.device
+        self.resid, self.psd, self.walker_psd = resid, psd, walker_psd
+        self.k_lo, self.n_f = int(k_lo), int(resid.shape[2])
+        self.n_walkers, self.n_psd = int(resid.shape[0]), int(psd.shape[0])
+        if walker_psd is None and self.n_psd not in (1, self.n_walkers):
+            raise ValueError("walker_psd is required when n_psd is neither 1 nor n_walkers")
+        self.psd_is_inverse = bool(psd_is_inverse)
+        self.device = dev
+        self._c = GbData(_dev_ptr(resid, (torch.complex128, torch.float64), dev, "resid"),
+                         _dev_ptr(psd, torch.float64, dev, "psd"),
+                         _dev_ptr(walker_psd, torch.int32, dev, "walker_psd"),
+                         self.k_lo, self.n_f, self.n_walkers, self.n_psd, int(self.psd_is_inverse), 0)
+
+    def c(self):
+        return C.byref(self._c)
+
+
+class Context:
+    """gb_ctx: orbit tables, twiddles and scratch on one device."""
+
+    def __init__(self, device: int = 0, **cfg):
+        L = lib()
+        c = GbConfig()
+        L.gb_default_config(C.byref(c))
+        for k, v in cfg.items():
+            if not hasattr(c, k) or k in ("device", "reserved"):
+                raise TypeError(f"unknown gb_config field {k}")
+            setattr(c, k, float(v))
+        c.device = int(device)
+        self.config = c
+        self.device = torch.device("cuda", int(device))
+        self._h = C.c_void_p()
+        rc = L.gb_create(C.byref(c), C.byref(self._h))
+        if rc != GB_OK:
+            msg = L.gb_last_error(self._h).decode() if self._h else "gb_create failed"
+            if self._h:
+                L.gb_destroy(self._h)
+                self._h = C.c_void_p()
+            raise GbError(rc, msg)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().gb_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _ok(self, rc: int):
+        if rc != GB_OK:
+            raise GbError(rc, lib().gb_last_error(self._h).decode())
+
+    def last_error(self) -> str:
+        return lib().gb_last_error(self._h).decode()
+
+    def launch_count(self) -> int:
+        return int(lib().gb_launch_count(self._h))
+
+    def check(self, stream=None):
+        """Synchronise the stream and raise if any row of an earlier call was invalid."""
+        self._ok(lib().gb_check(self._h, _stream_ptr(stream, self.device)))
+
+    # ------------------------------------------------------------------------------- device forms
+    def waveform(self, params: torch.Tensor, N: int = 0, n_bins: Optional[torch.Tensor] = None,
+                 Nmax: Optional[int] = None, out: Optional[torch.Tensor] = None,
+                 kmin_out: Optional[torch.Tensor] = None, stream=None):
+        """gb_waveform: returns (AE [B, 2, Nmax] complex128, kmin [B] int64), both CUDA tensors."""
+        dev = self.device
+        B = int(params.shape[0])
+        if Nmax is None:
+            Nmax = int(N) if n_bins is None else 1024
+        if out is None:
+            out = torch.zeros((B, 2, Nmax), dtype=torch.complex128, device=dev)
+        if kmin_out is None:
+            kmin_out = torch.empty((B,), dtype=torch.int64, device=dev)
+        self._ok(lib().gb_waveform(self._h, _dev_ptr(params, torch.float64, dev, "params"), B, int(N),
+                                   _dev_ptr(n_bins, torch.int32, dev, "n_bins"), int(Nmax),
+                                   _dev_ptr(out, (torch.complex128, torch.float64), dev, "out"),
+                                   _dev_ptr(kmin_out, torch.int64, dev, "kmin_out"),
+                                   _stream_ptr(stream, dev)))
+        return out, kmin_out
+
+    def delta_loglike(self, data: Data, params_new: Optional[torch.Tensor], params_old: Optional[torch.Tensor],
+                      walker_index: torch.Tensor, move: Optional[torch.Tensor] = None, move_all: int = ADD,
+                      N: int = 0, n_bins: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None,
+                      aux: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """gb_delta_loglike: returns dlnL [B] float64 (CUDA)."""
+        dev = self.device
+        B = int(walker_index.shape[0])
+        if out is None:
+            out = torch.empty((B,), dtype=torch.float64, device=dev)
+        self._ok(lib().gb_delta_loglike(self._h, data.c(), _dev_ptr(params_new, torch.float64, dev, "params_new"),
+                                        _dev_ptr(params_old, torch.float64, dev, "params_old"),
+                                        _dev_ptr(walker_index, torch.int32, dev, "walker_index"),
+                                        _dev_ptr(move, torch.int8, dev, "move"), int(move_all), int(N),
+                                        _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B,
+                                        _dev_ptr(out, torch.float64, dev, "out"),
+                                        _dev_ptr(aux, torch.float64, dev, "aux"), _stream_ptr(stream, dev)))
+        return out
+
+    def residual_update(self, data: Data, params_new: Optional[torch.Tensor], params_old: Optional[torch.Tensor],
+                        walker_index: torch.Tensor, move: Optional[torch.Tensor] = None, move_all: int = ADD,
+                        accepted: Optional[torch.Tensor] = None, N: int = 0,
+                        n_bins: Optional[torch.Tensor] = None, stream=None) -> None:
+        """gb_residual_update: scatter accepted rows into data.resid in place."""
+        dev = self.device
+        B = int(walker_index.shape[0])
+        self._ok(lib().gb_residual_update(self._h, data.c(), _dev_ptr(params_new, torch.float64, dev, "params_new"),
+                                          _dev_ptr(params_old, torch.float64, dev, "params_old"),
+                                          _dev_ptr(walker_index, torch.int32, dev, "walker_index"),
+                                          _dev_ptr(move, torch.int8, dev, "move"), int(move_all),
+                                          _dev_ptr(accepted, torch.uint8, dev, "accepted"), int(N),
+                                          _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B,
+                                          _stream_ptr(stream, dev)))
+
+    # --------------------------------------------------------------------------------- host forms
+    def waveform_host(self, params, N: int = 0, n_bins=None, Nmax: Optional[int] = None, out=None,
+                      kmin_out=None, stream=None):
+        """gb_waveform_host: HOST params in, HOST (AE, kmin) out (numpy unless buffers are given)."""
+        p, k0 = _host_ptr(params, np.float64, "params")
+        B = int(np.prod(k0.shape) // 8)
+        nb, k1 = _host_ptr(n_bins, np.int32, "n_bins")
+        if Nmax is None:
+            Nmax = int(N) if n_bins is None else 1024
+        if out is None:
+            out = np.zeros((B, 2, Nmax), np.complex128)
+        if kmin_out is None:
+            kmin_out = np.zeros((B,), np.int64)
+        o, k2 = _host_ptr(out, np.complex128, "out")
+        km, k3 = _host_ptr(kmin_out, np.int64, "kmin_out")
+        self._ok(lib().gb_waveform_host(self._h, p, B, int(N), nb, int(Nmax), o, km,
+                                        _stream_ptr(stream, self.device)))
+        return k2, k3
+
+    def delta_loglike_host(self, data: Data, params_new, params_old, walker_index, move=None,
+                           move_all: int = ADD, N: int = 0, n_bins=None, out=None, aux=None, stream=None):
+        """gb_delta_loglike_host: HOST proposal arrays in, HOST dlnL out; `data` stays on the device."""
+        pn, k0 = _host_ptr(params_new, np.float64, "params_new")
+        po, k1 = _host_ptr(params_old, np.float64, "params_old")
+        w, k2 = _host_ptr(walker_index, np.int32, "walker_index")
+        B = int(k2.shape[0])
+        mv, k3 = _host_ptr(move, np.int8, "move")
+        nb, k4 = _host_ptr(n_bins, np.int32, "n_bins")
+        if out is None:
+            out = np.zeros((B,), np.float64)
+        o, k5 = _host_ptr(out, np.float64, "out")
+        ax, k6 = _host_ptr(aux, np.float64, "aux")
+        self._ok(lib().gb_delta_loglike_host(self._h, data.c(), pn, po, w, mv, int(move_all), int(N), nb, B, o, ax,
+                                             _stream_ptr(stream, self.device)))
+        return k5
+
+    def residual_update_host(self, data: Data, params_new, params_old, walker_index, move=None,
+                             move_all: int = ADD, accepted=None, N: int = 0, n_bins=None, stream=None) -> None:
+        """gb_residual_update_host: HOST proposal arrays in; data.resid (device) updated in place."""
+        pn, k0 = _host_ptr(params_new, np.float64, "params_new")
+        po, k1 = _host_ptr(params_old, np.float64, "params_old")
+        w, k2 = _host_ptr(walker_index, np.int32, "walker_index")
+        B = int(k2.shape[0])
+        mv, k3 = _host_ptr(move, np.int8, "move")
+        acc, k4 = _host_ptr(accepted, np.uint8, "accepted")
+        nb, k5 = _host_ptr(n_bins, np.int32, "n_bins")
+        self._ok(lib().gb_residual_update_host(self._h, data.c(), pn, po, w, mv, int(move_all), acc, int(N), nb, B,
+                                               _stream_ptr(stream, self.device)))
