@@ -4,4 +4,4 @@ The product is the C-ABI library libgbfit.so (include/gbfit.h, csrc/); this pack
 Python binding.  Names follow the header: Context.waveform / delta_loglike / residual_update.
 """
 from .gbfit import (ADD, REMOVE, SWAP, Context, Data, GbError, EXPORTS, lib, lib_path, version)  # noqa: F401
-from .build import build  # noqa: F401
+from . import build  # noqa: F401  (module: build.build() compiles libgbfit.so)
