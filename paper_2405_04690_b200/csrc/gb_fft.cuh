@@ -136,11 +136,17 @@ GB_HD void fft_stage_write(cx* bA, cx* bE, const cx* tw, int tid, StageRegs<N, G
     }
 }
 
-// Radix plans: N = 128: 4,4,4,2   256: 8,8,4   512: 8,8,8   1024: 8,8,4,4
+// Radix plans (group size G, then the stages as X(N, G, radix, Ns) with Ns = product of the earlier radices):
+//   N = 128: 4,4,4,2   256: 8,8,4   512: 8,8,8   1024: 8,8,4,4
+// The kernels expand X into read / barrier / write / barrier; the host logic test replays the same list.
 template <int N> struct Plan;
-template <> struct Plan<128>  { static constexpr int n = 4; static constexpr int R[4] = {4, 4, 4, 2}; static constexpr int G = 32; };
-template <> struct Plan<256>  { static constexpr int n = 3; static constexpr int R[4] = {8, 8, 4, 1}; static constexpr int G = 32; };
-template <> struct Plan<512>  { static constexpr int n = 3; static constexpr int R[4] = {8, 8, 8, 1}; static constexpr int G = 64; };
-template <> struct Plan<1024> { static constexpr int n = 4; static constexpr int R[4] = {8, 8, 4, 4}; static constexpr int G = 128; };
+template <> struct Plan<128>  { static constexpr int G = 32; };
+template <> struct Plan<256>  { static constexpr int G = 32; };
+template <> struct Plan<512>  { static constexpr int G = 64; };
+template <> struct Plan<1024> { static constexpr int G = 128; };
+#define GB_FFT_PLAN_128(X)  X(128, 32, 4, 1) X(128, 32, 4, 4) X(128, 32, 4, 16) X(128, 32, 2, 64)
+#define GB_FFT_PLAN_256(X)  X(256, 32, 8, 1) X(256, 32, 8, 8) X(256, 32, 4, 64)
+#define GB_FFT_PLAN_512(X)  X(512, 64, 8, 1) X(512, 64, 8, 8) X(512, 64, 8, 64)
+#define GB_FFT_PLAN_1024(X) X(1024, 128, 8, 1) X(1024, 128, 8, 8) X(1024, 128, 4, 64) X(1024, 128, 4, 256)
 
 }  // namespace gbk

@@ -51,16 +51,17 @@ struct SrcConst {
     double k[3];        // propagation direction
     double u[3];        // polarisation basis vector u
     double v[2];        // polarisation basis vector v (v_z = 0)
-    cd DP, DC;          // polarisation constants
+    cd DP, DC2;         // polarisation constants; DC2 = 2 DC (the factor 2 of d_cross = 2 nu_u nu_v)
     double w0;          // 2 pi f0
     double pifd;        // pi fdot
     double c1;          // (2/3) fdot / f0
     double phi0;
     double twopidelta;  // 2 pi (f0 T - q)
-    double x0;          // 2 pi f0 L / c
-    double xd;          // 2 pi fdot L / c
+    double hx0;         // pi f0 L / c      (x/2 at t = 0, x = 2 pi f L/c)
+    double hxd;         // pi fdot L / c
     int64_t kmin;       // q - N/2
-    double pad[4];
+    int64_t fast;       // 1: inside the limits of slow_sample_fast (gb_fast.cuh)
+    double pad[3];
 };
 static_assert(sizeof(SrcConst) == 192, "SrcConst layout");
 
@@ -82,7 +83,7 @@ GB_HD void source_constants(const double* p, double Tobs, double tau, int N, Src
     s.k[0] = -cosb * cl; s.k[1] = -cosb * sl; s.k[2] = -sinb;
     const double Ap = amp * (1.0 + ci * ci), Ac = -2.0 * amp * ci;
     s.DP = {Ap * c2p, -Ac * s2p};
-    s.DC = {-Ap * s2p, -Ac * c2p};
+    s.DC2 = {-2.0 * Ap * s2p, -2.0 * Ac * c2p};
     const double q = floor(mul_rn(f0, Tobs) + 0.5);
     const double delta = fma(f0, Tobs, -q);
     s.w0 = kTwoPi * f0;
@@ -90,10 +91,11 @@ GB_HD void source_constants(const double* p, double Tobs, double tau, int N, Src
     s.c1 = (2.0 / 3.0) * (fdot / f0);
     s.phi0 = phi0;
     s.twopidelta = kTwoPi * delta;
-    s.x0 = kTwoPi * f0 * tau;
-    s.xd = kTwoPi * fdot * tau;
+    s.hx0 = kPi * f0 * tau;
+    s.hxd = kPi * fdot * tau;
     s.kmin = (int64_t)q - N / 2;
-    s.pad[0] = s.pad[1] = s.pad[2] = s.pad[3] = 0.0;
+    s.fast = 0;
+    s.pad[0] = s.pad[1] = s.pad[2] = 0.0;
 }
 
 GB_HD double sinc_plain(double th, double sn) { return fabs(th) < 1e-8 ? 1.0 - th * th / 6.0 : sn / th; }
@@ -122,12 +124,12 @@ GB_HD void slow_sample(const SrcConst& s, const OrbitSample& o, double t, double
     const double va = s.v[0] * o.a[0] + s.v[1] * o.a[1];
     const double vb = s.v[0] * o.b[0] + s.v[1] * o.b[1];
     const double vc = s.v[0] * o.c[0] + s.v[1] * o.c[1];
-    const double dpa = ua * ua - va * va, dca = 2.0 * ua * va;
-    const double dpb = ub * ub - vb * vb, dcb = 2.0 * ub * vb;
-    const double dpc = uc * uc - vc * vc, dcc = 2.0 * uc * vc;
-    const cd Da = {dpa * s.DP.re + dca * s.DC.re, dpa * s.DP.im + dca * s.DC.im};   // D_12 = D_21
-    const cd Db = {dpb * s.DP.re + dcb * s.DC.re, dpb * s.DP.im + dcb * s.DC.im};   // D_23 = D_32
-    const cd Dc = {dpc * s.DP.re + dcc * s.DC.re, dpc * s.DP.im + dcc * s.DC.im};   // D_31 = D_13
+    const double dpa = ua * ua - va * va, dca = ua * va;   // the factor 2 of d_cross is in DC2
+    const double dpb = ub * ub - vb * vb, dcb = ub * vb;
+    const double dpc = uc * uc - vc * vc, dcc = uc * vc;
+    const cd Da = {dpa * s.DP.re + dca * s.DC2.re, dpa * s.DP.im + dca * s.DC2.im};   // D_12 = D_21
+    const cd Db = {dpb * s.DP.re + dcb * s.DC2.re, dpb * s.DP.im + dcb * s.DC2.im};   // D_23 = D_32
+    const cd Dc = {dpc * s.DP.re + dcc * s.DC2.re, dpc * s.DP.im + dcc * s.DC2.im};   // D_31 = D_13
 
     // k.x_r / c = k.R/c + (tau/3) * (kappa of the two links leaving r), since x_r = R + (L/3)(n_rs + n_rs')
     const double kR = s.k[0] * o.Rx + s.k[1] * o.Ry;
@@ -152,8 +154,8 @@ GB_HD void slow_sample(const SrcConst& s, const OrbitSample& o, double t, double
     }
 
     // transfer functions of the six links: theta_rs = x/2 (1 - kappa_rs)
-    const double x = s.x0 + s.xd * t;
-    const double hx = 0.5 * x;
+    const double hx = s.hx0 + s.hxd * t;
+    const double x = 2.0 * hx;
     const cd T12 = transfer(hx * (1.0 - ka)), T21 = transfer(hx * (1.0 + ka));
     const cd T23 = transfer(hx * (1.0 - kb)), T32 = transfer(hx * (1.0 + kb));
     const cd T31 = transfer(hx * (1.0 - kc)), T13 = transfer(hx * (1.0 + kc));

@@ -19,6 +19,7 @@
 #include <vector>
 
 #include "../../include/gbfit.h"
+#include "gb_fast.cuh"
 #include "gb_fft.cuh"
 #include "gb_math.cuh"
 #include "gb_tables.hpp"
@@ -28,7 +29,7 @@ using namespace gbk;
 namespace {
 
 enum Mode { MODE_WAVEFORM = 0, MODE_DLNL = 1, MODE_UPDATE = 2 };
-constexpr int kNumClasses = 8;   // class = 2 * log2(N / 128) + swap
+constexpr int kNumClasses = 16;  // class = 4 * log2(N / 128) + 2 * general + swap  (general: outside the fast path)
 
 // ------------------------------------------------------------------------------------------------ args
 struct PrepArgs {
@@ -40,7 +41,7 @@ struct PrepArgs {
     const int32_t* n_bins;
     int move_all, N, mode, n_walkers;
     int64_t B;
-    double Tobs, tau;
+    double Tobs, tau, Rmax;  // Rmax = AU / c
     int64_t kmax;            // largest valid global bin (Nyquist)
     SrcConst* src_new;
     SrcConst* src_old;
@@ -101,19 +102,24 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
             atomicOr(a.errflag, 1);
             if (a.dlnL_out) a.dlnL_out[b] = __longlong_as_double(0x7ff8000000000000LL);
         } else if (active) {
+            bool fast = true;
             if (mv != GB_REMOVE) {
                 SrcConst s;
                 source_constants(a.params_new + 8 * b, a.Tobs, a.tau, N, s);
+                s.fast = fast_path_ok(a.params_new + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                fast = fast && s.fast;
                 if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                 a.src_new[b] = s;
             }
             if (mv != GB_ADD) {
                 SrcConst s;
                 source_constants(a.params_old + 8 * b, a.Tobs, a.tau, N, s);
+                s.fast = fast_path_ok(a.params_old + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                fast = fast && s.fast;
                 if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                 a.src_old[b] = s;
             }
-            cls = 2 * cN + (mv == GB_SWAP ? 1 : 0);
+            cls = 4 * cN + (fast ? 0 : 2) + (mv == GB_SWAP ? 1 : 0);
         }
     }
     // warp-aggregated append: one atomic per (warp, class)
@@ -145,24 +151,24 @@ __device__ __forceinline__ void fft_all(cx* bA, cx* bE, const cx* tw, int tid);
 
 template <>
 __device__ __forceinline__ void fft_all<128, 32>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_STAGE(128, 32, 4, 1) GB_STAGE(128, 32, 4, 4) GB_STAGE(128, 32, 4, 16) GB_STAGE(128, 32, 2, 64)
+    GB_FFT_PLAN_128(GB_STAGE)
 }
 template <>
 __device__ __forceinline__ void fft_all<256, 32>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_STAGE(256, 32, 8, 1) GB_STAGE(256, 32, 8, 8) GB_STAGE(256, 32, 4, 64)
+    GB_FFT_PLAN_256(GB_STAGE)
 }
 template <>
 __device__ __forceinline__ void fft_all<512, 64>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_STAGE(512, 64, 8, 1) GB_STAGE(512, 64, 8, 8) GB_STAGE(512, 64, 8, 64)
+    GB_FFT_PLAN_512(GB_STAGE)
 }
 template <>
 __device__ __forceinline__ void fft_all<1024, 128>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_STAGE(1024, 128, 8, 1) GB_STAGE(1024, 128, 8, 8) GB_STAGE(1024, 128, 4, 64) GB_STAGE(1024, 128, 4, 256)
+    GB_FFT_PLAN_1024(GB_STAGE)
 }
 
 // slow part at this thread's samples n = tid + G j, then the FFT: bA, bE end up holding the window,
 // element j <-> global bin kmin + j.  s_src is the group's shared copy of the source constants.
-template <int N, int G>
+template <int N, int G, bool FAST>
 __device__ __forceinline__ void generate_waveform(const SrcConst* __restrict__ gsrc, SrcConst* s_src,
                                                   const double* __restrict__ orbit, const cx* __restrict__ tw,
                                                   cx* bA, cx* bE, double Tobs, double tau, int tid) {
@@ -175,17 +181,29 @@ __device__ __forceinline__ void generate_waveform(const SrcConst* __restrict__ g
 #pragma unroll 1
     for (int j = 0; j < S; j++) {
         const int n = tid + G * j;
-        OrbitSample o;
-        o.Rx = __ldg(orbit + 0 * N + n);
-        o.Ry = __ldg(orbit + 1 * N + n);
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            o.a[d] = __ldg(orbit + (2 + d) * N + n);
-            o.b[d] = __ldg(orbit + (5 + d) * N + n);
-            o.c[d] = __ldg(orbit + (8 + d) * N + n);
-        }
         cd As, Es;
-        slow_sample(*s_src, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
+        if (FAST) {
+            OrbitSampleAB o;
+            o.Rx = __ldg(orbit + 0 * N + n);
+            o.Ry = __ldg(orbit + 1 * N + n);
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                o.a[d] = __ldg(orbit + (2 + d) * N + n);
+                o.b[d] = __ldg(orbit + (5 + d) * N + n);
+            }
+            slow_sample_fast(*s_src, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
+        } else {
+            OrbitSample o;
+            o.Rx = __ldg(orbit + 0 * N + n);
+            o.Ry = __ldg(orbit + 1 * N + n);
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                o.a[d] = __ldg(orbit + (2 + d) * N + n);
+                o.b[d] = __ldg(orbit + (5 + d) * N + n);
+                o.c[d] = __ldg(orbit + (8 + d) * N + n);
+            }
+            slow_sample(*s_src, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
+        }
         bA[pad_idx(n)] = {As.re, As.im};
         bE[pad_idx(n)] = {Es.re, Es.im};
     }
@@ -224,12 +242,12 @@ __device__ __forceinline__ cx ld_cx(const double* p) {
     return {v.x, v.y};
 }
 
-template <int N, bool SWAP>
+template <int N, bool SWAP, bool FAST>
 __global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(MainArgs a) {
     constexpr int G = Plan<N>::G;
     constexpr int S = N / G;
     constexpr int PN = padded_len(N);
-    constexpr int cls = 2 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (SWAP ? 1 : 0);
+    constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx* bufA0 = reinterpret_cast<cx*>(smem_raw);      // first (or only) waveform
     cx* bufE0 = bufA0 + PN;
@@ -254,10 +272,10 @@ __global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(M
 
         // ---- waveform(s)
         if (SWAP) {
-            generate_waveform<N, G>(a.src_old + b, &s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
-            generate_waveform<N, G>(a.src_new + b, &s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
+            generate_waveform<N, G, FAST>(a.src_old + b, &s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
+            generate_waveform<N, G, FAST>(a.src_new + b, &s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
         } else {
-            generate_waveform<N, G>((mv == GB_REMOVE ? a.src_old : a.src_new) + b, &s_src[0], a.orbit, a.tw,
+            generate_waveform<N, G, FAST>((mv == GB_REMOVE ? a.src_old : a.src_new) + b, &s_src[0], a.orbit, a.tw,
                                     bufA0, bufE0, a.Tobs, a.tau, tid);
         }
         const int64_t kmin0 = s_src[0].kmin;
@@ -446,26 +464,37 @@ int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
     return GB_OK;
 }
 
-template <int N, bool SWAP>
-int setup_kernel(gb_ctx* ctx, int cls) {
+template <int N, bool SWAP, bool FAST>
+int setup_kernel(gb_ctx* ctx) {
+    constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
     const size_t smem = main_smem_bytes<N, SWAP>();
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP, FAST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP>, Plan<N>::G, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST>, Plan<N>::G, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_CUDA, "kernel class %d does not fit on an SM", cls);
     ctx->grid_blocks[cls] = nb * ctx->num_sms;
     return GB_OK;
 }
 
-template <int N, bool SWAP>
-int launch_main(gb_ctx* ctx, MainArgs& a, int cls, int64_t B, cudaStream_t st) {
-    a.orbit = ctx->d_orbit[cls >> 1];
+template <int N, bool SWAP, bool FAST>
+int launch_main(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
+    constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
+    a.orbit = ctx->d_orbit[cls >> 2];
     int64_t grid = ctx->grid_blocks[cls];
     if (grid > B) grid = B;
-    gb_main_kernel<N, SWAP><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP>(), st>>>(a);
+    gb_main_kernel<N, SWAP, FAST><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP>(), st>>>(a);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
+}
+
+// the fast-path kernel of a class, then the general one for the rows outside its limits (usually none:
+// that launch finds an empty list and returns at once)
+template <int N, bool SWAP>
+int launch_pair(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
+    int rc = launch_main<N, SWAP, true>(ctx, a, B, st);
+    if (rc) return rc;
+    return launch_main<N, SWAP, false>(ctx, a, B, st);
 }
 
 struct Call {
@@ -534,6 +563,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.B = c.B;
     p.Tobs = ctx->cfg.Tobs;
     p.tau = ctx->cfg.armlength / kCLight;
+    p.Rmax = ctx->cfg.au / kCLight;
     p.kmax = (int64_t)floor(ctx->cfg.Tobs / (2.0 * ctx->cfg.dt));
     p.src_new = ctx->d_src_new;
     p.src_old = ctx->d_src_old;
@@ -584,19 +614,19 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
         if (!c.n_bins && Nc != c.N) continue;
         if (may_swap) {
             switch (Nc) {
-                case 128: rc = launch_main<128, true>(ctx, a, 2 * cN + 1, c.B, st); break;
-                case 256: rc = launch_main<256, true>(ctx, a, 2 * cN + 1, c.B, st); break;
-                case 512: rc = launch_main<512, true>(ctx, a, 2 * cN + 1, c.B, st); break;
-                default: rc = launch_main<1024, true>(ctx, a, 2 * cN + 1, c.B, st); break;
+                case 128: rc = launch_pair<128, true>(ctx, a, c.B, st); break;
+                case 256: rc = launch_pair<256, true>(ctx, a, c.B, st); break;
+                case 512: rc = launch_pair<512, true>(ctx, a, c.B, st); break;
+                default: rc = launch_pair<1024, true>(ctx, a, c.B, st); break;
             }
             if (rc) return rc;
         }
         if (may_single) {
             switch (Nc) {
-                case 128: rc = launch_main<128, false>(ctx, a, 2 * cN, c.B, st); break;
-                case 256: rc = launch_main<256, false>(ctx, a, 2 * cN, c.B, st); break;
-                case 512: rc = launch_main<512, false>(ctx, a, 2 * cN, c.B, st); break;
-                default: rc = launch_main<1024, false>(ctx, a, 2 * cN, c.B, st); break;
+                case 128: rc = launch_pair<128, false>(ctx, a, c.B, st); break;
+                case 256: rc = launch_pair<256, false>(ctx, a, c.B, st); break;
+                case 512: rc = launch_pair<512, false>(ctx, a, c.B, st); break;
+                default: rc = launch_pair<1024, false>(ctx, a, c.B, st); break;
             }
             if (rc) return rc;
         }
@@ -655,14 +685,13 @@ int gb_create(const gb_config* cfg, gb_ctx** out) {
     GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->d_counts), sizeof(int32_t) * (2 * kNumClasses + 1)));
     GB_CUDA(ctx, cudaMemset(ctx->d_counts, 0, sizeof(int32_t) * (2 * kNumClasses + 1)));
     int rc;
-    if ((rc = setup_kernel<128, false>(ctx, 0))) return rc;
-    if ((rc = setup_kernel<128, true>(ctx, 1))) return rc;
-    if ((rc = setup_kernel<256, false>(ctx, 2))) return rc;
-    if ((rc = setup_kernel<256, true>(ctx, 3))) return rc;
-    if ((rc = setup_kernel<512, false>(ctx, 4))) return rc;
-    if ((rc = setup_kernel<512, true>(ctx, 5))) return rc;
-    if ((rc = setup_kernel<1024, false>(ctx, 6))) return rc;
-    if ((rc = setup_kernel<1024, true>(ctx, 7))) return rc;
+#define GB_SETUP(N_)                                                    \
+    if ((rc = setup_kernel<N_, false, true>(ctx))) return rc;           \
+    if ((rc = setup_kernel<N_, true, true>(ctx))) return rc;            \
+    if ((rc = setup_kernel<N_, false, false>(ctx))) return rc;          \
+    if ((rc = setup_kernel<N_, true, false>(ctx))) return rc;
+    GB_SETUP(128) GB_SETUP(256) GB_SETUP(512) GB_SETUP(1024)
+#undef GB_SETUP
     return GB_OK;
 }
 
