@@ -223,9 +223,11 @@ def run_ours(args):
             if i < n_keep:
                 keep[i] = row
     torch.cuda.synchronize()
-    d_psd = torch.from_numpy(wl.psd).to(dev)
+    # the noise weights live on the GPU as 1/S_n (formed once when a PSD row is set; the library
+    # takes S_n as well and then divides per bin, see gb_data.psd_is_inverse)
+    d_psd = torch.from_numpy(1.0 / wl.psd).to(dev)
     d_wpsd = torch.from_numpy(wl.walker_psd).to(dev)
-    data = gbfit.Data(d_resid, d_psd, wl.k_lo, walker_psd=d_wpsd)
+    data = gbfit.Data(d_resid, d_psd, wl.k_lo, walker_psd=d_wpsd, psd_is_inverse=True)
 
     # ---- proposals: pinned host copies (e2e) and device copies (kernel-only)
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -374,7 +376,7 @@ def run_ours(args):
             "config": {"workload": WORKLOAD if full else f"cfg5_reduced_{args.walkers}x{args.per_walker}",
                        "evals_per_step_per_gpu": int(B), "n_residuals": int(wl.n_walkers), "n_f": int(wl.n_f),
                        "accepted_fraction": float(wl.accepted.mean()), "mean_N": float(nb.mean()),
-                       "l2": "inputs_exceed_l2 (10.8 GB of residuals, no flush)",
+                       "l2": "inputs_exceed_l2 (10.8 GB of residuals, no flush)", "psd_layout": "1/S_n rows (psd_is_inverse=1)",
                        "parallelism": f"replicas{world}" if world > 1 else "single_gpu",
                        "ms_dlnl": ms_dlnl, "ms_update": ms_upd, "setup_s": setup_s},
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,

@@ -28,6 +28,23 @@ using namespace gbk;
 
 namespace {
 
+// tunables (defaults chosen from A/B runs on B200, see profiles/README.md)
+#ifndef GB_TPSM
+#define GB_TPSM 512        // resident threads per SM the main kernels are register-limited to (launch bounds)
+#endif
+#ifndef GB_ORBIT_PREFETCH
+#define GB_ORBIT_PREFETCH 1   // request the orbit rows of sample j+1 before evaluating sample j
+#endif
+#ifndef GB_L2_PREFETCH
+#define GB_L2_PREFETCH 1      // delta lnL: request the next item's residual / PSD window into L2
+#endif
+#ifndef GB_STREAM_LOADS
+#define GB_STREAM_LOADS 1     // window loads bypass L1 allocation
+#endif
+#ifndef GB_UNROLL
+#define GB_UNROLL 1        // unroll factor of the per-thread time-sample loop
+#endif
+
 enum Mode { MODE_WAVEFORM = 0, MODE_DLNL = 1, MODE_UPDATE = 2 };
 constexpr int kNumClasses = 16;  // class = 4 * log2(N / 128) + 2 * general + swap  (general: outside the fast path)
 
@@ -39,7 +56,8 @@ struct PrepArgs {
     const int8_t* move;
     const uint8_t* accepted;
     const int32_t* n_bins;
-    int move_all, N, mode, n_walkers;
+    const int32_t* walker_psd;
+    int move_all, N, mode, n_walkers, n_psd;
     int64_t B;
     double Tobs, tau, Rmax;  // Rmax = AU / c
     int64_t kmax;            // largest valid global bin (Nyquist)
@@ -88,14 +106,17 @@ __device__ __forceinline__ int class_of_N(int N) {
 __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int cls = -1;
+    bool use_old = false;   // the row's single source is the OLD one (REMOVE)
     if (b < a.B) {
         const int mv = a.mode == MODE_WAVEFORM ? GB_ADD : (a.move ? (int)a.move[b] : a.move_all);
         const int N = a.n_bins ? a.n_bins[b] : a.N;
         const int cN = class_of_N(N);
         bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP;
+        int w = 0, prow = 0;
         if (a.mode != MODE_WAVEFORM) {
-            const int w = a.walker_index[b];
+            w = a.walker_index[b];
             ok = ok && w >= 0 && w < a.n_walkers;
+            if (ok) prow = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
         }
         const bool active = a.accepted ? a.accepted[b] != 0 : true;
         if (!ok) {
@@ -108,6 +129,7 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
                 source_constants(a.params_new + 8 * b, a.Tobs, a.tau, N, s);
                 s.fast = fast_path_ok(a.params_new + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
                 fast = fast && s.fast;
+                s.walker = w;  s.psd_row = prow;  s.move = mv;
                 if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                 a.src_new[b] = s;
             }
@@ -116,10 +138,12 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
                 source_constants(a.params_old + 8 * b, a.Tobs, a.tau, N, s);
                 s.fast = fast_path_ok(a.params_old + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
                 fast = fast && s.fast;
+                s.walker = w;  s.psd_row = prow;  s.move = mv;
                 if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                 a.src_old[b] = s;
             }
             cls = 4 * cN + (fast ? 0 : 2) + (mv == GB_SWAP ? 1 : 0);
+            use_old = mv == GB_REMOVE;
         }
     }
     // warp-aggregated append: one atomic per (warp, class)
@@ -132,7 +156,7 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         int base = 0;
         if ((int)lane == leader) base = atomicAdd(a.counts + c, __popc(m));
         base = __shfl_sync(0xffffffffu, base, leader);
-        if (cls == c) a.lists[(int64_t)c * a.B + base + __popc(m & ((1u << lane) - 1))] = (int32_t)b;
+        if (cls == c) a.lists[(int64_t)c * a.B + base + __popc(m & ((1u << lane) - 1))] = (int32_t)b | (use_old ? (int32_t)0x80000000 : 0);
     }
 }
 
@@ -166,44 +190,70 @@ __device__ __forceinline__ void fft_all<1024, 128>(cx* bA, cx* bE, const cx* tw,
     GB_FFT_PLAN_1024(GB_STAGE)
 }
 
+// orbit table rows at sample n (coalesced across the group; the table stays L1/L2 resident)
+template <int N, bool FAST>
+struct OrbitRegs;
+template <int N>
+struct OrbitRegs<N, true> {
+    OrbitSampleAB o;
+    __device__ __forceinline__ void load(const double* __restrict__ orbit, int n) {
+        o.Rx = __ldg(orbit + 0 * N + n);
+        o.Ry = __ldg(orbit + 1 * N + n);
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            o.a[d] = __ldg(orbit + (2 + d) * N + n);
+            o.b[d] = __ldg(orbit + (5 + d) * N + n);
+        }
+    }
+    __device__ __forceinline__ void eval(const SrcConst& s, double t, double nfrac, double tau, double scale, cd& As,
+                                         cd& Es) const {
+        slow_sample_fast(s, o, t, nfrac, tau, scale, As, Es);
+    }
+};
+template <int N>
+struct OrbitRegs<N, false> {
+    OrbitSample o;
+    __device__ __forceinline__ void load(const double* __restrict__ orbit, int n) {
+        o.Rx = __ldg(orbit + 0 * N + n);
+        o.Ry = __ldg(orbit + 1 * N + n);
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            o.a[d] = __ldg(orbit + (2 + d) * N + n);
+            o.b[d] = __ldg(orbit + (5 + d) * N + n);
+            o.c[d] = __ldg(orbit + (8 + d) * N + n);
+        }
+    }
+    __device__ __forceinline__ void eval(const SrcConst& s, double t, double nfrac, double tau, double scale, cd& As,
+                                         cd& Es) const {
+        slow_sample(s, o, t, nfrac, tau, scale, As, Es);
+    }
+};
+
 // slow part at this thread's samples n = tid + G j, then the FFT: bA, bE end up holding the window,
-// element j <-> global bin kmin + j.  s_src is the group's shared copy of the source constants.
+// element j <-> global bin kmin + j.  s_src is the group's shared copy of the source record (already
+// visible to the whole group).  The orbit rows of sample j+1 are requested before sample j is evaluated.
 template <int N, int G, bool FAST>
-__device__ __forceinline__ void generate_waveform(const SrcConst* __restrict__ gsrc, SrcConst* s_src,
-                                                  const double* __restrict__ orbit, const cx* __restrict__ tw,
-                                                  cx* bA, cx* bE, double Tobs, double tau, int tid) {
+__device__ __forceinline__ void generate_waveform(const SrcConst* s_src, const double* __restrict__ orbit,
+                                                  const cx* __restrict__ tw, cx* bA, cx* bE, double Tobs, double tau,
+                                                  int tid) {
     constexpr int S = N / G;
-    // stage the 24 doubles of the source constants in shared memory (one broadcast read per use)
-    if (tid < 24) reinterpret_cast<double*>(s_src)[tid] = __ldg(reinterpret_cast<const double*>(gsrc) + tid);
-    __syncthreads();
     const double dtN = Tobs / (double)N;
     const double scale = (tid & 1) ? -Tobs / (2.0 * N) : Tobs / (2.0 * N);   // G is even: parity of n = parity of tid
-#pragma unroll 1
+    OrbitRegs<N, FAST> nxt;
+    nxt.load(orbit, tid);
+    constexpr int kUnroll = GB_UNROLL;
+#pragma unroll kUnroll
     for (int j = 0; j < S; j++) {
         const int n = tid + G * j;
+#if GB_ORBIT_PREFETCH
+        const OrbitRegs<N, FAST> cur = nxt;
+        if (j + 1 < S) nxt.load(orbit, n + G);
+#else
+        if (j > 0) nxt.load(orbit, n);
+        const OrbitRegs<N, FAST>& cur = nxt;
+#endif
         cd As, Es;
-        if (FAST) {
-            OrbitSampleAB o;
-            o.Rx = __ldg(orbit + 0 * N + n);
-            o.Ry = __ldg(orbit + 1 * N + n);
-#pragma unroll
-            for (int d = 0; d < 3; d++) {
-                o.a[d] = __ldg(orbit + (2 + d) * N + n);
-                o.b[d] = __ldg(orbit + (5 + d) * N + n);
-            }
-            slow_sample_fast(*s_src, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
-        } else {
-            OrbitSample o;
-            o.Rx = __ldg(orbit + 0 * N + n);
-            o.Ry = __ldg(orbit + 1 * N + n);
-#pragma unroll
-            for (int d = 0; d < 3; d++) {
-                o.a[d] = __ldg(orbit + (2 + d) * N + n);
-                o.b[d] = __ldg(orbit + (5 + d) * N + n);
-                o.c[d] = __ldg(orbit + (8 + d) * N + n);
-            }
-            slow_sample(*s_src, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
-        }
+        cur.eval(*s_src, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
         bA[pad_idx(n)] = {As.re, As.im};
         bE[pad_idx(n)] = {Es.re, Es.im};
     }
@@ -237,48 +287,173 @@ __device__ __forceinline__ void group_reduce(double* v, double* s_red, int tid) 
     }
 }
 
-__device__ __forceinline__ cx ld_cx(const double* p) {
-    const double2 v = *reinterpret_cast<const double2*>(p);
-    return {v.x, v.y};
+// One batch of window bins of a thread: residual (A, E) and weights 1/S_n (A, E) at elements i_first + G c.
+// The loads are unconditional (index clamped, values zeroed when the bin lies outside the stored band) so
+// that all of them are in flight together, and they are cached in L2 only (ld.global.cg): the orbit tables
+// and twiddles, re-read by every item, keep the L1.
+template <int CH>
+struct WinBatch {
+    cx ra[CH], re[CH];
+    double wa[CH], we[CH];
+    template <int G>
+    __device__ __forceinline__ void load(const double* __restrict__ rA, const double* __restrict__ rE,
+                                         const double* __restrict__ SA, const double* __restrict__ SE, int64_t i_first,
+                                         int64_t n_f, bool inv) {
+        bool ok[CH];
+#pragma unroll
+        for (int c = 0; c < CH; c++) {
+            const int64_t i = i_first + G * c;
+            ok[c] = i >= 0 && i < n_f;
+            const int64_t ic = ok[c] ? i : 0;
+#if GB_STREAM_LOADS
+            const double2 a2 = __ldcg(reinterpret_cast<const double2*>(rA + 2 * ic));
+            const double2 e2 = __ldcg(reinterpret_cast<const double2*>(rE + 2 * ic));
+            wa[c] = __ldcg(SA + ic);
+            we[c] = __ldcg(SE + ic);
+#else
+            const double2 a2 = *reinterpret_cast<const double2*>(rA + 2 * ic);
+            const double2 e2 = *reinterpret_cast<const double2*>(rE + 2 * ic);
+            wa[c] = SA[ic];
+            we[c] = SE[ic];
+#endif
+            ra[c] = {a2.x, a2.y};
+            re[c] = {e2.x, e2.y};
+        }
+        if (!inv) {
+#pragma unroll
+            for (int c = 0; c < CH; c++) {
+                wa[c] = 1.0 / wa[c];
+                we[c] = 1.0 / we[c];
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < CH; c++) {
+            if (!ok[c]) {
+                wa[c] = we[c] = 0.0;
+                ra[c] = re[c] = {0.0, 0.0};
+            }
+        }
+    }
+};
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int K>
+__device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;" ::"n"(K) : "memory");
 }
 
+constexpr int kRecChunks = (int)(sizeof(SrcConst) / 16);   // 16-byte pieces of one source record
+
+// Work distribution: items of a class are handed out by a global ticket counter, in list order, so the CTAs
+// that run at the same time work on neighbouring rows -- consecutive sources of one walker -- and share that
+// walker's residual in L2 (a fixed round-robin deal lets the CTAs drift apart and more than doubles the DRAM
+// traffic).  The ticket is taken three items ahead, its list entry is read two items ahead, the 192-byte
+// source record(s) of the next item are copied into the other half of s_src with cp.async while the current
+// item computes, and (delta lnL) the next item's residual / PSD window is requested into L2 one whole item
+// before its inner products read it: no global-memory round trip is exposed between items.
+// A list entry is the row index, with bit 31 set when the row's single source is the OLD one (REMOVE);
+// -1 marks the end of the list.
 template <int N, bool SWAP, bool FAST>
-__global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(MainArgs a) {
+__global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kernel(MainArgs a) {
     constexpr int G = Plan<N>::G;
     constexpr int S = N / G;
     constexpr int PN = padded_len(N);
+    constexpr int NS = SWAP ? 2 : 1;
     constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx* bufA0 = reinterpret_cast<cx*>(smem_raw);      // first (or only) waveform
     cx* bufE0 = bufA0 + PN;
     cx* bufA1 = bufE0 + PN;                           // SWAP: the new source; first = old
     cx* bufE1 = bufA1 + PN;
-    __shared__ SrcConst s_src[SWAP ? 2 : 1];
+    __shared__ __align__(16) SrcConst s_src[2][NS];   // [buffer][0 = old or only, 1 = new (SWAP)]
     __shared__ double s_red[(G / 32) * 5 + 1];
-    __shared__ int s_item;
+
+    __shared__ int s_ent[2];
 
     const int tid = threadIdx.x;
     const int count = a.counts[cls];
+    if (count == 0) return;
     const int32_t* __restrict__ list = a.lists + (int64_t)cls * a.B;
 
+    auto fetch = [&](int entry, int bufi) {
+        const int64_t row = entry & 0x7fffffff;
+        if (SWAP) {
+            if (tid < kRecChunks)
+                cp_async16(reinterpret_cast<char*>(&s_src[bufi][0]) + 16 * tid,
+                           reinterpret_cast<const char*>(a.src_old + row) + 16 * tid);
+            else if (tid < 2 * kRecChunks)
+                cp_async16(reinterpret_cast<char*>(&s_src[bufi][NS - 1]) + 16 * (tid - kRecChunks),
+                           reinterpret_cast<const char*>(a.src_new + row) + 16 * (tid - kRecChunks));
+        } else if (tid < kRecChunks) {
+            const SrcConst* g = (entry < 0 ? a.src_old : a.src_new) + row;
+            cp_async16(reinterpret_cast<char*>(&s_src[bufi][0]) + 16 * tid, reinterpret_cast<const char*>(g) + 16 * tid);
+        }
+    };
+
+    int t_nx2 = 0;   // (thread 0) ticket of the item after next
+    if (tid == 0) {
+        const int t = atomicAdd(a.counters + cls, 3);
+        s_ent[0] = t < count ? __ldg(list + t) : -1;
+        s_ent[1] = t + 1 < count ? __ldg(list + t + 1) : -1;
+        t_nx2 = t + 2;
+    }
+    __syncthreads();
+    int e_cur = s_ent[0], e_nxt = s_ent[1];
+    if (e_cur == -1) return;
+    fetch(e_cur, 0);
+    cp_async_commit();
+    int buf = 0;
+
     for (;;) {
-        if (tid == 0) s_item = atomicAdd(a.counters + cls, 1);
+        int t_nx3 = 0, e_nx2 = -1;
+        if (tid == 0) {   // issued now, consumed at the end of this item
+            t_nx3 = atomicAdd(a.counters + cls, 1);
+            if (t_nx2 < count) e_nx2 = __ldg(list + t_nx2);
+        }
+        const bool has_nxt = e_nxt != -1;
+        if (has_nxt) fetch(e_nxt, buf ^ 1);
+        cp_async_commit();
+        cp_async_wait<1>();            // this item's record(s) have landed (the next item's may be in flight)
         __syncthreads();
-        const int item = s_item;
-        __syncthreads();
-        if (item >= count) break;
-        const int64_t b = list[item];
-        const int mv = a.mode == MODE_WAVEFORM ? GB_ADD : (a.move ? (int)a.move[b] : a.move_all);
+        const SrcConst* rec = s_src[buf];
+        const int64_t b = e_cur & 0x7fffffff;
+        const int mv = rec[0].move;
 
         // ---- waveform(s)
-        if (SWAP) {
-            generate_waveform<N, G, FAST>(a.src_old + b, &s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
-            generate_waveform<N, G, FAST>(a.src_new + b, &s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
-        } else {
-            generate_waveform<N, G, FAST>((mv == GB_REMOVE ? a.src_old : a.src_new) + b, &s_src[0], a.orbit, a.tw,
-                                    bufA0, bufE0, a.Tobs, a.tau, tid);
+        generate_waveform<N, G, FAST>(&rec[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
+        if (SWAP) generate_waveform<N, G, FAST>(&rec[NS - 1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
+        const int64_t kmin0 = rec[0].kmin;
+
+        // ---- ask L2 for the next item's residual / PSD window
+        if (GB_L2_PREFETCH && a.mode == MODE_DLNL && has_nxt) {
+            cp_async_wait<0>();
+            __syncthreads();
+            const SrcConst& nx = s_src[buf ^ 1][NS - 1];
+            const int64_t i0 = nx.kmin - a.k_lo;
+            const size_t nf = (size_t)a.n_f;
+            const double* rAn = a.resid + ((size_t)nx.walker * 2 + 0) * nf * 2;
+            const double* rEn = a.resid + ((size_t)nx.walker * 2 + 1) * nf * 2;
+            const double* SAn = a.psd + ((size_t)nx.psd_row * 2 + 0) * nf;
+            const double* SEn = a.psd + ((size_t)nx.psd_row * 2 + 1) * nf;
+            for (int l = tid; l <= N / 8; l += G) {        // 128-byte lines of the complex128 windows
+                const int64_t i = i0 + 8 * l;
+                if (i >= 0 && i < a.n_f) {
+                    prefetch_l2(rAn + 2 * i);
+                    prefetch_l2(rEn + 2 * i);
+                }
+            }
+            for (int l = tid; l <= N / 16; l += G) {       // and of the f64 PSD windows
+                const int64_t i = i0 + 16 * l;
+                if (i >= 0 && i < a.n_f) {
+                    prefetch_l2(SAn + i);
+                    prefetch_l2(SEn + i);
+                }
+            }
         }
-        const int64_t kmin0 = s_src[0].kmin;
 
         // ---- epilogue
         if (a.mode == MODE_WAVEFORM) {
@@ -293,27 +468,29 @@ __global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(M
             }
             if (tid == 0 && a.kmin_out) a.kmin_out[b] = kmin0;
         } else {
-            const int w = a.walker_index[b];
+            const int w = rec[0].walker;
             const size_t nf = (size_t)a.n_f;
             double* rA = a.resid + ((size_t)w * 2 + 0) * nf * 2;
             double* rE = a.resid + ((size_t)w * 2 + 1) * nf * 2;
             if (a.mode == MODE_DLNL) {
-                const int prow = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
+                const int prow = rec[0].psd_row;
                 const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
                 const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
                 const bool inv = a.psd_is_inverse != 0;
                 const double norm = 4.0 / a.Tobs;
+                constexpr int CH = SWAP ? 2 : (S < 4 ? S : 4);   // bins per thread whose loads are in flight together
                 if (!SWAP) {
                     double v[2] = {0.0, 0.0};   // <h|h>, <r|h>
 #pragma unroll
-                    for (int m = 0; m < S; m++) {
-                        const int j = tid + G * m;
-                        const int64_t i = kmin0 + j - a.k_lo;
-                        if (i >= 0 && i < a.n_f) {
+                    for (int m0 = 0; m0 < S; m0 += CH) {
+                        WinBatch<CH> wb;
+                        wb.template load<G>(rA, rE, SA, SE, kmin0 + tid + G * m0 - a.k_lo, a.n_f, inv);
+#pragma unroll
+                        for (int c = 0; c < CH; c++) {
+                            const int j = tid + G * (m0 + c);
                             const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
-                            const cx ra = ld_cx(rA + 2 * i), re = ld_cx(rE + 2 * i);
-                            const double wa = inv ? SA[i] : 1.0 / SA[i];
-                            const double we = inv ? SE[i] : 1.0 / SE[i];
+                            const cx ra = wb.ra[c], re = wb.re[c];
+                            const double wa = wb.wa[c], we = wb.we[c];
                             v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
                             v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
                         }
@@ -329,34 +506,37 @@ __global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(M
                     }
                 } else {
                     // buffers: 0 = old (o), 1 = new (a)
-                    const int64_t kmin1 = s_src[1].kmin;
+                    const int64_t kmin1 = rec[NS - 1].kmin;
                     const int64_t shift = kmin1 - kmin0;   // o index of a's bin j is j + shift
                     double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // aa, ra, ao, oo, ro
 #pragma unroll
-                    for (int m = 0; m < S; m++) {
-                        const int j = tid + G * m;
-                        int64_t i = kmin1 + j - a.k_lo;
-                        if (i >= 0 && i < a.n_f) {
-                            const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
-                            const cx ra = ld_cx(rA + 2 * i), re = ld_cx(rE + 2 * i);
-                            const double wa = inv ? SA[i] : 1.0 / SA[i];
-                            const double we = inv ? SE[i] : 1.0 / SE[i];
-                            v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
-                            v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
-                            const int64_t jo = j + shift;
-                            if (jo >= 0 && jo < N) {
-                                const cx oa = bufA0[pad_idx((int)jo)], oe = bufE0[pad_idx((int)jo)];
-                                v[2] += wa * (ha.re * oa.re + ha.im * oa.im) + we * (he.re * oe.re + he.im * oe.im);
+                    for (int m0 = 0; m0 < S; m0 += CH) {
+                        WinBatch<CH> wn, wo;   // the new source's window and the old one's (equal when shift == 0)
+                        wn.template load<G>(rA, rE, SA, SE, kmin1 + tid + G * m0 - a.k_lo, a.n_f, inv);
+                        if (shift != 0) wo.template load<G>(rA, rE, SA, SE, kmin0 + tid + G * m0 - a.k_lo, a.n_f, inv);
+                        else wo = wn;
+#pragma unroll
+                        for (int c = 0; c < CH; c++) {
+                            const int j = tid + G * (m0 + c);
+                            {
+                                const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
+                                const cx ra = wn.ra[c], re = wn.re[c];
+                                const double wa = wn.wa[c], we = wn.we[c];
+                                v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
+                                v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
+                                const int64_t jo = j + shift;
+                                if (jo >= 0 && jo < N) {
+                                    const cx oa = bufA0[pad_idx((int)jo)], oe = bufE0[pad_idx((int)jo)];
+                                    v[2] += wa * (ha.re * oa.re + ha.im * oa.im) + we * (he.re * oe.re + he.im * oe.im);
+                                }
                             }
-                        }
-                        i = kmin0 + j - a.k_lo;
-                        if (i >= 0 && i < a.n_f) {
-                            const cx oa = bufA0[pad_idx(j)], oe = bufE0[pad_idx(j)];
-                            const cx ra = ld_cx(rA + 2 * i), re = ld_cx(rE + 2 * i);
-                            const double wa = inv ? SA[i] : 1.0 / SA[i];
-                            const double we = inv ? SE[i] : 1.0 / SE[i];
-                            v[3] += wa * (oa.re * oa.re + oa.im * oa.im) + we * (oe.re * oe.re + oe.im * oe.im);
-                            v[4] += wa * (ra.re * oa.re + ra.im * oa.im) + we * (re.re * oe.re + re.im * oe.im);
+                            {
+                                const cx oa = bufA0[pad_idx(j)], oe = bufE0[pad_idx(j)];
+                                const cx ra = wo.ra[c], re = wo.re[c];
+                                const double wa = wo.wa[c], we = wo.we[c];
+                                v[3] += wa * (oa.re * oa.re + oa.im * oa.im) + we * (oe.re * oe.re + oe.im * oe.im);
+                                v[4] += wa * (ra.re * oa.re + ra.im * oa.im) + we * (re.re * oe.re + re.im * oe.im);
+                            }
                         }
                     }
                     group_reduce<G, 5>(v, s_red, tid);
@@ -384,7 +564,7 @@ __global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(M
                         atomicAdd(rE + 2 * i + 1, sgn0 * he.im);
                     }
                     if (SWAP) {
-                        i = s_src[1].kmin + j - a.k_lo;
+                        i = rec[NS - 1].kmin + j - a.k_lo;
                         if (i >= 0 && i < a.n_f) {
                             const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
                             atomicAdd(rA + 2 * i, -ha.re);
@@ -396,7 +576,15 @@ __global__ void __launch_bounds__(Plan<N>::G, 512 / Plan<N>::G) gb_main_kernel(M
                 }
             }
         }
-        __syncthreads();   // buffers and s_src are reused by the next item
+        if (tid == 0) {
+            s_ent[0] = e_nx2;
+            t_nx2 = t_nx3;
+        }
+        __syncthreads();   // the waveform buffers, s_red and this half of s_src are reused from here on
+        if (!has_nxt) break;
+        e_cur = e_nxt;
+        e_nxt = s_ent[0];
+        buf ^= 1;
     }
 }
 
@@ -560,6 +748,8 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.N = c.N;
     p.mode = c.mode;
     p.n_walkers = c.data ? c.data->n_walkers : 0;
+    p.n_psd = c.data ? c.data->n_psd : 0;
+    p.walker_psd = c.data ? c.data->walker_psd : nullptr;
     p.B = c.B;
     p.Tobs = ctx->cfg.Tobs;
     p.tau = ctx->cfg.armlength / kCLight;
