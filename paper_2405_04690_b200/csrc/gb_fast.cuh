@@ -25,37 +25,55 @@
 
 namespace gbk {
 
+// Numeric constants of the fast path.  On the device they sit in __constant__ memory so that every use is a
+// c[bank][offset] operand of the DFMA / DMUL itself: a 64-bit literal would cost two extra issue slots (a pair
+// of 32-bit moves) per use, and the issue slot is the second bound of this kernel after the FP64 pipe.
+struct FastConsts {
+    double wS[6], wC[6];   // |x| <= 0.8
+    double nS[5], nC[4];   // |x| <= 0.27
+    double two_over_pi, pio2_hi, pio2_lo;
+    double third, rsqrt2, rsqrt6, r120, msixth;
+};
+#define GB_FAST_CONSTS_INIT                                                                                   \
+    {GB_POLY_W_SIN, GB_POLY_W_COS, GB_POLY_N_SIN, GB_POLY_N_COS, GB_TWO_OVER_PI, GB_PIO2_HI, GB_PIO2_LO,      \
+     1.0 / 3.0, 0.70710678118654752440, 0.40824829046386301637, 1.0 / 120.0, -1.0 / 6.0}
+#if defined(__CUDACC__)
+__constant__ FastConsts d_fast_consts = GB_FAST_CONSTS_INIT;
+#endif
+static const FastConsts h_fast_consts = GB_FAST_CONSTS_INIT;
+#if defined(__CUDA_ARCH__)
+#define GB_K(field) (d_fast_consts.field)
+#else
+#define GB_K(field) (h_fast_consts.field)
+#endif
+
 // sin, cos for |x| <= 0.8 (no range reduction)
 GB_HD void sincos_w(double x, double& s, double& c) {
-    constexpr double S[6] = GB_POLY_W_SIN;
-    constexpr double C[6] = GB_POLY_W_COS;
     const double z = x * x;
-    double ps = fma(S[5], z, S[4]);
-    double pc = fma(C[5], z, C[4]);
-    ps = fma(ps, z, S[3]);
-    pc = fma(pc, z, C[3]);
-    ps = fma(ps, z, S[2]);
-    pc = fma(pc, z, C[2]);
-    ps = fma(ps, z, S[1]);
-    pc = fma(pc, z, C[1]);
-    ps = fma(ps, z, S[0]);
-    pc = fma(pc, z, C[0]);
+    double ps = fma(GB_K(wS[5]), z, GB_K(wS[4]));
+    double pc = fma(GB_K(wC[5]), z, GB_K(wC[4]));
+    ps = fma(ps, z, GB_K(wS[3]));
+    pc = fma(pc, z, GB_K(wC[3]));
+    ps = fma(ps, z, GB_K(wS[2]));
+    pc = fma(pc, z, GB_K(wC[2]));
+    ps = fma(ps, z, GB_K(wS[1]));
+    pc = fma(pc, z, GB_K(wC[1]));
+    ps = fma(ps, z, GB_K(wS[0]));
+    pc = fma(pc, z, GB_K(wC[0]));
     s = fma(x * z, ps, x);
     c = fma(z, fma(z, pc, -0.5), 1.0);
 }
 
 // sin, cos for |x| <= 0.27
 GB_HD void sincos_n(double x, double& s, double& c) {
-    constexpr double S[5] = GB_POLY_N_SIN;
-    constexpr double C[4] = GB_POLY_N_COS;
     const double z = x * x;
-    double ps = fma(S[4], z, S[3]);
-    double pc = fma(C[3], z, C[2]);
-    ps = fma(ps, z, S[2]);
-    pc = fma(pc, z, C[1]);
-    ps = fma(ps, z, S[1]);
-    pc = fma(pc, z, C[0]);
-    ps = fma(ps, z, S[0]);
+    double ps = fma(GB_K(nS[4]), z, GB_K(nS[3]));
+    double pc = fma(GB_K(nC[3]), z, GB_K(nC[2]));
+    ps = fma(ps, z, GB_K(nS[2]));
+    pc = fma(pc, z, GB_K(nC[1]));
+    ps = fma(ps, z, GB_K(nS[1]));
+    pc = fma(pc, z, GB_K(nC[0]));
+    ps = fma(ps, z, GB_K(nS[0]));
     s = fma(x * z, ps, x);
     c = fma(z, fma(z, pc, -0.5), 1.0);
 }
@@ -73,11 +91,11 @@ GB_HD int lo32_of(double v) {
 // sin, cos for |x| < 3000: two-constant Cody-Waite reduction by pi/2, then sincos_w and the quadrant
 GB_HD void sincos_cw(double x, double& s, double& c) {
     constexpr double kMagic = 6755399441055744.0;   // 1.5 * 2^52: the low word of x*2/pi + magic is rint()
-    const double kd = fma(x, GB_TWO_OVER_PI, kMagic);
+    const double kd = fma(x, GB_K(two_over_pi), kMagic);
     const int q = lo32_of(kd);
     const double kf = kd - kMagic;
-    double r = fma(-kf, GB_PIO2_HI, x);
-    r = fma(-kf, GB_PIO2_LO, r);
+    double r = fma(-kf, GB_K(pio2_hi), x);
+    r = fma(-kf, GB_K(pio2_lo), r);
     double sr, cr;
     sincos_w(r, sr, cr);
     double a = (q & 1) ? cr : sr;
@@ -120,7 +138,7 @@ struct OrbitSampleAB {
 GB_HD double sinc_guarded(double hx, double sn, double d) {
     if (fabs(d) >= 1e-4) return sn / d;
     const double th = hx * d, z = th * th;
-    return hx * fma(z, fma(z, 1.0 / 120.0, -1.0 / 6.0), 1.0);
+    return hx * fma(z, fma(z, GB_K(r120), GB_K(msixth)), 1.0);
 }
 
 // Slow envelopes A_s(t_n), E_s(t_n) times `scale`; arguments as slow_sample().
@@ -147,7 +165,7 @@ GB_HD void slow_sample_fast(const SrcConst& s, const OrbitSampleAB& o, double t,
     const double kR = s.k[0] * o.Rx + s.k[1] * o.Ry;
     const double xiR = t - kR;
     const double hx = fma(s.hxd, t, s.hx0);
-    const double hx3 = hx * (1.0 / 3.0);
+    const double hx3 = hx * GB_K(third);
     double sh, ch, sa, ca, sb, cb;
     sincos_w(hx, sh, ch);
     sincos_n(hx3 * ka, sa, ca);
@@ -163,7 +181,7 @@ GB_HD void slow_sample_fast(const SrcConst& s, const OrbitSampleAB& o, double t,
 
     // ---- receiver factors g_r = a_r exp(i (phase_r - Phi_R)) = Q_r (a_r, a_r eps_r)   (O4)
     //      Q_1 = conj(Pa2) Pc2, Q_2 = conj(Pb2) Pa2, Q_3 = conj(Pc2) Pb2
-    const double t3 = tau * (1.0 / 3.0);
+    const double t3 = tau * GB_K(third);
     const double d1 = t3 * (ka - kc), d2 = t3 * (kb - ka), d3 = t3 * (kc - kb);
     const double aR = fma(s.c1, xiR, 1.0);
     const double a1 = fma(-s.c1, d1, aR), a2 = fma(-s.c1, d2, aR), a3 = fma(-s.c1, d3, aR);
@@ -224,8 +242,8 @@ GB_HD void slow_sample_fast(const SrcConst& s, const OrbitSampleAB& o, double t,
     const cd F = cmul({f2 * cx, -(f2 * sx)}, {cR, sR});
     const cd Ap = csub(Zp, Xp);                                                    // sqrt2 A'
     const cd Ep = {Xp.re - 2.0 * Yp.re + Zp.re, Xp.im - 2.0 * Yp.im + Zp.im};      // sqrt6 E'
-    As = cscale(0.70710678118654752440, cmul(F, Ap));
-    Es = cscale(0.40824829046386301637, cmul(F, Ep));
+    As = cscale(GB_K(rsqrt2), cmul(F, Ap));
+    Es = cscale(GB_K(rsqrt6), cmul(F, Ep));
 }
 
 }  // namespace gbk

@@ -41,6 +41,9 @@ namespace {
 #ifndef GB_STREAM_LOADS
 #define GB_STREAM_LOADS 1     // window loads bypass L1 allocation
 #endif
+#ifndef GB_WARP_SYNC
+#define GB_WARP_SYNC 1        // one-warp groups (N = 128, 256) use __syncwarp instead of the CTA barrier
+#endif
 #ifndef GB_UNROLL
 #define GB_UNROLL 1        // unroll factor of the per-thread time-sample loop
 #endif
@@ -161,6 +164,17 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------ main
+// barrier of the group that owns an item (= the CTA): a one-warp group only needs the warp-level barrier
+template <int G>
+__device__ __forceinline__ void group_sync() {
+#if GB_WARP_SYNC
+    if (G == 32) __syncwarp();
+    else __syncthreads();
+#else
+    __syncthreads();
+#endif
+}
+
 template <int N, int G>
 __device__ __forceinline__ void fft_all(cx* bA, cx* bE, const cx* tw, int tid);
 
@@ -168,9 +182,9 @@ __device__ __forceinline__ void fft_all(cx* bA, cx* bE, const cx* tw, int tid);
     {                                                                \
         StageRegs<N_, G_, R_> rg;                                    \
         fft_stage_read<N_, G_, R_>(bA, bE, tid, rg);                 \
-        __syncthreads();                                             \
+        group_sync<G_>();                                            \
         fft_stage_write<N_, G_, R_, Ns_>(bA, bE, tw, tid, rg);       \
-        __syncthreads();                                             \
+        group_sync<G_>();                                            \
     }
 
 template <>
@@ -229,13 +243,13 @@ struct OrbitRegs<N, false> {
     }
 };
 
-// slow part at this thread's samples n = tid + G j, then the FFT: bA, bE end up holding the window,
-// element j <-> global bin kmin + j.  s_src is the group's shared copy of the source record (already
-// visible to the whole group).  The orbit rows of sample j+1 are requested before sample j is evaluated.
+// slow part at this thread's samples n = tid + G j: bA, bE receive (-1)^n T/(2N) (A_s, E_s)(t_n); after
+// fft_all they hold the window, element j <-> global bin kmin + j.  s_src is the group's shared copy of the
+// source record (already visible to the whole group).  The orbit rows of sample j+1 are requested before
+// sample j is evaluated.
 template <int N, int G, bool FAST>
-__device__ __forceinline__ void generate_waveform(const SrcConst* s_src, const double* __restrict__ orbit,
-                                                  const cx* __restrict__ tw, cx* bA, cx* bE, double Tobs, double tau,
-                                                  int tid) {
+__device__ __forceinline__ void slow_part(const SrcConst* s_src, const double* __restrict__ orbit, cx* bA, cx* bE,
+                                          double Tobs, double tau, int tid) {
     constexpr int S = N / G;
     const double dtN = Tobs / (double)N;
     const double scale = (tid & 1) ? -Tobs / (2.0 * N) : Tobs / (2.0 * N);   // G is even: parity of n = parity of tid
@@ -257,8 +271,7 @@ __device__ __forceinline__ void generate_waveform(const SrcConst* s_src, const d
         bA[pad_idx(n)] = {As.re, As.im};
         bE[pad_idx(n)] = {Es.re, Es.im};
     }
-    __syncthreads();
-    fft_all<N, G>(bA, bE, tw, tid);
+    group_sync<G>();
 }
 
 // sum NV per-thread values over the group; result valid in thread 0
@@ -275,7 +288,7 @@ __device__ __forceinline__ void group_reduce(double* v, double* s_red, int tid) 
 #pragma unroll
             for (int i = 0; i < NV; i++) s_red[warp * NV + i] = v[i];
         }
-        __syncthreads();
+        group_sync<G>();
         if (tid == 0) {
 #pragma unroll
             for (int w = 1; w < G / 32; w++) {
@@ -283,7 +296,7 @@ __device__ __forceinline__ void group_reduce(double* v, double* s_red, int tid) 
                 for (int i = 0; i < NV; i++) v[i] += s_red[w * NV + i];
             }
         }
-        __syncthreads();
+        group_sync<G>();
     }
 }
 
@@ -295,7 +308,7 @@ template <int CH>
 struct WinBatch {
     cx ra[CH], re[CH];
     double wa[CH], we[CH];
-    template <int G>
+    template <int G, bool CHECK>
     __device__ __forceinline__ void load(const double* __restrict__ rA, const double* __restrict__ rE,
                                          const double* __restrict__ SA, const double* __restrict__ SE, int64_t i_first,
                                          int64_t n_f, bool inv) {
@@ -303,7 +316,7 @@ struct WinBatch {
 #pragma unroll
         for (int c = 0; c < CH; c++) {
             const int64_t i = i_first + G * c;
-            ok[c] = i >= 0 && i < n_f;
+            ok[c] = CHECK ? (i >= 0 && i < n_f) : true;   // !CHECK: the whole window lies inside the stored band
             const int64_t ic = ok[c] ? i : 0;
 #if GB_STREAM_LOADS
             const double2 a2 = __ldcg(reinterpret_cast<const double2*>(rA + 2 * ic));
@@ -401,7 +414,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         s_ent[1] = t + 1 < count ? __ldg(list + t + 1) : -1;
         t_nx2 = t + 2;
     }
-    __syncthreads();
+    group_sync<G>();
     int e_cur = s_ent[0], e_nxt = s_ent[1];
     if (e_cur == -1) return;
     fetch(e_cur, 0);
@@ -409,29 +422,36 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     int buf = 0;
 
     for (;;) {
-        int t_nx3 = 0, e_nx2 = -1;
-        if (tid == 0) {   // issued now, consumed at the end of this item
-            t_nx3 = atomicAdd(a.counters + cls, 1);
-            if (t_nx2 < count) e_nx2 = __ldg(list + t_nx2);
-        }
         const bool has_nxt = e_nxt != -1;
         if (has_nxt) fetch(e_nxt, buf ^ 1);
         cp_async_commit();
         cp_async_wait<1>();            // this item's record(s) have landed (the next item's may be in flight)
-        __syncthreads();
+        group_sync<G>();
         const SrcConst* rec = s_src[buf];
         const int64_t b = e_cur & 0x7fffffff;
         const int mv = rec[0].move;
 
         // ---- waveform(s)
-        generate_waveform<N, G, FAST>(&rec[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
-        if (SWAP) generate_waveform<N, G, FAST>(&rec[NS - 1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
+        slow_part<N, G, FAST>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+        if (SWAP) {
+            fft_all<N, G>(bufA0, bufE0, a.tw, tid);
+            slow_part<N, G, FAST>(&rec[NS - 1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
+        }
+        // (thread 0) next ticket and the list entry of the ticket taken one item ago: issued here, after the
+        // register-hungry slow part, and consumed at the end of the item, behind the FFT and the epilogue
+        int t_nx3 = 0, e_nx2 = -1;
+        if (tid == 0) {
+            t_nx3 = atomicAdd(a.counters + cls, 1);
+            if (t_nx2 < count) e_nx2 = __ldg(list + t_nx2);
+        }
+        if (SWAP) fft_all<N, G>(bufA1, bufE1, a.tw, tid);
+        else fft_all<N, G>(bufA0, bufE0, a.tw, tid);
         const int64_t kmin0 = rec[0].kmin;
 
         // ---- ask L2 for the next item's residual / PSD window
         if (GB_L2_PREFETCH && a.mode == MODE_DLNL && has_nxt) {
             cp_async_wait<0>();
-            __syncthreads();
+            group_sync<G>();
             const SrcConst& nx = s_src[buf ^ 1][NS - 1];
             const int64_t i0 = nx.kmin - a.k_lo;
             const size_t nf = (size_t)a.n_f;
@@ -439,18 +459,39 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             const double* rEn = a.resid + ((size_t)nx.walker * 2 + 1) * nf * 2;
             const double* SAn = a.psd + ((size_t)nx.psd_row * 2 + 0) * nf;
             const double* SEn = a.psd + ((size_t)nx.psd_row * 2 + 1) * nf;
-            for (int l = tid; l <= N / 8; l += G) {        // 128-byte lines of the complex128 windows
-                const int64_t i = i0 + 8 * l;
-                if (i >= 0 && i < a.n_f) {
-                    prefetch_l2(rAn + 2 * i);
-                    prefetch_l2(rEn + 2 * i);
+            if (i0 >= 0 && i0 + N + 16 <= a.n_f) {           // window (plus the line it may end in) is stored
+                const double* pA = rAn + 2 * (i0 + 8 * tid);
+                const double* pE = rEn + 2 * (i0 + 8 * tid);
+#pragma unroll
+                for (int l = 0; l <= N / 8; l += G) {      // 128-byte lines of the complex128 windows
+                    if (l + tid <= N / 8) {
+                        prefetch_l2(pA + 16 * l);
+                        prefetch_l2(pE + 16 * l);
+                    }
                 }
-            }
-            for (int l = tid; l <= N / 16; l += G) {       // and of the f64 PSD windows
-                const int64_t i = i0 + 16 * l;
-                if (i >= 0 && i < a.n_f) {
-                    prefetch_l2(SAn + i);
-                    prefetch_l2(SEn + i);
+                const double* pSA = SAn + i0 + 16 * tid;
+                const double* pSE = SEn + i0 + 16 * tid;
+#pragma unroll
+                for (int l = 0; l <= N / 16; l += G) {     // and of the f64 PSD windows
+                    if (l + tid <= N / 16) {
+                        prefetch_l2(pSA + 16 * l);
+                        prefetch_l2(pSE + 16 * l);
+                    }
+                }
+            } else {
+                for (int l = tid; l <= N / 8; l += G) {
+                    const int64_t i = i0 + 8 * l;
+                    if (i >= 0 && i < a.n_f) {
+                        prefetch_l2(rAn + 2 * i);
+                        prefetch_l2(rEn + 2 * i);
+                    }
+                }
+                for (int l = tid; l <= N / 16; l += G) {
+                    const int64_t i = i0 + 16 * l;
+                    if (i >= 0 && i < a.n_f) {
+                        prefetch_l2(SAn + i);
+                        prefetch_l2(SEn + i);
+                    }
                 }
             }
         }
@@ -472,6 +513,8 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             const size_t nf = (size_t)a.n_f;
             double* rA = a.resid + ((size_t)w * 2 + 0) * nf * 2;
             double* rE = a.resid + ((size_t)w * 2 + 1) * nf * 2;
+            const int64_t i0w = kmin0 - a.k_lo;                         // residual element of window bin 0
+            const bool inband0 = i0w >= 0 && i0w + N <= a.n_f;          // the whole window is stored
             if (a.mode == MODE_DLNL) {
                 const int prow = rec[0].psd_row;
                 const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
@@ -484,7 +527,8 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
 #pragma unroll
                     for (int m0 = 0; m0 < S; m0 += CH) {
                         WinBatch<CH> wb;
-                        wb.template load<G>(rA, rE, SA, SE, kmin0 + tid + G * m0 - a.k_lo, a.n_f, inv);
+                        if (inband0) wb.template load<G, false>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                        else wb.template load<G, true>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
 #pragma unroll
                         for (int c = 0; c < CH; c++) {
                             const int j = tid + G * (m0 + c);
@@ -508,13 +552,20 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     // buffers: 0 = old (o), 1 = new (a)
                     const int64_t kmin1 = rec[NS - 1].kmin;
                     const int64_t shift = kmin1 - kmin0;   // o index of a's bin j is j + shift
+                    const int64_t i1w = kmin1 - a.k_lo;
+                    const bool inband1 = i1w >= 0 && i1w + N <= a.n_f;
                     double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // aa, ra, ao, oo, ro
 #pragma unroll
                     for (int m0 = 0; m0 < S; m0 += CH) {
                         WinBatch<CH> wn, wo;   // the new source's window and the old one's (equal when shift == 0)
-                        wn.template load<G>(rA, rE, SA, SE, kmin1 + tid + G * m0 - a.k_lo, a.n_f, inv);
-                        if (shift != 0) wo.template load<G>(rA, rE, SA, SE, kmin0 + tid + G * m0 - a.k_lo, a.n_f, inv);
-                        else wo = wn;
+                        if (inband0 && inband1) {
+                            wn.template load<G, false>(rA, rE, SA, SE, i1w + tid + G * m0, a.n_f, inv);
+                            if (shift != 0) wo.template load<G, false>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                            else wo = wn;
+                        } else {
+                            wn.template load<G, true>(rA, rE, SA, SE, i1w + tid + G * m0, a.n_f, inv);
+                            wo.template load<G, true>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                        }
 #pragma unroll
                         for (int c = 0; c < CH; c++) {
                             const int j = tid + G * (m0 + c);
@@ -552,6 +603,19 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 }
             } else {   // MODE_UPDATE: r -= a (ADD), r += h (REMOVE), r += o - a (SWAP)
                 const double sgn0 = SWAP ? 1.0 : (mv == GB_REMOVE ? 1.0 : -1.0);
+                if (!SWAP && inband0) {   // common case: no per-bin range checks
+                    double* pA = rA + 2 * (i0w + tid);
+                    double* pE = rE + 2 * (i0w + tid);
+#pragma unroll
+                    for (int m = 0; m < S; m++) {
+                        const int j = tid + G * m;
+                        const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
+                        atomicAdd(pA + 2 * G * m, sgn0 * ha.re);
+                        atomicAdd(pA + 2 * G * m + 1, sgn0 * ha.im);
+                        atomicAdd(pE + 2 * G * m, sgn0 * he.re);
+                        atomicAdd(pE + 2 * G * m + 1, sgn0 * he.im);
+                    }
+                } else
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -580,7 +644,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             s_ent[0] = e_nx2;
             t_nx2 = t_nx3;
         }
-        __syncthreads();   // the waveform buffers, s_red and this half of s_src are reused from here on
+        group_sync<G>();   // the waveform buffers, s_red and this half of s_src are reused from here on
         if (!has_nxt) break;
         e_cur = e_nxt;
         e_nxt = s_ent[0];
