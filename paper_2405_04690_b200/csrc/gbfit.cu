@@ -175,33 +175,44 @@ __device__ __forceinline__ void group_sync() {
 #endif
 }
 
-template <int N, int G>
-__device__ __forceinline__ void fft_all(cx* bA, cx* bE, const cx* tw, int tid);
-
-#define GB_STAGE(N_, G_, R_, Ns_)                                    \
-    {                                                                \
-        StageRegs<N_, G_, R_> rg;                                    \
-        fft_stage_read<N_, G_, R_>(bA, bE, tid, rg);                 \
-        group_sync<G_>();                                            \
-        fft_stage_write<N_, G_, R_, Ns_>(bA, bE, tw, tid, rg);       \
-        group_sync<G_>();                                            \
+// FFT of both channels of one item: threads [0, G/2) transform A, threads [G/2, G) transform E (gb_fft.cuh).
+//   fft_store: every stage written back, the buffers end up holding the window in natural order;
+//   fft_regs:  the last stage stays in registers, h[m] = bin ht + (G/2) m of this thread's channel.
+#define GB_STAGE_X(N_, R_, Ns_)                                       \
+    {                                                                 \
+        StageRegs<N_, R_> rg;                                         \
+        fft_stage_read<N_, R_>(buf, ht, rg);                          \
+        group_sync<Plan<N_>::G>();                                    \
+        fft_stage_compute<N_, R_, Ns_>(tw, ht, rg);                   \
+        fft_stage_store<N_, R_, Ns_>(buf, ht, rg);                    \
+        group_sync<Plan<N_>::G>();                                    \
     }
-
-template <>
-__device__ __forceinline__ void fft_all<128, 32>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_FFT_PLAN_128(GB_STAGE)
+#define GB_STAGE_L(N_, R_, Ns_)                                       \
+    {                                                                 \
+        StageRegs<N_, R_> rg;                                         \
+        fft_stage_read<N_, R_>(buf, ht, rg);                          \
+        fft_stage_compute<N_, R_, Ns_>(tw, ht, rg);                   \
+        fft_last_to_bins<N_, R_>(rg, h);                              \
+    }
+template <int N>
+__device__ __forceinline__ void fft_store(cx* bA, cx* bE, const cx* __restrict__ tw, int tid) {
+    constexpr int H = Plan<N>::G / 2;
+    cx* buf = tid < H ? bA : bE;
+    const int ht = tid < H ? tid : tid - H;
+    if constexpr (N == 128) { GB_FFT_PLAN_128(GB_STAGE_X, GB_STAGE_X) }
+    if constexpr (N == 256) { GB_FFT_PLAN_256(GB_STAGE_X, GB_STAGE_X) }
+    if constexpr (N == 512) { GB_FFT_PLAN_512(GB_STAGE_X, GB_STAGE_X) }
+    if constexpr (N == 1024) { GB_FFT_PLAN_1024(GB_STAGE_X, GB_STAGE_X) }
 }
-template <>
-__device__ __forceinline__ void fft_all<256, 32>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_FFT_PLAN_256(GB_STAGE)
-}
-template <>
-__device__ __forceinline__ void fft_all<512, 64>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_FFT_PLAN_512(GB_STAGE)
-}
-template <>
-__device__ __forceinline__ void fft_all<1024, 128>(cx* bA, cx* bE, const cx* tw, int tid) {
-    GB_FFT_PLAN_1024(GB_STAGE)
+template <int N>
+__device__ __forceinline__ void fft_regs(cx* bA, cx* bE, const cx* __restrict__ tw, int tid, cx* h) {
+    constexpr int H = Plan<N>::G / 2;
+    cx* buf = tid < H ? bA : bE;
+    const int ht = tid < H ? tid : tid - H;
+    if constexpr (N == 128) { GB_FFT_PLAN_128(GB_STAGE_X, GB_STAGE_L) }
+    if constexpr (N == 256) { GB_FFT_PLAN_256(GB_STAGE_X, GB_STAGE_L) }
+    if constexpr (N == 512) { GB_FFT_PLAN_512(GB_STAGE_X, GB_STAGE_L) }
+    if constexpr (N == 1024) { GB_FFT_PLAN_1024(GB_STAGE_X, GB_STAGE_L) }
 }
 
 // orbit table rows at sample n (coalesced across the group; the table stays L1/L2 resident)
@@ -268,8 +279,8 @@ __device__ __forceinline__ void slow_part(const SrcConst* s_src, const double* _
 #endif
         cd As, Es;
         cur.eval(*s_src, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
-        bA[pad_idx(n)] = {As.re, As.im};
-        bE[pad_idx(n)] = {Es.re, Es.im};
+        bA[pad_idx<N>(n)] = {As.re, As.im};
+        bE[pad_idx<N>(n)] = {Es.re, Es.im};
     }
     group_sync<G>();
 }
@@ -299,6 +310,44 @@ __device__ __forceinline__ void group_reduce(double* v, double* s_red, int tid) 
         group_sync<G>();
     }
 }
+
+// One batch of window bins of ONE channel: residual r and weight 1/S_n at elements i_first + H c (the
+// non-SWAP epilogue, fed from registers).  Same load policy as WinBatch below.
+template <int CH>
+struct WinBatch1 {
+    cx r[CH];
+    double w[CH];
+    template <int H, bool CHECK>
+    __device__ __forceinline__ void load(const double* __restrict__ rC, const double* __restrict__ SC, int64_t i_first,
+                                         int64_t n_f, bool inv) {
+        bool ok[CH];
+#pragma unroll
+        for (int c = 0; c < CH; c++) {
+            const int64_t i = i_first + H * c;
+            ok[c] = CHECK ? (i >= 0 && i < n_f) : true;   // !CHECK: the whole window lies inside the stored band
+            const int64_t ic = ok[c] ? i : 0;
+#if GB_STREAM_LOADS
+            const double2 a2 = __ldcg(reinterpret_cast<const double2*>(rC + 2 * ic));
+            w[c] = __ldcg(SC + ic);
+#else
+            const double2 a2 = *reinterpret_cast<const double2*>(rC + 2 * ic);
+            w[c] = SC[ic];
+#endif
+            r[c] = {a2.x, a2.y};
+        }
+        if (!inv) {
+#pragma unroll
+            for (int c = 0; c < CH; c++) w[c] = 1.0 / w[c];
+        }
+#pragma unroll
+        for (int c = 0; c < CH; c++) {
+            if (!ok[c]) {
+                w[c] = 0.0;
+                r[c] = {0.0, 0.0};
+            }
+        }
+    }
+};
 
 // One batch of window bins of a thread: residual (A, E) and weights 1/S_n (A, E) at elements i_first + G c.
 // The loads are unconditional (index clamped, values zeroed when the bin lies outside the stored band) so
@@ -374,7 +423,7 @@ template <int N, bool SWAP, bool FAST>
 __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kernel(MainArgs a) {
     constexpr int G = Plan<N>::G;
     constexpr int S = N / G;
-    constexpr int PN = padded_len(N);
+    constexpr int PN = padded_len<N>();
     constexpr int NS = SWAP ? 2 : 1;
     constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -434,7 +483,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         // ---- waveform(s)
         slow_part<N, G, FAST>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
         if (SWAP) {
-            fft_all<N, G>(bufA0, bufE0, a.tw, tid);
+            fft_store<N>(bufA0, bufE0, a.tw, tid);
             slow_part<N, G, FAST>(&rec[NS - 1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
         }
         // (thread 0) next ticket and the list entry of the ticket taken one item ago: issued here, after the
@@ -444,8 +493,6 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             t_nx3 = atomicAdd(a.counters + cls, 1);
             if (t_nx2 < count) e_nx2 = __ldg(list + t_nx2);
         }
-        if (SWAP) fft_all<N, G>(bufA1, bufE1, a.tw, tid);
-        else fft_all<N, G>(bufA0, bufE0, a.tw, tid);
         const int64_t kmin0 = rec[0].kmin;
 
         // ---- ask L2 for the next item's residual / PSD window
@@ -496,17 +543,21 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             }
         }
 
+        // ---- FFT: SWAP keeps both windows in shared memory; otherwise the last stage stays in registers,
+        //      h[m] = bin ht + H m of this thread's channel (threads [0, H): A, [H, G): E)
+        constexpr int H = G / 2, M = N / H;
+        cx h[M];
+        if (SWAP) fft_store<N>(bufA1, bufE1, a.tw, tid);
+        else fft_regs<N>(bufA0, bufE0, a.tw, tid, h);
+        const int ch = tid >= H ? 1 : 0;
+        const int ht = tid - ch * H;
+
         // ---- epilogue
         if (a.mode == MODE_WAVEFORM) {
             double2* outA = reinterpret_cast<double2*>(a.AE_out) + ((size_t)b * 2 + 0) * (size_t)a.Nmax;
             double2* outE = reinterpret_cast<double2*>(a.AE_out) + ((size_t)b * 2 + 1) * (size_t)a.Nmax;
 #pragma unroll
-            for (int m = 0; m < S; m++) {
-                const int j = tid + G * m;
-                const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
-                outA[j] = make_double2(ha.re, ha.im);
-                outE[j] = make_double2(he.re, he.im);
-            }
+            for (int m = 0; m < M; m++) (ch ? outE : outA)[ht + H * m] = make_double2(h[m].re, h[m].im);
             if (tid == 0 && a.kmin_out) a.kmin_out[b] = kmin0;
         } else {
             const int w = rec[0].walker;
@@ -523,20 +574,21 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 const double norm = 4.0 / a.Tobs;
                 constexpr int CH = SWAP ? 2 : (S < 4 ? S : 4);   // bins per thread whose loads are in flight together
                 if (!SWAP) {
+                    // this thread's channel: bins ht + H m (consecutive threads, consecutive bins)
+                    const double* rC = ch ? rE : rA;
+                    const double* SC = ch ? SE : SA;
+                    constexpr int CH1 = 4;      // bins per thread whose loads are in flight together
                     double v[2] = {0.0, 0.0};   // <h|h>, <r|h>
 #pragma unroll
-                    for (int m0 = 0; m0 < S; m0 += CH) {
-                        WinBatch<CH> wb;
-                        if (inband0) wb.template load<G, false>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
-                        else wb.template load<G, true>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                    for (int m0 = 0; m0 < M; m0 += CH1) {
+                        WinBatch1<CH1> wb;
+                        if (inband0) wb.template load<H, false>(rC, SC, i0w + ht + H * m0, a.n_f, inv);
+                        else wb.template load<H, true>(rC, SC, i0w + ht + H * m0, a.n_f, inv);
 #pragma unroll
-                        for (int c = 0; c < CH; c++) {
-                            const int j = tid + G * (m0 + c);
-                            const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
-                            const cx ra = wb.ra[c], re = wb.re[c];
-                            const double wa = wb.wa[c], we = wb.we[c];
-                            v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
-                            v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
+                        for (int c = 0; c < CH1; c++) {
+                            const cx hc = h[m0 + c], rc = wb.r[c];
+                            v[0] += wb.w[c] * (hc.re * hc.re + hc.im * hc.im);
+                            v[1] += wb.w[c] * (rc.re * hc.re + rc.im * hc.im);
                         }
                     }
                     group_reduce<G, 2>(v, s_red, tid);
@@ -570,19 +622,19 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                         for (int c = 0; c < CH; c++) {
                             const int j = tid + G * (m0 + c);
                             {
-                                const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
+                                const cx ha = bufA1[pad_idx<N>(j)], he = bufE1[pad_idx<N>(j)];
                                 const cx ra = wn.ra[c], re = wn.re[c];
                                 const double wa = wn.wa[c], we = wn.we[c];
                                 v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
                                 v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
                                 const int64_t jo = j + shift;
                                 if (jo >= 0 && jo < N) {
-                                    const cx oa = bufA0[pad_idx((int)jo)], oe = bufE0[pad_idx((int)jo)];
+                                    const cx oa = bufA0[pad_idx<N>((int)jo)], oe = bufE0[pad_idx<N>((int)jo)];
                                     v[2] += wa * (ha.re * oa.re + ha.im * oa.im) + we * (he.re * oe.re + he.im * oe.im);
                                 }
                             }
                             {
-                                const cx oa = bufA0[pad_idx(j)], oe = bufE0[pad_idx(j)];
+                                const cx oa = bufA0[pad_idx<N>(j)], oe = bufE0[pad_idx<N>(j)];
                                 const cx ra = wo.ra[c], re = wo.re[c];
                                 const double wa = wo.wa[c], we = wo.we[c];
                                 v[3] += wa * (oa.re * oa.re + oa.im * oa.im) + we * (oe.re * oe.re + oe.im * oe.im);
@@ -603,17 +655,23 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 }
             } else {   // MODE_UPDATE: r -= a (ADD), r += h (REMOVE), r += o - a (SWAP)
                 const double sgn0 = SWAP ? 1.0 : (mv == GB_REMOVE ? 1.0 : -1.0);
-                if (!SWAP && inband0) {   // common case: no per-bin range checks
-                    double* pA = rA + 2 * (i0w + tid);
-                    double* pE = rE + 2 * (i0w + tid);
+                if (!SWAP) {
+                    double* rC = (ch ? rE : rA) + 2 * (i0w + ht);
+                    if (inband0) {            // common case: no per-bin range checks
 #pragma unroll
-                    for (int m = 0; m < S; m++) {
-                        const int j = tid + G * m;
-                        const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
-                        atomicAdd(pA + 2 * G * m, sgn0 * ha.re);
-                        atomicAdd(pA + 2 * G * m + 1, sgn0 * ha.im);
-                        atomicAdd(pE + 2 * G * m, sgn0 * he.re);
-                        atomicAdd(pE + 2 * G * m + 1, sgn0 * he.im);
+                        for (int m = 0; m < M; m++) {
+                            atomicAdd(rC + 2 * H * m, sgn0 * h[m].re);
+                            atomicAdd(rC + 2 * H * m + 1, sgn0 * h[m].im);
+                        }
+                    } else {
+#pragma unroll
+                        for (int m = 0; m < M; m++) {
+                            const int64_t i = i0w + ht + H * m;
+                            if (i >= 0 && i < a.n_f) {
+                                atomicAdd(rC + 2 * H * m, sgn0 * h[m].re);
+                                atomicAdd(rC + 2 * H * m + 1, sgn0 * h[m].im);
+                            }
+                        }
                     }
                 } else
 #pragma unroll
@@ -621,7 +679,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     const int j = tid + G * m;
                     int64_t i = kmin0 + j - a.k_lo;
                     if (i >= 0 && i < a.n_f) {
-                        const cx ha = bufA0[pad_idx(j)], he = bufE0[pad_idx(j)];
+                        const cx ha = bufA0[pad_idx<N>(j)], he = bufE0[pad_idx<N>(j)];
                         atomicAdd(rA + 2 * i, sgn0 * ha.re);
                         atomicAdd(rA + 2 * i + 1, sgn0 * ha.im);
                         atomicAdd(rE + 2 * i, sgn0 * he.re);
@@ -630,7 +688,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     if (SWAP) {
                         i = rec[NS - 1].kmin + j - a.k_lo;
                         if (i >= 0 && i < a.n_f) {
-                            const cx ha = bufA1[pad_idx(j)], he = bufE1[pad_idx(j)];
+                            const cx ha = bufA1[pad_idx<N>(j)], he = bufE1[pad_idx<N>(j)];
                             atomicAdd(rA + 2 * i, -ha.re);
                             atomicAdd(rA + 2 * i + 1, -ha.im);
                             atomicAdd(rE + 2 * i, -he.re);
@@ -654,7 +712,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
 
 template <int N, bool SWAP>
 constexpr size_t main_smem_bytes() {
-    return (size_t)padded_len(N) * sizeof(cx) * 2 * (SWAP ? 2 : 1);
+    return (size_t)padded_len<N>() * sizeof(cx) * 2 * (SWAP ? 2 : 1);
 }
 
 }  // namespace

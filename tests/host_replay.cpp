@@ -18,22 +18,35 @@ using namespace gbk;
 
 namespace {
 
-template <int N, int G, int R, int Ns>
+// one stage for both channels: threads [0, H) own channel A, threads [H, 2H) own channel E
+template <int N, int R, int Ns, bool LAST>
 void replay_stage(cx* bA, cx* bE, const cx* tw) {
-    std::vector<StageRegs<N, G, R>> regs(G);
-    for (int tid = 0; tid < G; tid++) fft_stage_read<N, G, R>(bA, bE, tid, regs[tid]);
+    constexpr int G = Plan<N>::G, H = G / 2;
+    std::vector<StageRegs<N, R>> regs(G);
+    for (int tid = 0; tid < G; tid++) fft_stage_read<N, R>(tid < H ? bA : bE, tid % H, regs[tid]);
     // (barrier)
-    for (int tid = 0; tid < G; tid++) fft_stage_write<N, G, R, Ns>(bA, bE, tw, tid, regs[tid]);
+    for (int tid = 0; tid < G; tid++) {
+        fft_stage_compute<N, R, Ns>(tw, tid % H, regs[tid]);
+        cx* buf = tid < H ? bA : bE;
+        if (!LAST) {
+            fft_stage_store<N, R, Ns>(buf, tid % H, regs[tid]);
+        } else {   // the kernels keep these in registers: bin j = ht + H m
+            cx h[N / H];
+            fft_last_to_bins<N, R>(regs[tid], h);
+            for (int m = 0; m < N / H; m++) buf[pad_idx<N>(tid % H + H * m)] = h[m];
+        }
+    }
     // (barrier)
 }
-#define REPLAY_STAGE(N_, G_, R_, Ns_) replay_stage<N_, G_, R_, Ns_>(bA, bE, tw);
+#define REPLAY_X(N_, R_, Ns_) replay_stage<N_, R_, Ns_, false>(bA, bE, tw);
+#define REPLAY_L(N_, R_, Ns_) replay_stage<N_, R_, Ns_, true>(bA, bE, tw);
 
 template <int N>
 void replay_fft(cx* bA, cx* bE, const cx* tw);
-template <> void replay_fft<128>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_128(REPLAY_STAGE) }
-template <> void replay_fft<256>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_256(REPLAY_STAGE) }
-template <> void replay_fft<512>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_512(REPLAY_STAGE) }
-template <> void replay_fft<1024>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_1024(REPLAY_STAGE) }
+template <> void replay_fft<128>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_128(REPLAY_X, REPLAY_L) }
+template <> void replay_fft<256>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_256(REPLAY_X, REPLAY_L) }
+template <> void replay_fft<512>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_512(REPLAY_X, REPLAY_L) }
+template <> void replay_fft<1024>(cx* bA, cx* bE, const cx* tw) { GB_FFT_PLAN_1024(REPLAY_X, REPLAY_L) }
 
 template <int N>
 int replay(const double* params, const OrbitParams& op, int path, double* AE, int64_t* kmin, int* used_fast) {
@@ -50,7 +63,7 @@ int replay(const double* params, const OrbitParams& op, int path, double* AE, in
     const bool fast = path == 1 || (path == 2 && ok);
     *used_fast = fast ? 1 : 0;
     *kmin = s.kmin;
-    std::vector<cx> bufA(padded_len(N)), bufE(padded_len(N));
+    std::vector<cx> bufA(padded_len<N>()), bufE(padded_len<N>());
     const double dtN = Tobs / (double)N;
     for (int tid = 0; tid < G; tid++) {
         const double scale = (tid & 1) ? -Tobs / (2.0 * N) : Tobs / (2.0 * N);
@@ -77,16 +90,16 @@ int replay(const double* params, const OrbitParams& op, int path, double* AE, in
                 }
                 slow_sample(s, o, (double)n * dtN, (double)n * (1.0 / N), tau, scale, As, Es);
             }
-            bufA[pad_idx(n)] = {As.re, As.im};
-            bufE[pad_idx(n)] = {Es.re, Es.im};
+            bufA[pad_idx<N>(n)] = {As.re, As.im};
+            bufE[pad_idx<N>(n)] = {Es.re, Es.im};
         }
     }
     replay_fft<N>(bufA.data(), bufE.data(), tw);
     for (int j = 0; j < N; j++) {
-        AE[2 * j] = bufA[pad_idx(j)].re;
-        AE[2 * j + 1] = bufA[pad_idx(j)].im;
-        AE[2 * (N + j)] = bufE[pad_idx(j)].re;
-        AE[2 * (N + j) + 1] = bufE[pad_idx(j)].im;
+        AE[2 * j] = bufA[pad_idx<N>(j)].re;
+        AE[2 * j + 1] = bufA[pad_idx<N>(j)].im;
+        AE[2 * (N + j)] = bufE[pad_idx<N>(j)].re;
+        AE[2 * (N + j) + 1] = bufE[pad_idx<N>(j)].im;
     }
     return 0;
 }
