@@ -39,6 +39,7 @@ WORKLOAD = "cfg5_full_ensemble_sweep_10x36x12000"
 
 # ---- algorithmic work per evaluation (frozen in BASELINE.md before optimisation) ----
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
+NCU_DRAM_BYTES_DLNL = 15.64e9                           # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1_v6
 
 
 def flops_eval(N):
@@ -263,6 +264,8 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     K, W = args.steps, args.warmup
+    # ---- measured DFMA rate of this device (register-only stream; diagnostic entry point of the library)
+    dfma_tflops, dfma_lanes = ctx.measure_fp64_peak(clock_mhz=1965.0)
     # ---- kernel-only arm
     for i in range(W):
         step_device(i)
@@ -332,10 +335,15 @@ def run_ours(args):
     hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
     ach_tf = flops_dlnl / (ms_dlnl * 1e-3) / 1e12
     roofline = {
-        "bound": "alu", "kernel": "gb_main_kernel<N,false> x {1024,512,256,128} (+ gb_prep_kernel) of gb_delta_loglike",
+        "bound": "alu", "kernel": "gb_main_kernel<N,false,true> x {1024,512,256,128} (+ gb_prep_kernel) of gb_delta_loglike",
         "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tf / FP64_PEAK_TFLOPS,
         "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz (no FP64 figure in MEASURED_PEAKS.json)",
-        "flops_per_launch": flops_dlnl, "ms_per_launch": ms_dlnl, "traffic": None,
+        "peak_measured_dfma": dfma_tflops, "frac_of_measured_dfma": ach_tf / dfma_tflops if dfma_tflops > 0 else None,
+        "dfma_lanes_per_clk_sm_at_1965mhz": dfma_lanes,
+        "flops_per_launch": flops_dlnl, "ms_per_launch": ms_dlnl,
+        # DRAM bytes (read + write) of the four delta-lnL kernels of one step, from the ncu --set full capture
+        # profiles/r1_v6_ncu_full_summary.csv (full workload only); algorithmic bytes are in "hbm"
+        "traffic": NCU_DRAM_BYTES_DLNL if full else None, "traffic_unit": "bytes per delta-lnL call (ncu, r1_v6)",
         "hbm": {"achieved": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "bytes_per_launch": bytes_dlnl},

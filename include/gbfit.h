@@ -100,6 +100,18 @@ const char *gb_version(void);
 int64_t gb_launch_count(const gb_ctx *ctx);
 
 /*
+ * gb_measure_fp64_peak -- diagnostic, not on the hot path: times a register-only stream of independent DFMAs
+ * (8 chains per thread, 512 threads per SM, every SM) on the context's device and returns the sustained rate.
+ * This is the measured denominator of the "alu" roofline bench.py reports beside the nominal
+ * 148 SMs x 64 DFMA/clk x 2 x clock figure (the delta-lnL path is bound by the plain FP64 pipe).
+ *   tflops_out            HOST, 2 flop per DFMA
+ *   dfma_per_clk_sm_out   HOST, DFMA lanes per SM per clock at clock_mhz (may be NULL)
+ *   clock_mhz             SM clock to normalise by (e.g. the max SM clock); ignored if dfma_per_clk_sm_out is NULL
+ * Synchronises `stream`.  Returns GB_OK or GB_ERR_INVALID / GB_ERR_CUDA.
+ */
+int gb_measure_fp64_peak(gb_ctx *ctx, double *tflops_out, double *dfma_per_clk_sm_out, double clock_mhz, void *stream);
+
+/*
  * gb_waveform -- A/E windows of B sources.
  *   params   [B][8] f64
  *   N        window length used for every row when n_bins == NULL; one of 128, 256, 512, 1024

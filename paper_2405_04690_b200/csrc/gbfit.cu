@@ -717,6 +717,25 @@ constexpr size_t main_smem_bytes() {
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------ FP64 peak
+// 8 independent DFMA chains per thread, registers only (gb_measure_fp64_peak)
+__global__ void __launch_bounds__(128) gb_dfma_peak_kernel(double* sink, int iters, double a, double b) {
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) x[i] = threadIdx.x * 1e-3 + i;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int r = 0; r < 8; r++) {
+#pragma unroll
+            for (int i = 0; i < 8; i++) x[i] = fma(x[i], a, b);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) s += x[i];
+    if (s == 12345.678) sink[0] = s;   // never true: keeps the chains alive
+}
+
 // ------------------------------------------------------------------------------------------------ context
 struct gb_ctx {
     gb_config cfg;
@@ -1024,6 +1043,36 @@ void gb_destroy(gb_ctx* ctx) {
 const char* gb_last_error(const gb_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
 
 int64_t gb_launch_count(const gb_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int gb_measure_fp64_peak(gb_ctx* ctx, double* tflops_out, double* dfma_per_clk_sm_out, double clock_mhz, void* stream) {
+    if (!ctx || !tflops_out) return GB_ERR_INVALID;
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    double* d_sink = nullptr;
+    GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&d_sink), sizeof(double)));
+    cudaEvent_t e0, e1;
+    GB_CUDA(ctx, cudaEventCreate(&e0));
+    GB_CUDA(ctx, cudaEventCreate(&e1));
+    const int iters = 8192, threads = 128, grid = ctx->num_sms * 4;
+    float best = 0.0f;
+    for (int rep = 0; rep < 4; rep++) {   // first repetition warms up
+        GB_CUDA(ctx, cudaEventRecord(e0, st));
+        gb_dfma_peak_kernel<<<grid, threads, 0, st>>>(d_sink, iters, 1.0000001, 1e-9);
+        GB_CUDA(ctx, cudaEventRecord(e1, st));
+        GB_CUDA(ctx, cudaEventSynchronize(e1));
+        float ms = 0.0f;
+        GB_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && (best == 0.0f || ms < best)) best = ms;
+    }
+    ctx->launches += 4;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_sink);
+    const double dfma = (double)grid * threads * (double)iters * 8.0 * 8.0;
+    *tflops_out = 2.0 * dfma / (best * 1e-3) / 1e12;
+    if (dfma_per_clk_sm_out) *dfma_per_clk_sm_out = clock_mhz > 0 ? dfma / (best * 1e-3) / ctx->num_sms / (clock_mhz * 1e6) : 0.0;
+    return GB_OK;
+}
 
 int gb_check(gb_ctx* ctx, void* stream) {
     if (!ctx) return GB_ERR_INVALID;

@@ -20,7 +20,7 @@ ADD, REMOVE, SWAP = 0, 1, 2
 GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
-           "gb_launch_count", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
+           "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
            "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host")
 
 
@@ -74,6 +74,8 @@ def lib() -> C.CDLL:
         L.gb_version.restype = C.c_char_p
         L.gb_launch_count.argtypes = [vp]
         L.gb_launch_count.restype = i64
+        L.gb_measure_fp64_peak.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, vp]
+        L.gb_measure_fp64_peak.restype = ci
         wf = [vp, vp, i64, ci, vp, ci, vp, vp, vp]
         dl = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, vp, vp, vp]
         ru = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, vp, ci, vp, i64, vp]
@@ -218,6 +220,13 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().gb_launch_count(self._h))
+
+    def measure_fp64_peak(self, clock_mhz: float = 0.0, stream=None):
+        """Diagnostic: sustained DFMA rate of the device -> (TFLOP/s, DFMA lanes per SM per clock at clock_mhz)."""
+        tf, lanes = C.c_double(0.0), C.c_double(0.0)
+        self._ok(lib().gb_measure_fp64_peak(self._h, C.byref(tf), C.byref(lanes), C.c_double(clock_mhz),
+                                            _stream_ptr(stream, self.device)))
+        return float(tf.value), float(lanes.value)
 
     def check(self, stream=None):
         """Synchronise the stream and raise if any row of an earlier call was invalid."""

@@ -391,6 +391,73 @@ def test_highest_bins_up_to_nyquist(oracle, torch_cuda, gb):
         ctx.check()
 
 
+# ----------------------------------------------------- fast / general slow-part dispatch (csrc/gb_fast.cuh)
+def test_rows_inside_and_outside_the_fast_path_limits_in_one_batch(oracle, torch_cuda, gb):
+    """gb_prep_kernel routes a row to the polynomial fast path or to the general kernels by its parameters
+    (f0 > 30.5 mHz, |fdot| >~ 5e-13, |phi0| in the thousands, f0 <= 0 go the general way).  One batch with
+    both kinds, mixed window lengths and all three moves must match the oracle row by row."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=96, n_walkers=3)
+    pn, po = wl.params_new.copy(), wl.params_old.copy()
+    move = wl.move.copy()
+    move[::4] = gbfit.SWAP
+    pn[::4] = po[::4]
+    pn[::4, 1] += 3e-9
+    pn[::4, 3] += 0.02
+    for arr in (pn, po):                # every 3rd row leaves the fast limits in one of three ways
+        arr[1::6, 2] = 4e-12            # |fdot| beyond the first-order limit
+        arr[2::6, 3] += 3500.0          # phase beyond the Cody-Waite range of the fast path
+        arr[4::12, 1] = 4.2e-2          # above 30.5 mHz (window outside the stored band: delta lnL = 0)
+    nb = wl.n_bins.copy()
+    nb[4::12] = 1024
+    resid = wl.resid()
+    data, d_resid = upload(torch, gbfit, wl, resid)
+    od = oracle.Data(resid.copy(), wl.psd, wl.k_lo, walker_psd=wl.walker_psd)
+    ref = oracle.delta_loglike(oracle.Config(), od, pn, po, wl.walker_index, move=move, n_bins=nb,
+                               nthreads=oracle.max_threads())
+    got = ctx.delta_loglike(data, dev(torch, pn), dev(torch, po), dev(torch, wl.walker_index),
+                            move=dev(torch, move), n_bins=dev(torch, nb)).cpu().numpy()
+    ctx.check()
+    assert np.abs(got - ref).max() <= TOL_DLNL
+    refw, refk = oracle.waveform_batch(oracle.Config(), pn, n_bins=nb, nthreads=oracle.max_threads())
+    gw, gk = ctx.waveform(dev(torch, pn), n_bins=dev(torch, nb), Nmax=int(refw.shape[2]))
+    ctx.check()
+    assert np.array_equal(gk.cpu().numpy(), refk)
+    assert wf_err(gw.cpu().numpy(), refw, nb) <= TOL_WF
+    acc = (np.arange(wl.B) % 2 == 0).astype(np.uint8)
+    ctx.residual_update(data, dev(torch, pn), dev(torch, po), dev(torch, wl.walker_index), move=dev(torch, move),
+                        accepted=dev(torch, acc), n_bins=dev(torch, nb))
+    ctx.check()
+    oracle.residual_update(oracle.Config(), od, pn, po, wl.walker_index, move=move, accepted=acc, n_bins=nb,
+                           nthreads=oracle.max_threads())
+    dref = od.resid - resid
+    assert np.abs((d_resid.cpu().numpy() - resid) - dref).max() <= 1e-9 * np.abs(dref).max()
+
+
+def test_sources_along_link_directions(oracle, torch_cuda, gb):
+    """kappa -> +-1 at some time samples: the fast path's shared reciprocal is singular there and the sinc
+    series takes over for that link (a degenerate case of the restructured arithmetic)."""
+    gbfit, ctx = gb
+    cfg = oracle.Config()
+    rows = []
+    for t in (0.0, 0.31 * cfg.Tobs, 0.77 * cfg.Tobs):
+        x = oracle.orbits(cfg, float(t))
+        for (r, s_), sign in (((0, 1), 1.0), ((2, 0), -1.0), ((1, 2), 1.0)):
+            n = (x[r] - x[s_]) / cfg.armlength
+            kdir = sign * n / np.linalg.norm(n)          # k = -(cos b cos l, cos b sin l, sin b)
+            lam = np.arctan2(-kdir[1], -kdir[0]) % (2 * np.pi)
+            for f0 in (2.5e-4, 2e-3, 1.2e-2):
+                rows.append([1e-22, f0, 2e-17, 1.0, 0.3, 0.7, lam, -kdir[2]])
+    p = np.array(rows)
+    nb = n_bins_for_f0(p[:, 1])
+    ref, refk = oracle.waveform_batch(cfg, p, n_bins=nb, nthreads=oracle.max_threads())
+    got, k = ctx.waveform(dev(torch_cuda, p), n_bins=dev(torch_cuda, nb), Nmax=int(ref.shape[2]))
+    ctx.check()
+    assert np.array_equal(k.cpu().numpy(), refk)
+    assert wf_err(got.cpu().numpy(), ref, nb) <= TOL_WF
+
+
 # ------------------------------------------------------------------------ config 5: full-size launch
 def test_config5_full_size_sampled(oracle, torch_cuda, gb):
     """The bench's launch configuration: 360 residuals (10.8 GB), 4.32 M ADD-type evaluations in one call,
