@@ -213,3 +213,73 @@ def make_workload(config: int, B: Optional[int] = None, n_walkers: Optional[int]
         return Workload(5, "cfg5_ensemble_sweep", TOBS, DT, k_lo, n_f, nw, psd, walker_psd, p, None,
                         w, None, ADD, 0, n_bins_for_f0(p[:, 1]), acc, sc)
     raise ValueError(f"unknown config {config}")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Band tasks for the Algorithm-1 primitive: sub-bands of N bins
+# (PAPER.md:288), one task per (walker, ODD sub-band) -- the paper's odd/even schedule -- staging
+# sub-bands b-1, b, b+1; n_src sources with f0 inside sub-band b; n_prop proposals "theta' = theta + jitter" on
+# randomly picked sources of the band (PAPER.md:595 randint), each with its log-uniform draw.
+_S_BAND = 7
+
+
+@dataclass
+class BandTasks:
+    N: int
+    tasks: dict                 # equal-length arrays: walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first,
+                                # write_back, beta
+    params: np.ndarray          # [n_src_total, 8] current sources (in/out)
+    prop_k: np.ndarray          # [n_prop_total] int32 index of the source within its band
+    prop_params: np.ndarray     # [n_prop_total, 8]
+    prop_logq: np.ndarray       # [n_prop_total] log prior/proposal ratio term (0 here)
+    prop_logu: np.ndarray       # [n_prop_total] log of the uniform draw
+    max_stage: int
+
+
+def make_band_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_src: int, n_prop: int,
+                    betas=(1.0, 0.6), stream: int = 0, amp_lo: float = 2e-23, amp_hi: float = 2e-22) -> BandTasks:
+    """n_bands odd sub-bands per walker of `wl`, starting near f_lo.  Deterministic in (wl.config, N, stream)."""
+    g = _rng(wl.config, 100 * _S_BAND + stream + N)
+    T = wl.Tobs
+    kb0 = int(np.ceil(f_lo * T / N)) * N                       # global bin of sub-band 0 (a multiple of N)
+    nw = wl.n_walkers
+    nt = nw * n_bands
+    walker = np.repeat(np.arange(nw, dtype=np.int32), n_bands)
+    b = np.tile(2 * np.arange(n_bands, dtype=np.int64) + 1, nw)  # odd sub-bands
+    tasks = {
+        "walker": walker,
+        "n_src": np.full(nt, n_src, np.int32),
+        "src_begin": (np.arange(nt) * n_src).astype(np.int32),
+        "n_prop": np.full(nt, n_prop, np.int32),
+        "prop_begin": (np.arange(nt) * n_prop).astype(np.int32),
+        "n_stage": np.full(nt, 3 * N, np.int32),
+        "k_first": kb0 + (b - 1) * N,
+        "write_back": np.ones(nt, np.int32),
+        "beta": np.asarray(betas, np.float64)[walker % len(betas)],
+    }
+    u = g.random((nt, n_src, 8))
+    p = np.empty((nt, n_src, 8))
+    p[..., 0] = amp_lo * (amp_hi / amp_lo) ** u[..., 0]
+    p[..., 1] = (kb0 + (b[:, None] + u[..., 1]) * N) / T          # f0 inside sub-band b
+    p[..., 2] = (2.0 * u[..., 2] - 1.0) * 1e-16
+    p[..., 3] = 2.0 * np.pi * u[..., 3]
+    p[..., 4] = 2.0 * u[..., 4] - 1.0
+    p[..., 5] = np.pi * u[..., 5]
+    p[..., 6] = 2.0 * np.pi * u[..., 6]
+    p[..., 7] = 2.0 * u[..., 7] - 1.0
+    params = np.ascontiguousarray(p.reshape(nt * n_src, 8))
+    prop_k = g.integers(0, n_src, (nt, n_prop)).astype(np.int32)
+    z = g.standard_normal((nt, n_prop, 8))
+    base = p[np.arange(nt)[:, None], prop_k]                     # proposals jitter the INITIAL parameters
+    q = base.copy()
+    q[..., 0] = base[..., 0] * (1.0 + 0.02 * z[..., 0])
+    q[..., 1] = base[..., 1] + 2e-9 * z[..., 1]
+    q[..., 3] = base[..., 3] + 0.05 * z[..., 3]
+    q[..., 5] = base[..., 5] + 0.05 * z[..., 5]
+    q[..., 6] = base[..., 6] + 0.02 * z[..., 6]
+    q[..., 4] = np.clip(base[..., 4] + 0.02 * z[..., 4], -1.0, 1.0)
+    q[..., 7] = np.clip(base[..., 7] + 0.02 * z[..., 7], -1.0, 1.0)
+    logu = np.log(g.random((nt, n_prop)))
+    return BandTasks(N, tasks, params, np.ascontiguousarray(prop_k.reshape(-1)),
+                     np.ascontiguousarray(q.reshape(nt * n_prop, 8)), np.zeros(nt * n_prop),
+                     np.ascontiguousarray(logu.reshape(-1)), 3 * N)

@@ -402,6 +402,93 @@ double gbo_inner_windows(const gbo_config *c, const gbo_data *d, int psd_row,
     return o7_inner(c, d, psd_row, bA, bE, kb, nb, cA, cE, kc, nc);
 }
 
+/* ---- Algorithm 1: sequential proposals of one band against a staged residual --------
+ * One task = one band j = (t, w, b): the residual r' of walker `walker` on the staged bins
+ * [k_first, k_first + n_stage) (the paper's sub-bands b-1, b, b+1; reading F1-a: the caller's
+ * per-(t,w) residual already has the current sources subtracted, r = d - H), the band's n_src sources
+ * params[src_begin ..], and n_prop proposals applied IN ORDER: proposal p replaces
+ * source k_p by theta'_p; delta lnL by Eq. 5 with every inner product restricted to the
+ * staged bins (and the stored band); accepted iff beta * dlnL + logq_p >= logu_p (Eq. 13
+ * in log form with the tempered likelihood of PAPER.md:674; logq_p = log prior/proposal ratio and logu_p =
+ * log of the uniform draw are inputs: the random numbers of the method are passed in).  On acceptance
+ * theta_j[k] <- theta', r' <- r' + h(theta_k) - h(theta'_k).  If write_back, the net
+ * change of r' is added to the walker's stored residual at the end.  Tasks are processed
+ * one after the other in task order.                                                                   */
+typedef struct {
+    int32_t walker, n_src, src_begin, n_prop, prop_begin, n_stage;
+    int64_t k_first;
+    int32_t write_back, reserved;
+    double beta;
+} gbo_band_task;
+
+int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks, int64_t n_tasks, int N,
+                   double *params, const int32_t *prop_k, const double *prop_params, const double *prop_logq,
+                   const double *prop_logu, uint8_t *accepted_out, double *dlnL_out) {
+    if (!valid_N(N)) return GBO_ERR_INVALID;
+    double *h = (double *)malloc(sizeof(double) * 8 * (size_t)N);
+    double *oA = h, *oE = h + 2 * (size_t)N, *aA = h + 4 * (size_t)N, *aE = h + 6 * (size_t)N;
+    for (int64_t it = 0; it < n_tasks; it++) {
+        const gbo_band_task *t = &tasks[it];
+        if (t->walker < 0 || t->walker >= d->n_walkers || t->n_stage < 0) { free(h); return GBO_ERR_INVALID; }
+        /* staged bins that are stored: global bins [lo, hi) */
+        int64_t lo = t->k_first > d->k_lo ? t->k_first : d->k_lo;
+        int64_t hi = t->k_first + t->n_stage < d->k_lo + d->n_f ? t->k_first + t->n_stage : d->k_lo + d->n_f;
+        int64_t n = hi > lo ? hi - lo : 0;
+        /* r' and the PSD of the walker on those bins, as a one-walker data view */
+        double *rv = (double *)malloc(sizeof(double) * 4 * (size_t)(n > 0 ? n : 1));
+        double *r0 = (double *)malloc(sizeof(double) * 4 * (size_t)(n > 0 ? n : 1));
+        double *sv = (double *)malloc(sizeof(double) * 2 * (size_t)(n > 0 ? n : 1));
+        int row = psd_row_of(d, t->walker);
+        for (int ch = 0; ch < 2; ch++) {
+            const double *r = resid_ch(d, t->walker, ch) + 2 * (lo - d->k_lo);
+            const double *S = d->psd + ((size_t)row * 2 + (size_t)ch) * (size_t)d->n_f + (lo - d->k_lo);
+            for (int64_t i = 0; i < n; i++) {
+                rv[2 * ((size_t)ch * n + i)] = r[2 * i];
+                rv[2 * ((size_t)ch * n + i) + 1] = r[2 * i + 1];
+                sv[(size_t)ch * n + i] = S[i];
+            }
+        }
+        memcpy(r0, rv, sizeof(double) * 4 * (size_t)n);
+        gbo_data v = {rv, sv, NULL, lo, n, 1, 1, d->psd_is_inverse};
+        for (int p = 0; p < t->n_prop && n > 0; p++) {
+            int64_t ip = t->prop_begin + p;
+            int k = prop_k[ip];
+            if (k < 0 || k >= t->n_src) { free(rv); free(r0); free(sv); free(h); return GBO_ERR_INVALID; }
+            double *theta_k = params + 8 * ((size_t)t->src_begin + k);
+            const double *theta_p = prop_params + 8 * ip;
+            double dl = 0.0;
+            o8_row(c, &v, theta_p, theta_k, 0, GBO_SWAP, N, &dl, NULL);            /* Eq. 5 against r' */
+            int acc = t->beta * dl + prop_logq[ip] >= prop_logu[ip];
+            dlnL_out[ip] = dl;
+            accepted_out[ip] = (uint8_t)acc;
+            if (acc) {
+                int64_t ko, ka;
+                gbo_waveform(c, theta_k, N, oA, oE, &ko);
+                gbo_waveform(c, theta_p, N, aA, aE, &ka);
+                add_window(&v, 0, oA, oE, ko, N, +1.0);                             /* r' += h(theta_k)  */
+                add_window(&v, 0, aA, aE, ka, N, -1.0);                             /* r' -= h(theta'_k) */
+                memcpy(theta_k, theta_p, sizeof(double) * 8);
+            }
+        }
+        for (int p = 0; p < t->n_prop && n <= 0; p++) {   /* nothing staged: every dlnL is 0 */
+            int64_t ip = t->prop_begin + p;
+            int acc = prop_logq[ip] >= prop_logu[ip];
+            dlnL_out[ip] = 0.0;
+            accepted_out[ip] = (uint8_t)acc;
+            if (acc) memcpy(params + 8 * ((size_t)t->src_begin + prop_k[ip]), prop_params + 8 * ip, sizeof(double) * 8);
+        }
+        if (t->write_back) {
+            for (int ch = 0; ch < 2; ch++) {
+                double *r = (double *)resid_ch(d, t->walker, ch) + 2 * (lo - d->k_lo);
+                for (int64_t i = 0; i < 2 * n; i++) r[i] += rv[2 * (size_t)ch * n + i] - r0[2 * (size_t)ch * n + i];
+            }
+        }
+        free(rv); free(r0); free(sv);
+    }
+    free(h);
+    return GBO_OK;
+}
+
 /* orbit positions at time t, row-major [3][3] (exposed for the orbit pin) */
 void gbo_orbits(const gbo_config *c, double t, double *x_out) {
     double x[3][3];

@@ -179,6 +179,32 @@ def residual_update(cfg: Config, data: Data, params_new, params_old, walker_inde
         raise ValueError(f"gbo_residual_update rc={rc}")
 
 
+_BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
+                       ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
+                       ("write_back", np.int32), ("reserved", np.int32), ("beta", np.float64)], align=True)
+
+
+def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, prop_params, prop_logq, prop_logu):
+    """Algorithm 1, task after task, proposal after proposal.  `tasks` is a dict of equal-length
+    arrays (walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta).  `params` [n_src_total, 8]
+    and data.resid are updated in place.  Returns (accepted[n_prop_total] uint8, dlnL[n_prop_total])."""
+    n = len(tasks["walker"])
+    t = np.zeros(n, _BAND_TASK)
+    for key in ("walker", "n_src", "src_begin", "n_prop", "prop_begin", "n_stage", "k_first", "write_back", "beta"):
+        t[key] = tasks[key]
+    assert params.dtype == np.float64 and params.flags.c_contiguous
+    pk = np.ascontiguousarray(prop_k, dtype=np.int32)
+    pp, lq, lu = _f64(prop_params), _f64(prop_logq), _f64(prop_logu)
+    acc = np.zeros(pk.shape[0], np.uint8)
+    dl = np.zeros(pk.shape[0], np.float64)
+    cc, dd = cfg.c(), data.c()
+    rc = lib().gbo_band_sweep(C.byref(cc), C.byref(dd), _ptr(t), C.c_int64(n), C.c_int(N), _ptr(params), _ptr(pk),
+                              _ptr(pp), _ptr(lq), _ptr(lu), _ptr(acc), _ptr(dl))
+    if rc != 0:
+        raise ValueError(f"gbo_band_sweep rc={rc}")
+    return acc, dl
+
+
 def inner_windows(cfg: Config, data: Data, psd_row: int, bA, bE, kb: int, cA, cE, kc: int) -> float:
     """<b|c> of two explicit windows (step O7)."""
     bA, bE, cA, cE = (np.ascontiguousarray(z, dtype=np.complex128) for z in (bA, bE, cA, cE))

@@ -360,3 +360,111 @@ def test_p7_noise_normalisation_and_psd_values():
     for f, S in g:
         assert abs(instrument_psd(f) / S - 1.0) < 5e-4
     assert band_bins(1e-3, 4e-3) == (31458, 94372) and band_bins(0.1e-3, 30e-3) == (3146, 940573)
+
+
+# ------------------------------------------------------------- Algorithm 1, row f1
+def _band_case(oracle, N=128, n_bands=3, n_src=4, n_prop=10, f_lo=6e-4):
+    from gb_inputs import make_workload, make_band_tasks
+    wl = make_workload(3, B=1, n_walkers=2)
+    bt = make_band_tasks(wl, N, f_lo, n_bands, n_src, n_prop)
+    resid = wl.resid()
+    return wl, bt, resid
+
+
+def _staged_lnL(wl, resid, w, k_first, n_stage):
+    """-1/2 <r|r> on the staged bins straight from the definition (Eq. 1-2)."""
+    i0 = k_first - wl.k_lo
+    r = resid[w, :, i0:i0 + n_stage]
+    S = wl.psd[wl.psd_row_of(w), :, i0:i0 + n_stage]
+    return -0.5 * (4.0 / wl.Tobs) * float((np.abs(r) ** 2 / S).sum())
+
+
+def test_band_sweep_sum_of_accepted_dlnL_is_the_lnL_difference(oracle):
+    """Eq. 5 is a likelihood DIFFERENCE: over a whole task the accepted delta lnL must add up to
+    lnL(final r') - lnL(initial r') computed from the definition on the staged bins."""
+    wl, bt, resid = _band_case(oracle)
+    cfg = oracle.Config()
+    data = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params = bt.params.copy()
+    t = bt.tasks
+    acc = np.zeros(bt.prop_k.size, np.uint8)
+    dl = np.zeros(bt.prop_k.size)
+    for i in range(len(t["walker"])):      # task by task (staged ranges of neighbouring tasks share a sub-band)
+        one = {k: v[i:i + 1] for k, v in t.items()}
+        l0 = _staged_lnL(wl, data.resid, t["walker"][i], t["k_first"][i], t["n_stage"][i])
+        a_i, d_i = oracle.band_sweep(cfg, data, one, bt.N, params, bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
+        l1 = _staged_lnL(wl, data.resid, t["walker"][i], t["k_first"][i], t["n_stage"][i])
+        sl = slice(t["prop_begin"][i], t["prop_begin"][i] + t["n_prop"][i])
+        acc[sl], dl[sl] = a_i[sl], d_i[sl]
+        tot = float(dl[sl][acc[sl] != 0].sum())
+        assert abs(tot - (l1 - l0)) <= 1e-9 * max(1.0, abs(l0)), (i, tot, l1 - l0)
+    assert 0 < acc.sum() < acc.size                       # a mixture of accepted and rejected proposals
+    # all tasks in one call give the same decisions, values and residuals as task-by-task calls
+    data2 = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params2 = bt.params.copy()
+    acc2, dl2 = oracle.band_sweep(cfg, data2, t, bt.N, params2, bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
+    assert np.array_equal(acc2, acc) and np.array_equal(dl2, dl) and np.array_equal(params2, params)
+    assert np.array_equal(data2.resid, data.resid)
+    # the acceptance rule itself (Eq. 13 in log form, tempered): beta dlnL + logq >= logu
+    beta = np.repeat(t["beta"], t["n_prop"])
+    assert np.array_equal(acc != 0, beta * dl + bt.prop_logq >= bt.prop_logu)
+
+
+def test_band_sweep_all_accepted_telescopes_and_all_rejected_is_identity(oracle):
+    wl, bt, resid = _band_case(oracle, N=256, f_lo=2e-3)
+    cfg = oracle.Config()
+    t = bt.tasks
+    # every proposal accepted: r' changes by h(initial) - h(final) of each source, whatever the path
+    data = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params = bt.params.copy()
+    acc, _ = oracle.band_sweep(cfg, data, t, bt.N, params, bt.prop_k, bt.prop_params, bt.prop_logq,
+                               np.full_like(bt.prop_logu, -np.inf))
+    assert acc.all()
+    expect = resid.copy()
+    for i in range(len(t["walker"])):
+        w, k0, ns = int(t["walker"][i]), int(t["k_first"][i]), int(t["n_stage"][i])
+        for s in range(t["n_src"][i]):
+            row = t["src_begin"][i] + s
+            hits = np.nonzero(bt.prop_k[t["prop_begin"][i]:t["prop_begin"][i] + t["n_prop"][i]] == s)[0]
+            if hits.size == 0:
+                assert np.array_equal(params[row], bt.params[row])
+                continue
+            last = t["prop_begin"][i] + hits[-1]
+            assert np.array_equal(params[row], bt.prop_params[last])
+            for p, sign in ((bt.params[row], +1.0), (bt.prop_params[last], -1.0)):
+                A, E, kmin = oracle.waveform(cfg, p, bt.N)
+                for ch, h in enumerate((A, E)):
+                    for j in range(bt.N):
+                        k = kmin + j
+                        if k0 <= k < k0 + ns:
+                            expect[w, ch, k - wl.k_lo] += sign * h[j]
+    scale = np.abs(expect - resid).max()
+    assert scale > 0 and np.abs(data.resid - expect).max() <= 1e-12 * scale + 4e-16 * np.abs(resid).max()
+    # every proposal rejected: nothing changes; write_back = 0 leaves the stored residual alone even if accepted
+    data = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params = bt.params.copy()
+    acc, _ = oracle.band_sweep(cfg, data, t, bt.N, params, bt.prop_k, bt.prop_params, bt.prop_logq,
+                               np.full_like(bt.prop_logu, np.inf))
+    assert not acc.any() and np.array_equal(params, bt.params) and np.array_equal(data.resid, resid)
+    t2 = dict(t, write_back=np.zeros_like(t["write_back"]))
+    params = bt.params.copy()
+    acc, _ = oracle.band_sweep(cfg, data, t2, bt.N, params, bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
+    assert acc.any() and np.array_equal(data.resid, resid) and not np.array_equal(params, bt.params)
+
+
+def test_band_sweep_single_proposal_is_eq5_on_the_staged_bins(oracle):
+    """One proposal per task: delta lnL = Eq. 5 evaluated with the residual zeroed outside the staged bins and a
+    huge PSD there (so those bins drop out of every inner product)."""
+    wl, bt, resid = _band_case(oracle, N=128, n_bands=2, n_src=2, n_prop=1)
+    cfg = oracle.Config()
+    t = bt.tasks
+    data = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    acc, dl = oracle.band_sweep(cfg, data, t, bt.N, bt.params.copy(), bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
+    for i in range(len(t["walker"])):
+        w, k0, ns = int(t["walker"][i]), int(t["k_first"][i]), int(t["n_stage"][i])
+        psd = np.full_like(wl.psd, 1e300)
+        psd[:, :, k0 - wl.k_lo:k0 - wl.k_lo + ns] = wl.psd[:, :, k0 - wl.k_lo:k0 - wl.k_lo + ns]
+        old = bt.params[t["src_begin"][i] + bt.prop_k[t["prop_begin"][i]]]
+        ref = oracle.delta_loglike(cfg, oracle.Data(resid.copy(), psd, wl.k_lo), bt.prop_params[t["prop_begin"][i]][None],
+                                   old[None], np.array([w], np.int32), move_all=oracle.SWAP, N=bt.N)[0]
+        assert abs(dl[t["prop_begin"][i]] - ref) <= 1e-9 * max(1.0, abs(ref))
