@@ -168,6 +168,48 @@ int gb_residual_update_host(gb_ctx *ctx, const gb_data *data, const double *para
                             const int8_t *move /*HOST*/, int move_all, const uint8_t *accepted /*HOST*/,
                             int N, const int32_t *n_bins /*HOST*/, int64_t B, void *stream);
 
+/*
+ * gb_band_sweep -- Algorithm 1 of the paper ("Galaxy sampling algorithm"): for each band task the
+ * walker's residual on the staged bins is held on chip and the task's proposals are applied IN ORDER, each one a swap
+ * theta_k -> theta'_k evaluated by Eq. 5 against the staged residual r', accepted iff
+ *     beta * dlnL + logq >= logu          (Eq. 13, in log form; tempering PAPER.md:674)
+ * and, when accepted, r' <- r' + h(theta_k) - h(theta'_k), theta_j[k] <- theta'_k.  The random
+ * numbers of the method are inputs: logu = log of the uniform draw, logq = log prior / proposal-density ratio of the
+ * proposal (0 for a symmetric in-model move); proposal generation (stretch / group / RJ) is
+ * the caller's.  An RJ add or remove is the paper's amplitude switch: amp = 0 on one side.
+ *
+ *   tasks        [n_tasks] DEVICE array of gb_band_task
+ *   N            window length of every source in this call (128, 256, 512, 1024); group bands by N
+ *   max_stage    >= every task's n_stage, <= GB_BAND_MAX_STAGE; sizes the on-chip staging area
+ *   params       [sum n_src][8] DEVICE, in/out: the current sources of every band (task i owns rows
+ *                src_begin .. src_begin + n_src)
+ *   prop_k       [sum n_prop] DEVICE int32: which source of its band proposal p replaces (0 .. n_src-1)
+ *   prop_params  [sum n_prop][8], prop_logq [sum n_prop], prop_logu [sum n_prop]   DEVICE f64
+ *   accepted_out [sum n_prop] DEVICE uint8, dlnL_out [sum n_prop] DEVICE f64 (the T = 1 delta lnL of every proposal)
+ * Inner products use only the staged bins that lie in the stored band.  With write_back != 0 every accepted change
+ * is also added to data->resid with FP64 atomics, so concurrent tasks of one walker must not propose into the same
+ * bins: the paper's odd/even sub-band schedule -- one call per parity -- guarantees it.  Tasks are
+ * independent and run concurrently; the proposals of one task run sequentially.
+ * Errors: GB_ERR_INVALID for bad arguments; a task with a bad walker / n_stage or a proposal with a bad prop_k sets
+ * the sticky row flag (gb_check) and gives NaN.  Asynchronous on `stream`.
+ */
+#define GB_BAND_MAX_STAGE 3072
+typedef struct {
+    int32_t walker;      /* residual row                                                        */
+    int32_t n_src;       /* g_j: sources of the band                                            */
+    int32_t src_begin;   /* first row of the band in params                                     */
+    int32_t n_prop;      /* proposals of the band                                               */
+    int32_t prop_begin;  /* first row of the band in prop_*                                     */
+    int32_t n_stage;     /* staged bins                                                         */
+    int64_t k_first;     /* global bin of staged bin 0                                          */
+    int32_t write_back;  /* != 0: accepted changes also go to data->resid                       */
+    int32_t reserved;
+    double beta;         /* inverse temperature of the band's chain                             */
+} gb_band_task;
+int gb_band_sweep(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, int64_t n_tasks, int N, int max_stage,
+                  double *params, const int32_t *prop_k, const double *prop_params, const double *prop_logq,
+                  const double *prop_logu, uint8_t *accepted_out, double *dlnL_out, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -1,0 +1,219 @@
+// gb_band.cuh -- Algorithm 1 of the paper as a kernel.
+// Included by gbfit.cu inside its anonymous namespace, after slow_part / fft_store / group_reduce.
+//
+// One CTA owns one band task j = (t, w, b) at a time: it stages the walker's residual r' and the noise weights
+// 1/S_n of the task's bins [k_first, k_first + n_stage) (the paper's sub-bands b-1, b, b+1) in shared memory,
+// then runs the task's proposals IN ORDER.  Each proposal is the SWAP evaluation of the batched path (two slow
+// parts, two shared-memory FFTs, the five sums of Eq. 5) with the inner products read from the staged copy
+// instead of global memory, the accept / reject decision beta dlnL + logq >= logu taken by thread 0 in FP64, and,
+// when accepted, r' <- r' + h(theta_k) - h(theta'_k) in shared memory, theta_j[k] <- theta'_k in the caller's
+// parameter array, and (write_back) the same window change added to the stored residual with FP64 atomics --
+// the paper's "remove starting waveforms, add new group waveforms" of lines :608-613 done incrementally, so two
+// bands of one walker that share a neighbour sub-band (b and b+2) never overwrite each other.
+// Parallelism is across tasks only (the paper's design: the proposals of a band are a sequential chain).
+#pragma once
+
+struct BandArgs {
+    const gb_band_task* tasks;
+    int64_t n_tasks;
+    double* params;
+    const int32_t* prop_k;
+    const double* prop_params;
+    const double* prop_logq;
+    const double* prop_logu;
+    uint8_t* accepted_out;
+    double* dlnL_out;
+    const double* orbit;
+    const cx* tw;
+    double* resid;
+    const double* psd;
+    const int32_t* walker_psd;
+    int64_t k_lo, n_f;
+    int32_t n_walkers, n_psd, psd_is_inverse, max_stage;
+    double Tobs, tau, Rmax;
+    int64_t kmax;
+    int32_t* errflag;
+};
+
+template <int N>
+constexpr size_t band_smem_bytes(int max_stage) {
+    return (size_t)padded_len<N>() * sizeof(cx) * 4 + (size_t)max_stage * 48;
+}
+
+template <int N>
+__global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
+    constexpr int G = Plan<N>::G;
+    constexpr int S = N / G;
+    constexpr int PN = padded_len<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx* bufA0 = reinterpret_cast<cx*>(smem_raw);      // old source theta_k
+    cx* bufE0 = bufA0 + PN;
+    cx* bufA1 = bufE0 + PN;                           // proposed source theta'_k
+    cx* bufE1 = bufA1 + PN;
+    cx* sRA = bufE1 + PN;                             // staged residual r' (A, E) and weights 1/S_n (A, E)
+    cx* sRE = sRA + a.max_stage;
+    double* sWA = reinterpret_cast<double*>(sRE + a.max_stage);
+    double* sWE = sWA + a.max_stage;
+    __shared__ __align__(16) SrcConst s_src[2];
+    __shared__ double s_red[(G / 32) * 5 + 1];
+    __shared__ int s_acc;
+    const int tid = threadIdx.x;
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+
+    for (int64_t it = blockIdx.x; it < a.n_tasks; it += gridDim.x) {
+        const gb_band_task t = a.tasks[it];
+        if (t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0) {
+            if (tid == 0) atomicOr(a.errflag, 1);
+            for (int p = tid; p < t.n_prop; p += G) {
+                a.dlnL_out[t.prop_begin + p] = nan;
+                a.accepted_out[t.prop_begin + p] = 0;
+            }
+            continue;
+        }
+        // ---- stage r' and the weights (zero weight marks a bin outside the stored band)
+        const size_t nf = (size_t)a.n_f;
+        double* rA = a.resid + ((size_t)t.walker * 2 + 0) * nf * 2;
+        double* rE = a.resid + ((size_t)t.walker * 2 + 1) * nf * 2;
+        const int prow = a.walker_psd ? a.walker_psd[t.walker] : (a.n_psd == 1 ? 0 : t.walker);
+        const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
+        const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
+        const int64_t i_first = t.k_first - a.k_lo;   // stored element of staged bin 0
+        for (int i = tid; i < t.n_stage; i += G) {
+            const int64_t e = i_first + i;
+            const bool ok = e >= 0 && e < a.n_f;
+            cx ra = {0.0, 0.0}, re = {0.0, 0.0};
+            double wa = 0.0, we = 0.0;
+            if (ok) {
+                const double2 a2 = __ldcg(reinterpret_cast<const double2*>(rA + 2 * e));
+                const double2 e2 = __ldcg(reinterpret_cast<const double2*>(rE + 2 * e));
+                ra = {a2.x, a2.y};
+                re = {e2.x, e2.y};
+                wa = a.psd_is_inverse ? SA[e] : 1.0 / SA[e];
+                we = a.psd_is_inverse ? SE[e] : 1.0 / SE[e];
+            }
+            sRA[i] = ra;
+            sRE[i] = re;
+            sWA[i] = wa;
+            sWE[i] = we;
+        }
+        group_sync<G>();
+
+        // ---- the proposals of the band, in order
+        for (int p = 0; p < t.n_prop; p++) {
+            const int64_t ip = (int64_t)t.prop_begin + p;
+            const int k = a.prop_k[ip];
+            if (k < 0 || k >= t.n_src) {   // uniform over the CTA
+                if (tid == 0) {
+                    atomicOr(a.errflag, 1);
+                    a.dlnL_out[ip] = nan;
+                    a.accepted_out[ip] = 0;
+                }
+                continue;
+            }
+            double* theta_k = a.params + 8 * ((size_t)t.src_begin + k);
+            const double* theta_p = a.prop_params + 8 * ip;
+            if (tid < 2) {   // step O1 for the old (thread 0) and the proposed (thread 1) source
+                const double* src = tid == 0 ? theta_k : theta_p;
+                SrcConst s;
+                source_constants(src, a.Tobs, a.tau, N, s);
+                s.fast = fast_path_ok(src, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                s_src[tid] = s;
+            }
+            group_sync<G>();
+            if (s_src[0].fast && s_src[1].fast) {
+                slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+                fft_store<N>(bufA0, bufE0, a.tw, tid);
+                slow_part<N, G, true>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
+                fft_store<N>(bufA1, bufE1, a.tw, tid);
+            } else {
+                slow_part<N, G, false>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+                fft_store<N>(bufA0, bufE0, a.tw, tid);
+                slow_part<N, G, false>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
+                fft_store<N>(bufA1, bufE1, a.tw, tid);
+            }
+            // ---- the five sums of Eq. 5 against the staged r' (buffers: 0 = old o, 1 = new a)
+            const int64_t j0o = s_src[0].kmin - t.k_first;   // staged bin of window bin 0, old and new
+            const int64_t j0a = s_src[1].kmin - t.k_first;
+            const int64_t shift = s_src[1].kmin - s_src[0].kmin;
+            double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // aa, ra, ao, oo, ro
+#pragma unroll
+            for (int m = 0; m < S; m++) {
+                const int j = tid + G * m;
+                int64_t i = j0a + j;
+                if (i >= 0 && i < t.n_stage) {
+                    const cx ha = bufA1[pad_idx<N>(j)], he = bufE1[pad_idx<N>(j)];
+                    const cx ra = sRA[i], re = sRE[i];
+                    const double wa = sWA[i], we = sWE[i];
+                    v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
+                    v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
+                    const int64_t jo = j + shift;
+                    if (jo >= 0 && jo < N) {
+                        const cx oa = bufA0[pad_idx<N>((int)jo)], oe = bufE0[pad_idx<N>((int)jo)];
+                        v[2] += wa * (ha.re * oa.re + ha.im * oa.im) + we * (he.re * oe.re + he.im * oe.im);
+                    }
+                }
+                i = j0o + j;
+                if (i >= 0 && i < t.n_stage) {
+                    const cx oa = bufA0[pad_idx<N>(j)], oe = bufE0[pad_idx<N>(j)];
+                    const cx ra = sRA[i], re = sRE[i];
+                    const double wa = sWA[i], we = sWE[i];
+                    v[3] += wa * (oa.re * oa.re + oa.im * oa.im) + we * (oe.re * oe.re + oe.im * oe.im);
+                    v[4] += wa * (ra.re * oa.re + ra.im * oa.im) + we * (re.re * oe.re + re.im * oe.im);
+                }
+            }
+            group_reduce<G, 5>(v, s_red, tid);
+            if (tid == 0) {
+                const double norm = 4.0 / a.Tobs;
+                const double dl = -0.5 * norm * (v[0] + v[3] - 2.0 * v[2] - 2.0 * v[1] + 2.0 * v[4]);
+                const int acc = t.beta * dl + a.prop_logq[ip] >= a.prop_logu[ip] ? 1 : 0;
+                a.dlnL_out[ip] = dl;
+                a.accepted_out[ip] = (uint8_t)acc;
+                s_acc = acc;
+            }
+            group_sync<G>();
+            if (s_acc) {
+                // r' += h(theta_k), then r' -= h(theta'_k) (two passes: the windows overlap), and the same change
+                // to the stored residual (only bins inside the stored band exist)
+                const bool wb = t.write_back != 0;
+#pragma unroll
+                for (int m = 0; m < S; m++) {
+                    const int j = tid + G * m;
+                    const int64_t i = j0o + j;
+                    const int64_t e = i_first + i;
+                    if (i >= 0 && i < t.n_stage && e >= 0 && e < a.n_f) {
+                        const cx oa = bufA0[pad_idx<N>(j)], oe = bufE0[pad_idx<N>(j)];
+                        sRA[i] = {sRA[i].re + oa.re, sRA[i].im + oa.im};
+                        sRE[i] = {sRE[i].re + oe.re, sRE[i].im + oe.im};
+                        if (wb) {
+                            atomicAdd(rA + 2 * e, oa.re);
+                            atomicAdd(rA + 2 * e + 1, oa.im);
+                            atomicAdd(rE + 2 * e, oe.re);
+                            atomicAdd(rE + 2 * e + 1, oe.im);
+                        }
+                    }
+                }
+                group_sync<G>();
+#pragma unroll
+                for (int m = 0; m < S; m++) {
+                    const int j = tid + G * m;
+                    const int64_t i = j0a + j;
+                    const int64_t e = i_first + i;
+                    if (i >= 0 && i < t.n_stage && e >= 0 && e < a.n_f) {
+                        const cx ha = bufA1[pad_idx<N>(j)], he = bufE1[pad_idx<N>(j)];
+                        sRA[i] = {sRA[i].re - ha.re, sRA[i].im - ha.im};
+                        sRE[i] = {sRE[i].re - he.re, sRE[i].im - he.im};
+                        if (wb) {
+                            atomicAdd(rA + 2 * e, -ha.re);
+                            atomicAdd(rA + 2 * e + 1, -ha.im);
+                            atomicAdd(rE + 2 * e, -he.re);
+                            atomicAdd(rE + 2 * e + 1, -he.im);
+                        }
+                    }
+                }
+                if (tid < 8) theta_k[tid] = theta_p[tid];   // theta_j[k] <- theta'_k
+            }
+            group_sync<G>();   // r', s_src, the waveform buffers and theta_j are reused by the next proposal
+        }
+    }
+}

@@ -710,6 +710,8 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     }
 }
 
+#include "gb_band.cuh"
+
 template <int N, bool SWAP>
 constexpr size_t main_smem_bytes() {
     return (size_t)padded_len<N>() * sizeof(cx) * 2 * (SWAP ? 2 : 1);
@@ -967,6 +969,24 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
 
 }  // namespace
 
+namespace {
+template <int N>
+int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
+    const size_t smem = band_smem_bytes<N>(a.max_stage);
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int nb = 0;
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N>, Plan<N>::G, smem));
+    if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
+    int64_t grid = (int64_t)nb * ctx->num_sms;
+    if (grid > a.n_tasks) grid = a.n_tasks;
+    gb_band_kernel<N><<<(unsigned)grid, Plan<N>::G, smem, st>>>(a);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+    return GB_OK;
+}
+
+}  // namespace
+
 // ------------------------------------------------------------------------------------------------ C ABI
 extern "C" {
 
@@ -1137,6 +1157,54 @@ int gb_residual_update(gb_ctx* ctx, const gb_data* data, const double* params_ne
     c.n_bins = n_bins;
     c.B = B;
     return run_call(ctx, c, stream);
+}
+
+int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
+                  double* params, const int32_t* prop_k, const double* prop_params, const double* prop_logq,
+                  const double* prop_logu, uint8_t* accepted_out, double* dlnL_out, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (n_tasks < 0 || n_tasks > 0x7fffffff) return set_err(ctx, GB_ERR_INVALID, "n_tasks out of range");
+    if (n_tasks == 0) return GB_OK;
+    if (!data || !data->resid || !data->psd || data->n_f <= 0 || data->n_walkers <= 0)
+        return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
+    if (!tasks || !params || !prop_k || !prop_params || !prop_logq || !prop_logu || !accepted_out || !dlnL_out)
+        return set_err(ctx, GB_ERR_INVALID, "NULL argument");
+    if (!(N == 128 || N == 256 || N == 512 || N == 1024)) return set_err(ctx, GB_ERR_INVALID, "N must be 128, 256, 512 or 1024");
+    if (max_stage < 1 || max_stage > GB_BAND_MAX_STAGE) return set_err(ctx, GB_ERR_INVALID, "max_stage out of range");
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    BandArgs a{};
+    a.tasks = tasks;
+    a.n_tasks = n_tasks;
+    a.params = params;
+    a.prop_k = prop_k;
+    a.prop_params = prop_params;
+    a.prop_logq = prop_logq;
+    a.prop_logu = prop_logu;
+    a.accepted_out = accepted_out;
+    a.dlnL_out = dlnL_out;
+    a.orbit = ctx->d_orbit[N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3];
+    a.tw = ctx->d_tw;
+    a.resid = data->resid;
+    a.psd = data->psd;
+    a.walker_psd = data->walker_psd;
+    a.k_lo = data->k_lo;
+    a.n_f = data->n_f;
+    a.n_walkers = data->n_walkers;
+    a.n_psd = data->n_psd;
+    a.psd_is_inverse = data->psd_is_inverse;
+    a.max_stage = max_stage;
+    a.Tobs = ctx->cfg.Tobs;
+    a.tau = ctx->cfg.armlength / kCLight;
+    a.Rmax = ctx->cfg.au / kCLight;
+    a.kmax = (int64_t)floor(ctx->cfg.Tobs / (2.0 * ctx->cfg.dt));
+    a.errflag = ctx->d_counts + 2 * kNumClasses;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    switch (N) {
+        case 128: return launch_band<128>(ctx, a, st);
+        case 256: return launch_band<256>(ctx, a, st);
+        case 512: return launch_band<512>(ctx, a, st);
+        default: return launch_band<1024>(ctx, a, st);
+    }
 }
 
 }  // extern "C"

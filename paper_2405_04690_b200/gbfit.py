@@ -21,7 +21,23 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
-           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host")
+           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep")
+
+BAND_MAX_STAGE = 3072
+# layout of gb_band_task (include/gbfit.h)
+BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
+                      ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
+                      ("write_back", np.int32), ("reserved", np.int32), ("beta", np.float64)], align=True)
+
+
+def pack_band_tasks(walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta) -> np.ndarray:
+    """Host array of gb_band_task records from equal-length columns (upload it as bytes: torch.from_numpy(t.view(np.uint8)))."""
+    t = np.zeros(len(walker), BAND_TASK)
+    for key, val in (("walker", walker), ("n_src", n_src), ("src_begin", src_begin), ("n_prop", n_prop),
+                     ("prop_begin", prop_begin), ("n_stage", n_stage), ("k_first", k_first),
+                     ("write_back", write_back), ("beta", beta)):
+        t[key] = val
+    return t
 
 
 class GbConfig(C.Structure):
@@ -79,6 +95,8 @@ def lib() -> C.CDLL:
         wf = [vp, vp, i64, ci, vp, ci, vp, vp, vp]
         dl = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, vp, vp, vp]
         ru = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, vp, ci, vp, i64, vp]
+        L.gb_band_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.gb_band_sweep.restype = ci
         for name, sig in (("gb_waveform", wf), ("gb_waveform_host", wf), ("gb_delta_loglike", dl),
                           ("gb_delta_loglike_host", dl), ("gb_residual_update", ru),
                           ("gb_residual_update_host", ru)):
@@ -284,6 +302,29 @@ class Context:
                                           _dev_ptr(accepted, torch.uint8, dev, "accepted"), int(N),
                                           _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B,
                                           _stream_ptr(stream, dev)))
+
+    def band_sweep(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
+                   prop_k: torch.Tensor, prop_params: torch.Tensor, prop_logq: torch.Tensor, prop_logu: torch.Tensor,
+                   accepted_out: Optional[torch.Tensor] = None, dlnL_out: Optional[torch.Tensor] = None, stream=None):
+        """gb_band_sweep (Algorithm 1): `tasks` is a CUDA uint8 tensor holding packed gb_band_task records
+        (pack_band_tasks); params [n_src_total, 8] and data.resid are updated in place.
+        Returns (accepted [n_prop_total] uint8, dlnL [n_prop_total] float64), CUDA tensors."""
+        dev = self.device
+        n_tasks = int(tasks.numel() // BAND_TASK.itemsize)
+        P = int(prop_k.shape[0])
+        if accepted_out is None:
+            accepted_out = torch.zeros((P,), dtype=torch.uint8, device=dev)
+        if dlnL_out is None:
+            dlnL_out = torch.zeros((P,), dtype=torch.float64, device=dev)
+        self._ok(lib().gb_band_sweep(self._h, data.c(), _dev_ptr(tasks, torch.uint8, dev, "tasks"), n_tasks, int(N),
+                                     int(max_stage), _dev_ptr(params, torch.float64, dev, "params"),
+                                     _dev_ptr(prop_k, torch.int32, dev, "prop_k"),
+                                     _dev_ptr(prop_params, torch.float64, dev, "prop_params"),
+                                     _dev_ptr(prop_logq, torch.float64, dev, "prop_logq"),
+                                     _dev_ptr(prop_logu, torch.float64, dev, "prop_logu"),
+                                     _dev_ptr(accepted_out, torch.uint8, dev, "accepted_out"),
+                                     _dev_ptr(dlnL_out, torch.float64, dev, "dlnL_out"), _stream_ptr(stream, dev)))
+        return accepted_out, dlnL_out
 
     # --------------------------------------------------------------------------------- host forms
     def waveform_host(self, params, N: int = 0, n_bins=None, Nmax: Optional[int] = None, out=None,

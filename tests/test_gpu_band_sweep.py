@@ -1,0 +1,125 @@
+"""Parity of gb_band_sweep (Algorithm 1) with the CPU oracle on the
+same seeded band tasks: accept / reject decisions and final parameters bit-exact (both sides decide
+beta dlnL + logq >= logu in FP64), delta lnL <= 1e-6 absolute, final residuals <= 1e-9 of the largest change.
+"""
+import numpy as np
+import pytest
+
+from gb_inputs import make_band_tasks, make_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_DLNL = 1e-6
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked parity tests must run on a B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gb(torch_cuda):
+    from paper_2405_04690_b200 import gbfit
+    ctx = gbfit.Context(0)
+    yield gbfit, ctx
+    ctx.close()
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def run_gpu(torch, gbfit, ctx, wl, bt, resid, tasks=None, logu=None, psd=None, inverse=False):
+    t = bt.tasks if tasks is None else tasks
+    packed = gbfit.pack_band_tasks(**t)
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd if psd is None else psd), wl.k_lo, psd_is_inverse=inverse)
+    d_params = dev(torch, bt.params)
+    acc, dl = ctx.band_sweep(data, dev(torch, packed.view(np.uint8)), bt.N, int(max(t["n_stage"].max(), 1)), d_params,
+                             dev(torch, bt.prop_k), dev(torch, bt.prop_params), dev(torch, bt.prop_logq),
+                             dev(torch, bt.prop_logu if logu is None else logu))
+    ctx.check()
+    return acc.cpu().numpy(), dl.cpu().numpy(), d_params.cpu().numpy(), d_resid.cpu().numpy()
+
+
+def run_oracle(oracle, wl, bt, resid, tasks=None, logu=None):
+    data = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params = bt.params.copy()
+    acc, dl = oracle.band_sweep(oracle.Config(), data, bt.tasks if tasks is None else tasks, bt.N, params, bt.prop_k,
+                                bt.prop_params, bt.prop_logq, bt.prop_logu if logu is None else logu)
+    return acc, dl, params, data.resid
+
+
+def compare(got, ref, resid):
+    acc, dl, params, r1 = got
+    racc, rdl, rparams, rr1 = ref
+    assert np.array_equal(acc, racc), int((acc != racc).sum())
+    assert np.abs(dl - rdl).max() <= TOL_DLNL
+    assert np.array_equal(params, rparams)
+    change = np.abs(rr1 - resid).max()
+    assert np.abs(r1 - rr1).max() <= 1e-9 * change + 4e-16 * np.abs(resid).max()
+
+
+@pytest.mark.parametrize("N,f_lo,n_bands,amp", [(128, 5e-4, 6, 2e-22), (256, 2e-3, 6, 2e-22), (512, 6e-3, 4, 4e-23),
+                                                 (1024, 1.2e-2, 3, 1e-23)])
+def test_band_sweep_each_window_length(oracle, torch_cuda, gb, N, f_lo, n_bands, amp):
+    gbfit, ctx = gb
+    wl = make_workload(3, B=1, n_walkers=3)
+    bt = make_band_tasks(wl, N, f_lo, n_bands, n_src=5, n_prop=14, amp_lo=0.1 * amp, amp_hi=amp)
+    resid = wl.resid()
+    ref = run_oracle(oracle, wl, bt, resid)
+    assert 0 < ref[0].sum() < ref[0].size
+    compare(run_gpu(torch_cuda, gbfit, ctx, wl, bt, resid), ref, resid)
+
+
+def test_band_sweep_all_accepted_all_rejected_no_write_back_and_inverse_psd(oracle, torch_cuda, gb):
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=1, n_walkers=2)
+    bt = make_band_tasks(wl, 256, 2.5e-3, 5, n_src=4, n_prop=12, stream=1)
+    resid = wl.resid()
+    for logu in (np.full_like(bt.prop_logu, -np.inf), np.full_like(bt.prop_logu, np.inf)):
+        compare(run_gpu(torch, gbfit, ctx, wl, bt, resid, logu=logu), run_oracle(oracle, wl, bt, resid, logu=logu), resid)
+    t2 = dict(bt.tasks, write_back=np.zeros_like(bt.tasks["write_back"]))
+    got = run_gpu(torch, gbfit, ctx, wl, bt, resid, tasks=t2)
+    ref = run_oracle(oracle, wl, bt, resid, tasks=t2)
+    assert np.array_equal(got[3], resid) and np.array_equal(ref[3], resid)
+    assert np.array_equal(got[0], ref[0]) and np.array_equal(got[2], ref[2]) and np.abs(got[1] - ref[1]).max() <= TOL_DLNL
+    got = run_gpu(torch, gbfit, ctx, wl, bt, resid, psd=1.0 / wl.psd, inverse=True)
+    compare(got, run_oracle(oracle, wl, bt, resid), resid)
+
+
+def test_band_sweep_edges_rj_amplitude_switch_and_bad_tasks(oracle, torch_cuda, gb):
+    """Staged range partly outside the stored band, an empty task, n_prop = 0, the RJ amplitude switch of
+    PAPER.md:564 (amp = 0 on one side), a proposal outside the fast-path limits, and invalid tasks."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(1)                                   # band 1-4 mHz only (k_lo = 31458)
+    bt = make_band_tasks(wl, 128, 1e-3, 4, n_src=3, n_prop=8, stream=2)
+    t = {k: v.copy() for k, v in bt.tasks.items()}
+    t["k_first"][0] = wl.k_lo - 200                          # staged bins below the stored band
+    t["n_prop"][1] = 0                                       # a task with nothing to do
+    bt.params[t["src_begin"][0]:t["src_begin"][0] + 3, 1] = (wl.k_lo + 20 + np.arange(3) * 30) / wl.Tobs
+    bt.prop_params[0:8, 1] = bt.params[t["src_begin"][0] + bt.prop_k[0:8], 1] + 1e-9
+    p2 = t["prop_begin"][2]
+    bt.prop_params[p2] = bt.params[t["src_begin"][2] + bt.prop_k[p2]]
+    bt.prop_params[p2, 0] = 0.0                              # proposed removal: amplitude -> 0
+    bt.prop_params[p2 + 1, 2] = 3e-12                        # outside the fast-path limits: general kernels' arithmetic
+    resid = wl.resid()
+    compare(run_gpu(torch, gbfit, ctx, wl, bt, resid, tasks=t), run_oracle(oracle, wl, bt, resid, tasks=t), resid)
+    # invalid: walker out of range -> sticky flag, NaN rows
+    bad = {k: v.copy() for k, v in bt.tasks.items()}
+    bad["walker"][0] = 7
+    packed = gbfit.pack_band_tasks(**bad)
+    data = gbfit.Data(dev(torch, resid), dev(torch, wl.psd), wl.k_lo)
+    acc, dl = ctx.band_sweep(data, dev(torch, packed.view(np.uint8)), 128, 384, dev(torch, bt.params), dev(torch, bt.prop_k),
+                             dev(torch, bt.prop_params), dev(torch, bt.prop_logq), dev(torch, bt.prop_logu))
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    assert np.isnan(dl.cpu().numpy()[:8]).all() and np.isfinite(dl.cpu().numpy()[8:]).all()
+    with pytest.raises(gbfit.GbError):
+        ctx.band_sweep(data, dev(torch, packed.view(np.uint8)), 128, gbfit.BAND_MAX_STAGE + 1, dev(torch, bt.params),
+                       dev(torch, bt.prop_k), dev(torch, bt.prop_params), dev(torch, bt.prop_logq), dev(torch, bt.prop_logu))
