@@ -319,6 +319,41 @@ def run_ours(args):
     h2d = 2 * (h_p.numel() * 8 + h_w.numel() * 4 + h_nb.numel() * 4) + h_acc.numel()
     d2h = h_out.numel() * 8
 
+    # ---- SURVEY 8(f) row f1, outside the timed step: Algorithm 1 (gb_band_sweep) on the same residuals --
+    # every odd 256-bin sub-band of 1-4 mHz of every walker, 9 sources and 30 sequential proposals per band
+    band = None
+    if rank == 0 and full and not args.no_band_sweep:
+        from gb_inputs import make_band_tasks
+        bt = make_band_tasks(wl, 256, 1e-3, n_bands=183, n_src=9, n_prop=30)
+        packed = gbfit.pack_band_tasks(**bt.tasks)
+        d_tasks = torch.from_numpy(packed.view(np.uint8)).to(dev)
+        d_bp0 = torch.from_numpy(bt.params).to(dev)
+        d_bp = d_bp0.clone()
+        d_bk, d_bq = torch.from_numpy(bt.prop_k).to(dev), torch.from_numpy(bt.prop_params).to(dev)
+        d_lq, d_lu = torch.from_numpy(bt.prop_logq).to(dev), torch.from_numpy(bt.prop_logu).to(dev)
+        d_acc_b = torch.zeros(bt.prop_k.size, dtype=torch.uint8, device=dev)
+        d_dl_b = torch.zeros(bt.prop_k.size, dtype=torch.float64, device=dev)
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 3
+        for i in range(reps + 1):          # first call warms up; every call starts from the same parameters
+            d_bp.copy_(d_bp0)
+            if i == 1:
+                b0.record(stream)
+            ctx.band_sweep(data, d_tasks, 256, bt.max_stage, d_bp, d_bk, d_bq, d_lq, d_lu, d_acc_b, d_dl_b)
+        b1.record(stream)
+        torch.cuda.synchronize()
+        ctx.check()
+        ms_band = b0.elapsed_time(b1) / reps
+        band = {"call": "gb_band_sweep (Algorithm 1)", "N": 256, "tasks": int(len(bt.tasks["walker"])),
+                "sources_per_band": 9, "proposals_per_band": 30, "proposals": int(bt.prop_k.size),
+                "ms_per_call": ms_band, "proposals_per_s": bt.prop_k.size / (ms_band * 1e-3),
+                "accepted_fraction_last_call": float(d_acc_b.float().mean().item()),
+                # nominal work of a swap evaluation: 2 (711 N + 10 N log2 N) + 60 N flop
+                "alu_frac": bt.prop_k.size * (2 * (711 * 256 + 10 * 256 * 8) + 60 * 256) / (ms_band * 1e-3) / 1e12
+                            / FP64_PEAK_TFLOPS,
+                "note": "each proposal = 2 waveforms + Eq. 5 against the staged residual + accept/reject + update; "
+                        "includes the device-side reset of the 38 MB parameter array before each call"}
+
     # ---- roofline of the delta-lnL kernels (the dominant launches) and of the scatter
     nb = wl.n_bins.astype(np.float64)
     flops_dlnl = float(flops_eval(nb).sum())
@@ -390,6 +425,7 @@ def run_ours(args):
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+            "band_sweep": band,
         }
         print(json.dumps(line), flush=True)
     ctx.close()
@@ -407,6 +443,7 @@ def main(argv=None):
     ap.add_argument("--walkers", type=int, default=360, help="debug: fewer residuals (default = the full config)")
     ap.add_argument("--per-walker", type=int, default=12000, help="debug: fewer sources per walker")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-band-sweep", action="store_true", help="skip the Algorithm-1 (gb_band_sweep) measurement")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3)
     args.steps = max(args.steps, 1)
