@@ -402,6 +402,35 @@ double gbo_inner_windows(const gbo_config *c, const gbo_data *d, int psd_row,
     return o7_inner(c, d, psd_row, bA, bE, kb, nb, cA, cE, kc, nc);
 }
 
+/* ---- normalised overlap of two sources (cataloging) -------------
+ * O(a, c) = <a|c> / sqrt(<a|a> <c|c>) with Eq. 2 against PSD row psd_row[b], <a|c> over the bins common to
+ * the two windows, every term over the stored band only.  The paper uses the overlap (threshold 0.9) and the
+ * optimal SNR sqrt(<h|h>) (cut at 7) without printing the formula; this is the standard definition
+ * (reading F4-a).  O = 0 when either norm vanishes (reading F4-b).  aux = (<a|a>, <c|c>).          */
+int gbo_overlap(const gbo_config *c, const gbo_data *d, const double *params_a, const double *params_c,
+                const int32_t *psd_row, int N, const int32_t *n_bins, int64_t B, double *overlap_out,
+                double *aux_out, int nthreads) {
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads > 0 ? nthreads : 1)
+    for (int64_t b = 0; b < B; b++) {
+        int Nb = n_bins ? n_bins[b] : N;
+        int row = psd_row ? psd_row[b] : 0;
+        if (!valid_N(Nb) || row < 0 || row >= d->n_psd) { bad = 1; continue; }
+        double *buf = (double *)malloc(sizeof(double) * 8 * (size_t)Nb);
+        double *aA = buf, *aE = buf + 2 * (size_t)Nb, *cA = buf + 4 * (size_t)Nb, *cE = buf + 6 * (size_t)Nb;
+        int64_t ka, kc;
+        gbo_waveform(c, params_a + 8 * b, Nb, aA, aE, &ka);
+        gbo_waveform(c, params_c + 8 * b, Nb, cA, cE, &kc);
+        double aa = o7_inner(c, d, row, aA, aE, ka, Nb, aA, aE, ka, Nb);
+        double cc = o7_inner(c, d, row, cA, cE, kc, Nb, cA, cE, kc, Nb);
+        double ac = o7_inner(c, d, row, aA, aE, ka, Nb, cA, cE, kc, Nb);
+        overlap_out[b] = (aa > 0.0 && cc > 0.0) ? ac / sqrt(aa * cc) : 0.0;
+        if (aux_out) { aux_out[2 * b] = aa; aux_out[2 * b + 1] = cc; }
+        free(buf);
+    }
+    return bad ? GBO_ERR_INVALID : GBO_OK;
+}
+
 /* ---- Algorithm 1: sequential proposals of one band against a staged residual --------
  * One task = one band j = (t, w, b): the residual r' of walker `walker` on the staged bins
  * [k_first, k_first + n_stage) (the paper's sub-bands b-1, b, b+1; reading F1-a: the caller's

@@ -179,6 +179,23 @@ def residual_update(cfg: Config, data: Data, params_new, params_old, walker_inde
         raise ValueError(f"gbo_residual_update rc={rc}")
 
 
+def overlap(cfg: Config, data: Data, params_a, params_c, psd_row=None, N: int = 0, n_bins=None, nthreads: int = 1):
+    """Normalised overlap <a|c>/sqrt(<a|a><c|c>) of B source pairs against PSD row psd_row[b] (row 0 if None).
+    Returns (overlap[B], aux[B, 2] = (<a|a>, <c|c>)).  data.resid is not used."""
+    pa, pc = _f64(params_a).reshape(-1, 8), _f64(params_c).reshape(-1, 8)
+    B = pa.shape[0]
+    pr = None if psd_row is None else np.ascontiguousarray(psd_row, dtype=np.int32)
+    nb = None if n_bins is None else np.ascontiguousarray(n_bins, dtype=np.int32)
+    out = np.zeros(B, np.float64)
+    aux = np.zeros((B, 2), np.float64)
+    cc, dd = cfg.c(), data.c()
+    rc = lib().gbo_overlap(C.byref(cc), C.byref(dd), _ptr(pa), _ptr(pc), _ptr(pr), C.c_int(N), _ptr(nb), C.c_int64(B),
+                           _ptr(out), _ptr(aux), C.c_int(nthreads))
+    if rc != 0:
+        raise ValueError(f"gbo_overlap rc={rc}")
+    return out, aux
+
+
 _BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
                        ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
                        ("write_back", np.int32), ("reserved", np.int32), ("beta", np.float64)], align=True)

@@ -468,3 +468,41 @@ def test_band_sweep_single_proposal_is_eq5_on_the_staged_bins(oracle):
         ref = oracle.delta_loglike(cfg, oracle.Data(resid.copy(), psd, wl.k_lo), bt.prop_params[t["prop_begin"][i]][None],
                                    old[None], np.array([w], np.int32), move_all=oracle.SWAP, N=bt.N)[0]
         assert abs(dl[t["prop_begin"][i]] - ref) <= 1e-9 * max(1.0, abs(ref))
+
+
+# ------------------------------------------------------------- normalised overlap, row f4
+def test_overlap_closed_forms(oracle):
+    """O(a, a) = 1; O is symmetric and amplitude-free; a phase offset gives O = cos(dphi) exactly (the window is
+    linear in exp(i phi0)); |O| <= 1; <a|a> equals the Parseval form of P4 for a flat PSD."""
+    from gb_inputs import make_workload
+    wl = make_workload(2, B=24)
+    cfg = oracle.Config()
+    data = oracle.Data(np.zeros((1, 2, wl.n_f), np.complex128), wl.psd, wl.k_lo)
+    p = wl.params_new
+    nb = np.where(p[:, 1] < 1e-3, 128, np.where(p[:, 1] < 4e-3, 256, np.where(p[:, 1] < 1e-2, 512, 1024))).astype(np.int32)
+    o, aux = oracle.overlap(cfg, data, p, p, n_bins=nb)
+    assert np.abs(o - 1.0).max() < 1e-14 and np.all(aux[:, 0] == aux[:, 1]) and np.all(aux > 0)
+    q = p.copy()
+    q[:, 0] *= 3.7
+    dphi = np.linspace(-3.0, 3.0, p.shape[0])
+    q[:, 3] += dphi
+    o2, aux2 = oracle.overlap(cfg, data, p, q, n_bins=nb)
+    assert np.abs(o2 - np.cos(dphi)).max() < 1e-11
+    assert np.abs(aux2[:, 1] / aux2[:, 0] - 3.7 ** 2).max() < 1e-12
+    o3, aux3 = oracle.overlap(cfg, data, q, p, n_bins=nb)
+    assert np.abs(o3 - o2).max() < 1e-14 and np.allclose(aux3[:, ::-1], aux2, rtol=1e-15)
+    r = p.copy()
+    r[:, 1] += 1.5e-8                    # half a bin away: partial overlap, offset windows for some rows
+    r[:, 6] += 0.3
+    o4, _ = oracle.overlap(cfg, data, p, r, n_bins=nb)
+    assert np.all(np.abs(o4) < 1.0) and np.abs(o4).max() > 0.01
+    # <a|a> against the time-domain (Parseval) form with a flat PSD
+    flat = oracle.Data(np.zeros((1, 2, wl.n_f), np.complex128), np.full((1, 2, wl.n_f), 2.5e-40), wl.k_lo)
+    row = np.array([2e-22, 3.1e-3, 1e-17, 0.4, 0.3, 0.9, 2.2, 0.35])
+    _, a = oracle.overlap(cfg, flat, row[None], row[None], N=256)
+    As, Es = oracle.slow_envelope(cfg, row, 256)
+    assert abs(a[0, 0] - cfg.Tobs / (256 * 2.5e-40) * float((np.abs(As) ** 2 + np.abs(Es) ** 2).sum())) <= 1e-12 * a[0, 0]
+    z = p[:2].copy()
+    z[:, 0] = 0.0
+    o5, _ = oracle.overlap(cfg, data, p[:2], z, n_bins=nb[:2])
+    assert np.all(o5 == 0.0)
