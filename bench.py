@@ -354,6 +354,31 @@ def run_ours(args):
                 "note": "each proposal = 2 waveforms + Eq. 5 against the staged residual + accept/reject + update; "
                         "includes the device-side reset of the 38 MB parameter array before each call"}
 
+    # ---- SURVEY 8(f) row f4, outside the timed step: normalised overlaps of 1 M source pairs (gb_overlap) ----
+    ovl = None
+    if rank == 0 and full and not args.no_band_sweep:
+        n_pairs = 1 << 20
+        d_pa = d_p[:n_pairs].contiguous()
+        jit = torch.zeros((n_pairs, 8), dtype=torch.float64, device=dev)
+        jit[:, 1] = 4e-9
+        jit[:, 3] = 0.05
+        d_pc = d_pa + jit
+        d_rows = (torch.arange(n_pairs, device=dev, dtype=torch.int32) % wl.psd.shape[0]).contiguous()
+        d_ov = torch.empty(n_pairs, dtype=torch.float64, device=dev)
+        o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        view = gbfit.Data.psd_only(d_psd, wl.k_lo, psd_is_inverse=True)
+        nb_pairs = d_nb[:n_pairs].contiguous()
+        for i in range(4):
+            if i == 1:
+                o0.record(stream)
+            ctx.overlap(view, d_pa, d_pc, psd_row=d_rows, n_bins=nb_pairs, out=d_ov)
+        o1.record(stream)
+        torch.cuda.synchronize()
+        ctx.check()
+        ms_ov = o0.elapsed_time(o1) / 3
+        ovl = {"call": "gb_overlap", "pairs": n_pairs, "ms_per_call": ms_ov, "pairs_per_s": n_pairs / (ms_ov * 1e-3),
+               "mean_N": float(wl.n_bins[:n_pairs].mean()), "median_overlap": float(d_ov.median().item())}
+
     # ---- roofline of the delta-lnL kernels (the dominant launches) and of the scatter
     nb = wl.n_bins.astype(np.float64)
     flops_dlnl = float(flops_eval(nb).sum())
@@ -425,7 +450,7 @@ def run_ours(args):
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "band_sweep": band,
+            "band_sweep": band, "overlap": ovl,
         }
         print(json.dumps(line), flush=True)
     ctx.close()

@@ -169,6 +169,19 @@ int gb_residual_update_host(gb_ctx *ctx, const gb_data *data, const double *para
                             int N, const int32_t *n_bins /*HOST*/, int64_t B, void *stream);
 
 /*
+ * gb_overlap -- normalised overlap of B source pairs (cataloging; the search / catalog workloads
+ * of PAPER.md:710-718 use the same kernels with this batch shape):
+ *     O_b = <a_b|c_b> / sqrt(<a_b|a_b> <c_b|c_b>),   Eq. 2 against PSD row psd_row[b],
+ * <a|c> over the bins common to the two windows, every term over the stored band only; O_b = 0 if a norm vanishes.
+ *   data        only psd, psd_is_inverse, n_psd, k_lo, n_f are used (resid may be NULL)
+ *   params_a, params_c  [B][8] DEVICE;  psd_row [B] DEVICE int32 or NULL (row 0)
+ *   overlap_out [B] DEVICE f64;  aux_out optional [B][2] DEVICE: <a|a>, <c|c> (the optimal SNR^2 of each source)
+ * N / n_bins as for gb_waveform.  Asynchronous on `stream`; a bad row sets the sticky flag and gives NaN.
+ */
+int gb_overlap(gb_ctx *ctx, const gb_data *data, const double *params_a, const double *params_c, const int32_t *psd_row,
+               int N, const int32_t *n_bins, int64_t B, double *overlap_out, double *aux_out, void *stream);
+
+/*
  * gb_band_sweep -- Algorithm 1 of the paper ("Galaxy sampling algorithm"): for each band task the
  * walker's residual on the staged bins is held on chip and the task's proposals are applied IN ORDER, each one a swap
  * theta_k -> theta'_k evaluated by Eq. 5 against the staged residual r', accepted iff

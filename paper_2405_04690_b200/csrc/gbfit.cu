@@ -48,7 +48,7 @@ namespace {
 #define GB_UNROLL 1        // unroll factor of the per-thread time-sample loop
 #endif
 
-enum Mode { MODE_WAVEFORM = 0, MODE_DLNL = 1, MODE_UPDATE = 2 };
+enum Mode { MODE_WAVEFORM = 0, MODE_DLNL = 1, MODE_UPDATE = 2, MODE_OVERLAP = 3 };   // OVERLAP: SWAP kernels, no residual
 constexpr int kNumClasses = 16;  // class = 4 * log2(N / 128) + 2 * general + swap  (general: outside the fast path)
 
 // ------------------------------------------------------------------------------------------------ args
@@ -116,7 +116,10 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         const int cN = class_of_N(N);
         bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP;
         int w = 0, prow = 0;
-        if (a.mode != MODE_WAVEFORM) {
+        if (a.mode == MODE_OVERLAP) {          // walker_index carries the PSD row itself (NULL: row 0)
+            prow = a.walker_index ? a.walker_index[b] : 0;
+            ok = ok && prow >= 0 && prow < a.n_psd;
+        } else if (a.mode != MODE_WAVEFORM) {
             w = a.walker_index[b];
             ok = ok && w >= 0 && w < a.n_walkers;
             if (ok) prow = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
@@ -396,6 +399,21 @@ struct WinBatch {
             }
         }
     }
+    // weights only (gb_overlap has no residual): r = 0
+    template <int G>
+    __device__ __forceinline__ void load_weights(const double* __restrict__ SA, const double* __restrict__ SE,
+                                                 int64_t i_first, int64_t n_f, bool inv) {
+#pragma unroll
+        for (int c = 0; c < CH; c++) {
+            const int64_t i = i_first + G * c;
+            const bool ok = i >= 0 && i < n_f;
+            const int64_t ic = ok ? i : 0;
+            const double sa = __ldcg(SA + ic), se = __ldcg(SE + ic);
+            wa[c] = ok ? (inv ? sa : 1.0 / sa) : 0.0;
+            we[c] = ok ? (inv ? se : 1.0 / se) : 0.0;
+            ra[c] = re[c] = {0.0, 0.0};
+        }
+    }
 };
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
@@ -566,7 +584,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             double* rE = a.resid + ((size_t)w * 2 + 1) * nf * 2;
             const int64_t i0w = kmin0 - a.k_lo;                         // residual element of window bin 0
             const bool inband0 = i0w >= 0 && i0w + N <= a.n_f;          // the whole window is stored
-            if (a.mode == MODE_DLNL) {
+            if (a.mode == MODE_DLNL || a.mode == MODE_OVERLAP) {
                 const int prow = rec[0].psd_row;
                 const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
                 const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
@@ -610,7 +628,10 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
 #pragma unroll
                     for (int m0 = 0; m0 < S; m0 += CH) {
                         WinBatch<CH> wn, wo;   // the new source's window and the old one's (equal when shift == 0)
-                        if (inband0 && inband1) {
+                        if (a.mode == MODE_OVERLAP) {      // no residual: weights only
+                            wn.template load_weights<G>(SA, SE, i1w + tid + G * m0, a.n_f, inv);
+                            wo.template load_weights<G>(SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                        } else if (inband0 && inband1) {
                             wn.template load<G, false>(rA, rE, SA, SE, i1w + tid + G * m0, a.n_f, inv);
                             if (shift != 0) wo.template load<G, false>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
                             else wo = wn;
@@ -646,10 +667,18 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     if (tid == 0) {
                         const double aa = norm * v[0], ra = norm * v[1], ao = norm * v[2], oo = norm * v[3],
                                      ro = norm * v[4];
-                        a.dlnL_out[b] = -0.5 * (aa + oo - 2.0 * ao - 2.0 * ra + 2.0 * ro);
-                        if (a.aux_out) {
-                            a.aux_out[2 * b] = aa;
-                            a.aux_out[2 * b + 1] = ra;
+                        if (a.mode == MODE_OVERLAP) {   // <a|c> / sqrt(<a|a><c|c>), 0 when a norm vanishes
+                            a.dlnL_out[b] = (aa > 0.0 && oo > 0.0) ? ao / sqrt(aa * oo) : 0.0;
+                            if (a.aux_out) {
+                                a.aux_out[2 * b] = aa;
+                                a.aux_out[2 * b + 1] = oo;
+                            }
+                        } else {
+                            a.dlnL_out[b] = -0.5 * (aa + oo - 2.0 * ao - 2.0 * ra + 2.0 * ro);
+                            if (a.aux_out) {
+                                a.aux_out[2 * b] = aa;
+                                a.aux_out[2 * b + 1] = ra;
+                            }
                         }
                     }
                 }
@@ -853,7 +882,10 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     if (c.B == 0) return GB_OK;
     const bool need_new = c.mode == MODE_WAVEFORM || c.move != nullptr || c.move_all != GB_REMOVE;
     const bool need_old = c.mode != MODE_WAVEFORM && (c.move != nullptr || c.move_all != GB_ADD);
-    if (c.mode != MODE_WAVEFORM) {
+    if (c.mode == MODE_OVERLAP) {
+        if (!c.data || !c.data->psd || c.data->n_f <= 0 || c.data->n_psd <= 0) return set_err(ctx, GB_ERR_INVALID, "NULL / empty PSD view");
+        if (!c.params_new || !c.params_old || !c.dlnL_out) return set_err(ctx, GB_ERR_INVALID, "NULL params / output");
+    } else if (c.mode != MODE_WAVEFORM) {
         if (!c.data || !c.data->resid || !c.walker_index) return set_err(ctx, GB_ERR_INVALID, "NULL data / walker_index");
         if (c.mode == MODE_DLNL && (!c.data->psd || !c.dlnL_out)) return set_err(ctx, GB_ERR_INVALID, "NULL psd / dlnL_out");
         if (c.data->n_f <= 0 || c.data->n_walkers <= 0) return set_err(ctx, GB_ERR_INVALID, "empty data view");
@@ -903,7 +935,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.lists = ctx->d_lists;
     p.counts = ctx->d_counts;
     p.errflag = ctx->d_counts + 2 * kNumClasses;
-    p.dlnL_out = c.mode == MODE_DLNL ? c.dlnL_out : nullptr;
+    p.dlnL_out = (c.mode == MODE_DLNL || c.mode == MODE_OVERLAP) ? c.dlnL_out : nullptr;
     const unsigned pgrid = (unsigned)((c.B + 255) / 256);
     gb_prep_kernel<<<pgrid, 256, 0, st>>>(p);
     ctx->launches++;
@@ -940,7 +972,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     a.tau = p.tau;
 
     // launch only the classes that can occur; largest windows first
-    const bool may_swap = c.mode != MODE_WAVEFORM && (c.move ? true : c.move_all == GB_SWAP);
+    const bool may_swap = c.mode != MODE_WAVEFORM && (c.move ? true : c.move_all == GB_SWAP);   // MODE_OVERLAP: move_all = SWAP
     const bool may_single = c.mode == MODE_WAVEFORM || (c.move ? true : c.move_all != GB_SWAP);
     for (int cN = 3; cN >= 0; cN--) {
         const int Nc = 128 << cN;
@@ -1137,6 +1169,23 @@ int gb_delta_loglike(gb_ctx* ctx, const gb_data* data, const double* params_new,
     c.n_bins = n_bins;
     c.B = B;
     c.dlnL_out = dlnL_out;
+    c.aux_out = aux_out;
+    return run_call(ctx, c, stream);
+}
+
+int gb_overlap(gb_ctx* ctx, const gb_data* data, const double* params_a, const double* params_c, const int32_t* psd_row,
+               int N, const int32_t* n_bins, int64_t B, double* overlap_out, double* aux_out, void* stream) {
+    Call c{};
+    c.mode = MODE_OVERLAP;
+    c.data = data;
+    c.params_new = params_a;
+    c.params_old = params_c;
+    c.walker_index = psd_row;
+    c.move_all = GB_SWAP;
+    c.N = N;
+    c.n_bins = n_bins;
+    c.B = B;
+    c.dlnL_out = overlap_out;
     c.aux_out = aux_out;
     return run_call(ctx, c, stream);
 }

@@ -21,7 +21,7 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
-           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep")
+           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap")
 
 BAND_MAX_STAGE = 3072
 # layout of gb_band_task (include/gbfit.h)
@@ -97,6 +97,8 @@ def lib() -> C.CDLL:
         ru = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, vp, ci, vp, i64, vp]
         L.gb_band_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gb_band_sweep.restype = ci
+        L.gb_overlap.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, ci, vp, i64, vp, vp, vp]
+        L.gb_overlap.restype = ci
         for name, sig in (("gb_waveform", wf), ("gb_waveform_host", wf), ("gb_delta_loglike", dl),
                           ("gb_delta_loglike_host", dl), ("gb_residual_update", ru),
                           ("gb_residual_update_host", ru)):
@@ -187,6 +189,21 @@ class Data:
 
     def c(self):
         return C.byref(self._c)
+
+    @classmethod
+    def psd_only(cls, psd: torch.Tensor, k_lo: int, psd_is_inverse: bool = False) -> "Data":
+        """A view without residuals, for gb_overlap: psd CUDA float64 [n_psd, 2, n_f]."""
+        if psd.dim() != 3 or psd.shape[1] != 2:
+            raise ValueError("psd must be [n_psd, 2, n_f] float64")
+        self = cls.__new__(cls)
+        self.resid, self.psd, self.walker_psd = None, psd, None
+        self.k_lo, self.n_f = int(k_lo), int(psd.shape[2])
+        self.n_walkers, self.n_psd = 0, int(psd.shape[0])
+        self.psd_is_inverse = bool(psd_is_inverse)
+        self.device = psd.device
+        self._c = GbData(None, _dev_ptr(psd, torch.float64, psd.device, "psd"), None, self.k_lo, self.n_f, 0,
+                         self.n_psd, int(self.psd_is_inverse), 0)
+        return self
 
 
 class Context:
@@ -302,6 +319,22 @@ class Context:
                                           _dev_ptr(accepted, torch.uint8, dev, "accepted"), int(N),
                                           _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B,
                                           _stream_ptr(stream, dev)))
+
+    def overlap(self, data: Data, params_a: torch.Tensor, params_c: torch.Tensor,
+                psd_row: Optional[torch.Tensor] = None, N: int = 0, n_bins: Optional[torch.Tensor] = None,
+                out: Optional[torch.Tensor] = None, aux: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """gb_overlap: normalised overlap [B] float64 (CUDA); aux [B, 2] receives <a|a>, <c|c> when given."""
+        dev = self.device
+        B = int(params_a.shape[0])
+        if out is None:
+            out = torch.empty((B,), dtype=torch.float64, device=dev)
+        self._ok(lib().gb_overlap(self._h, data.c(), _dev_ptr(params_a, torch.float64, dev, "params_a"),
+                                  _dev_ptr(params_c, torch.float64, dev, "params_c"),
+                                  _dev_ptr(psd_row, torch.int32, dev, "psd_row"), int(N),
+                                  _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B,
+                                  _dev_ptr(out, torch.float64, dev, "out"),
+                                  _dev_ptr(aux, torch.float64, dev, "aux"), _stream_ptr(stream, dev)))
+        return out
 
     def band_sweep(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
                    prop_k: torch.Tensor, prop_params: torch.Tensor, prop_logq: torch.Tensor, prop_logu: torch.Tensor,

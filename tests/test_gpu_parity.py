@@ -511,3 +511,40 @@ def test_config5_full_size_sampled(oracle, torch_cuda, gb):
         dgot = d_resid[w].cpu().numpy() - keep[w]
         assert np.abs(dref).max() > 0
         assert np.abs(dgot - dref).max() <= 1e-9 * np.abs(dref).max(), w
+
+
+# ------------------------------------------------------------------- row f4: normalised overlap of source pairs
+def test_overlap_pairs_against_oracle(oracle, torch_cuda, gb):
+    """gb_overlap on config-4-shaped pairs (jittered copies, some with offset windows), mixed window lengths,
+    several PSD rows, S_n and 1/S_n layouts, a zero-amplitude row and a row outside the fast-path limits."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(4, B=300, n_walkers=4)
+    a, c = wl.params_new.copy(), wl.params_old.copy()
+    a[:100, 1] = np.linspace(2e-4, 1.4e-2, 100)               # spread the first 100 over all window lengths
+    c[:100] = a[:100]
+    c[:100, 1] += 8e-9
+    c[:100, 6] += 0.1
+    c[100:110, 1] += 2.0 / wl.Tobs * np.arange(10)            # up to 18 bins apart
+    a[120, 0] = 0.0
+    a[121, 2] = c[121, 2] = 2e-12
+    nb = n_bins_for_f0(a[:, 1])
+    rows = (np.arange(300) % 4).astype(np.int32)
+    data_o = oracle.Data(np.zeros((1, 2, wl.n_f), np.complex128), wl.psd, wl.k_lo)
+    ref, raux = oracle.overlap(oracle.Config(), data_o, a, c, psd_row=rows, n_bins=nb, nthreads=oracle.max_threads())
+    for psd, inv in ((wl.psd, False), (1.0 / wl.psd, True)):
+        view = gbfit.Data.psd_only(dev(torch, psd), wl.k_lo, psd_is_inverse=inv)
+        aux = torch.zeros((300, 2), dtype=torch.float64, device="cuda:0")
+        got = ctx.overlap(view, dev(torch, a), dev(torch, c), psd_row=dev(torch, rows), n_bins=dev(torch, nb), aux=aux)
+        ctx.check()
+        got, aux = got.cpu().numpy(), aux.cpu().numpy()
+        assert np.abs(got - ref).max() <= 1e-10
+        assert np.abs(aux - raux).max() <= 1e-9 * raux.max() and np.abs(aux / np.maximum(raux, 1e-300) - 1)[raux > 0].max() <= 1e-9
+    assert got[120] == 0.0 and abs(got[:100]).max() <= 1.0 + 1e-12
+    same = ctx.overlap(view, dev(torch, c), dev(torch, c), N=512).cpu().numpy()     # psd_row = NULL -> row 0
+    assert np.abs(same[100:] - 1.0).max() <= 1e-12
+    bad = rows.copy(); bad[5] = 9
+    out = ctx.overlap(view, dev(torch, a), dev(torch, c), psd_row=dev(torch, bad), n_bins=dev(torch, nb))
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    assert np.isnan(out.cpu().numpy()[5])
