@@ -283,3 +283,69 @@ def make_band_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_src: int,
     return BandTasks(N, tasks, params, np.ascontiguousarray(prop_k.reshape(-1)),
                      np.ascontiguousarray(q.reshape(nt * n_prop, 8)), np.zeros(nt * n_prop),
                      np.ascontiguousarray(logu.reshape(-1)), 3 * N)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Temperature-swap tasks for the Algorithm-2 primitive: one task per
+# odd sub-band; a ladder of n_t chains on distinct walkers (a random permutation), inverse
+# temperatures 1.2^-t, each chain holding its own jittered copy of the band's "true" sources (hotter chains
+# jitter more; every other chain carries one extra weak source so the sets differ in size).
+@dataclass
+class TemperTasks:
+    N: int
+    tasks: dict                  # n_t, chain_begin, n_stage, write_back, k_first   (one entry per task)
+    params: np.ndarray           # [n_src_total, 8] all chain sets, read-only
+    truth: np.ndarray            # [n_tasks, n_src, 8] the sources the chains scatter around (to build residuals)
+    chain_walker: np.ndarray     # [n_chain] int32
+    chain_beta: np.ndarray       # [n_chain]
+    chain_set_begin: np.ndarray  # [n_chain] int32
+    chain_set_n: np.ndarray      # [n_chain] int32
+    chain_logu: np.ndarray       # [n_chain] log of the uniform draw of pair (t, t-1); entry t = 0 unused
+    max_stage: int
+
+
+def make_temper_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_t: int, n_src: int, stream: int = 0,
+                      amp_lo: float = 2e-23, amp_hi: float = 2e-22, jitter: float = 1.0) -> TemperTasks:
+    assert wl.n_walkers >= n_t
+    g = _rng(wl.config, 200 * _S_BAND + stream + N)
+    T = wl.Tobs
+    kb0 = int(np.ceil(f_lo * T / N)) * N
+    b = 2 * np.arange(n_bands, dtype=np.int64) + 1
+    u = g.random((n_bands, n_src, 8))
+    tr = np.empty((n_bands, n_src, 8))
+    tr[..., 0] = amp_lo * (amp_hi / amp_lo) ** u[..., 0]
+    tr[..., 1] = (kb0 + (b[:, None] + 0.1 + 0.8 * u[..., 1]) * N) / T
+    tr[..., 2] = (2.0 * u[..., 2] - 1.0) * 1e-16
+    tr[..., 3] = 2.0 * np.pi * u[..., 3]
+    tr[..., 4] = 1.8 * u[..., 4] - 0.9
+    tr[..., 5] = np.pi * u[..., 5]
+    tr[..., 6] = 2.0 * np.pi * u[..., 6]
+    tr[..., 7] = 1.8 * u[..., 7] - 0.9
+    sets, set_begin, set_n, walkers = [], [], [], []
+    row = 0
+    for i in range(n_bands):
+        walkers.append(g.permutation(wl.n_walkers)[:n_t].astype(np.int32))
+        for t in range(n_t):
+            z = g.standard_normal((n_src, 8)) * jitter * (1.0 + 0.5 * t)
+            s = tr[i].copy()
+            s[:, 0] *= 1.0 + 0.01 * z[:, 0]
+            s[:, 1] += 3e-10 * z[:, 1]
+            s[:, 3] += 0.01 * z[:, 3]
+            s[:, 5] += 0.01 * z[:, 5]
+            s[:, 6] += 0.005 * z[:, 6]
+            if t % 2 == 1:                                   # one extra weak source: sets of different size
+                e = tr[i, :1].copy()
+                e[0, 0] = 0.05 * amp_lo
+                e[0, 1] = (kb0 + (b[i] + g.random()) * N) / T
+                s = np.concatenate([s, e])
+            sets.append(s)
+            set_begin.append(row)
+            set_n.append(len(s))
+            row += len(s)
+    nc = n_bands * n_t
+    tasks = {"n_t": np.full(n_bands, n_t, np.int32), "chain_begin": (np.arange(n_bands) * n_t).astype(np.int32),
+             "n_stage": np.full(n_bands, 3 * N, np.int32), "write_back": np.ones(n_bands, np.int32),
+             "k_first": kb0 + (b - 1) * N}
+    return TemperTasks(N, tasks, np.ascontiguousarray(np.concatenate(sets)), tr, np.concatenate(walkers),
+                       np.tile(1.2 ** -np.arange(n_t, dtype=np.float64), n_bands), np.asarray(set_begin, np.int32),
+                       np.asarray(set_n, np.int32), np.log(g.random(nc)), 3 * N)

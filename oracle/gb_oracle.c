@@ -518,6 +518,102 @@ int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks,
     return GBO_OK;
 }
 
+/* ---- Algorithm 2 (Eq. D2): temperature swaps of one sub-band ------------
+ * One task = one sub-band b with a ladder of n_t chains.  Chain t has a residual row chain_walker[t] (the
+ * paper's permuted walker p[t]; r = d - H of that chain, reading F1-a), an inverse temperature
+ * chain_beta[t] and the set of the band's sources it currently holds, params rows
+ * [chain_set_begin[t], + chain_set_n[t]).  From the hottest pair down (t = n_t-1 .. 1) chains
+ * i = t and j = t-1 propose to exchange their sets S_i <-> S_j.  With delta = sum_{S_i} h - sum_{S_j} h on the
+ * staged bins (both residuals change by +-delta if the sets are exchanged),
+ *     D_i = lnL_i(S_j) - lnL_i(S_i) = -1/2 <delta|delta>_i - <r_i|delta>_i
+ *     D_j = lnL_j(S_i) - lnL_j(S_j) = -1/2 <delta|delta>_j + <r_j|delta>_j       (Eq. 1-2 with each chain's PSD row)
+ * and the swap is accepted iff beta_i D_i + beta_j D_j >= logu[t]   (Eq. D2 in log form; logu is an input).
+ * If accepted the sets are exchanged, r_i += delta, r_j -= delta on the staged bins of every
+ * chain whose write_back flag is set (the paper stores only the cold chain, :652-658; here every chain owns a
+ * residual), and the next pair sees the new holder of chain t-1.  Outputs per chain entry t: accepted[t] and
+ * dlnl[t] = (D_i, D_j) of the pair (t, t-1) (entry 0 unused), perm[t] = the chain whose INITIAL set ends in t. */
+typedef struct {
+    int32_t n_t, chain_begin, n_stage, write_back;
+    int64_t k_first;
+} gbo_temper_task;
+
+int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *tasks, int64_t n_tasks, int N,
+                     const double *params, const int32_t *chain_walker, const double *chain_beta,
+                     const int32_t *chain_set_begin, const int32_t *chain_set_n, const double *chain_logu,
+                     int32_t *perm_out, uint8_t *accepted_out, double *dlnl_out) {
+    if (!valid_N(N)) return GBO_ERR_INVALID;
+    double *hA = (double *)malloc(sizeof(double) * 4 * (size_t)N), *hE = hA + 2 * (size_t)N;
+    for (int64_t it = 0; it < n_tasks; it++) {
+        const gbo_temper_task *t = &tasks[it];
+        int64_t lo = t->k_first > d->k_lo ? t->k_first : d->k_lo;
+        int64_t hi = t->k_first + t->n_stage < d->k_lo + d->n_f ? t->k_first + t->n_stage : d->k_lo + d->n_f;
+        int64_t n = hi > lo ? hi - lo : 0;
+        double complex *dl = (double complex *)malloc(sizeof(double complex) * 2 * (size_t)(n > 0 ? n : 1));
+        int *holder = (int *)malloc(sizeof(int) * (size_t)(t->n_t > 0 ? t->n_t : 1));   /* whose initial set chain t holds */
+        for (int q = 0; q < t->n_t; q++) { holder[q] = q; perm_out[t->chain_begin + q] = q; accepted_out[t->chain_begin + q] = 0;
+                                           dlnl_out[2 * (t->chain_begin + q)] = dlnl_out[2 * (t->chain_begin + q) + 1] = 0.0; }
+        for (int q = t->n_t - 1; q >= 1; q--) {
+            int ci = t->chain_begin + q, cj = ci - 1;
+            int wi = chain_walker[ci], wj = chain_walker[cj];
+            if (wi < 0 || wi >= d->n_walkers || wj < 0 || wj >= d->n_walkers) { free(dl); free(holder); free(hA); return GBO_ERR_INVALID; }
+            /* delta = sum over the set chain i holds - sum over the set chain j holds, on the staged stored bins */
+            for (int64_t x = 0; x < 2 * n; x++) dl[x] = 0.0;
+            for (int side = 0; side < 2; side++) {
+                int src = t->chain_begin + holder[side == 0 ? q : q - 1];
+                double sign = side == 0 ? +1.0 : -1.0;
+                for (int sidx = 0; sidx < chain_set_n[src]; sidx++) {
+                    int64_t kh;
+                    gbo_waveform(c, params + 8 * ((size_t)chain_set_begin[src] + sidx), N, hA, hE, &kh);
+                    for (int jb = 0; jb < N; jb++) {
+                        int64_t k = kh + jb;
+                        if (k < lo || k >= hi) continue;
+                        dl[k - lo] += sign * (hA[2 * jb] + I * hA[2 * jb + 1]);
+                        dl[n + k - lo] += sign * (hE[2 * jb] + I * hE[2 * jb + 1]);
+                    }
+                }
+            }
+            double D[2];
+            for (int side = 0; side < 2; side++) {                 /* side 0: chain i (+<r|delta> enters with -), side 1: chain j */
+                int w = side == 0 ? wi : wj, row = psd_row_of(d, w);
+                double dd = 0.0, rd = 0.0;
+                for (int ch = 0; ch < 2; ch++) {
+                    const double *r = resid_ch(d, w, ch) + 2 * (lo - d->k_lo);
+                    const double *S = d->psd + ((size_t)row * 2 + (size_t)ch) * (size_t)d->n_f + (lo - d->k_lo);
+                    for (int64_t x = 0; x < n; x++) {
+                        double complex de = dl[(size_t)ch * n + x], rr = r[2 * x] + I * r[2 * x + 1];
+                        double wgt = d->psd_is_inverse ? S[x] : 1.0 / S[x];
+                        dd += wgt * creal(conj(de) * de);
+                        rd += wgt * creal(conj(rr) * de);
+                    }
+                }
+                dd *= 4.0 / c->Tobs; rd *= 4.0 / c->Tobs;
+                D[side] = side == 0 ? -0.5 * dd - rd : -0.5 * dd + rd;
+            }
+            int acc = chain_beta[ci] * D[0] + chain_beta[cj] * D[1] >= chain_logu[ci];
+            accepted_out[ci] = (uint8_t)acc;
+            dlnl_out[2 * ci] = D[0]; dlnl_out[2 * ci + 1] = D[1];
+            if (acc) {
+                int tmp = holder[q]; holder[q] = holder[q - 1]; holder[q - 1] = tmp;
+                if (t->write_back) {
+                    for (int ch = 0; ch < 2; ch++) {
+                        double *ri = (double *)resid_ch(d, wi, ch) + 2 * (lo - d->k_lo);
+                        double *rj = (double *)resid_ch(d, wj, ch) + 2 * (lo - d->k_lo);
+                        for (int64_t x = 0; x < n; x++) {
+                            double complex de = dl[(size_t)ch * n + x];
+                            ri[2 * x] += creal(de); ri[2 * x + 1] += cimag(de);
+                            rj[2 * x] -= creal(de); rj[2 * x + 1] -= cimag(de);
+                        }
+                    }
+                }
+            }
+        }
+        for (int q = 0; q < t->n_t; q++) perm_out[t->chain_begin + q] = holder[q];
+        free(dl); free(holder);
+    }
+    free(hA);
+    return GBO_OK;
+}
+
 /* orbit positions at time t, row-major [3][3] (exposed for the orbit pin) */
 void gbo_orbits(const gbo_config *c, double t, double *x_out) {
     double x[3][3];

@@ -222,6 +222,36 @@ def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, pro
     return acc, dl
 
 
+_TEMPER_TASK = np.dtype([("n_t", np.int32), ("chain_begin", np.int32), ("n_stage", np.int32), ("write_back", np.int32),
+                         ("k_first", np.int64)], align=True)
+
+
+def temper_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, chain_walker, chain_beta, chain_set_begin,
+                 chain_set_n, chain_logu):
+    """Algorithm 2 with Eq. D2, task after task.  `tasks`: dict of equal-length arrays n_t, chain_begin,
+    n_stage, write_back, k_first.  data.resid is updated in place.
+    Returns (perm[n_chain] int32, accepted[n_chain] uint8, dlnl[n_chain, 2])."""
+    n = len(tasks["n_t"])
+    t = np.zeros(n, _TEMPER_TASK)
+    for key in ("n_t", "chain_begin", "n_stage", "write_back", "k_first"):
+        t[key] = tasks[key]
+    p = _f64(params)
+    cw = np.ascontiguousarray(chain_walker, dtype=np.int32)
+    sb = np.ascontiguousarray(chain_set_begin, dtype=np.int32)
+    sn = np.ascontiguousarray(chain_set_n, dtype=np.int32)
+    cb, lu = _f64(chain_beta), _f64(chain_logu)
+    nc = cw.shape[0]
+    perm = np.zeros(nc, np.int32)
+    acc = np.zeros(nc, np.uint8)
+    dl = np.zeros((nc, 2), np.float64)
+    cc, dd = cfg.c(), data.c()
+    rc = lib().gbo_temper_sweep(C.byref(cc), C.byref(dd), _ptr(t), C.c_int64(n), C.c_int(N), _ptr(p), _ptr(cw), _ptr(cb),
+                                _ptr(sb), _ptr(sn), _ptr(lu), _ptr(perm), _ptr(acc), _ptr(dl))
+    if rc != 0:
+        raise ValueError(f"gbo_temper_sweep rc={rc}")
+    return perm, acc, dl
+
+
 def inner_windows(cfg: Config, data: Data, psd_row: int, bA, bE, kb: int, cA, cE, kc: int) -> float:
     """<b|c> of two explicit windows (step O7)."""
     bA, bE, cA, cE = (np.ascontiguousarray(z, dtype=np.complex128) for z in (bA, bE, cA, cE))

@@ -506,3 +506,80 @@ def test_overlap_closed_forms(oracle):
     z[:, 0] = 0.0
     o5, _ = oracle.overlap(cfg, data, p[:2], z, n_bins=nb[:2])
     assert np.all(o5 == 0.0)
+
+
+# ------------------------------------------------------------- Algorithm 2 (Eq. D2), row f2
+def _chain_lnL(wl, resid, w, k_first, n_stage):
+    return _staged_lnL(wl, resid, w, k_first, n_stage)
+
+
+def test_temper_sweep_matches_the_likelihood_definition_and_eq_d2(oracle):
+    """Every pair: D_i, D_j are the lnL differences obtained by actually exchanging the sets in the residuals and
+    evaluating -1/2 <r|r> on the staged bins; the decision is Eq. D2 in log form; accepted exchanges move the sets."""
+    from temper_setup import temper_case
+    wl, tt, resid = temper_case(oracle)
+    cfg = oracle.Config()
+    t = tt.tasks
+    r_run = resid.copy()
+    perm, acc, dl = oracle.temper_sweep(cfg, oracle.Data(r_run, wl.psd, wl.k_lo), t, tt.N, tt.params, tt.chain_walker,
+                                        tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)
+    assert 0 < acc.sum() < (t["n_t"] - 1).sum()
+    r_ref = resid.copy()                                      # replay with the plain update primitive
+    data = oracle.Data(r_ref, wl.psd, wl.k_lo)
+    for i in range(len(t["n_t"])):
+        cb, nt, k0, ns = int(t["chain_begin"][i]), int(t["n_t"][i]), int(t["k_first"][i]), int(t["n_stage"][i])
+        holder = list(range(nt))
+        for q in range(nt - 1, 0, -1):
+            wi, wj = int(tt.chain_walker[cb + q]), int(tt.chain_walker[cb + q - 1])
+            Si = tt.params[tt.chain_set_begin[cb + holder[q]]:][:tt.chain_set_n[cb + holder[q]]]
+            Sj = tt.params[tt.chain_set_begin[cb + holder[q - 1]]:][:tt.chain_set_n[cb + holder[q - 1]]]
+            before = (_chain_lnL(wl, r_ref, wi, k0, ns), _chain_lnL(wl, r_ref, wj, k0, ns))
+            trial = r_ref.copy()
+            dtrial = oracle.Data(trial, wl.psd, wl.k_lo)
+            for w, old, new in ((wi, Si, Sj), (wj, Sj, Si)):
+                for src in old:
+                    oracle.residual_update(cfg, dtrial, None, src[None], np.full(1, w, np.int32), move_all=oracle.REMOVE, N=tt.N)
+                for src in new:
+                    oracle.residual_update(cfg, dtrial, src[None], None, np.full(1, w, np.int32), move_all=oracle.ADD, N=tt.N)
+            after = (_chain_lnL(wl, trial, wi, k0, ns), _chain_lnL(wl, trial, wj, k0, ns))
+            Di, Dj = after[0] - before[0], after[1] - before[1]
+            assert abs(dl[cb + q, 0] - Di) <= 1e-9 * max(1.0, abs(before[0])), (i, q)
+            assert abs(dl[cb + q, 1] - Dj) <= 1e-9 * max(1.0, abs(before[1])), (i, q)
+            ok = tt.chain_beta[cb + q] * dl[cb + q, 0] + tt.chain_beta[cb + q - 1] * dl[cb + q, 1] >= tt.chain_logu[cb + q]
+            assert bool(acc[cb + q]) == bool(ok)
+            if ok:
+                holder[q], holder[q - 1] = holder[q - 1], holder[q]
+                r_ref[...] = trial
+        assert list(perm[cb:cb + nt]) == holder
+    scale = np.abs(r_ref - resid).max()
+    assert scale > 0 and np.abs(r_run - r_ref).max() <= 1e-10 * scale + 4e-16 * np.abs(resid).max()
+
+
+def test_temper_sweep_reduces_to_eq_d1_for_a_shared_likelihood_and_bubbles_when_all_accepted(oracle):
+    from temper_setup import temper_case
+    wl, tt, resid = temper_case(oracle, n_bands=2)
+    cfg = oracle.Config()
+    # same data and PSD for every chain (noise of walker 0 everywhere): D_j = -D_i, Eq. D2 -> Eq. D1 (PAPER.md:674-687)
+    same = resid.copy()
+    base = wl.resid()
+    same += base[:1] - base
+    psd1 = np.repeat(wl.psd[:1], wl.psd.shape[0], axis=0)
+    perm, acc, dl = oracle.temper_sweep(cfg, oracle.Data(same.copy(), psd1, wl.k_lo), tt.tasks, tt.N, tt.params,
+                                        tt.chain_walker, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n,
+                                        np.full_like(tt.chain_logu, np.inf))          # nothing accepted: pure evaluation
+    used = np.ones(len(tt.chain_walker), bool)
+    used[tt.tasks["chain_begin"]] = False
+    assert not acc.any() and np.abs(dl[used, 0] + dl[used, 1]).max() <= 1e-8 * np.abs(dl[used]).max()
+    # everything accepted: the hottest chain's set bubbles down to the cold chain, the others move up by one
+    r = resid.copy()
+    perm, acc, _ = oracle.temper_sweep(cfg, oracle.Data(r, wl.psd, wl.k_lo), tt.tasks, tt.N, tt.params, tt.chain_walker,
+                                       tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, np.full_like(tt.chain_logu, -np.inf))
+    nt = int(tt.tasks["n_t"][0])
+    for cb in tt.tasks["chain_begin"]:
+        assert list(perm[cb:cb + nt]) == [nt - 1] + list(range(nt - 1)) and acc[cb + 1:cb + nt].all() and not acc[cb]
+    # write_back = 0: decisions and permutation as before, residuals untouched
+    t0 = dict(tt.tasks, write_back=np.zeros_like(tt.tasks["write_back"]))
+    r0 = resid.copy()
+    p0, a0, _ = oracle.temper_sweep(cfg, oracle.Data(r0, wl.psd, wl.k_lo), t0, tt.N, tt.params, tt.chain_walker, tt.chain_beta,
+                                    tt.chain_set_begin, tt.chain_set_n, np.full_like(tt.chain_logu, np.inf))
+    assert np.array_equal(r0, resid) and not a0.any() and list(p0[:nt]) == list(range(nt))
