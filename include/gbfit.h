@@ -223,6 +223,35 @@ int gb_band_sweep(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, i
                   double *params, const int32_t *prop_k, const double *prop_params, const double *prop_logq,
                   const double *prop_logu, uint8_t *accepted_out, double *dlnL_out, void *stream);
 
+/*
+ * gb_temper_sweep -- Algorithm 2 of the paper ("Galaxy Tempering algorithm") with the swap acceptance
+ * of Eq. D2 for walkers that carry different residuals / PSDs.  One task = one sub-band with a ladder of
+ * n_t chains (n_t <= GB_TEMPER_MAX_LADDER); chain entry c = chain_begin + t has
+ *   chain_walker[c]     residual row of chain t (the paper's permuted walker p[t]; r = d - H of that chain)
+ *   chain_beta[c]       inverse temperature
+ *   chain_set_begin[c], chain_set_n[c]   the band's sources the chain holds at entry: rows of params (read-only)
+ *   chain_logu[c]       log of the uniform draw of the pair (t, t-1); entry t = 0 unused
+ * From t = n_t - 1 down to 1 chains i = t and j = t - 1 propose to exchange the sets S_i, S_j they currently hold.  With
+ * delta = sum_{S_i} h - sum_{S_j} h on the staged bins,  D_i = lnL_i(S_j) - lnL_i(S_i) = -1/2 <delta|delta>_i - <r_i|delta>_i,
+ * D_j = lnL_j(S_i) - lnL_j(S_j) = -1/2 <delta|delta>_j + <r_j|delta>_j  (each chain's own PSD row), accepted iff
+ * beta_i D_i + beta_j D_j >= logu.  Accepted: the holders are exchanged and, if write_back, r_i += delta, r_j -= delta in
+ * data->resid (FP64 atomics; the paper keeps only the cold chain's residual, here every chain owns one).
+ * Outputs [n_chain]: perm_out[c] = ladder position whose INITIAL set ends in chain t; accepted_out[c]; dlnl_out[c][2] =
+ * (D_i, D_j) of pair (t, t-1).  All arrays DEVICE.  N, max_stage, odd/even rule, errors and asynchrony as gb_band_sweep.
+ */
+#define GB_TEMPER_MAX_LADDER 64
+typedef struct {
+    int32_t n_t;          /* chains of the ladder                    */
+    int32_t chain_begin;  /* first chain entry of the task           */
+    int32_t n_stage;      /* staged bins                             */
+    int32_t write_back;   /* != 0: accepted exchanges update data->resid */
+    int64_t k_first;      /* global bin of staged bin 0              */
+} gb_temper_task;
+int gb_temper_sweep(gb_ctx *ctx, const gb_data *data, const gb_temper_task *tasks, int64_t n_tasks, int N, int max_stage,
+                    const double *params, const int32_t *chain_walker, const double *chain_beta,
+                    const int32_t *chain_set_begin, const int32_t *chain_set_n, const double *chain_logu,
+                    int32_t *perm_out, uint8_t *accepted_out, double *dlnl_out, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgbfit.so")
 SOURCES = ["gbfit.cu"]
-HEADERS = ["gb_math.cuh", "gb_fast.cuh", "gb_sincos_poly.h", "gb_fft.cuh", "gb_band.cuh", "gb_tables.hpp", os.path.join("..", "..", "include", "gbfit.h")]
+HEADERS = ["gb_math.cuh", "gb_fast.cuh", "gb_sincos_poly.h", "gb_fft.cuh", "gb_band.cuh", "gb_temper.cuh", "gb_tables.hpp", os.path.join("..", "..", "include", "gbfit.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

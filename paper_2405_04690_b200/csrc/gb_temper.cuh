@@ -1,0 +1,193 @@
+// gb_temper.cuh -- Algorithm 2 of the paper as a kernel (Eq. D2).
+// Included by gbfit.cu inside its anonymous namespace, after slow_part / fft_store / group_reduce.
+//
+// One CTA owns one sub-band's temperature ladder.  From the hottest pair down, chains i = t and j = t-1 propose to
+// exchange the source sets they hold: the CTA builds delta = sum_{S_i} h - sum_{S_j} h on the staged bins in shared
+// memory (one slow part + FFT per source, accumulated with its sign), reduces <delta|delta> and <r|delta> against
+// both chains' residuals and PSD rows (read through L2), and thread 0 decides beta_i D_i + beta_j D_j >= logu
+// with D_i = -1/2 <d|d>_i - <r_i|d>_i, D_j = -1/2 <d|d>_j + <r_j|d>_j.  An accepted exchange swaps the holders and
+// (write_back) adds +-delta to the two stored residuals with FP64 atomics; the next pair then reads the updated
+// residual of chain t-1 (the atomics resolve in L2, the reads are ld.global.cg after a fence and a barrier).
+#pragma once
+
+constexpr int kMaxLadder = 64;
+
+struct TemperArgs {
+    const gb_temper_task* tasks;
+    int64_t n_tasks;
+    const double* params;
+    const int32_t* chain_walker;
+    const double* chain_beta;
+    const int32_t* chain_set_begin;
+    const int32_t* chain_set_n;
+    const double* chain_logu;
+    int32_t* perm_out;
+    uint8_t* accepted_out;
+    double* dlnl_out;
+    const double* orbit;
+    const cx* tw;
+    double* resid;
+    const double* psd;
+    const int32_t* walker_psd;
+    int64_t k_lo, n_f;
+    int32_t n_walkers, n_psd, psd_is_inverse, max_stage;
+    double Tobs, tau, Rmax;
+    int64_t kmax;
+    int32_t* errflag;
+};
+
+template <int N>
+constexpr size_t temper_smem_bytes(int max_stage) {
+    return (size_t)padded_len<N>() * sizeof(cx) * 2 + (size_t)max_stage * 32;
+}
+
+template <int N>
+__global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
+    constexpr int G = Plan<N>::G;
+    constexpr int S = N / G;
+    constexpr int PN = padded_len<N>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx* bufA = reinterpret_cast<cx*>(smem_raw);
+    cx* bufE = bufA + PN;
+    cx* dA = bufE + PN;                 // delta on the staged bins
+    cx* dE = dA + a.max_stage;
+    __shared__ __align__(16) SrcConst s_src;
+    __shared__ double s_red[(G / 32) * 4 + 1];
+    __shared__ int s_holder[kMaxLadder];
+    __shared__ int s_acc;
+    const int tid = threadIdx.x;
+    const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    const size_t nf = (size_t)a.n_f;
+
+    for (int64_t it = blockIdx.x; it < a.n_tasks; it += gridDim.x) {
+        const gb_temper_task t = a.tasks[it];
+        bool ok = t.n_t >= 0 && t.n_t <= kMaxLadder && t.n_stage >= 0 && t.n_stage <= a.max_stage;
+        for (int q = 0; ok && q < t.n_t; q++) {
+            const int w = a.chain_walker[t.chain_begin + q];
+            ok = w >= 0 && w < a.n_walkers && a.chain_set_n[t.chain_begin + q] >= 0;
+        }
+        for (int q = tid; q < t.n_t; q += G) {
+            const int c = t.chain_begin + q;
+            if (q < kMaxLadder) s_holder[q] = q;
+            a.perm_out[c] = q;
+            a.accepted_out[c] = 0;
+            a.dlnl_out[2 * c] = a.dlnl_out[2 * c + 1] = (ok || q == 0) ? 0.0 : nan;
+        }
+        if (!ok) {
+            if (tid == 0) atomicOr(a.errflag, 1);
+            continue;
+        }
+        group_sync<G>();
+        const int64_t i_first = t.k_first - a.k_lo;
+        for (int q = t.n_t - 1; q >= 1; q--) {
+            const int ci = t.chain_begin + q, cj = ci - 1;
+            // ---- delta = sum over the set chain i holds - sum over the set chain j holds
+            for (int i = tid; i < t.n_stage; i += G) {
+                dA[i] = {0.0, 0.0};
+                dE[i] = {0.0, 0.0};
+            }
+            group_sync<G>();
+            for (int side = 0; side < 2; side++) {
+                const int src = t.chain_begin + s_holder[side == 0 ? q : q - 1];
+                const double sign = side == 0 ? 1.0 : -1.0;
+                const int n_set = a.chain_set_n[src];
+                const double* set = a.params + 8 * (size_t)a.chain_set_begin[src];
+                for (int sidx = 0; sidx < n_set; sidx++) {
+                    if (tid == 0) {
+                        SrcConst s;
+                        source_constants(set + 8 * sidx, a.Tobs, a.tau, N, s);
+                        s.fast = fast_path_ok(set + 8 * sidx, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                        if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                        s_src = s;
+                    }
+                    group_sync<G>();
+                    if (s_src.fast) slow_part<N, G, true>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
+                    else slow_part<N, G, false>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
+                    fft_store<N>(bufA, bufE, a.tw, tid);
+                    const int64_t j0 = s_src.kmin - t.k_first;
+#pragma unroll
+                    for (int m = 0; m < S; m++) {
+                        const int j = tid + G * m;
+                        const int64_t i = j0 + j;
+                        if (i >= 0 && i < t.n_stage) {
+                            const cx ha = bufA[pad_idx<N>(j)], he = bufE[pad_idx<N>(j)];
+                            dA[i] = {dA[i].re + sign * ha.re, dA[i].im + sign * ha.im};
+                            dE[i] = {dE[i].re + sign * he.re, dE[i].im + sign * he.im};
+                        }
+                    }
+                    group_sync<G>();
+                }
+            }
+            // ---- <delta|delta> and <r|delta> for both chains, stored bins only
+            const int wi = a.chain_walker[ci], wj = a.chain_walker[cj];
+            const int rowi = a.walker_psd ? a.walker_psd[wi] : (a.n_psd == 1 ? 0 : wi);
+            const int rowj = a.walker_psd ? a.walker_psd[wj] : (a.n_psd == 1 ? 0 : wj);
+            double* rAi = a.resid + ((size_t)wi * 2 + 0) * nf * 2;
+            double* rEi = a.resid + ((size_t)wi * 2 + 1) * nf * 2;
+            double* rAj = a.resid + ((size_t)wj * 2 + 0) * nf * 2;
+            double* rEj = a.resid + ((size_t)wj * 2 + 1) * nf * 2;
+            const double* SAi = a.psd + ((size_t)rowi * 2 + 0) * nf;
+            const double* SEi = a.psd + ((size_t)rowi * 2 + 1) * nf;
+            const double* SAj = a.psd + ((size_t)rowj * 2 + 0) * nf;
+            const double* SEj = a.psd + ((size_t)rowj * 2 + 1) * nf;
+            const bool inv = a.psd_is_inverse != 0;
+            double v[4] = {0.0, 0.0, 0.0, 0.0};   // dd_i, rd_i, dd_j, rd_j
+            for (int i = tid; i < t.n_stage; i += G) {
+                const int64_t e = i_first + i;
+                if (e < 0 || e >= a.n_f) continue;
+                const cx da = dA[i], de = dE[i];
+                const double na = da.re * da.re + da.im * da.im, ne = de.re * de.re + de.im * de.im;
+                {
+                    const double2 ra = __ldcg(reinterpret_cast<const double2*>(rAi + 2 * e));
+                    const double2 re = __ldcg(reinterpret_cast<const double2*>(rEi + 2 * e));
+                    const double wa = inv ? SAi[e] : 1.0 / SAi[e], we = inv ? SEi[e] : 1.0 / SEi[e];
+                    v[0] += wa * na + we * ne;
+                    v[1] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
+                }
+                {
+                    const double2 ra = __ldcg(reinterpret_cast<const double2*>(rAj + 2 * e));
+                    const double2 re = __ldcg(reinterpret_cast<const double2*>(rEj + 2 * e));
+                    const double wa = inv ? SAj[e] : 1.0 / SAj[e], we = inv ? SEj[e] : 1.0 / SEj[e];
+                    v[2] += wa * na + we * ne;
+                    v[3] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
+                }
+            }
+            group_reduce<G, 4>(v, s_red, tid);
+            if (tid == 0) {
+                const double norm = 4.0 / a.Tobs;
+                const double Di = -0.5 * norm * v[0] - norm * v[1];
+                const double Dj = -0.5 * norm * v[2] + norm * v[3];
+                const int acc = a.chain_beta[ci] * Di + a.chain_beta[cj] * Dj >= a.chain_logu[ci] ? 1 : 0;
+                a.accepted_out[ci] = (uint8_t)acc;
+                a.dlnl_out[2 * ci] = Di;
+                a.dlnl_out[2 * ci + 1] = Dj;
+                s_acc = acc;
+                if (acc) {
+                    const int h = s_holder[q];
+                    s_holder[q] = s_holder[q - 1];
+                    s_holder[q - 1] = h;
+                }
+            }
+            group_sync<G>();
+            if (s_acc && t.write_back) {   // r_i += delta, r_j -= delta
+                for (int i = tid; i < t.n_stage; i += G) {
+                    const int64_t e = i_first + i;
+                    if (e < 0 || e >= a.n_f) continue;
+                    const cx da = dA[i], de = dE[i];
+                    atomicAdd(rAi + 2 * e, da.re);
+                    atomicAdd(rAi + 2 * e + 1, da.im);
+                    atomicAdd(rEi + 2 * e, de.re);
+                    atomicAdd(rEi + 2 * e + 1, de.im);
+                    atomicAdd(rAj + 2 * e, -da.re);
+                    atomicAdd(rAj + 2 * e + 1, -da.im);
+                    atomicAdd(rEj + 2 * e, -de.re);
+                    atomicAdd(rEj + 2 * e + 1, -de.im);
+                }
+                __threadfence();
+            }
+            group_sync<G>();
+        }
+        for (int q = tid; q < t.n_t; q += G) a.perm_out[t.chain_begin + q] = s_holder[q];
+        group_sync<G>();
+    }
+}

@@ -740,6 +740,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
 }
 
 #include "gb_band.cuh"
+#include "gb_temper.cuh"
 
 template <int N, bool SWAP>
 constexpr size_t main_smem_bytes() {
@@ -1017,6 +1018,20 @@ int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
     return GB_OK;
 }
 
+template <int N>
+int launch_temper(gb_ctx* ctx, const TemperArgs& a, cudaStream_t st) {
+    const size_t smem = temper_smem_bytes<N>(a.max_stage);
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_temper_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int nb = 0;
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_temper_kernel<N>, Plan<N>::G, smem));
+    if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
+    int64_t grid = (int64_t)nb * ctx->num_sms;
+    if (grid > a.n_tasks) grid = a.n_tasks;
+    gb_temper_kernel<N><<<(unsigned)grid, Plan<N>::G, smem, st>>>(a);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+    return GB_OK;
+}
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------ C ABI
@@ -1253,6 +1268,58 @@ int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, i
         case 256: return launch_band<256>(ctx, a, st);
         case 512: return launch_band<512>(ctx, a, st);
         default: return launch_band<1024>(ctx, a, st);
+    }
+}
+
+int gb_temper_sweep(gb_ctx* ctx, const gb_data* data, const gb_temper_task* tasks, int64_t n_tasks, int N, int max_stage,
+                    const double* params, const int32_t* chain_walker, const double* chain_beta,
+                    const int32_t* chain_set_begin, const int32_t* chain_set_n, const double* chain_logu,
+                    int32_t* perm_out, uint8_t* accepted_out, double* dlnl_out, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (n_tasks < 0 || n_tasks > 0x7fffffff) return set_err(ctx, GB_ERR_INVALID, "n_tasks out of range");
+    if (n_tasks == 0) return GB_OK;
+    if (!data || !data->resid || !data->psd || data->n_f <= 0 || data->n_walkers <= 0)
+        return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
+    if (!tasks || !params || !chain_walker || !chain_beta || !chain_set_begin || !chain_set_n || !chain_logu || !perm_out ||
+        !accepted_out || !dlnl_out)
+        return set_err(ctx, GB_ERR_INVALID, "NULL argument");
+    if (!(N == 128 || N == 256 || N == 512 || N == 1024)) return set_err(ctx, GB_ERR_INVALID, "N must be 128, 256, 512 or 1024");
+    if (max_stage < 1 || max_stage > GB_BAND_MAX_STAGE) return set_err(ctx, GB_ERR_INVALID, "max_stage out of range");
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    TemperArgs a{};
+    a.tasks = tasks;
+    a.n_tasks = n_tasks;
+    a.params = params;
+    a.chain_walker = chain_walker;
+    a.chain_beta = chain_beta;
+    a.chain_set_begin = chain_set_begin;
+    a.chain_set_n = chain_set_n;
+    a.chain_logu = chain_logu;
+    a.perm_out = perm_out;
+    a.accepted_out = accepted_out;
+    a.dlnl_out = dlnl_out;
+    a.orbit = ctx->d_orbit[N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3];
+    a.tw = ctx->d_tw;
+    a.resid = data->resid;
+    a.psd = data->psd;
+    a.walker_psd = data->walker_psd;
+    a.k_lo = data->k_lo;
+    a.n_f = data->n_f;
+    a.n_walkers = data->n_walkers;
+    a.n_psd = data->n_psd;
+    a.psd_is_inverse = data->psd_is_inverse;
+    a.max_stage = max_stage;
+    a.Tobs = ctx->cfg.Tobs;
+    a.tau = ctx->cfg.armlength / kCLight;
+    a.Rmax = ctx->cfg.au / kCLight;
+    a.kmax = (int64_t)floor(ctx->cfg.Tobs / (2.0 * ctx->cfg.dt));
+    a.errflag = ctx->d_counts + 2 * kNumClasses;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    switch (N) {
+        case 128: return launch_temper<128>(ctx, a, st);
+        case 256: return launch_temper<256>(ctx, a, st);
+        case 512: return launch_temper<512>(ctx, a, st);
+        default: return launch_temper<1024>(ctx, a, st);
     }
 }
 

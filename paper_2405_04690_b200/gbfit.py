@@ -21,13 +21,28 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
-           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap")
+           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep")
 
 BAND_MAX_STAGE = 3072
 # layout of gb_band_task (include/gbfit.h)
 BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
                       ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
                       ("write_back", np.int32), ("reserved", np.int32), ("beta", np.float64)], align=True)
+
+
+TEMPER_MAX_LADDER = 64
+# layout of gb_temper_task (include/gbfit.h)
+TEMPER_TASK = np.dtype([("n_t", np.int32), ("chain_begin", np.int32), ("n_stage", np.int32), ("write_back", np.int32),
+                        ("k_first", np.int64)], align=True)
+
+
+def pack_temper_tasks(n_t, chain_begin, n_stage, write_back, k_first) -> np.ndarray:
+    """Host array of gb_temper_task records from equal-length columns."""
+    t = np.zeros(len(n_t), TEMPER_TASK)
+    for key, val in (("n_t", n_t), ("chain_begin", chain_begin), ("n_stage", n_stage), ("write_back", write_back),
+                     ("k_first", k_first)):
+        t[key] = val
+    return t
 
 
 def pack_band_tasks(walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta) -> np.ndarray:
@@ -99,6 +114,8 @@ def lib() -> C.CDLL:
         L.gb_band_sweep.restype = ci
         L.gb_overlap.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, ci, vp, i64, vp, vp, vp]
         L.gb_overlap.restype = ci
+        L.gb_temper_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.gb_temper_sweep.restype = ci
         for name, sig in (("gb_waveform", wf), ("gb_waveform_host", wf), ("gb_delta_loglike", dl),
                           ("gb_delta_loglike_host", dl), ("gb_residual_update", ru),
                           ("gb_residual_update_host", ru)):
@@ -335,6 +352,29 @@ class Context:
                                   _dev_ptr(out, torch.float64, dev, "out"),
                                   _dev_ptr(aux, torch.float64, dev, "aux"), _stream_ptr(stream, dev)))
         return out
+
+    def temper_sweep(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
+                     chain_walker: torch.Tensor, chain_beta: torch.Tensor, chain_set_begin: torch.Tensor,
+                     chain_set_n: torch.Tensor, chain_logu: torch.Tensor, stream=None):
+        """gb_temper_sweep (Algorithm 2, Eq. D2): `tasks` is a CUDA uint8 tensor of packed gb_temper_task records
+        (pack_temper_tasks).  Returns (perm int32, accepted uint8, dlnl [n_chain, 2] float64), CUDA tensors;
+        data.resid is updated in place for accepted exchanges of tasks with write_back."""
+        dev = self.device
+        n_tasks = int(tasks.numel() // TEMPER_TASK.itemsize)
+        nc = int(chain_walker.shape[0])
+        perm = torch.zeros((nc,), dtype=torch.int32, device=dev)
+        acc = torch.zeros((nc,), dtype=torch.uint8, device=dev)
+        dl = torch.zeros((nc, 2), dtype=torch.float64, device=dev)
+        self._ok(lib().gb_temper_sweep(self._h, data.c(), _dev_ptr(tasks, torch.uint8, dev, "tasks"), n_tasks, int(N),
+                                       int(max_stage), _dev_ptr(params, torch.float64, dev, "params"),
+                                       _dev_ptr(chain_walker, torch.int32, dev, "chain_walker"),
+                                       _dev_ptr(chain_beta, torch.float64, dev, "chain_beta"),
+                                       _dev_ptr(chain_set_begin, torch.int32, dev, "chain_set_begin"),
+                                       _dev_ptr(chain_set_n, torch.int32, dev, "chain_set_n"),
+                                       _dev_ptr(chain_logu, torch.float64, dev, "chain_logu"),
+                                       _dev_ptr(perm, torch.int32, dev, "perm"), _dev_ptr(acc, torch.uint8, dev, "acc"),
+                                       _dev_ptr(dl, torch.float64, dev, "dl"), _stream_ptr(stream, dev)))
+        return perm, acc, dl
 
     def band_sweep(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
                    prop_k: torch.Tensor, prop_params: torch.Tensor, prop_logq: torch.Tensor, prop_logu: torch.Tensor,

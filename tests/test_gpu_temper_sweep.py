@@ -1,0 +1,92 @@
+"""Parity of gb_temper_sweep (Algorithm 2 with Eq. D2) with the CPU
+oracle on the same seeded ladders: decisions and final permutations bit-exact, (D_i, D_j) <= 1e-6 absolute, final
+residuals <= 1e-9 of the largest change."""
+import numpy as np
+import pytest
+
+from temper_setup import temper_case
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu-marked parity tests must run on a B200 box")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def gb(torch_cuda):
+    from paper_2405_04690_b200 import gbfit
+    ctx = gbfit.Context(0)
+    yield gbfit, ctx
+    ctx.close()
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def run_both(oracle, torch, gbfit, ctx, wl, tt, resid, tasks=None, logu=None, psd=None, inverse=False):
+    t = tt.tasks if tasks is None else tasks
+    lu = tt.chain_logu if logu is None else logu
+    r_ref = resid.copy()
+    ref = oracle.temper_sweep(oracle.Config(), oracle.Data(r_ref, wl.psd, wl.k_lo), t, tt.N, tt.params, tt.chain_walker,
+                              tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, lu)
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd if psd is None else psd), wl.k_lo, psd_is_inverse=inverse)
+    packed = gbfit.pack_temper_tasks(**t)
+    got = ctx.temper_sweep(data, dev(torch, packed.view(np.uint8)), tt.N, int(t["n_stage"].max()), dev(torch, tt.params),
+                           dev(torch, tt.chain_walker), dev(torch, tt.chain_beta), dev(torch, tt.chain_set_begin),
+                           dev(torch, tt.chain_set_n), dev(torch, lu))
+    ctx.check()
+    perm, acc, dl = (x.cpu().numpy() for x in got)
+    assert np.array_equal(acc, ref[1]), int((acc != ref[1]).sum())
+    assert np.array_equal(perm, ref[0])
+    assert np.abs(dl - ref[2]).max() <= 1e-6
+    change = np.abs(r_ref - resid).max()
+    assert np.abs(d_resid.cpu().numpy() - r_ref).max() <= 1e-9 * change + 4e-16 * np.abs(resid).max()
+    return ref
+
+
+@pytest.mark.parametrize("N,f_lo,amp", [(128, 6e-4, 2e-22), (256, 2e-3, 1e-22), (512, 6e-3, 3e-23), (1024, 1.2e-2, 8e-24)])
+def test_temper_sweep_each_window_length(oracle, torch_cuda, gb, N, f_lo, amp):
+    gbfit, ctx = gb
+    wl, tt, resid = temper_case(oracle, N=N, f_lo=f_lo, n_bands=3, n_t=5, n_src=3, n_walkers=6, amp=(0.1 * amp, amp))
+    ref = run_both(oracle, torch_cuda, gbfit, ctx, wl, tt, resid)
+    assert ref[1].any()
+
+
+def test_temper_sweep_all_accepted_none_accepted_no_write_back_inverse_psd_and_bad_tasks(oracle, torch_cuda, gb):
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl, tt, resid = temper_case(oracle, N=256, f_lo=2.5e-3, n_bands=4, n_t=6, n_src=2, n_walkers=7, stream=3)
+    for lu in (np.full_like(tt.chain_logu, -np.inf), np.full_like(tt.chain_logu, np.inf)):
+        run_both(oracle, torch, gbfit, ctx, wl, tt, resid, logu=lu)
+    t0 = dict(tt.tasks, write_back=np.zeros_like(tt.tasks["write_back"]))
+    run_both(oracle, torch, gbfit, ctx, wl, tt, resid, tasks=t0, logu=np.full_like(tt.chain_logu, -np.inf))
+    run_both(oracle, torch, gbfit, ctx, wl, tt, resid, psd=1.0 / wl.psd, inverse=True)
+    # staged range partly below the stored band, a ladder of one chain (nothing to do), an empty set
+    t1 = {k: v.copy() for k, v in tt.tasks.items()}
+    t1["k_first"][0] = wl.k_lo - 5 * tt.N
+    t1["n_t"][1] = 1
+    sn = tt.chain_set_n.copy()
+    sn[t1["chain_begin"][2] + 1] = 0
+    import copy
+    tt2 = copy.copy(tt)
+    tt2.chain_set_n = sn
+    run_both(oracle, torch, gbfit, ctx, wl, tt2, resid, tasks=t1)
+    # invalid walker -> sticky flag and NaN for that ladder
+    bad = tt.chain_walker.copy()
+    bad[tt.tasks["chain_begin"][1] + 2] = 99
+    data = gbfit.Data(dev(torch, resid), dev(torch, wl.psd), wl.k_lo)
+    packed = gbfit.pack_temper_tasks(**tt.tasks)
+    perm, acc, dl = ctx.temper_sweep(data, dev(torch, packed.view(np.uint8)), tt.N, tt.max_stage, dev(torch, tt.params),
+                                     dev(torch, bad), dev(torch, tt.chain_beta), dev(torch, tt.chain_set_begin),
+                                     dev(torch, tt.chain_set_n), dev(torch, tt.chain_logu))
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    cb = tt.tasks["chain_begin"][1]
+    assert np.isnan(dl.cpu().numpy()[cb + 1:cb + 6]).all() and np.isfinite(dl.cpu().numpy()[:cb]).all()
