@@ -354,6 +354,36 @@ def run_ours(args):
                 "note": "each proposal = 2 waveforms + Eq. 5 against the staged residual + accept/reject + update; "
                         "includes the device-side reset of the 38 MB parameter array before each call"}
 
+    # ---- SURVEY 8(f) row f2, outside the timed step: Algorithm 2 (gb_temper_sweep), 10-chain ladders ------
+    # every odd 256-bin sub-band of 1-4 mHz, 36 ladders per band on disjoint residuals, 9-10 sources per chain
+    tmp = None
+    if rank == 0 and full and not args.no_band_sweep:
+        from gb_inputs import make_temper_tasks
+        tt = make_temper_tasks(wl, 256, 1e-3, n_bands=183, n_t=10, n_src=9, n_groups=36)
+        d_tt = torch.from_numpy(gbfit.pack_temper_tasks(**tt.tasks).view(np.uint8)).to(dev)
+        # the bench residuals hold no signals, so hardly any exchange would pass Eq. D2: force a seeded quarter of the
+        # pairs to be accepted (logu = -inf) so that the holder swap and the atomic residual update are in the timing
+        lu = tt.chain_logu.copy()
+        lu[np.random.Generator(np.random.Philox(key=[5, 77])).random(lu.size) < 0.25] = -np.inf
+        targs = [torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in
+                 (tt.params, tt.chain_walker, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, lu)]
+        t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(4):
+            if i == 1:
+                t0e.record(stream)
+            t_perm, t_acc, t_dl = ctx.temper_sweep(data, d_tt, 256, tt.max_stage, *targs)
+        t1e.record(stream)
+        torch.cuda.synchronize()
+        ctx.check()
+        ms_t = t0e.elapsed_time(t1e) / 3
+        n_pairs_t = int((tt.tasks["n_t"] - 1).sum())
+        n_wave = int(sum(int(tt.chain_set_n[c:c + 10].sum()) * 2 - int(tt.chain_set_n[c]) - int(tt.chain_set_n[c + 9])
+                         for c in tt.tasks["chain_begin"]))
+        tmp = {"call": "gb_temper_sweep (Algorithm 2, Eq. D2)", "N": 256, "ladders": int(len(tt.tasks["n_t"])), "chains": 10,
+               "swap_proposals": n_pairs_t, "waveforms_per_call_at_least": n_wave, "ms_per_call": ms_t,
+               "swap_proposals_per_s": n_pairs_t / (ms_t * 1e-3), "waveforms_per_s": n_wave / (ms_t * 1e-3),
+               "accepted_fraction_last_call": float(t_acc.float().sum().item()) / n_pairs_t}
+
     # ---- SURVEY 8(f) row f4, outside the timed step: normalised overlaps of 1 M source pairs (gb_overlap) ----
     ovl = None
     if rank == 0 and full and not args.no_band_sweep:
@@ -450,7 +480,7 @@ def run_ours(args):
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "band_sweep": band, "overlap": ovl,
+            "band_sweep": band, "temper_sweep": tmp, "overlap": ovl,
         }
         print(json.dumps(line), flush=True)
     ctx.close()

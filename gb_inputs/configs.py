@@ -305,8 +305,9 @@ class TemperTasks:
 
 
 def make_temper_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_t: int, n_src: int, stream: int = 0,
-                      amp_lo: float = 2e-23, amp_hi: float = 2e-22, jitter: float = 1.0) -> TemperTasks:
-    assert wl.n_walkers >= n_t
+                      amp_lo: float = 2e-23, amp_hi: float = 2e-22, jitter: float = 1.0, n_groups: int = 1) -> TemperTasks:
+    """n_groups ladders per sub-band on disjoint walkers (tasks are ordered band-major); truth is per band."""
+    assert wl.n_walkers >= n_t * n_groups
     g = _rng(wl.config, 200 * _S_BAND + stream + N)
     T = wl.Tobs
     kb0 = int(np.ceil(f_lo * T / N)) * N
@@ -323,8 +324,10 @@ def make_temper_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_t: int,
     tr[..., 7] = 1.8 * u[..., 7] - 0.9
     sets, set_begin, set_n, walkers = [], [], [], []
     row = 0
-    for i in range(n_bands):
-        walkers.append(g.permutation(wl.n_walkers)[:n_t].astype(np.int32))
+    for i in [ib for ib in range(n_bands) for _ in range(n_groups)]:
+        if len(walkers) % n_groups == 0:
+            pw = g.permutation(wl.n_walkers).astype(np.int32)
+        walkers.append(pw[(len(walkers) % n_groups) * n_t:(len(walkers) % n_groups + 1) * n_t])
         for t in range(n_t):
             z = g.standard_normal((n_src, 8)) * jitter * (1.0 + 0.5 * t)
             s = tr[i].copy()
@@ -342,10 +345,11 @@ def make_temper_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_t: int,
             set_begin.append(row)
             set_n.append(len(s))
             row += len(s)
-    nc = n_bands * n_t
-    tasks = {"n_t": np.full(n_bands, n_t, np.int32), "chain_begin": (np.arange(n_bands) * n_t).astype(np.int32),
-             "n_stage": np.full(n_bands, 3 * N, np.int32), "write_back": np.ones(n_bands, np.int32),
-             "k_first": kb0 + (b - 1) * N}
+    ntask = n_bands * n_groups
+    nc = ntask * n_t
+    tasks = {"n_t": np.full(ntask, n_t, np.int32), "chain_begin": (np.arange(ntask) * n_t).astype(np.int32),
+             "n_stage": np.full(ntask, 3 * N, np.int32), "write_back": np.ones(ntask, np.int32),
+             "k_first": np.repeat(kb0 + (b - 1) * N, n_groups)}
     return TemperTasks(N, tasks, np.ascontiguousarray(np.concatenate(sets)), tr, np.concatenate(walkers),
-                       np.tile(1.2 ** -np.arange(n_t, dtype=np.float64), n_bands), np.asarray(set_begin, np.int32),
+                       np.tile(1.2 ** -np.arange(n_t, dtype=np.float64), ntask), np.asarray(set_begin, np.int32),
                        np.asarray(set_n, np.int32), np.log(g.random(nc)), 3 * N)
