@@ -344,10 +344,28 @@ def run_ours(args):
         torch.cuda.synchronize()
         ctx.check()
         ms_band = b0.elapsed_time(b1) / reps
+        # row f3: the same tasks in the odd/even cold-chain buffer mode: residual rows 2w / 2w+1 stand for
+        # the even / odd buffer of "walker" w, r' is formed on chip (9 extra waveforms per task), write-back to the odd row
+        wv = bt.tasks["walker"]
+        packed_oe = gbfit.pack_band_tasks(**dict(bt.tasks, walker=(wv // 2) * 2), subtract_current=np.ones_like(wv),
+                                          write_walker=(wv // 2) * 2 + 1)
+        d_tasks_oe = torch.from_numpy(packed_oe.view(np.uint8)).to(dev)
+        for i in range(reps + 1):
+            d_bp.copy_(d_bp0)
+            if i == 1:
+                b0.record(stream)
+            ctx.band_sweep(data, d_tasks_oe, 256, bt.max_stage, d_bp, d_bk, d_bq, d_lq, d_lu, d_acc_b, d_dl_b)
+        b1.record(stream)
+        torch.cuda.synchronize()
+        ctx.check()
+        ms_band_oe = b0.elapsed_time(b1) / reps
         band = {"call": "gb_band_sweep (Algorithm 1)", "N": 256, "tasks": int(len(bt.tasks["walker"])),
                 "sources_per_band": 9, "proposals_per_band": 30, "proposals": int(bt.prop_k.size),
                 "ms_per_call": ms_band, "proposals_per_s": bt.prop_k.size / (ms_band * 1e-3),
                 "accepted_fraction_last_call": float(d_acc_b.float().mean().item()),
+                "odd_even_buffers": {"ms_per_call": ms_band_oe, "proposals_per_s": bt.prop_k.size / (ms_band_oe * 1e-3),
+                                     "note": "GB_BAND_SUBTRACT_CURRENT | GB_BAND_WRITE_OTHER: residual rows needed per "
+                                             "walker 2 instead of n_t (72 rows = 2.2 GB instead of 360 = 10.8 GB here)"},
                 # nominal work of a swap evaluation: 2 (711 N + 10 N log2 N) + 60 N flop
                 "alu_frac": bt.prop_k.size * (2 * (711 * 256 + 10 * 256 * 8) + 60 * 256) / (ms_band * 1e-3) / 1e12
                             / FP64_PEAK_TFLOPS,

@@ -199,7 +199,7 @@ int gb_overlap(gb_ctx *ctx, const gb_data *data, const double *params_a, const d
  *   prop_k       [sum n_prop] DEVICE int32: which source of its band proposal p replaces (0 .. n_src-1)
  *   prop_params  [sum n_prop][8], prop_logq [sum n_prop], prop_logu [sum n_prop]   DEVICE f64
  *   accepted_out [sum n_prop] DEVICE uint8, dlnL_out [sum n_prop] DEVICE f64 (the T = 1 delta lnL of every proposal)
- * Inner products use only the staged bins that lie in the stored band.  With write_back != 0 every accepted change
+ * Inner products use only the staged bins that lie in the stored band.  With GB_BAND_WRITE_BACK every accepted change
  * is also added to data->resid with FP64 atomics, so concurrent tasks of one walker must not propose into the same
  * bins: the paper's odd/even sub-band schedule -- one call per parity -- guarantees it.  Tasks are
  * independent and run concurrently; the proposals of one task run sequentially.
@@ -207,6 +207,15 @@ int gb_overlap(gb_ctx *ctx, const gb_data *data, const double *params_a, const d
  * the sticky row flag (gb_check) and gives NaN.  Asynchronous on `stream`.
  */
 #define GB_BAND_MAX_STAGE 3072
+/* task flags.  The last two implement the paper's odd/even cold-chain buffers (Fig. 4): per walker
+ * only two residual rows are stored -- the data minus the cold-chain sources of the even sub-bands, and of the odd ones --
+ * instead of one row per (temperature, walker).  A task of an odd sub-band stages from the EVEN row, which holds none of
+ * the band's own sources, subtracts the band's current sources while staging (GB_BAND_SUBTRACT_CURRENT),
+ * and, for the cold chain only, writes its accepted changes into the ODD row (GB_BAND_WRITE_OTHER); even
+ * sub-bands the other way round.  Hotter chains stage from the same cold-chain row and write nothing. */
+#define GB_BAND_WRITE_BACK 1        /* accepted changes are added to a stored residual row                      */
+#define GB_BAND_SUBTRACT_CURRENT 2  /* r' = staged row - sum of the band's current sources (formed on chip)      */
+#define GB_BAND_WRITE_OTHER 4       /* the write-back row is write_walker instead of walker                      */
 typedef struct {
     int32_t walker;      /* residual row                                                        */
     int32_t n_src;       /* g_j: sources of the band                                            */
@@ -215,8 +224,8 @@ typedef struct {
     int32_t prop_begin;  /* first row of the band in prop_*                                     */
     int32_t n_stage;     /* staged bins                                                         */
     int64_t k_first;     /* global bin of staged bin 0                                          */
-    int32_t write_back;  /* != 0: accepted changes also go to data->resid                       */
-    int32_t reserved;
+    int32_t flags;       /* GB_BAND_WRITE_BACK | GB_BAND_SUBTRACT_CURRENT | GB_BAND_WRITE_OTHER   */
+    int32_t write_walker;/* residual row that receives accepted changes when GB_BAND_WRITE_OTHER */
     double beta;         /* inverse temperature of the band's chain                             */
 } gb_band_task;
 int gb_band_sweep(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, int64_t n_tasks, int N, int max_stage,

@@ -442,11 +442,17 @@ int gbo_overlap(const gbo_config *c, const gbo_data *d, const double *params_a, 
  * log of the uniform draw are inputs: the random numbers of the method are passed in).  On acceptance
  * theta_j[k] <- theta', r' <- r' + h(theta_k) - h(theta'_k).  If write_back, the net
  * change of r' is added to the walker's stored residual at the end.  Tasks are processed
- * one after the other in task order.                                                                   */
+ * one after the other in task order.
+ * Odd/even cold-chain buffers (Fig. 4; row f3), flags bits 1 and 2:
+ *   bit 1 (2): r' is formed ONLINE: the staged row holds the data minus the cold-chain sources of the OTHER
+ *              parity only, and the band's own current sources are subtracted while staging
+ *              ("We subtract from the buffer residual the waveforms contained in (w, t, b)", :360);
+ *   bit 2 (4): the write-back goes to row `write_walker` (the buffer of the band's own parity, :362) instead
+ *              of the staged row.                                                                       */
 typedef struct {
     int32_t walker, n_src, src_begin, n_prop, prop_begin, n_stage;
     int64_t k_first;
-    int32_t write_back, reserved;
+    int32_t flags, write_walker;     /* flags: 1 write back, 2 subtract current sources, 4 write to write_walker */
     double beta;
 } gbo_band_task;
 
@@ -477,8 +483,15 @@ int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks,
                 sv[(size_t)ch * n + i] = S[i];
             }
         }
-        memcpy(r0, rv, sizeof(double) * 4 * (size_t)n);
         gbo_data v = {rv, sv, NULL, lo, n, 1, 1, d->psd_is_inverse};
+        if ((t->flags & 2) && n > 0) {                     /* r' <- r' - sum of the band's current sources (:360) */
+            for (int sidx = 0; sidx < t->n_src; sidx++) {
+                int64_t kh;
+                gbo_waveform(c, params + 8 * ((size_t)t->src_begin + sidx), N, oA, oE, &kh);
+                add_window(&v, 0, oA, oE, kh, N, -1.0);
+            }
+        }
+        memcpy(r0, rv, sizeof(double) * 4 * (size_t)n);
         for (int p = 0; p < t->n_prop && n > 0; p++) {
             int64_t ip = t->prop_begin + p;
             int k = prop_k[ip];
@@ -506,9 +519,11 @@ int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks,
             accepted_out[ip] = (uint8_t)acc;
             if (acc) memcpy(params + 8 * ((size_t)t->src_begin + prop_k[ip]), prop_params + 8 * ip, sizeof(double) * 8);
         }
-        if (t->write_back) {
+        if (t->flags & 1) {
+            int wrow = (t->flags & 4) ? t->write_walker : t->walker;
+            if (wrow < 0 || wrow >= d->n_walkers) { free(rv); free(r0); free(sv); free(h); return GBO_ERR_INVALID; }
             for (int ch = 0; ch < 2; ch++) {
-                double *r = (double *)resid_ch(d, t->walker, ch) + 2 * (lo - d->k_lo);
+                double *r = (double *)resid_ch(d, wrow, ch) + 2 * (lo - d->k_lo);
                 for (int64_t i = 0; i < 2 * n; i++) r[i] += rv[2 * (size_t)ch * n + i] - r0[2 * (size_t)ch * n + i];
             }
         }

@@ -198,17 +198,25 @@ def overlap(cfg: Config, data: Data, params_a, params_c, psd_row=None, N: int = 
 
 _BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
                        ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
-                       ("write_back", np.int32), ("reserved", np.int32), ("beta", np.float64)], align=True)
+                       ("flags", np.int32), ("write_walker", np.int32), ("beta", np.float64)], align=True)
 
 
 def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, prop_params, prop_logq, prop_logu):
     """Algorithm 1, task after task, proposal after proposal.  `tasks` is a dict of equal-length
-    arrays (walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta).  `params` [n_src_total, 8]
+    arrays (walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta; optional subtract_current
+    and write_walker for the odd/even buffers of PAPER.md:354-362).  `params` [n_src_total, 8]
     and data.resid are updated in place.  Returns (accepted[n_prop_total] uint8, dlnL[n_prop_total])."""
     n = len(tasks["walker"])
     t = np.zeros(n, _BAND_TASK)
-    for key in ("walker", "n_src", "src_begin", "n_prop", "prop_begin", "n_stage", "k_first", "write_back", "beta"):
+    for key in ("walker", "n_src", "src_begin", "n_prop", "prop_begin", "n_stage", "k_first", "beta"):
         t[key] = tasks[key]
+    flags = (np.asarray(tasks["write_back"]) != 0).astype(np.int32)
+    if "subtract_current" in tasks:
+        flags |= 2 * (np.asarray(tasks["subtract_current"]) != 0).astype(np.int32)
+    if "write_walker" in tasks:
+        flags |= 4
+        t["write_walker"] = tasks["write_walker"]
+    t["flags"] = flags
     assert params.dtype == np.float64 and params.flags.c_contiguous
     pk = np.ascontiguousarray(prop_k, dtype=np.int32)
     pp, lq, lu = _f64(prop_params), _f64(prop_logq), _f64(prop_logu)

@@ -62,7 +62,10 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
 
     for (int64_t it = blockIdx.x; it < a.n_tasks; it += gridDim.x) {
         const gb_band_task t = a.tasks[it];
-        if (t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0) {
+        const bool wb = (t.flags & GB_BAND_WRITE_BACK) != 0;
+        const int wrow = (t.flags & GB_BAND_WRITE_OTHER) ? t.write_walker : t.walker;
+        if (t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0 ||
+            (wb && (wrow < 0 || wrow >= a.n_walkers))) {
             if (tid == 0) atomicOr(a.errflag, 1);
             for (int p = tid; p < t.n_prop; p += G) {
                 a.dlnL_out[t.prop_begin + p] = nan;
@@ -72,8 +75,10 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
         }
         // ---- stage r' and the weights (zero weight marks a bin outside the stored band)
         const size_t nf = (size_t)a.n_f;
-        double* rA = a.resid + ((size_t)t.walker * 2 + 0) * nf * 2;
-        double* rE = a.resid + ((size_t)t.walker * 2 + 1) * nf * 2;
+        const double* rA = a.resid + ((size_t)t.walker * 2 + 0) * nf * 2;   // staged from this row
+        const double* rE = a.resid + ((size_t)t.walker * 2 + 1) * nf * 2;
+        double* wA = a.resid + ((size_t)(wb ? wrow : t.walker) * 2 + 0) * nf * 2;   // accepted changes go to this row
+        double* wE = a.resid + ((size_t)(wb ? wrow : t.walker) * 2 + 1) * nf * 2;
         const int prow = a.walker_psd ? a.walker_psd[t.walker] : (a.n_psd == 1 ? 0 : t.walker);
         const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
         const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
@@ -97,6 +102,36 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
             sWE[i] = we;
         }
         group_sync<G>();
+        // ---- odd/even buffers: the staged row holds none of the band's own sources; subtract them
+        if (t.flags & GB_BAND_SUBTRACT_CURRENT) {
+            for (int sidx = 0; sidx < t.n_src; sidx++) {
+                const double* theta = a.params + 8 * ((size_t)t.src_begin + sidx);
+                if (tid == 0) {
+                    SrcConst s;
+                    source_constants(theta, a.Tobs, a.tau, N, s);
+                    s.fast = fast_path_ok(theta, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                    if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                    s_src[0] = s;
+                }
+                group_sync<G>();
+                if (s_src[0].fast) slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+                else slow_part<N, G, false>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+                fft_store<N>(bufA0, bufE0, a.tw, tid);
+                const int64_t j0 = s_src[0].kmin - t.k_first;
+#pragma unroll
+                for (int m = 0; m < S; m++) {
+                    const int j = tid + G * m;
+                    const int64_t i = j0 + j;
+                    const int64_t e = i_first + i;
+                    if (i >= 0 && i < t.n_stage && e >= 0 && e < a.n_f) {
+                        const cx ha = bufA0[pad_idx<N>(j)], he = bufE0[pad_idx<N>(j)];
+                        sRA[i] = {sRA[i].re - ha.re, sRA[i].im - ha.im};
+                        sRE[i] = {sRE[i].re - he.re, sRE[i].im - he.im};
+                    }
+                }
+                group_sync<G>();
+            }
+        }
 
         // ---- the proposals of the band, in order
         for (int p = 0; p < t.n_prop; p++) {
@@ -175,7 +210,6 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
             if (s_acc) {
                 // r' += h(theta_k), then r' -= h(theta'_k) (two passes: the windows overlap), and the same change
                 // to the stored residual (only bins inside the stored band exist)
-                const bool wb = t.write_back != 0;
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -186,10 +220,10 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                         sRA[i] = {sRA[i].re + oa.re, sRA[i].im + oa.im};
                         sRE[i] = {sRE[i].re + oe.re, sRE[i].im + oe.im};
                         if (wb) {
-                            atomicAdd(rA + 2 * e, oa.re);
-                            atomicAdd(rA + 2 * e + 1, oa.im);
-                            atomicAdd(rE + 2 * e, oe.re);
-                            atomicAdd(rE + 2 * e + 1, oe.im);
+                            atomicAdd(wA + 2 * e, oa.re);
+                            atomicAdd(wA + 2 * e + 1, oa.im);
+                            atomicAdd(wE + 2 * e, oe.re);
+                            atomicAdd(wE + 2 * e + 1, oe.im);
                         }
                     }
                 }
@@ -204,10 +238,10 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                         sRA[i] = {sRA[i].re - ha.re, sRA[i].im - ha.im};
                         sRE[i] = {sRE[i].re - he.re, sRE[i].im - he.im};
                         if (wb) {
-                            atomicAdd(rA + 2 * e, -ha.re);
-                            atomicAdd(rA + 2 * e + 1, -ha.im);
-                            atomicAdd(rE + 2 * e, -he.re);
-                            atomicAdd(rE + 2 * e + 1, -he.im);
+                            atomicAdd(wA + 2 * e, -ha.re);
+                            atomicAdd(wA + 2 * e + 1, -ha.im);
+                            atomicAdd(wE + 2 * e, -he.re);
+                            atomicAdd(wE + 2 * e + 1, -he.im);
                         }
                     }
                 }

@@ -27,7 +27,8 @@ BAND_MAX_STAGE = 3072
 # layout of gb_band_task (include/gbfit.h)
 BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
                       ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
-                      ("write_back", np.int32), ("reserved", np.int32), ("beta", np.float64)], align=True)
+                      ("flags", np.int32), ("write_walker", np.int32), ("beta", np.float64)], align=True)
+BAND_WRITE_BACK, BAND_SUBTRACT_CURRENT, BAND_WRITE_OTHER = 1, 2, 4
 
 
 TEMPER_MAX_LADDER = 64
@@ -45,13 +46,22 @@ def pack_temper_tasks(n_t, chain_begin, n_stage, write_back, k_first) -> np.ndar
     return t
 
 
-def pack_band_tasks(walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta) -> np.ndarray:
-    """Host array of gb_band_task records from equal-length columns (upload it as bytes: torch.from_numpy(t.view(np.uint8)))."""
+def pack_band_tasks(walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta,
+                    subtract_current=None, write_walker=None) -> np.ndarray:
+    """Host array of gb_band_task records from equal-length columns (upload it as bytes:
+    torch.from_numpy(t.view(np.uint8))).  subtract_current / write_walker select the odd/even cold-chain buffer mode
+    of PAPER.md:354-362 (GB_BAND_SUBTRACT_CURRENT, GB_BAND_WRITE_OTHER)."""
     t = np.zeros(len(walker), BAND_TASK)
     for key, val in (("walker", walker), ("n_src", n_src), ("src_begin", src_begin), ("n_prop", n_prop),
-                     ("prop_begin", prop_begin), ("n_stage", n_stage), ("k_first", k_first),
-                     ("write_back", write_back), ("beta", beta)):
+                     ("prop_begin", prop_begin), ("n_stage", n_stage), ("k_first", k_first), ("beta", beta)):
         t[key] = val
+    flags = BAND_WRITE_BACK * (np.asarray(write_back) != 0).astype(np.int32)
+    if subtract_current is not None:
+        flags |= BAND_SUBTRACT_CURRENT * (np.asarray(subtract_current) != 0).astype(np.int32)
+    if write_walker is not None:
+        flags |= BAND_WRITE_OTHER
+        t["write_walker"] = write_walker
+    t["flags"] = flags
     return t
 
 

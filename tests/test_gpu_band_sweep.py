@@ -123,3 +123,30 @@ def test_band_sweep_edges_rj_amplitude_switch_and_bad_tasks(oracle, torch_cuda, 
     with pytest.raises(gbfit.GbError):
         ctx.band_sweep(data, dev(torch, packed.view(np.uint8)), 128, gbfit.BAND_MAX_STAGE + 1, dev(torch, bt.params),
                        dev(torch, bt.prop_k), dev(torch, bt.prop_params), dev(torch, bt.prop_logq), dev(torch, bt.prop_logu))
+
+
+def test_band_sweep_odd_even_cold_chain_buffers(oracle, torch_cuda, gb):
+    """Row f3 (Fig. 4): tasks stage from the EVEN buffer of their walker, subtract the band's current
+    sources on chip, and the cold chain writes its accepted changes into the ODD buffer; hot chains store nothing."""
+    from oddeven_setup import oddeven_case
+    gbfit, ctx = gb
+    torch = torch_cuda
+    for N, f_lo, amp in ((128, 6e-4, 2e-22), (512, 6e-3, 4e-23)):
+        wl, d, buf, wpsd, cold, tcold, hot, thot, ev = oddeven_case(oracle, N=N, f_lo=f_lo, n_bands=4, n_src=4, n_prop=12,
+                                                                  n_walkers=3, amp=(0.1 * amp, amp))
+        for bt, tt in ((cold, tcold), (hot, thot)):
+            r_ref = buf.copy()
+            p_ref = bt.params.copy()
+            racc, rdl = oracle.band_sweep(oracle.Config(), oracle.Data(r_ref, wl.psd, wl.k_lo, walker_psd=wpsd), tt, N, p_ref,
+                                          bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
+            d_resid = dev(torch, buf)
+            data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo, walker_psd=dev(torch, wpsd))
+            d_params = dev(torch, bt.params)
+            acc, dl = ctx.band_sweep(data, dev(torch, gbfit.pack_band_tasks(**tt).view(np.uint8)), N, 3 * N, d_params,
+                                     dev(torch, bt.prop_k), dev(torch, bt.prop_params), dev(torch, bt.prop_logq),
+                                     dev(torch, bt.prop_logu))
+            ctx.check()
+            assert 0 < racc.sum() < racc.size
+            compare((acc.cpu().numpy(), dl.cpu().numpy(), d_params.cpu().numpy(), d_resid.cpu().numpy()),
+                    (racc, rdl, p_ref, r_ref), buf if tt["write_back"].any() else buf + 1e-30)
+            assert np.array_equal(d_resid.cpu().numpy()[0::2], buf[0::2])     # even buffers are only read

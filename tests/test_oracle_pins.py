@@ -583,3 +583,48 @@ def test_temper_sweep_reduces_to_eq_d1_for_a_shared_likelihood_and_bubbles_when_
     p0, a0, _ = oracle.temper_sweep(cfg, oracle.Data(r0, wl.psd, wl.k_lo), t0, tt.N, tt.params, tt.chain_walker, tt.chain_beta,
                                     tt.chain_set_begin, tt.chain_set_n, np.full_like(tt.chain_logu, np.inf))
     assert np.array_equal(r0, resid) and not a0.any() and list(p0[:nt]) == list(range(nt))
+
+
+# ------------------------------------------------- odd/even cold-chain buffers (Fig. 4), row f3
+def test_oddeven_buffers_equal_the_explicit_residual_and_keep_the_odd_buffer_consistent(oracle):
+    from oddeven_setup import oddeven_case
+    wl, d, buf, wpsd, cold, tcold, hot, thot, ev = oddeven_case(oracle)
+    cfg = oracle.Config()
+    N = cold.N
+    for bt, tt, is_cold in ((cold, tcold, True), (hot, thot, False)):
+        run = buf.copy()
+        params = bt.params.copy()
+        acc, dl = oracle.band_sweep(cfg, oracle.Data(run, wl.psd, wl.k_lo, walker_psd=wpsd), tt, N, params, bt.prop_k,
+                                    bt.prop_params, bt.prop_logq, bt.prop_logu)
+        assert 0 < acc.sum() < acc.size
+        # (1) the same tasks on EXPLICIT residual rows r = even buffer - sum(current sources), plain mode
+        nt = len(tt["walker"])
+        expl = np.empty((nt, 2, wl.n_f), np.complex128)
+        de = oracle.Data(expl, wl.psd, wl.k_lo, walker_psd=(tt["walker"] // 2).astype(np.int32))
+        for i in range(nt):
+            expl[i] = buf[tt["walker"][i]]
+            for src in bt.params[bt.tasks["src_begin"][i]:bt.tasks["src_begin"][i] + bt.tasks["n_src"][i]]:
+                oracle.residual_update(cfg, de, src[None], None, np.full(1, i, np.int32), move_all=oracle.ADD, N=N)
+        e0 = expl.copy()
+        plain = dict(bt.tasks, walker=np.arange(nt, dtype=np.int32), write_back=np.ones(nt, np.int32))
+        p2 = bt.params.copy()
+        acc2, dl2 = oracle.band_sweep(cfg, de, plain, N, p2, bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
+        assert np.array_equal(acc, acc2) and np.array_equal(params, p2) and np.abs(dl - dl2).max() <= 1e-9
+        if not is_cold:
+            assert np.array_equal(run, buf)                          # hot chains store nothing
+            continue
+        assert np.array_equal(run[0::2], buf[0::2])                  # the even buffers are only read
+        change = np.zeros_like(buf)                                  # the odd buffer received each task's net change
+        for i in range(nt):
+            sl = slice(int(tt["k_first"][i] - wl.k_lo), int(tt["k_first"][i] - wl.k_lo + tt["n_stage"][i]))
+            change[tt["write_walker"][i], :, sl] += (expl[i] - e0[i])[:, sl]
+        scale = np.abs(change).max()
+        assert scale > 0 and np.abs((run - buf) - change).max() <= 1e-12 * scale + 4e-16 * np.abs(buf).max()
+        # (2) PAPER.md:362: the odd buffer is again "data minus the (new) cold sources of the odd sub-bands"
+        chk = oracle.Data(run.copy(), wl.psd, wl.k_lo, walker_psd=wpsd)
+        for i in range(nt):
+            for src in params[bt.tasks["src_begin"][i]:bt.tasks["src_begin"][i] + bt.tasks["n_src"][i]]:
+                oracle.residual_update(cfg, chk, None, src[None], np.full(1, tt["write_walker"][i], np.int32),
+                                       move_all=oracle.REMOVE, N=N)
+        assert np.abs(chk.resid[1::2] - d).max() <= 1e-12 * np.abs(buf - d[np.repeat(np.arange(len(d)), 2)]).max() \
+            + 4e-16 * np.abs(d).max()
