@@ -769,6 +769,8 @@ __global__ void __launch_bounds__(128) gb_dfma_peak_kernel(double* sink, int ite
 }
 
 // ------------------------------------------------------------------------------------------------ context
+constexpr int kHostChunks = 8;
+
 struct gb_ctx {
     gb_config cfg;
     int num_sms;
@@ -783,6 +785,9 @@ struct gb_ctx {
     // staging for the *_host entry points
     void* d_stage;
     size_t cap_stage;
+    // copy streams and events of the *_host forms (chunked: the copies of chunk i+1 overlap the kernels of chunk i)
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_start, ev_in[kHostChunks], ev_done[kHostChunks];
     int64_t launches;
     char err[512];
 };
@@ -1082,6 +1087,13 @@ int gb_create(const gb_config* cfg, gb_ctx** out) {
     GB_CUDA(ctx, cudaMemcpy(ctx->d_tw, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice));
     GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->d_counts), sizeof(int32_t) * (2 * kNumClasses + 1)));
     GB_CUDA(ctx, cudaMemset(ctx->d_counts, 0, sizeof(int32_t) * (2 * kNumClasses + 1)));
+    GB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking));
+    GB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking));
+    GB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming));
+    for (int i = 0; i < kHostChunks; i++) {
+        GB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_in[i], cudaEventDisableTiming));
+        GB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_done[i], cudaEventDisableTiming));
+    }
     int rc;
 #define GB_SETUP(N_)                                                    \
     if ((rc = setup_kernel<N_, false, true>(ctx))) return rc;           \
@@ -1104,6 +1116,13 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_src_old);
     cudaFree(ctx->d_lists);
     cudaFree(ctx->d_stage);
+    if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
+    if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
+    if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
+    for (int i = 0; i < kHostChunks; i++) {
+        if (ctx->ev_in[i]) cudaEventDestroy(ctx->ev_in[i]);
+        if (ctx->ev_done[i]) cudaEventDestroy(ctx->ev_done[i]);
+    }
     delete ctx;
 }
 
@@ -1392,19 +1411,47 @@ int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params
     GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     int rc = stage_reserve(ctx, (size_t)B * (64 + 64 + 4 + 1 + 4 + 8 + 16) + 8192);
     if (rc) return rc;
-    Stager s{ctx, reinterpret_cast<cudaStream_t>(stream), static_cast<char*>(ctx->d_stage), 0};
-    double* d_pn = params_new ? s.put(params_new, (size_t)B * 8) : nullptr;
-    double* d_po = params_old ? s.put(params_old, (size_t)B * 8) : nullptr;
-    int32_t* d_w = s.put(walker_index, (size_t)B);
-    int8_t* d_mv = move ? s.put(move, (size_t)B) : nullptr;
-    int32_t* d_nb = n_bins ? s.put(n_bins, (size_t)B) : nullptr;
+    // staging areas for the whole batch; the batch then flows through in chunks: H2D of chunk i+1 (stream s_in) overlaps
+    // the kernels of chunk i (caller's stream), whose results go back on s_out
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Stager s{ctx, st, static_cast<char*>(ctx->d_stage), 0};
+    double* d_pn = params_new ? s.put<double>(nullptr, (size_t)B * 8) : nullptr;
+    double* d_po = params_old ? s.put<double>(nullptr, (size_t)B * 8) : nullptr;
+    int32_t* d_w = s.put<int32_t>(nullptr, (size_t)B);
+    int8_t* d_mv = move ? s.put<int8_t>(nullptr, (size_t)B) : nullptr;
+    int32_t* d_nb = n_bins ? s.put<int32_t>(nullptr, (size_t)B) : nullptr;
     double* d_out = s.put<double>(nullptr, (size_t)B);
     double* d_aux = aux_out ? s.put<double>(nullptr, (size_t)B * 2) : nullptr;
-    rc = gb_delta_loglike(ctx, data, d_pn, d_po, d_w, d_mv, move_all, N, d_nb, B, d_out, d_aux, stream);
-    if (rc) return rc;
-    GB_CUDA(ctx, cudaMemcpyAsync(dlnL_out, d_out, (size_t)B * 8, cudaMemcpyDeviceToHost, s.st));
-    if (aux_out) GB_CUDA(ctx, cudaMemcpyAsync(aux_out, d_aux, (size_t)B * 16, cudaMemcpyDeviceToHost, s.st));
-    GB_CUDA(ctx, cudaStreamSynchronize(s.st));
+    const int nch = B >= (1 << 18) ? kHostChunks : 1;
+    GB_CUDA(ctx, cudaEventRecord(ctx->ev_start, st));
+    GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ctx->ev_start, 0));   // earlier work on `stream` may still read the staging area
+    for (int c = 0; c < nch; c++) {
+        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        if (d_pn) GB_CUDA(ctx, cudaMemcpyAsync(d_pn + 8 * lo, params_new + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_po) GB_CUDA(ctx, cudaMemcpyAsync(d_po + 8 * lo, params_old + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaMemcpyAsync(d_w + lo, walker_index + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_mv) GB_CUDA(ctx, cudaMemcpyAsync(d_mv + lo, move + lo, (size_t)n, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_nb) GB_CUDA(ctx, cudaMemcpyAsync(d_nb + lo, n_bins + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaEventRecord(ctx->ev_in[c], ctx->s_in));
+    }
+    for (int c = 0; c < nch; c++) {
+        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        GB_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_in[c], 0));
+        rc = gb_delta_loglike(ctx, data, d_pn ? d_pn + 8 * lo : nullptr, d_po ? d_po + 8 * lo : nullptr, d_w + lo,
+                              d_mv ? d_mv + lo : nullptr, move_all, N, d_nb ? d_nb + lo : nullptr, n, d_out + lo,
+                              d_aux ? d_aux + 2 * lo : nullptr, stream);
+        if (rc) {
+            cudaStreamSynchronize(ctx->s_in);
+            cudaStreamSynchronize(ctx->s_out);
+            return rc;
+        }
+        GB_CUDA(ctx, cudaEventRecord(ctx->ev_done[c], st));
+        GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[c], 0));
+        GB_CUDA(ctx, cudaMemcpyAsync(dlnL_out + lo, d_out + lo, (size_t)n * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+        if (aux_out) GB_CUDA(ctx, cudaMemcpyAsync(aux_out + 2 * lo, d_aux + 2 * lo, (size_t)n * 16, cudaMemcpyDeviceToHost, ctx->s_out));
+    }
+    GB_CUDA(ctx, cudaStreamSynchronize(ctx->s_out));
+    GB_CUDA(ctx, cudaStreamSynchronize(st));
     return GB_OK;
 }
 
@@ -1417,16 +1464,39 @@ int gb_residual_update_host(gb_ctx* ctx, const gb_data* data, const double* para
     GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     int rc = stage_reserve(ctx, (size_t)B * (64 + 64 + 4 + 1 + 1 + 4) + 8192);
     if (rc) return rc;
-    Stager s{ctx, reinterpret_cast<cudaStream_t>(stream), static_cast<char*>(ctx->d_stage), 0};
-    double* d_pn = params_new ? s.put(params_new, (size_t)B * 8) : nullptr;
-    double* d_po = params_old ? s.put(params_old, (size_t)B * 8) : nullptr;
-    int32_t* d_w = s.put(walker_index, (size_t)B);
-    int8_t* d_mv = move ? s.put(move, (size_t)B) : nullptr;
-    uint8_t* d_acc = accepted ? s.put(accepted, (size_t)B) : nullptr;
-    int32_t* d_nb = n_bins ? s.put(n_bins, (size_t)B) : nullptr;
-    rc = gb_residual_update(ctx, data, d_pn, d_po, d_w, d_mv, move_all, d_acc, N, d_nb, B, stream);
-    if (rc) return rc;
-    GB_CUDA(ctx, cudaStreamSynchronize(s.st));
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Stager s{ctx, st, static_cast<char*>(ctx->d_stage), 0};
+    double* d_pn = params_new ? s.put<double>(nullptr, (size_t)B * 8) : nullptr;
+    double* d_po = params_old ? s.put<double>(nullptr, (size_t)B * 8) : nullptr;
+    int32_t* d_w = s.put<int32_t>(nullptr, (size_t)B);
+    int8_t* d_mv = move ? s.put<int8_t>(nullptr, (size_t)B) : nullptr;
+    uint8_t* d_acc = accepted ? s.put<uint8_t>(nullptr, (size_t)B) : nullptr;
+    int32_t* d_nb = n_bins ? s.put<int32_t>(nullptr, (size_t)B) : nullptr;
+    const int nch = B >= (1 << 18) ? kHostChunks : 1;   // chunked as gb_delta_loglike_host
+    GB_CUDA(ctx, cudaEventRecord(ctx->ev_start, st));
+    GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ctx->ev_start, 0));
+    for (int c = 0; c < nch; c++) {
+        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        if (d_acc) GB_CUDA(ctx, cudaMemcpyAsync(d_acc + lo, accepted + lo, (size_t)n, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_pn) GB_CUDA(ctx, cudaMemcpyAsync(d_pn + 8 * lo, params_new + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_po) GB_CUDA(ctx, cudaMemcpyAsync(d_po + 8 * lo, params_old + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaMemcpyAsync(d_w + lo, walker_index + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_mv) GB_CUDA(ctx, cudaMemcpyAsync(d_mv + lo, move + lo, (size_t)n, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_nb) GB_CUDA(ctx, cudaMemcpyAsync(d_nb + lo, n_bins + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaEventRecord(ctx->ev_in[c], ctx->s_in));
+    }
+    for (int c = 0; c < nch; c++) {
+        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        GB_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_in[c], 0));
+        rc = gb_residual_update(ctx, data, d_pn ? d_pn + 8 * lo : nullptr, d_po ? d_po + 8 * lo : nullptr, d_w + lo,
+                                d_mv ? d_mv + lo : nullptr, move_all, d_acc ? d_acc + lo : nullptr, N,
+                                d_nb ? d_nb + lo : nullptr, n, stream);
+        if (rc) {
+            cudaStreamSynchronize(ctx->s_in);
+            return rc;
+        }
+    }
+    GB_CUDA(ctx, cudaStreamSynchronize(st));
     return GB_OK;
 }
 
