@@ -548,3 +548,26 @@ def test_overlap_pairs_against_oracle(oracle, torch_cuda, gb):
     with pytest.raises(gbfit.GbError):
         ctx.check()
     assert np.isnan(out.cpu().numpy()[5])
+
+
+def test_repeated_calls_give_identical_bits(oracle, torch_cuda, gb):
+    """No sanitizer on this pool: a race in the ticket / record / window pipeline or in the shared-memory FFT would
+    show up as run-to-run differences.  delta lnL and waveforms have a fixed summation order, so repeated calls on the
+    same inputs must agree bit for bit (the atomic scatter of gb_residual_update is the one order-dependent step)."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=40000, n_walkers=6)
+    mv = wl.move.copy()
+    mv[::7] = gbfit.SWAP
+    data, _ = upload(torch, gbfit, wl, wl.resid())
+    args = (dev(torch, wl.params_new), dev(torch, wl.params_old), dev(torch, wl.walker_index))
+    kw = dict(move=dev(torch, mv), n_bins=dev(torch, wl.n_bins))
+    first = ctx.delta_loglike(data, *args, **kw).cpu().numpy()
+    wf0, _ = ctx.waveform(args[0][:4096], n_bins=kw["n_bins"][:4096], Nmax=1024)
+    wf0 = wf0.cpu().numpy()
+    for _ in range(4):
+        again = ctx.delta_loglike(data, *args, **kw).cpu().numpy()
+        assert np.array_equal(again, first)
+        wf, _ = ctx.waveform(args[0][:4096], n_bins=kw["n_bins"][:4096], Nmax=1024)
+        assert np.array_equal(wf.cpu().numpy(), wf0)
+    ctx.check()
