@@ -40,9 +40,10 @@ constexpr size_t band_smem_bytes(int max_stage) {
     return (size_t)padded_len<N>() * sizeof(cx) * 4 + (size_t)max_stage * 48;
 }
 
-template <int N>
-__global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
-    constexpr int G = Plan<N>::G;
+template <int N, int GM>
+__global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
+    constexpr int PG = Plan<N>::G;   // FFT group: the first PG threads
+    constexpr int G = PG * GM;       // threads of the CTA
     constexpr int S = N / G;
     constexpr int PN = padded_len<N>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
             sWA[i] = wa;
             sWE[i] = we;
         }
-        group_sync<G>();
+        cta_sync<G>();
         // ---- odd/even buffers: the staged row holds none of the band's own sources; subtract them
         if (t.flags & GB_BAND_SUBTRACT_CURRENT) {
             for (int sidx = 0; sidx < t.n_src; sidx++) {
@@ -113,10 +114,11 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                     if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                     s_src[0] = s;
                 }
-                group_sync<G>();
+                cta_sync<G>();
                 if (s_src[0].fast) slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
                 else slow_part<N, G, false>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                fft_store<N>(bufA0, bufE0, a.tw, tid);
+                if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
+                cta_sync<G>();
                 const int64_t j0 = s_src[0].kmin - t.k_first;
 #pragma unroll
                 for (int m = 0; m < S; m++) {
@@ -129,7 +131,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                         sRE[i] = {sRE[i].re - he.re, sRE[i].im - he.im};
                     }
                 }
-                group_sync<G>();
+                cta_sync<G>();
             }
         }
 
@@ -155,17 +157,21 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                 if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                 s_src[tid] = s;
             }
-            group_sync<G>();
+            cta_sync<G>();
             if (s_src[0].fast && s_src[1].fast) {
                 slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                fft_store<N>(bufA0, bufE0, a.tw, tid);
+                if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
+                cta_sync<G>();
                 slow_part<N, G, true>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
-                fft_store<N>(bufA1, bufE1, a.tw, tid);
+                if (tid < PG) fft_store<N>(bufA1, bufE1, a.tw, tid);
+                cta_sync<G>();
             } else {
                 slow_part<N, G, false>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                fft_store<N>(bufA0, bufE0, a.tw, tid);
+                if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
+                cta_sync<G>();
                 slow_part<N, G, false>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
-                fft_store<N>(bufA1, bufE1, a.tw, tid);
+                if (tid < PG) fft_store<N>(bufA1, bufE1, a.tw, tid);
+                cta_sync<G>();
             }
             // ---- the five sums of Eq. 5 against the staged r' (buffers: 0 = old o, 1 = new a)
             const int64_t j0o = s_src[0].kmin - t.k_first;   // staged bin of window bin 0, old and new
@@ -206,7 +212,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                 a.accepted_out[ip] = (uint8_t)acc;
                 s_acc = acc;
             }
-            group_sync<G>();
+            cta_sync<G>();
             if (s_acc) {
                 // r' += h(theta_k), then r' -= h(theta'_k) (two passes: the windows overlap), and the same change
                 // to the stored residual (only bins inside the stored band exist)
@@ -227,7 +233,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                         }
                     }
                 }
-                group_sync<G>();
+                cta_sync<G>();
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -247,7 +253,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_band_kernel(BandArgs a) {
                 }
                 if (tid < 8) theta_k[tid] = theta_p[tid];   // theta_j[k] <- theta'_k
             }
-            group_sync<G>();   // r', s_src, the waveform buffers and theta_j are reused by the next proposal
+            cta_sync<G>();   // r', s_src, the waveform buffers and theta_j are reused by the next proposal
         }
     }
 }

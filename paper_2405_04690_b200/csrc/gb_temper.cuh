@@ -41,9 +41,10 @@ constexpr size_t temper_smem_bytes(int max_stage) {
     return (size_t)padded_len<N>() * sizeof(cx) * 2 + (size_t)max_stage * 32;
 }
 
-template <int N>
-__global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
-    constexpr int G = Plan<N>::G;
+template <int N, int GM>
+__global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a) {
+    constexpr int PG = Plan<N>::G;   // FFT group: the first PG threads
+    constexpr int G = PG * GM;       // threads of the CTA
     constexpr int S = N / G;
     constexpr int PN = padded_len<N>();
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -77,7 +78,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
             if (tid == 0) atomicOr(a.errflag, 1);
             continue;
         }
-        group_sync<G>();
+        cta_sync<G>();
         const int64_t i_first = t.k_first - a.k_lo;
         for (int q = t.n_t - 1; q >= 1; q--) {
             const int ci = t.chain_begin + q, cj = ci - 1;
@@ -86,7 +87,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
                 dA[i] = {0.0, 0.0};
                 dE[i] = {0.0, 0.0};
             }
-            group_sync<G>();
+            cta_sync<G>();
             for (int side = 0; side < 2; side++) {
                 const int src = t.chain_begin + s_holder[side == 0 ? q : q - 1];
                 const double sign = side == 0 ? 1.0 : -1.0;
@@ -100,10 +101,11 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
                         if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                         s_src = s;
                     }
-                    group_sync<G>();
+                    cta_sync<G>();
                     if (s_src.fast) slow_part<N, G, true>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
                     else slow_part<N, G, false>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
-                    fft_store<N>(bufA, bufE, a.tw, tid);
+                    if (tid < PG) fft_store<N>(bufA, bufE, a.tw, tid);
+                    cta_sync<G>();
                     const int64_t j0 = s_src.kmin - t.k_first;
 #pragma unroll
                     for (int m = 0; m < S; m++) {
@@ -115,7 +117,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
                             dE[i] = {dE[i].re + sign * he.re, dE[i].im + sign * he.im};
                         }
                     }
-                    group_sync<G>();
+                    cta_sync<G>();
                 }
             }
             // ---- <delta|delta> and <r|delta> for both chains, stored bins only
@@ -168,7 +170,7 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
                     s_holder[q - 1] = h;
                 }
             }
-            group_sync<G>();
+            cta_sync<G>();
             if (s_acc && t.write_back) {   // r_i += delta, r_j -= delta
                 for (int i = tid; i < t.n_stage; i += G) {
                     const int64_t e = i_first + i;
@@ -185,9 +187,9 @@ __global__ void __launch_bounds__(Plan<N>::G) gb_temper_kernel(TemperArgs a) {
                 }
                 __threadfence();
             }
-            group_sync<G>();
+            cta_sync<G>();
         }
         for (int q = tid; q < t.n_t; q += G) a.perm_out[t.chain_begin + q] = s_holder[q];
-        group_sync<G>();
+        cta_sync<G>();
     }
 }

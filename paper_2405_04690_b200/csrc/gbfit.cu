@@ -44,6 +44,9 @@ namespace {
 #ifndef GB_WARP_SYNC
 #define GB_WARP_SYNC 1        // one-warp groups (N = 128, 256) use __syncwarp instead of the CTA barrier
 #endif
+#ifndef GB_BAND_GM
+#define GB_BAND_GM 2          // band / ladder kernels: threads per task = GB_BAND_GM x the FFT group (the slow part, the
+#endif                        // staging and the inner products use all of them, the FFT the first group)
 #ifndef GB_UNROLL
 #define GB_UNROLL 1        // unroll factor of the per-thread time-sample loop
 #endif
@@ -167,15 +170,23 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------ main
-// barrier of the group that owns an item (= the CTA): a one-warp group only needs the warp-level barrier
+// barrier of a group of G threads (the first G threads of the CTA, whole warps): a one-warp group only needs the
+// warp-level barrier; larger groups use named barrier 1 with a thread count, so that in the band / ladder kernels
+// (whose CTAs are wider than the FFT group) the first G threads can run the FFT while the others wait at cta_sync
 template <int G>
 __device__ __forceinline__ void group_sync() {
 #if GB_WARP_SYNC
     if (G == 32) __syncwarp();
-    else __syncthreads();
+    else asm volatile("bar.sync 1, %0;" ::"n"(G) : "memory");
 #else
-    __syncthreads();
+    asm volatile("bar.sync 1, %0;" ::"n"(G) : "memory");
 #endif
+}
+// barrier of the whole CTA of T threads (barrier 0)
+template <int T>
+__device__ __forceinline__ void cta_sync() {
+    if (T == 32) __syncwarp();
+    else __syncthreads();
 }
 
 // FFT of both channels of one item: threads [0, G/2) transform A, threads [G/2, G) transform E (gb_fft.cuh).
@@ -1011,13 +1022,13 @@ namespace {
 template <int N>
 int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
     const size_t smem = band_smem_bytes<N>(a.max_stage);
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N, GB_BAND_GM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N>, Plan<N>::G, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N, GB_BAND_GM>, Plan<N>::G * GB_BAND_GM, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
     int64_t grid = (int64_t)nb * ctx->num_sms;
     if (grid > a.n_tasks) grid = a.n_tasks;
-    gb_band_kernel<N><<<(unsigned)grid, Plan<N>::G, smem, st>>>(a);
+    gb_band_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(a);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -1026,13 +1037,13 @@ int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
 template <int N>
 int launch_temper(gb_ctx* ctx, const TemperArgs& a, cudaStream_t st) {
     const size_t smem = temper_smem_bytes<N>(a.max_stage);
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_temper_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_temper_kernel<N, GB_BAND_GM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_temper_kernel<N>, Plan<N>::G, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_temper_kernel<N, GB_BAND_GM>, Plan<N>::G * GB_BAND_GM, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
     int64_t grid = (int64_t)nb * ctx->num_sms;
     if (grid > a.n_tasks) grid = a.n_tasks;
-    gb_temper_kernel<N><<<(unsigned)grid, Plan<N>::G, smem, st>>>(a);
+    gb_temper_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(a);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
