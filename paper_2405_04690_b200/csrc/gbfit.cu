@@ -3,14 +3,19 @@
 // Launch structure of one call (all on the caller's stream, no host synchronisation):
 //   1. cudaMemsetAsync of the work counters
 //   2. gb_prep_kernel      one thread per proposal row: per-source constants (step O1) for the new and/or
-//                          old source, classification by (window length N, swap?) and warp-aggregated append
-//                          to that class's work list
-//   3. gb_main_kernel<N,SWAP>  one persistent launch per class that can occur: a group of G threads (one
-//                          CTA) takes a row from the class's list, evaluates the slow part at N time samples
-//                          (O2-O5), runs the length-N FFT of A and E in shared memory (O6), and finishes in
-//                          the same kernel with either the waveform store, the inner products + delta lnL
-//                          (O7, O8) or the atomic scatter into the residual (O9).  Waveforms never touch
-//                          global memory on the delta-lnL / update paths.
+//                          old source plus the row's walker / PSD row / move (one 192-byte record per side),
+//                          classification by (window length N, swap?, fast or general slow part) and
+//                          warp-aggregated append to that class's work list
+//   3. gb_main_kernel<N,SWAP,FAST>  one persistent launch per class that can occur: a group of G threads (one
+//                          CTA) takes rows of the class's list by a global ticket (taken three items ahead; the
+//                          next record arrives by cp.async while the current row computes), evaluates the slow
+//                          part at N time samples (O2-O5; gb_fast.cuh, or gb_math.cuh for rows outside its
+//                          limits), runs the length-N FFT of A and E in shared memory (O6; gb_fft.cuh), and
+//                          finishes in the same kernel with either the waveform store, the inner products +
+//                          delta lnL / overlap (O7, O8) or the atomic scatter into the residual (O9).  Waveforms
+//                          never touch global memory on the delta-lnL / update paths.
+// gb_band_sweep and gb_temper_sweep (Algorithms 1 and 2 of the paper) have their own kernels, gb_band.cuh and
+// gb_temper.cuh, built from the same slow part and FFT.
 #include <cuda_runtime.h>
 #include <stdarg.h>
 #include <stdio.h>
