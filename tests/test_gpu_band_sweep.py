@@ -150,3 +150,36 @@ def test_band_sweep_odd_even_cold_chain_buffers(oracle, torch_cuda, gb):
             compare((acc.cpu().numpy(), dl.cpu().numpy(), d_params.cpu().numpy(), d_resid.cpu().numpy()),
                     (racc, rdl, p_ref, r_ref), buf if tt["write_back"].any() else buf + 1e-30)
             assert np.array_equal(d_resid.cpu().numpy()[0::2], buf[0::2])     # even buffers are only read
+
+
+def test_band_sweep_many_tasks_sampled(oracle, torch_cuda, gb):
+    """The bench's launch shape at a tenth of its size: 36 walkers x 183 odd 256-bin sub-bands (6588 concurrent tasks,
+    more than one wave of CTAs), 9 sources and 30 proposals each.  Tasks of one walker only share bins that none of their
+    windows reach, so the oracle can run a seeded sample of tasks on the initial residual: decisions, delta lnL and final
+    parameters of those tasks must match."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=1, n_walkers=36)
+    bt = make_band_tasks(wl, 256, 1e-3, n_bands=183, n_src=9, n_prop=30)
+    resid = wl.resid()
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo)
+    d_params = dev(torch, bt.params)
+    acc, dl = ctx.band_sweep(data, dev(torch, gbfit.pack_band_tasks(**bt.tasks).view(np.uint8)), 256, bt.max_stage, d_params,
+                             dev(torch, bt.prop_k), dev(torch, bt.prop_params), dev(torch, bt.prop_logq), dev(torch, bt.prop_logu))
+    ctx.check()
+    acc, dl, params = acc.cpu().numpy(), dl.cpu().numpy(), d_params.cpu().numpy()
+    nt = len(bt.tasks["walker"])
+    assert nt == 6588 and np.isfinite(dl).all()
+    pick = np.random.Generator(np.random.Philox(key=[1, 256])).choice(nt, 64, replace=False)
+    sub = {k: v[pick] for k, v in bt.tasks.items()}
+    p_ref = bt.params.copy()
+    racc, rdl = oracle.band_sweep(oracle.Config(), oracle.Data(resid.copy(), wl.psd, wl.k_lo), sub, 256, p_ref, bt.prop_k,
+                                  bt.prop_params, bt.prop_logq, bt.prop_logu)
+    for i in pick:
+        ps = slice(bt.tasks["prop_begin"][i], bt.tasks["prop_begin"][i] + bt.tasks["n_prop"][i])
+        ss = slice(bt.tasks["src_begin"][i], bt.tasks["src_begin"][i] + bt.tasks["n_src"][i])
+        assert np.array_equal(acc[ps], racc[ps]), i
+        assert np.abs(dl[ps] - rdl[ps]).max() <= TOL_DLNL, i
+        assert np.array_equal(params[ss], p_ref[ss]), i
+    assert 0.02 < acc.mean() < 0.98

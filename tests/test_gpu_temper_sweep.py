@@ -90,3 +90,37 @@ def test_temper_sweep_all_accepted_none_accepted_no_write_back_inverse_psd_and_b
         ctx.check()
     cb = tt.tasks["chain_begin"][1]
     assert np.isnan(dl.cpu().numpy()[cb + 1:cb + 6]).all() and np.isfinite(dl.cpu().numpy()[:cb]).all()
+
+
+def test_temper_sweep_many_ladders_sampled(oracle, torch_cuda, gb):
+    """The bench's launch shape at reduced size: 183 odd 256-bin sub-bands x 4 disjoint walker groups = 732 ladders of
+    8 chains running concurrently.  Ladders of one sub-band use disjoint residual rows and ladders of different
+    sub-bands only share bins that no window of either reaches, so the oracle can run a seeded sample of ladders on the
+    initial residuals: decisions, (D_i, D_j) and permutations of those ladders must match."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    from gb_inputs import make_workload, make_temper_tasks
+    wl = make_workload(3, B=1, n_walkers=32)
+    tt = make_temper_tasks(wl, 256, 1e-3, n_bands=183, n_t=8, n_src=6, n_groups=4)
+    lu = tt.chain_logu.copy()
+    lu[np.random.Generator(np.random.Philox(key=[2, 256])).random(lu.size) < 0.3] = -np.inf      # some accepted exchanges
+    resid = wl.resid()
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo)
+    packed = gbfit.pack_temper_tasks(**tt.tasks)
+    perm, acc, dl = ctx.temper_sweep(data, dev(torch, packed.view(np.uint8)), 256, tt.max_stage, dev(torch, tt.params),
+                                     dev(torch, tt.chain_walker), dev(torch, tt.chain_beta), dev(torch, tt.chain_set_begin),
+                                     dev(torch, tt.chain_set_n), dev(torch, lu))
+    ctx.check()
+    perm, acc, dl = perm.cpu().numpy(), acc.cpu().numpy(), dl.cpu().numpy()
+    nt = len(tt.tasks["n_t"])
+    assert nt == 732 and np.isfinite(dl).all()
+    pick = np.random.Generator(np.random.Philox(key=[3, 256])).choice(nt, 40, replace=False)
+    sub = {k: v[pick] for k, v in tt.tasks.items()}
+    rperm, racc, rdl = oracle.temper_sweep(oracle.Config(), oracle.Data(resid.copy(), wl.psd, wl.k_lo), sub, 256, tt.params,
+                                           tt.chain_walker, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, lu)
+    for i in pick:
+        cs = slice(tt.tasks["chain_begin"][i], tt.tasks["chain_begin"][i] + tt.tasks["n_t"][i])
+        assert np.array_equal(acc[cs], racc[cs]) and np.array_equal(perm[cs], rperm[cs]), i
+        assert np.abs(dl[cs] - rdl[cs]).max() <= 1e-6, i
+    assert acc.sum() > 0
