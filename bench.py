@@ -372,6 +372,34 @@ def run_ours(args):
                 "note": "each proposal = 2 waveforms + Eq. 5 against the staged residual + accept/reject + update; "
                         "includes the device-side reset of the 38 MB parameter array before each call"}
 
+    # ---- BASELINE.json configs 1-4 (parity-test cases; each is <= 1 ms of work): latency of one call ----
+    small = None
+    if rank == 0 and full and not args.no_band_sweep:
+        small = {}
+        for cfg in (1, 2, 3, 4):
+            w2 = make_workload(cfg)
+            if cfg == 1:
+                r2 = torch.from_numpy(w2.resid()).to(dev)
+                dat2 = gbfit.Data(r2, torch.from_numpy(w2.psd).to(dev), w2.k_lo)
+            else:   # same band as the sweep: reuse its first residual rows (the values do not matter for timing)
+                nw2 = w2.n_walkers
+                dat2 = gbfit.Data(d_resid[:nw2], torch.from_numpy(w2.psd).to(dev), w2.k_lo)
+            up = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).to(dev)
+            a_n, a_o, a_w, a_m, a_nb = up(w2.params_new), up(w2.params_old), up(w2.walker_index), up(w2.move), up(w2.n_bins)
+            o2 = torch.empty(w2.B, dtype=torch.float64, device=dev)
+            call = lambda: ctx.delta_loglike(dat2, a_n, a_o, a_w, move=a_m, move_all=w2.move_all, N=w2.N, n_bins=a_nb, out=o2)
+            for _ in range(5):
+                call()
+            evs2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+            for e_a, e_b in evs2:
+                e_a.record(stream)
+                call()
+                e_b.record(stream)
+            torch.cuda.synchronize()
+            ctx.check()
+            ms2 = float(np.median([e_a.elapsed_time(e_b) for e_a, e_b in evs2]))
+            small[w2.name] = {"rows": int(w2.B), "ms_per_call_median": ms2, "evals_per_s": w2.B / (ms2 * 1e-3)}
+
     # ---- SURVEY 8(f) row f2, outside the timed step: Algorithm 2 (gb_temper_sweep), 10-chain ladders ------
     # every odd 256-bin sub-band of 1-4 mHz, 36 ladders per band on disjoint residuals, 9-10 sources per chain
     tmp = None
@@ -498,7 +526,7 @@ def run_ours(args):
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "band_sweep": band, "temper_sweep": tmp, "overlap": ovl,
+            "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "small_configs_latency": small,
         }
         print(json.dumps(line), flush=True)
     ctx.close()
