@@ -33,7 +33,15 @@ struct BandArgs {
     double Tobs, tau, Rmax;
     int64_t kmax;
     int32_t* errflag;
+    cx* cache;               // [gridDim.x][kBandCacheSlots][2][N] windows of the current sources of each CTA's task
 };
+
+// Current-source cache: a task with at most this many sources keeps the windows of its current sources in a per-CTA
+// scratch area in global memory (8 KB per source for N = 256; all CTAs together ~150 MB, the live part ~40 MB, i.e.
+// resident in the 126 MB L2).  A proposal then generates only the NEW waveform; the old one is copied in with
+// cp.async while the new one is computed.  Same bits as regenerating it, 39 instead of 60 waveforms for a task of
+// 9 sources and 30 proposals.
+constexpr int kBandCacheSlots = 32;
 
 template <int N>
 constexpr size_t band_smem_bytes(int max_stage) {
@@ -58,8 +66,10 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
     __shared__ __align__(16) SrcConst s_src[2];
     __shared__ double s_red[(G / 32) * 5 + 1];
     __shared__ int s_acc;
+    __shared__ int64_t s_kmin[kBandCacheSlots];       // window start of each cached current source
     const int tid = threadIdx.x;
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
+    cx* cache = a.cache ? a.cache + (size_t)blockIdx.x * kBandCacheSlots * 2 * N : nullptr;
 
     for (int64_t it = blockIdx.x; it < a.n_tasks; it += gridDim.x) {
         const gb_band_task t = a.tasks[it];
@@ -104,7 +114,9 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         }
         cta_sync<G>();
         // ---- odd/even buffers: the staged row holds none of the band's own sources; subtract them
-        if (t.flags & GB_BAND_SUBTRACT_CURRENT) {
+        const bool cached = cache != nullptr && t.n_src <= kBandCacheSlots;
+        const bool subtract = (t.flags & GB_BAND_SUBTRACT_CURRENT) != 0;
+        if (subtract || cached) {
             for (int sidx = 0; sidx < t.n_src; sidx++) {
                 const double* theta = a.params + 8 * ((size_t)t.src_begin + sidx);
                 if (tid == 0) {
@@ -120,13 +132,18 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
                 if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
                 cta_sync<G>();
                 const int64_t j0 = s_src[0].kmin - t.k_first;
+                if (cached && tid == 0) s_kmin[sidx] = s_src[0].kmin;
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
+                    const cx ha = bufA0[pad_idx<N>(j)], he = bufE0[pad_idx<N>(j)];
+                    if (cached) {
+                        cache[((size_t)sidx * 2 + 0) * N + j] = ha;
+                        cache[((size_t)sidx * 2 + 1) * N + j] = he;
+                    }
                     const int64_t i = j0 + j;
                     const int64_t e = i_first + i;
-                    if (i >= 0 && i < t.n_stage && e >= 0 && e < a.n_f) {
-                        const cx ha = bufA0[pad_idx<N>(j)], he = bufE0[pad_idx<N>(j)];
+                    if (subtract && i >= 0 && i < t.n_stage && e >= 0 && e < a.n_f) {
                         sRA[i] = {sRA[i].re - ha.re, sRA[i].im - ha.im};
                         sRE[i] = {sRE[i].re - he.re, sRE[i].im - he.im};
                     }
@@ -149,7 +166,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
             }
             double* theta_k = a.params + 8 * ((size_t)t.src_begin + k);
             const double* theta_p = a.prop_params + 8 * ip;
-            if (tid < 2) {   // step O1 for the old (thread 0) and the proposed (thread 1) source
+            if (cached ? tid == 1 : tid < 2) {   // step O1 for the old (thread 0) and the proposed (thread 1) source
                 const double* src = tid == 0 ? theta_k : theta_p;
                 SrcConst s;
                 source_constants(src, a.Tobs, a.tau, N, s);
@@ -157,8 +174,24 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
                 if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
                 s_src[tid] = s;
             }
+            if (cached) {   // the old window comes from the cache while the new one is generated
+                if (tid == 0) s_src[0].kmin = s_kmin[k];
+#pragma unroll
+                for (int m = 0; m < S; m++) {
+                    const int j = tid + G * m;
+                    cp_async16(&bufA0[pad_idx<N>(j)], &cache[((size_t)k * 2 + 0) * N + j]);
+                    cp_async16(&bufE0[pad_idx<N>(j)], &cache[((size_t)k * 2 + 1) * N + j]);
+                }
+                cp_async_commit();
+            }
             cta_sync<G>();
-            if (s_src[0].fast && s_src[1].fast) {
+            if (cached) {
+                if (s_src[1].fast) slow_part<N, G, true>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
+                else slow_part<N, G, false>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
+                if (tid < PG) fft_store<N>(bufA1, bufE1, a.tw, tid);
+                cp_async_wait<0>();
+                cta_sync<G>();
+            } else if (s_src[0].fast && s_src[1].fast) {
                 slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
                 if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
                 cta_sync<G>();
@@ -252,6 +285,15 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
                     }
                 }
                 if (tid < 8) theta_k[tid] = theta_p[tid];   // theta_j[k] <- theta'_k
+                if (cached) {                               // and its window replaces the cached one
+                    if (tid == 0) s_kmin[k] = s_src[1].kmin;
+#pragma unroll
+                    for (int m = 0; m < S; m++) {
+                        const int j = tid + G * m;
+                        cache[((size_t)k * 2 + 0) * N + j] = bufA1[pad_idx<N>(j)];
+                        cache[((size_t)k * 2 + 1) * N + j] = bufE1[pad_idx<N>(j)];
+                    }
+                }
             }
             cta_sync<G>();   // r', s_src, the waveform buffers and theta_j are reused by the next proposal
         }

@@ -796,7 +796,8 @@ struct gb_ctx {
     SrcConst* d_src_new;
     SrcConst* d_src_old;
     int32_t* d_lists;
-    int64_t cap_new, cap_old, cap_lists;
+    cx* d_band_cache;       // current-source windows of gb_band_sweep's CTAs (gb_band.cuh)
+    int64_t cap_new, cap_old, cap_lists, cap_band_cache;
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
     // staging for the *_host entry points
     void* d_stage;
@@ -1033,7 +1034,11 @@ int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
     if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
     int64_t grid = (int64_t)nb * ctx->num_sms;
     if (grid > a.n_tasks) grid = a.n_tasks;
-    gb_band_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(a);
+    BandArgs b = a;
+    int rc = ensure_cap(ctx, &ctx->d_band_cache, &ctx->cap_band_cache, grid * kBandCacheSlots * 2 * N);
+    if (rc) return rc;
+    b.cache = ctx->d_band_cache;
+    gb_band_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -1131,6 +1136,7 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_src_new);
     cudaFree(ctx->d_src_old);
     cudaFree(ctx->d_lists);
+    cudaFree(ctx->d_band_cache);
     cudaFree(ctx->d_stage);
     if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
     if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
