@@ -203,6 +203,8 @@ int gb_overlap(gb_ctx *ctx, const gb_data *data, const double *params_a, const d
  * is also added to data->resid with FP64 atomics, so concurrent tasks of one walker must not propose into the same
  * bins: the paper's odd/even sub-band schedule -- one call per parity -- guarantees it.  Tasks are
  * independent and run concurrently; the proposals of one task run sequentially.
+ * The library keeps the windows of each running task's current sources in context-owned scratch (about 150 MB, allocated at
+ * the first call and kept), so that a proposal generates only the proposed waveform.
  * Errors: GB_ERR_INVALID for bad arguments; a task with a bad walker / n_stage or a proposal with a bad prop_k sets
  * the sticky row flag (gb_check) and gives NaN.  Asynchronous on `stream`.
  */
@@ -245,6 +247,7 @@ int gb_band_sweep(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, i
  * D_j = lnL_j(S_i) - lnL_j(S_j) = -1/2 <delta|delta>_j + <r_j|delta>_j  (each chain's own PSD row), accepted iff
  * beta_i D_i + beta_j D_j >= logu.  Accepted: the holders are exchanged and, if write_back, r_i += delta, r_j -= delta in
  * data->resid (FP64 atomics; the paper keeps only the cold chain's residual, here every chain owns one).
+ * Ladders of up to 16 chains sum each chain's set once into context-owned scratch (allocated at the first call, <= 350 MB).
  * Outputs [n_chain]: perm_out[c] = ladder position whose INITIAL set ends in chain t; accepted_out[c]; dlnl_out[c][2] =
  * (D_i, D_j) of pair (t, t-1).  All arrays DEVICE.  N, max_stage, odd/even rule, errors and asynchrony as gb_band_sweep.
  */

@@ -34,7 +34,14 @@ struct TemperArgs {
     double Tobs, tau, Rmax;
     int64_t kmax;
     int32_t* errflag;
+    cx* cache;               // [gridDim.x][kTemperCacheChains][2][max_stage] summed windows of each chain's initial set
 };
+
+// Set-sum cache: a set takes part in up to two pairs (as S_j of pair (t+1, t), then as S_i of pair (t, t-1)) and only the
+// SUM of its windows on the staged bins is ever needed.  Ladders of at most this many chains compute every chain's sum
+// once into a per-CTA scratch area in global memory (L2 / HBM) and form delta = H_i - H_j from there: 95 instead of 171
+// waveforms for a ladder of 10 chains with 9-10 sources each.
+constexpr int kTemperCacheChains = 16;
 
 template <int N>
 constexpr size_t temper_smem_bytes(int max_stage) {
@@ -80,45 +87,73 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a
         }
         cta_sync<G>();
         const int64_t i_first = t.k_first - a.k_lo;
-        for (int q = t.n_t - 1; q >= 1; q--) {
-            const int ci = t.chain_begin + q, cj = ci - 1;
-            // ---- delta = sum over the set chain i holds - sum over the set chain j holds
+        // dA, dE += sign * (sum of the windows of the set held at chain entry `src`), on the staged bins
+        auto add_set = [&](int src, double sign) {
+            const int n_set = a.chain_set_n[src];
+            const double* set = a.params + 8 * (size_t)a.chain_set_begin[src];
+            for (int sidx = 0; sidx < n_set; sidx++) {
+                if (tid == 0) {
+                    SrcConst s;
+                    source_constants(set + 8 * sidx, a.Tobs, a.tau, N, s);
+                    s.fast = fast_path_ok(set + 8 * sidx, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                    if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                    s_src = s;
+                }
+                cta_sync<G>();
+                if (s_src.fast) slow_part<N, G, true>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
+                else slow_part<N, G, false>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
+                if (tid < PG) fft_store<N>(bufA, bufE, a.tw, tid);
+                cta_sync<G>();
+                const int64_t j0 = s_src.kmin - t.k_first;
+#pragma unroll
+                for (int m = 0; m < S; m++) {
+                    const int j = tid + G * m;
+                    const int64_t i = j0 + j;
+                    if (i >= 0 && i < t.n_stage) {
+                        const cx ha = bufA[pad_idx<N>(j)], he = bufE[pad_idx<N>(j)];
+                        dA[i] = {dA[i].re + sign * ha.re, dA[i].im + sign * ha.im};
+                        dE[i] = {dE[i].re + sign * he.re, dE[i].im + sign * he.im};
+                    }
+                }
+                cta_sync<G>();
+            }
+        };
+        auto zero_delta = [&]() {
             for (int i = tid; i < t.n_stage; i += G) {
                 dA[i] = {0.0, 0.0};
                 dE[i] = {0.0, 0.0};
             }
             cta_sync<G>();
-            for (int side = 0; side < 2; side++) {
-                const int src = t.chain_begin + s_holder[side == 0 ? q : q - 1];
-                const double sign = side == 0 ? 1.0 : -1.0;
-                const int n_set = a.chain_set_n[src];
-                const double* set = a.params + 8 * (size_t)a.chain_set_begin[src];
-                for (int sidx = 0; sidx < n_set; sidx++) {
-                    if (tid == 0) {
-                        SrcConst s;
-                        source_constants(set + 8 * sidx, a.Tobs, a.tau, N, s);
-                        s.fast = fast_path_ok(set + 8 * sidx, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                        if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                        s_src = s;
-                    }
-                    cta_sync<G>();
-                    if (s_src.fast) slow_part<N, G, true>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
-                    else slow_part<N, G, false>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
-                    if (tid < PG) fft_store<N>(bufA, bufE, a.tw, tid);
-                    cta_sync<G>();
-                    const int64_t j0 = s_src.kmin - t.k_first;
-#pragma unroll
-                    for (int m = 0; m < S; m++) {
-                        const int j = tid + G * m;
-                        const int64_t i = j0 + j;
-                        if (i >= 0 && i < t.n_stage) {
-                            const cx ha = bufA[pad_idx<N>(j)], he = bufE[pad_idx<N>(j)];
-                            dA[i] = {dA[i].re + sign * ha.re, dA[i].im + sign * ha.im};
-                            dE[i] = {dE[i].re + sign * he.re, dE[i].im + sign * he.im};
-                        }
-                    }
-                    cta_sync<G>();
+        };
+        cx* cache = a.cache ? a.cache + (size_t)blockIdx.x * kTemperCacheChains * 2 * a.max_stage : nullptr;
+        const bool cached = cache != nullptr && t.n_t <= kTemperCacheChains && t.n_t > 2;
+        if (cached) {   // H_c = sum of the windows of chain c's initial set
+            for (int c = 0; c < t.n_t; c++) {
+                zero_delta();
+                add_set(t.chain_begin + c, 1.0);
+                for (int i = tid; i < t.n_stage; i += G) {
+                    cache[((size_t)c * 2 + 0) * a.max_stage + i] = dA[i];
+                    cache[((size_t)c * 2 + 1) * a.max_stage + i] = dE[i];
                 }
+                cta_sync<G>();
+            }
+        }
+        for (int q = t.n_t - 1; q >= 1; q--) {
+            const int ci = t.chain_begin + q, cj = ci - 1;
+            // ---- delta = sum over the set chain i holds - sum over the set chain j holds
+            if (cached) {
+                const cx* Hi = cache + (size_t)s_holder[q] * 2 * a.max_stage;
+                const cx* Hj = cache + (size_t)s_holder[q - 1] * 2 * a.max_stage;
+                for (int i = tid; i < t.n_stage; i += G) {
+                    const cx ai = Hi[i], ei = Hi[a.max_stage + i], aj = Hj[i], ej = Hj[a.max_stage + i];
+                    dA[i] = {ai.re - aj.re, ai.im - aj.im};
+                    dE[i] = {ei.re - ej.re, ei.im - ej.im};
+                }
+                cta_sync<G>();
+            } else {
+                zero_delta();
+                add_set(t.chain_begin + s_holder[q], 1.0);
+                add_set(t.chain_begin + s_holder[q - 1], -1.0);
             }
             // ---- <delta|delta> and <r|delta> for both chains, stored bins only
             const int wi = a.chain_walker[ci], wj = a.chain_walker[cj];

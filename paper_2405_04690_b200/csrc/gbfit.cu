@@ -797,7 +797,8 @@ struct gb_ctx {
     SrcConst* d_src_old;
     int32_t* d_lists;
     cx* d_band_cache;       // current-source windows of gb_band_sweep's CTAs (gb_band.cuh)
-    int64_t cap_new, cap_old, cap_lists, cap_band_cache;
+    cx* d_temper_cache;     // set sums of gb_temper_sweep's CTAs (gb_temper.cuh)
+    int64_t cap_new, cap_old, cap_lists, cap_band_cache, cap_temper_cache;
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
     // staging for the *_host entry points
     void* d_stage;
@@ -1053,7 +1054,11 @@ int launch_temper(gb_ctx* ctx, const TemperArgs& a, cudaStream_t st) {
     if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
     int64_t grid = (int64_t)nb * ctx->num_sms;
     if (grid > a.n_tasks) grid = a.n_tasks;
-    gb_temper_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(a);
+    TemperArgs b = a;
+    int rc = ensure_cap(ctx, &ctx->d_temper_cache, &ctx->cap_temper_cache, grid * kTemperCacheChains * 2 * a.max_stage);
+    if (rc) return rc;
+    b.cache = ctx->d_temper_cache;
+    gb_temper_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -1137,6 +1142,7 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_src_old);
     cudaFree(ctx->d_lists);
     cudaFree(ctx->d_band_cache);
+    cudaFree(ctx->d_temper_cache);
     cudaFree(ctx->d_stage);
     if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
     if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
