@@ -1,15 +1,17 @@
 // gb_fast.cuh -- the slow part (steps O2-O5 of DESIGN.md) restructured for the FP64 pipe of sm_100a.
 //
-// Same definition as slow_sample() in gb_math.cuh, evaluated with 4 polynomial sin/cos pairs, no division
-// by an angle and one shared reciprocal per time sample instead of 10 library sincos + 6 divisions:
+// Same definition as slow_sample() in gb_math.cuh, evaluated with 3 polynomial sin/cos pairs, one small-angle
+// rotation of a per-source constant, no division by an angle and one shared reciprocal per time sample instead of
+// 10 library sincos + 6 divisions:
 //
 //   * a + b + c = 0 for the three link vectors, so kappa_c, nu_u,c, nu_v,c follow from the a and b links;
 //   * with psi_l = x kappa_l / 6 (x = 2 pi (f0 + fdot t) L/c) every angle of the response is an integer
 //     combination of x/2, psi_a, psi_b:   theta_rs = x/2 -+ 3 psi_l,   and the receiver phase offsets are
 //     -(x/3)(kappa_l - kappa_l') = -2 (psi_l - psi_l') up to eps_r = pi fdot d_r (2 k.R/c + d_r) (< 1e-8 rad,
 //     first order).  Double/triple-angle formulas (relative accuracy kept for small sines) and complex
-//     products give all phasors from sincos(x/2), sincos(psi_a), sincos(psi_b) -- small, bounded arguments
-//     that need no range reduction (gb_sincos_poly.h);
+//     products give all phasors from exp(i x/2), sincos(psi_a), sincos(psi_b) -- small, bounded arguments
+//     that need no range reduction (gb_sincos_poly.h); exp(i x/2) itself is the per-source constant exp(i x0/2)
+//     rotated by the tiny angle pi fdot t L/c (series);
 //   * (x/2) sinc(theta_rs) = sin(theta_rs) / (1 - kappa_rs): the six denominators share one reciprocal of
 //     (1-kappa_a^2)(1-kappa_b^2)(1-kappa_c^2); a link within ~1e-2 rad of the source direction takes the
 //     series of sinc instead (rare branch);
@@ -32,11 +34,11 @@ struct FastConsts {
     double wS[6], wC[6];   // |x| <= 0.8
     double nS[5], nC[4];   // |x| <= 0.27
     double two_over_pi, pio2_hi, pio2_lo;
-    double third, rsqrt2, rsqrt3, r120, msixth;
+    double third, rsqrt2, rsqrt3, r120, msixth, r24;
 };
 #define GB_FAST_CONSTS_INIT                                                                                   \
     {GB_POLY_W_SIN, GB_POLY_W_COS, GB_POLY_N_SIN, GB_POLY_N_COS, GB_TWO_OVER_PI, GB_PIO2_HI, GB_PIO2_LO,      \
-     1.0 / 3.0, 0.70710678118654752440, 0.57735026918962576451, 1.0 / 120.0, -1.0 / 6.0}
+     1.0 / 3.0, 0.70710678118654752440, 0.57735026918962576451, 1.0 / 120.0, -1.0 / 6.0, 1.0 / 24.0}
 #if defined(__CUDACC__)
 __constant__ FastConsts d_fast_consts = GB_FAST_CONSTS_INIT;
 #endif
@@ -165,7 +167,13 @@ GB_HD void slow_sample_fast(const SrcConst& s, const OrbitSampleAB& o, double t,
     const double hx = fma(s.hxd, t, s.hx0);
     const double hx3 = hx * GB_K(third);
     double sh, ch, sa, ca, sb, cb;
-    sincos_w(hx, sh, ch);
+    {   // exp(i hx) = exp(i hx0) exp(i eps), eps = hxd t: |eps| < 5e-4 inside the fast limits, series to eps^4 / eps^3
+        const double eps = s.hxd * t, e2 = eps * eps;
+        const double ce = fma(e2, fma(e2, GB_K(r24), -0.5), 1.0);
+        const double se = eps * fma(e2, GB_K(msixth), 1.0);
+        sh = fma(s.sh0, ce, s.ch0 * se);
+        ch = fma(s.ch0, ce, -(s.sh0 * se));
+    }
     sincos_n(hx3 * ka, sa, ca);
     sincos_n(hx3 * kb, sb, cb);
     // double and triple angles of psi_a, psi_b; psi_c = -(psi_a + psi_b) by products

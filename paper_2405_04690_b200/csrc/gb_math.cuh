@@ -60,13 +60,12 @@ struct SrcConst {
     double hx0;         // pi f0 L / c      (x/2 at t = 0, x = 2 pi f L/c)
     double hxd;         // pi fdot L / c
     int64_t kmin;       // q - N/2
-    int64_t fast;       // 1: inside the limits of slow_sample_fast (gb_fast.cuh)
+    int32_t fast;       // 1: inside the limits of slow_sample_fast (gb_fast.cuh)
     // row metadata copied in by gb_prep_kernel so that one 192-byte record is all a CTA needs per item
+    int32_t move;       // GB_ADD / GB_REMOVE / GB_SWAP
     int32_t walker;     // residual row
     int32_t psd_row;    // PSD row of that walker
-    int32_t move;       // GB_ADD / GB_REMOVE / GB_SWAP
-    int32_t pad_i;
-    double pad;
+    double ch0, sh0;    // cos, sin of hx0 (the fast path rotates them by the tiny angle hxd t instead of a sincos per sample)
 };
 static_assert(sizeof(SrcConst) == 192, "SrcConst layout");
 
@@ -100,8 +99,8 @@ GB_HD void source_constants(const double* p, double Tobs, double tau, int N, Src
     s.hxd = kPi * fdot * tau;
     s.kmin = (int64_t)q - N / 2;
     s.fast = 0;
-    s.walker = s.psd_row = s.move = s.pad_i = 0;
-    s.pad = 0.0;
+    s.walker = s.psd_row = s.move = 0;
+    sincos_full(s.hx0, &s.sh0, &s.ch0);
 }
 
 GB_HD double sinc_plain(double th, double sn) { return fabs(th) < 1e-8 ? 1.0 - th * th / 6.0 : sn / th; }
