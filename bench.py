@@ -238,13 +238,20 @@ def run_ours(args):
     d_out = torch.empty(B, dtype=torch.float64, device=dev)
     setup_s = time.perf_counter() - t_setup
 
+    sum_nb = int(wl.n_bins.astype(np.int64).sum())
+
     def step_device(i, ev=None):
         if ev:
             ev[0].record(stream)
-        ctx.delta_loglike(data, d_p, None, d_w, move_all=gbfit.ADD, n_bins=d_nb, out=d_out)
+        if (not args.kept_update):   # two independent calls: the update regenerates the accepted waveforms
+            ctx.delta_loglike(data, d_p, None, d_w, move_all=gbfit.ADD, n_bins=d_nb, out=d_out)
+        else:                        # the sweep pair: every window is kept (42 GB of scratch) and scattered from there
+            ctx.delta_loglike_keep(data, d_p, None, d_w, move_all=gbfit.ADD, n_bins=d_nb, sum_n_bins=sum_nb, out=d_out)
         if ev:
             ev[1].record(stream)
-        if i % 2 == 0:
+        if not (not args.kept_update):
+            ctx.residual_update_kept(data, d_acc, negate=(i % 2 == 1))
+        elif i % 2 == 0:
             ctx.residual_update(data, d_p, None, d_w, move_all=gbfit.ADD, accepted=d_acc, n_bins=d_nb)
         else:
             ctx.residual_update(data, None, d_p, d_w, move_all=gbfit.REMOVE, accepted=d_acc, n_bins=d_nb)
@@ -372,6 +379,30 @@ def run_ours(args):
                 "note": "each proposal = 2 waveforms + Eq. 5 against the staged residual + accept/reject + update; "
                         "includes the device-side reset of the 38 MB parameter array before each call"}
 
+    # ---- the same sweep as the gb_delta_loglike_keep + gb_residual_update_kept pair (outside the timed step unless
+    #      --kept-update): the accepted waveforms are not generated a second time
+    pair = None
+    if rank == 0 and full and not args.no_band_sweep and not args.kept_update:
+        k0, k1, k2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        t_d, t_u = [], []
+        for i in range(6):
+            k0.record(stream)
+            ctx.delta_loglike_keep(data, d_p, None, d_w, move_all=gbfit.ADD, n_bins=d_nb, sum_n_bins=sum_nb, out=d_out)
+            k1.record(stream)
+            ctx.residual_update_kept(data, d_acc, negate=(i % 2 == 1))
+            k2.record(stream)
+            torch.cuda.synchronize()
+            if i >= 2:
+                t_d.append(k0.elapsed_time(k1))
+                t_u.append(k1.elapsed_time(k2))
+        ctx.check()
+        ms_pair = float(np.mean(t_d) + np.mean(t_u))
+        pair = {"calls": "gb_delta_loglike_keep + gb_residual_update_kept", "ms_per_step": ms_pair,
+                "ms_dlnl_keep": float(np.mean(t_d)), "ms_update_kept": float(np.mean(t_u)),
+                "evals_per_s": B / (ms_pair * 1e-3), "scratch_bytes": 32.0 * sum_nb,
+                "note": "every window is stored by the delta-lnL epilogue (DRAM is at 5 % under that kernel) and the accepted "
+                        "rows are scattered from the store: a memory-bound update instead of a second generation"}
+
     # ---- BASELINE.json configs 1-4 (parity-test cases; each is <= 1 ms of work): latency of one call ----
     small = None
     if rank == 0 and full and not args.no_band_sweep:
@@ -482,10 +513,16 @@ def run_ours(args):
         "hbm": {"achieved": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "bytes_per_launch": bytes_dlnl},
-        "update": {"ms_per_launch": ms_upd, "flops": flops_upd, "bytes": bytes_upd,
-                   "alu_frac": flops_upd / (ms_upd * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
-                   "hbm_frac": bytes_upd / (ms_upd * 1e-3) / 1e9 / hbm_peak},
-        "step_frac": (flops_dlnl + flops_upd) / (ms_step * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+        "update": ({"call": "gb_residual_update (regenerates the accepted waveforms)", "ms_per_launch": ms_upd,
+                    "flops": flops_upd, "bytes": bytes_upd,
+                    "alu_frac": flops_upd / (ms_upd * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                    "hbm_frac": bytes_upd / (ms_upd * 1e-3) / 1e9 / hbm_peak} if (not args.kept_update) else
+                   {"call": "gb_residual_update_kept (scatter of the kept windows; bound hbm)", "ms_per_launch": ms_upd,
+                    "bytes": 1.5 * bytes_upd, "bytes_note": "32 N read + 64 N read-modify-write per accepted row",
+                    "hbm_frac": 1.5 * bytes_upd / (ms_upd * 1e-3) / 1e9 / hbm_peak,
+                    "kept_window_store_bytes_in_dlnl_call": 32.0 * float(nb.sum())}),
+        "step_frac": (flops_dlnl + (flops_upd if (not args.kept_update) else 0.0)) / (ms_step * 1e-3) / 1e12
+                     / FP64_PEAK_TFLOPS,
     }
 
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
@@ -520,12 +557,14 @@ def run_ours(args):
                        "evals_per_step_per_gpu": int(B), "n_residuals": int(wl.n_walkers), "n_f": int(wl.n_f),
                        "accepted_fraction": float(wl.accepted.mean()), "mean_N": float(nb.mean()),
                        "l2": "inputs_exceed_l2 (10.8 GB of residuals, no flush)", "psd_layout": "1/S_n rows (psd_is_inverse=1)",
+                       "update": "regenerate" if (not args.kept_update) else "kept windows (gb_delta_loglike_keep + "
+                                 "gb_residual_update_kept)",
                        "parallelism": f"replicas{world}" if world > 1 else "single_gpu",
                        "ms_dlnl": ms_dlnl, "ms_update": ms_upd, "setup_s": setup_s},
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "small_configs_latency": small,
+            "sweep_pair_kept": pair, "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "small_configs_latency": small,
         }
         print(json.dumps(line), flush=True)
     ctx.close()
@@ -543,6 +582,9 @@ def main(argv=None):
     ap.add_argument("--walkers", type=int, default=360, help="debug: fewer residuals (default = the full config)")
     ap.add_argument("--per-walker", type=int, default=12000, help="debug: fewer sources per walker")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kept-update", action="store_true",
+                    help="time the gb_delta_loglike_keep + gb_residual_update_kept pair (windows kept in 42 GB of scratch, "
+                         "accepted rows scattered from there) instead of gb_delta_loglike + gb_residual_update")
     ap.add_argument("--no-band-sweep", action="store_true", help="skip the Algorithm-1 (gb_band_sweep) measurement")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3)

@@ -169,6 +169,24 @@ int gb_residual_update_host(gb_ctx *ctx, const gb_data *data, const double *para
                             int N, const int32_t *n_bins /*HOST*/, int64_t B, void *stream);
 
 /*
+ * gb_delta_loglike_keep / gb_residual_update_kept -- the sweep pair "delta lnL of every source, then scatter of the accepted
+ * ones" (BASELINE config 5; Alg. 1 PAPER.md:599-613 in batched form) without generating the accepted waveforms twice.
+ * gb_delta_loglike_keep is gb_delta_loglike for ADD / REMOVE rows (a SWAP row is a row error) that also writes every row's
+ * window into context-owned scratch (2 x 16 bytes x sum_n_bins; DRAM is nearly idle under the compute-bound delta-lnL
+ * kernels, so the stores are almost free on a B200).  sum_n_bins = sum of the rows' window lengths when n_bins is given
+ * (ignored otherwise); too small a value sets row-error flag 4.
+ * gb_residual_update_kept must be the next call on the context after gb_delta_loglike_keep (any other gb_* call except
+ * gb_check / gb_band_sweep / gb_temper_sweep invalidates the kept state -> GB_ERR_INVALID).  It applies the moves of the
+ * rows with accepted[b] != 0 (NULL: all rows) from the kept windows: ADD r -= a, REMOVE r += h; negate != 0 applies the
+ * opposite signs (undo).  It may be called more than once.  Same result as gb_residual_update to the rounding order of
+ * the atomics.  Both asynchronous on `stream`.
+ */
+int gb_delta_loglike_keep(gb_ctx *ctx, const gb_data *data, const double *params_new, const double *params_old,
+                          const int32_t *walker_index, const int8_t *move, int move_all, int N, const int32_t *n_bins,
+                          int64_t B, int64_t sum_n_bins, double *dlnL_out, double *aux_out, void *stream);
+int gb_residual_update_kept(gb_ctx *ctx, const gb_data *data, const uint8_t *accepted, int negate, void *stream);
+
+/*
  * gb_overlap -- normalised overlap of B source pairs (cataloging; the search / catalog workloads
  * of PAPER.md:710-718 use the same kernels with this batch shape):
  *     O_b = <a_b|c_b> / sqrt(<a_b|a_b> <c_b|c_b>),   Eq. 2 against PSD row psd_row[b],

@@ -68,7 +68,7 @@ struct PrepArgs {
     const uint8_t* accepted;
     const int32_t* n_bins;
     const int32_t* walker_psd;
-    int move_all, N, mode, n_walkers, n_psd;
+    int move_all, N, mode, n_walkers, n_psd, keep;
     int64_t B;
     double Tobs, tau, Rmax;  // Rmax = AU / c
     int64_t kmax;            // largest valid global bin (Nyquist)
@@ -107,7 +107,17 @@ struct MainArgs {
     int64_t* kmin_out;
     int Nmax;
     double Tobs, tau;
+    cx* wkeep;               // gb_delta_loglike_keep: every row's window goes here (class base + list position)
+    int64_t wkeep_cap;       // capacity in elements
+    int32_t* errflag;
 };
+
+// element offset of a class's region of the kept windows: the classes before it, count x 2 N each
+__device__ __forceinline__ int64_t keep_class_base(const int32_t* counts, int cls) {
+    int64_t base = 0;
+    for (int c = 0; c < cls; c++) base += (int64_t)counts[c] * 2 * (128 << (c >> 2));
+    return base;
+}
 
 // ------------------------------------------------------------------------------------------------ prep
 __device__ __forceinline__ int class_of_N(int N) {
@@ -122,7 +132,7 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         const int mv = a.mode == MODE_WAVEFORM ? GB_ADD : (a.move ? (int)a.move[b] : a.move_all);
         const int N = a.n_bins ? a.n_bins[b] : a.N;
         const int cN = class_of_N(N);
-        bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP;
+        bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP && !(a.keep && mv == GB_SWAP);
         int w = 0, prow = 0;
         if (a.mode == MODE_OVERLAP) {          // walker_index carries the PSD row itself (NULL: row 0)
             prow = a.walker_index ? a.walker_index[b] : 0;
@@ -469,6 +479,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     __shared__ double s_red[(G / 32) * 5 + 1];
 
     __shared__ int s_ent[2];
+    __shared__ int s_pos[2];   // list positions of the entries in s_ent (gb_delta_loglike_keep)
 
     const int tid = threadIdx.x;
     const int count = a.counts[cls];
@@ -495,10 +506,14 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         const int t = atomicAdd(a.counters + cls, 3);
         s_ent[0] = t < count ? __ldg(list + t) : -1;
         s_ent[1] = t + 1 < count ? __ldg(list + t + 1) : -1;
+        s_pos[0] = t;
+        s_pos[1] = t + 1;
         t_nx2 = t + 2;
     }
     group_sync<G>();
     int e_cur = s_ent[0], e_nxt = s_ent[1];
+    int pos_cur = s_pos[0], pos_nxt = s_pos[1];
+    const int64_t keep_base = a.wkeep ? keep_class_base(a.counts, cls) : 0;
     if (e_cur == -1) return;
     fetch(e_cur, 0);
     cp_async_commit();
@@ -625,6 +640,15 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                             v[1] += wb.w[c] * (rc.re * hc.re + rc.im * hc.im);
                         }
                     }
+                    if (a.wkeep) {   // keep the window for gb_residual_update_kept: [position][channel][N]
+                        const int64_t off = keep_base + (int64_t)pos_cur * 2 * N + (int64_t)ch * N + ht;
+                        if (off - ht - (int64_t)ch * N + 2 * N <= a.wkeep_cap) {
+#pragma unroll
+                            for (int m = 0; m < M; m++) a.wkeep[off + H * m] = h[m];
+                        } else if (tid == 0) {
+                            atomicOr(a.errflag, 4);
+                        }
+                    }
                     group_reduce<G, 2>(v, s_red, tid);
                     if (tid == 0) {
                         const double hh = norm * v[0], rh = norm * v[1];
@@ -745,12 +769,15 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         }
         if (tid == 0) {
             s_ent[0] = e_nx2;
+            s_pos[0] = t_nx2;
             t_nx2 = t_nx3;
         }
         group_sync<G>();   // the waveform buffers, s_red and this half of s_src are reused from here on
         if (!has_nxt) break;
         e_cur = e_nxt;
         e_nxt = s_ent[0];
+        pos_cur = pos_nxt;
+        pos_nxt = s_pos[0];
         buf ^= 1;
     }
 }
@@ -764,6 +791,51 @@ constexpr size_t main_smem_bytes() {
 }
 
 }  // namespace
+
+// ------------------------------------------------------------------------------------------------ kept windows
+// gb_residual_update_kept: scatter of the accepted rows from the windows gb_delta_loglike_keep left in scratch.  The
+// class lists, their counts and the source records of that call are still in the context; one CTA per list entry.
+struct KeptArgs {
+    const int32_t* counts;
+    const int32_t* lists;
+    const SrcConst* src_new;
+    const SrcConst* src_old;
+    const cx* wkeep;
+    const uint8_t* accepted;
+    double* resid;
+    int64_t B, k_lo, n_f;
+    double sign;     // +1 applies the moves, -1 undoes them
+};
+
+__global__ void __launch_bounds__(128) gb_scatter_kept_kernel(KeptArgs a) {
+    int64_t base = 0;
+    for (int cls = 0; cls < kNumClasses; cls++) {
+        const int N = 128 << (cls >> 2);
+        const int count = a.counts[cls];
+        const int32_t* __restrict__ list = a.lists + (int64_t)cls * a.B;
+        for (int pos = blockIdx.x; pos < count; pos += gridDim.x) {
+            const int e = __ldg(list + pos);
+            const int64_t b = e & 0x7fffffff;
+            if (a.accepted && !a.accepted[b]) continue;
+            const SrcConst* rec = (e < 0 ? a.src_old : a.src_new) + b;
+            const int64_t i0 = rec->kmin - a.k_lo;
+            const double sgn = a.sign * (rec->move == GB_REMOVE ? 1.0 : -1.0);   // ADD: r -= a, REMOVE: r += h
+            const cx* w = a.wkeep + base + (int64_t)pos * 2 * N;
+            double* r = a.resid + (size_t)rec->walker * 2 * (size_t)a.n_f * 2;
+            for (int x = threadIdx.x; x < 2 * N; x += blockDim.x) {
+                const int ch = x >= N ? 1 : 0;
+                const int64_t i = i0 + (x - ch * N);
+                if (i >= 0 && i < a.n_f) {
+                    const cx h = w[x];
+                    double* p = r + ((size_t)ch * (size_t)a.n_f + (size_t)i) * 2;
+                    atomicAdd(p, sgn * h.re);
+                    atomicAdd(p + 1, sgn * h.im);
+                }
+            }
+        }
+        base += (int64_t)count * 2 * N;
+    }
+}
 
 // ------------------------------------------------------------------------------------------------ FP64 peak
 // 8 independent DFMA chains per thread, registers only (gb_measure_fp64_peak)
@@ -798,7 +870,9 @@ struct gb_ctx {
     int32_t* d_lists;
     cx* d_band_cache;       // current-source windows of gb_band_sweep's CTAs (gb_band.cuh)
     cx* d_temper_cache;     // set sums of gb_temper_sweep's CTAs (gb_temper.cuh)
-    int64_t cap_new, cap_old, cap_lists, cap_band_cache, cap_temper_cache;
+    cx* d_wkeep;            // windows kept by gb_delta_loglike_keep for gb_residual_update_kept
+    int64_t cap_new, cap_old, cap_lists, cap_band_cache, cap_temper_cache, cap_wkeep;
+    int64_t kept_B;         // > 0: lists, records and windows of the last gb_delta_loglike_keep call are still valid
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
     // staging for the *_host entry points
     void* d_stage;
@@ -898,6 +972,8 @@ struct Call {
     double* AE_out;
     int64_t* kmin_out;
     int Nmax;
+    int keep;               // gb_delta_loglike_keep
+    int64_t sum_bins;       // sum of the rows' window lengths (keep)
 };
 
 int run_call(gb_ctx* ctx, const Call& c, void* stream) {
@@ -933,6 +1009,11 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     if (need_new && (rc = ensure_cap(ctx, &ctx->d_src_new, &ctx->cap_new, c.B))) return rc;
     if (need_old && (rc = ensure_cap(ctx, &ctx->d_src_old, &ctx->cap_old, c.B))) return rc;
     if ((rc = ensure_cap(ctx, &ctx->d_lists, &ctx->cap_lists, c.B * kNumClasses))) return rc;
+    ctx->kept_B = 0;   // whatever an earlier keep call left is overwritten from here on
+    if (c.keep) {
+        if (c.sum_bins < 128 * c.B || c.sum_bins > 1024 * c.B) return set_err(ctx, GB_ERR_INVALID, "sum_n_bins out of range");
+        if ((rc = ensure_cap(ctx, &ctx->d_wkeep, &ctx->cap_wkeep, 2 * c.sum_bins))) return rc;
+    }
 
     GB_CUDA(ctx, cudaMemsetAsync(ctx->d_counts, 0, sizeof(int32_t) * 2 * kNumClasses, st));
 
@@ -948,6 +1029,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.mode = c.mode;
     p.n_walkers = c.data ? c.data->n_walkers : 0;
     p.n_psd = c.data ? c.data->n_psd : 0;
+    p.keep = c.keep;
     p.walker_psd = c.data ? c.data->walker_psd : nullptr;
     p.B = c.B;
     p.Tobs = ctx->cfg.Tobs;
@@ -994,6 +1076,9 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     a.Nmax = c.Nmax;
     a.Tobs = ctx->cfg.Tobs;
     a.tau = p.tau;
+    a.wkeep = c.keep ? ctx->d_wkeep : nullptr;
+    a.wkeep_cap = c.keep ? 2 * c.sum_bins : 0;
+    a.errflag = p.errflag;
 
     // launch only the classes that can occur; largest windows first
     const bool may_swap = c.mode != MODE_WAVEFORM && (c.move ? true : c.move_all == GB_SWAP);   // MODE_OVERLAP: move_all = SWAP
@@ -1020,6 +1105,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
             if (rc) return rc;
         }
     }
+    if (c.keep) ctx->kept_B = c.B;
     return GB_OK;
 }
 
@@ -1143,6 +1229,7 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_lists);
     cudaFree(ctx->d_band_cache);
     cudaFree(ctx->d_temper_cache);
+    cudaFree(ctx->d_wkeep);
     cudaFree(ctx->d_stage);
     if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
     if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
@@ -1197,7 +1284,7 @@ int gb_check(gb_ctx* ctx, void* stream) {
     GB_CUDA(ctx, cudaStreamSynchronize(st));
     if (flag) {
         GB_CUDA(ctx, cudaMemsetAsync(ctx->d_counts + 2 * kNumClasses, 0, sizeof(int32_t), st));
-        return set_err(ctx, GB_ERR_ROW, "row error flags 0x%x (1: bad N / move / walker index, 2: window beyond Nyquist)", flag);
+        return set_err(ctx, GB_ERR_ROW, "row error flags 0x%x (1: bad N / move / walker index, 2: window beyond Nyquist, 4: sum_n_bins too small)", flag);
     }
     return GB_OK;
 }
@@ -1233,6 +1320,51 @@ int gb_delta_loglike(gb_ctx* ctx, const gb_data* data, const double* params_new,
     c.dlnL_out = dlnL_out;
     c.aux_out = aux_out;
     return run_call(ctx, c, stream);
+}
+
+int gb_delta_loglike_keep(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                          const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                          int64_t B, int64_t sum_n_bins, double* dlnL_out, double* aux_out, void* stream) {
+    Call c{};
+    c.mode = MODE_DLNL;
+    c.data = data;
+    c.params_new = params_new;
+    c.params_old = params_old;
+    c.walker_index = walker_index;
+    c.move = move;
+    c.move_all = move_all;
+    c.N = N;
+    c.n_bins = n_bins;
+    c.B = B;
+    c.dlnL_out = dlnL_out;
+    c.aux_out = aux_out;
+    c.keep = 1;
+    c.sum_bins = n_bins ? sum_n_bins : (int64_t)N * B;
+    if (!move && move_all == GB_SWAP) return set_err(ctx, GB_ERR_INVALID, "gb_delta_loglike_keep takes ADD / REMOVE rows only");
+    return run_call(ctx, c, stream);
+}
+
+int gb_residual_update_kept(gb_ctx* ctx, const gb_data* data, const uint8_t* accepted, int negate, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (ctx->kept_B <= 0) return set_err(ctx, GB_ERR_INVALID, "no gb_delta_loglike_keep call to follow");
+    if (!data || !data->resid || data->n_f <= 0) return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    KeptArgs a{};
+    a.counts = ctx->d_counts;
+    a.lists = ctx->d_lists;
+    a.src_new = ctx->d_src_new;
+    a.src_old = ctx->d_src_old;
+    a.wkeep = ctx->d_wkeep;
+    a.accepted = accepted;
+    a.resid = data->resid;
+    a.B = ctx->kept_B;
+    a.k_lo = data->k_lo;
+    a.n_f = data->n_f;
+    a.sign = negate ? -1.0 : 1.0;
+    gb_scatter_kept_kernel<<<ctx->num_sms * 16, 128, 0, reinterpret_cast<cudaStream_t>(stream)>>>(a);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+    return GB_OK;
 }
 
 int gb_overlap(gb_ctx* ctx, const gb_data* data, const double* params_a, const double* params_c, const int32_t* psd_row,

@@ -21,7 +21,8 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
-           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep")
+           "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep",
+           "gb_delta_loglike_keep", "gb_residual_update_kept")
 
 BAND_MAX_STAGE = 3072
 # layout of gb_band_task (include/gbfit.h)
@@ -124,6 +125,10 @@ def lib() -> C.CDLL:
         L.gb_band_sweep.restype = ci
         L.gb_overlap.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, ci, vp, i64, vp, vp, vp]
         L.gb_overlap.restype = ci
+        L.gb_delta_loglike_keep.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, i64, vp, vp, vp]
+        L.gb_delta_loglike_keep.restype = ci
+        L.gb_residual_update_kept.argtypes = [vp, C.POINTER(GbData), vp, ci, vp]
+        L.gb_residual_update_kept.restype = ci
         L.gb_temper_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gb_temper_sweep.restype = ci
         for name, sig in (("gb_waveform", wf), ("gb_waveform_host", wf), ("gb_delta_loglike", dl),
@@ -331,6 +336,32 @@ class Context:
                                         _dev_ptr(out, torch.float64, dev, "out"),
                                         _dev_ptr(aux, torch.float64, dev, "aux"), _stream_ptr(stream, dev)))
         return out
+
+    def delta_loglike_keep(self, data: Data, params_new: Optional[torch.Tensor], params_old: Optional[torch.Tensor],
+                           walker_index: torch.Tensor, move: Optional[torch.Tensor] = None, move_all: int = ADD,
+                           N: int = 0, n_bins: Optional[torch.Tensor] = None, sum_n_bins: int = 0,
+                           out: Optional[torch.Tensor] = None, aux: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+        """gb_delta_loglike_keep: delta lnL of ADD / REMOVE rows; the windows stay in the context for residual_update_kept.
+        sum_n_bins = int(n_bins.sum()) when n_bins is given."""
+        dev = self.device
+        B = int(walker_index.shape[0])
+        if out is None:
+            out = torch.empty((B,), dtype=torch.float64, device=dev)
+        self._ok(lib().gb_delta_loglike_keep(self._h, data.c(), _dev_ptr(params_new, torch.float64, dev, "params_new"),
+                                             _dev_ptr(params_old, torch.float64, dev, "params_old"),
+                                             _dev_ptr(walker_index, torch.int32, dev, "walker_index"),
+                                             _dev_ptr(move, torch.int8, dev, "move"), int(move_all), int(N),
+                                             _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B, int(sum_n_bins),
+                                             _dev_ptr(out, torch.float64, dev, "out"),
+                                             _dev_ptr(aux, torch.float64, dev, "aux"), _stream_ptr(stream, dev)))
+        return out
+
+    def residual_update_kept(self, data: Data, accepted: Optional[torch.Tensor] = None, negate: bool = False,
+                             stream=None) -> None:
+        """gb_residual_update_kept: scatter the accepted rows of the preceding delta_loglike_keep call."""
+        dev = self.device
+        self._ok(lib().gb_residual_update_kept(self._h, data.c(), _dev_ptr(accepted, torch.uint8, dev, "accepted"),
+                                               int(bool(negate)), _stream_ptr(stream, dev)))
 
     def residual_update(self, data: Data, params_new: Optional[torch.Tensor], params_old: Optional[torch.Tensor],
                         walker_index: torch.Tensor, move: Optional[torch.Tensor] = None, move_all: int = ADD,

@@ -571,3 +571,41 @@ def test_repeated_calls_give_identical_bits(oracle, torch_cuda, gb):
         wf, _ = ctx.waveform(args[0][:4096], n_bins=kw["n_bins"][:4096], Nmax=1024)
         assert np.array_equal(wf.cpu().numpy(), wf0)
     ctx.check()
+
+
+def test_keep_and_update_kept_equal_the_two_call_form(oracle, torch_cuda, gb):
+    """gb_delta_loglike_keep gives the bits of gb_delta_loglike; gb_residual_update_kept equals the oracle's update (and
+    gb_residual_update) on the accepted rows, negate undoes it, and the kept state does not survive another call."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=6000, n_walkers=4)
+    wl.params_new[10, 1] = 4.1e-2                     # a general-path row (window outside the band)
+    wl.n_bins[10] = 1024
+    wl.params_old[10] = wl.params_new[10]
+    resid = wl.resid()
+    data, d_resid = upload(torch, gbfit, wl, resid)
+    args = (dev(torch, wl.params_new), dev(torch, wl.params_old), dev(torch, wl.walker_index))
+    kw = dict(move=dev(torch, wl.move), n_bins=dev(torch, wl.n_bins))
+    plain = ctx.delta_loglike(data, *args, **kw).cpu().numpy()
+    kept = ctx.delta_loglike_keep(data, *args, sum_n_bins=int(wl.n_bins.sum()), **kw).cpu().numpy()
+    assert np.array_equal(plain, kept)
+    acc = (np.random.Generator(np.random.Philox(key=[9, 9])).random(wl.B) < 0.3).astype(np.uint8)
+    ctx.residual_update_kept(data, dev(torch, acc))
+    ctx.check()
+    od = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    oracle.residual_update(oracle.Config(), od, wl.params_new, wl.params_old, wl.walker_index, move=wl.move, accepted=acc,
+                           n_bins=wl.n_bins, nthreads=oracle.max_threads())
+    dref = od.resid - resid
+    assert np.abs((d_resid.cpu().numpy() - resid) - dref).max() <= 1e-9 * np.abs(dref).max()
+    ctx.residual_update_kept(data, dev(torch, acc), negate=True)
+    assert np.abs(d_resid.cpu().numpy() - resid).max() <= 4e-16 * max(np.abs(resid).max(), np.abs(dref).max())
+    ctx.delta_loglike(data, *args, **kw)              # any other batched call drops the kept state
+    with pytest.raises(gbfit.GbError):
+        ctx.residual_update_kept(data, dev(torch, acc))
+    with pytest.raises(gbfit.GbError):                # too small a sum_n_bins: row-error flag
+        ctx.delta_loglike_keep(data, *args, sum_n_bins=128 * wl.B, **kw)
+        ctx.check()
+    mv = wl.move.copy(); mv[3] = gbfit.SWAP
+    ctx.delta_loglike_keep(data, *args, sum_n_bins=int(wl.n_bins.sum()), move=dev(torch, mv), n_bins=kw["n_bins"])
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
