@@ -39,7 +39,7 @@ WORKLOAD = "cfg5_full_ensemble_sweep_10x36x12000"
 
 # ---- algorithmic work per evaluation (frozen in BASELINE.md before optimisation) ----
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
-NCU_DRAM_BYTES_DLNL = 15.39e9                           # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1_v8
+NCU_DRAM_BYTES_DLNL = 13.70e9                           # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1_v9
 
 
 def flops_eval(N):
@@ -508,8 +508,8 @@ def run_ours(args):
         "dfma_lanes_per_clk_sm_at_1965mhz": dfma_lanes,
         "flops_per_launch": flops_dlnl, "ms_per_launch": ms_dlnl,
         # DRAM bytes (read + write) of the four delta-lnL kernels of one step, from the ncu --set full capture
-        # profiles/r1_v8_ncu_full_summary.csv (full workload only); algorithmic bytes are in "hbm"
-        "traffic": NCU_DRAM_BYTES_DLNL if full else None, "traffic_unit": "bytes per delta-lnL call (ncu, r1_v8)",
+        # profiles/r1_v9_ncu_full_summary.csv (full workload only); algorithmic bytes are in "hbm"
+        "traffic": NCU_DRAM_BYTES_DLNL if full else None, "traffic_unit": "bytes per delta-lnL call (ncu, r1_v9)",
         "hbm": {"achieved": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "bytes_per_launch": bytes_dlnl},
