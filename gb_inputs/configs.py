@@ -125,15 +125,28 @@ class Workload:
                         pick(self.accepted), self._psd_scale)
 
 
+# E-channel noise levels of the un-jittered configs 1-2 relative to the A channel.  The paper fits the noise
+# "in both channels (i.e., four parameters in total)", so S_A != S_E is the normal case; a fixed
+# offset keeps every PSD row's two channels distinguishable, so that a swapped or duplicated channel row cannot
+# pass a parity test.
+_E_OFFSET = (1.04, 0.97)      # (sqrt S_acc, sqrt S_oms) of E / nominal
+
+
 def _psd_rows(config: int, n_rows: int, k_lo: int, n_f: int, jitter: bool):
+    """PSD rows [n_rows, 2, n_f]: channel 0 = A, channel 1 = E, each with its own (sqrt S_acc, sqrt S_oms) pair
+    (four noise parameters, two per channel).  Returns (psd, scale[n_rows, 2 channels, 2 levels])."""
     f = (k_lo + np.arange(n_f, dtype=np.float64)) / TOBS
     psd = np.empty((n_rows, 2, n_f), np.float64)
     g = _rng(config, _S_PSD)
-    scale = 1.0 + 0.05 * (2.0 * g.random((n_rows, 2)) - 1.0) if jitter else np.ones((n_rows, 2))
+    scale = np.ones((n_rows, 2, 2))
+    if jitter:
+        scale[:, 0, :] = 1.0 + 0.05 * (2.0 * g.random((n_rows, 2)) - 1.0)      # A: the draws of the first recipe
+        scale[:, 1, :] = 1.0 + 0.05 * (2.0 * g.random((n_rows, 2)) - 1.0)      # E: its own draws
+    else:
+        scale[:, 1, :] = _E_OFFSET
     for r in range(n_rows):
-        S = instrument_psd(f, 3e-15 * scale[r, 0], 15e-12 * scale[r, 1])
-        psd[r, 0] = S
-        psd[r, 1] = S                                               # same S for A and E
+        for ch in range(2):
+            psd[r, ch] = instrument_psd(f, 3e-15 * scale[r, ch, 0], 15e-12 * scale[r, ch, 1])
     return psd, scale
 
 

@@ -305,6 +305,142 @@ def test_inverse_psd_flag(oracle):
     assert np.abs(a - b).max() < 1e-9 * np.abs(a).max()
 
 
+# ---------------------------------------------------------------- per-channel noise rows
+def _two_channel_psd(wl, n_rows):
+    """PSD rows whose channels differ strongly: S_E = 4 S_A times a tilt in frequency, and row r scaled by 1 + r."""
+    f = (wl.k_lo + np.arange(wl.n_f)) / wl.Tobs
+    SA = instrument_psd(f)
+    psd = np.empty((n_rows, 2, wl.n_f))
+    for r in range(n_rows):
+        psd[r, 0] = (1.0 + r) * SA
+        psd[r, 1] = (1.0 + r) * 4.0 * SA * (f / f[0]) ** 0.3
+    return psd
+
+
+def test_channel_psd_rows_are_addressed_per_channel(oracle):
+    """The paper fits the noise "in both channels (i.e., four parameters in total)", so S_A != S_E.
+    With S_E = 4 S_A x tilt, <h|h>, <r|h>, Eq. 4, Eq. 5 and the overlap must equal the numpy sums
+    4/T sum(|A|^2 / S_A + |E|^2 / S_E) written out per channel; the same sums with the channels' rows exchanged or
+    with the A row used twice are far away (the pin has power against `(row*2+0)` for both channels)."""
+    cfg = oracle.Config()
+    wl = make_workload(3, B=12, n_walkers=2)
+    psd = _two_channel_psd(wl, 2)
+    wpsd = np.array([1, 0], np.int32)                     # walker -> row map that is not the identity
+    resid = wl.resid()
+    data = oracle.Data(resid, psd, wl.k_lo, walker_psd=wpsd)
+    add = np.zeros(wl.B, np.int8)
+    d_add, aux = oracle.delta_loglike(cfg, data, wl.params_new, None, wl.walker_index, move=add, n_bins=wl.n_bins,
+                                      want_aux=True)
+    new = wl.params_new.copy()
+    new[:, 1] += 3.3 / cfg.Tobs
+    new[:, 3] += 0.4
+    d_sw = oracle.delta_loglike(cfg, data, new, wl.params_new, wl.walker_index, move_all=oracle.SWAP, n_bins=wl.n_bins)
+    ov, ovaux = oracle.overlap(cfg, data, new, wl.params_new, psd_row=wpsd[wl.walker_index], n_bins=wl.n_bins)
+    norm = 4.0 / cfg.Tobs
+
+    def sums(SA, SE, hA, hE, rA, rE):
+        hh = norm * ((np.abs(hA) ** 2 / SA).sum() + (np.abs(hE) ** 2 / SE).sum())
+        rh = norm * ((np.conj(rA) * hA / SA).real.sum() + (np.conj(rE) * hE / SE).real.sum())
+        return hh, rh
+
+    off = []
+    for b in range(wl.B):
+        w, N = int(wl.walker_index[b]), int(wl.n_bins[b])
+        row = int(wpsd[w])
+        A, E, kmin = oracle.waveform(cfg, wl.params_new[b], N)
+        A2, E2, kmin2 = oracle.waveform(cfg, new[b], N)
+        i0 = kmin - wl.k_lo
+        sl = slice(i0, i0 + N)
+        SA, SE = psd[row, 0, sl], psd[row, 1, sl]
+        hh, rh = sums(SA, SE, A, E, resid[w, 0, sl], resid[w, 1, sl])
+        assert abs(aux[b, 0] / hh - 1.0) < 1e-12 and abs(aux[b, 1] - rh) < 1e-11 * max(1.0, hh)
+        assert abs(d_add[b] - (rh - 0.5 * hh)) < 1e-11 * max(1.0, hh)
+        # the wrong addressings are nowhere near
+        for bad_SA, bad_SE in ((SE, SA), (SA, SA), (SE, SE), (psd[1 - row, 0, sl], psd[1 - row, 1, sl])):
+            hh_bad, _ = sums(bad_SA, bad_SE, A, E, resid[w, 0, sl], resid[w, 1, sl])
+            off.append(abs(hh_bad / hh - 1.0))
+        # Eq. 5 and the overlap with offset windows, per channel on the union / intersection
+        sl2 = slice(kmin2 - wl.k_lo, kmin2 - wl.k_lo + N)
+        aa, ra = sums(psd[row, 0, sl2], psd[row, 1, sl2], A2, E2, resid[w, 0, sl2], resid[w, 1, sl2])
+        sh = kmin2 - kmin                                 # bin j of the new window is bin j + sh of the old one
+        j = np.arange(N)
+        ok = (j + sh >= 0) & (j + sh < N)
+        ao = norm * ((np.conj(A2[ok]) * A[j[ok] + sh] / psd[row, 0, sl2][ok]).real.sum()
+                     + (np.conj(E2[ok]) * E[j[ok] + sh] / psd[row, 1, sl2][ok]).real.sum())
+        want = -0.5 * (aa + hh - 2.0 * ao - 2.0 * ra + 2.0 * rh)
+        assert abs(d_sw[b] - want) < 1e-10 * max(1.0, hh, aa)
+        assert abs(ov[b] - ao / np.sqrt(aa * hh)) < 1e-12
+        assert abs(ovaux[b, 0] / aa - 1.0) < 1e-12 and abs(ovaux[b, 1] / hh - 1.0) < 1e-12
+    off = np.asarray(off).reshape(wl.B, 4)                # per row: channels exchanged, A twice, E twice, other PSD row
+    assert np.median(off, axis=0).min() > 0.03 and off.max(axis=0).min() > 0.3 and off.min() > 1e-6   # against a 1e-12 agreement of the right addressing
+
+
+def test_band_and_temper_sweeps_use_each_channels_own_noise_row(oracle):
+    """Algorithm 1 and Algorithm 2 on data whose A and E rows differ by a factor 4: the accepted delta lnL of every band
+    task add up to the change of -1/2 <r|r> summed per channel, and every (D_i, D_j) of Eq. D2 is the lnL change obtained
+    by actually exchanging the sets, with each chain's own (A, E) rows."""
+    from temper_setup import temper_case
+    cfg = oracle.Config()
+    # ---- Algorithm 1
+    wl, bt, resid = _band_case(oracle)
+    psd = _two_channel_psd(wl, wl.n_walkers)
+
+    def lnl(r, w, k0, ns):
+        i0 = k0 - wl.k_lo
+        return -0.5 * (4.0 / wl.Tobs) * float((np.abs(r[w, 0, i0:i0 + ns]) ** 2 / psd[w, 0, i0:i0 + ns]).sum()
+                                              + (np.abs(r[w, 1, i0:i0 + ns]) ** 2 / psd[w, 1, i0:i0 + ns]).sum())
+
+    def lnl_swapped(r, w, k0, ns):
+        i0 = k0 - wl.k_lo
+        return -0.5 * (4.0 / wl.Tobs) * float((np.abs(r[w, 0, i0:i0 + ns]) ** 2 / psd[w, 1, i0:i0 + ns]).sum()
+                                              + (np.abs(r[w, 1, i0:i0 + ns]) ** 2 / psd[w, 0, i0:i0 + ns]).sum())
+
+    data = oracle.Data(resid.copy(), psd, wl.k_lo)
+    params = bt.params.copy()
+    t = bt.tasks
+    n_acc = 0
+    for i in range(len(t["walker"])):
+        one = {k: v[i:i + 1] for k, v in t.items()}
+        w, k0, ns = int(t["walker"][i]), int(t["k_first"][i]), int(t["n_stage"][i])
+        l0, l0s = lnl(data.resid, w, k0, ns), lnl_swapped(data.resid, w, k0, ns)
+        a_i, d_i = oracle.band_sweep(cfg, data, one, bt.N, params, bt.prop_k, bt.prop_params, bt.prop_logq,
+                                     np.full_like(bt.prop_logu, -np.inf))                    # accept everything
+        l1, l1s = lnl(data.resid, w, k0, ns), lnl_swapped(data.resid, w, k0, ns)
+        sl = slice(t["prop_begin"][i], t["prop_begin"][i] + t["n_prop"][i])
+        tot = float(d_i[sl].sum())
+        n_acc += int(a_i[sl].sum())
+        assert abs(tot - (l1 - l0)) <= 1e-9 * max(1.0, abs(l0))
+        assert abs(tot - (l1s - l0s)) > 1e-3 * abs(tot)                # exchanged channel rows do not fit
+    assert n_acc == bt.prop_k.size
+    # ---- Algorithm 2
+    wl, tt, resid = temper_case(oracle, n_bands=2)
+    psd = _two_channel_psd(wl, wl.n_walkers)
+    t = tt.tasks
+    perm, acc, dl = oracle.temper_sweep(cfg, oracle.Data(resid.copy(), psd, wl.k_lo), t, tt.N, tt.params, tt.chain_walker,
+                                        tt.chain_beta, tt.chain_set_begin, tt.chain_set_n,
+                                        np.full_like(tt.chain_logu, np.inf))                 # evaluate only
+    assert not acc.any()
+    for i in range(len(t["n_t"])):
+        cb, nt, k0, ns = int(t["chain_begin"][i]), int(t["n_t"][i]), int(t["k_first"][i]), int(t["n_stage"][i])
+        for q in range(nt - 1, 0, -1):
+            wi, wj = int(tt.chain_walker[cb + q]), int(tt.chain_walker[cb + q - 1])
+            Si = tt.params[tt.chain_set_begin[cb + q]:][:tt.chain_set_n[cb + q]]
+            Sj = tt.params[tt.chain_set_begin[cb + q - 1]:][:tt.chain_set_n[cb + q - 1]]
+            trial = resid.copy()
+            dtrial = oracle.Data(trial, psd, wl.k_lo)
+            for w, old, new in ((wi, Si, Sj), (wj, Sj, Si)):
+                for src in old:
+                    oracle.residual_update(cfg, dtrial, None, src[None], np.full(1, w, np.int32), move_all=oracle.REMOVE, N=tt.N)
+                for src in new:
+                    oracle.residual_update(cfg, dtrial, src[None], None, np.full(1, w, np.int32), move_all=oracle.ADD, N=tt.N)
+            Di = lnl(trial, wi, k0, ns) - lnl(resid, wi, k0, ns)
+            Dj = lnl(trial, wj, k0, ns) - lnl(resid, wj, k0, ns)
+            assert abs(dl[cb + q, 0] - Di) <= 1e-9 * max(1.0, abs(lnl(resid, wi, k0, ns)))
+            assert abs(dl[cb + q, 1] - Dj) <= 1e-9 * max(1.0, abs(lnl(resid, wj, k0, ns)))
+            Dis = lnl_swapped(trial, wi, k0, ns) - lnl_swapped(resid, wi, k0, ns)
+            assert abs(dl[cb + q, 0] - Dis) > 1e-3 * abs(Di)
+
+
 # ---------------------------------------------------------------- orbits: invariants of the first-order model
 def test_orbit_invariants(oracle):
     cfg = oracle.Config()
