@@ -22,9 +22,16 @@
  *   - All calls return an int status (GB_OK = 0, negative = error), never throw, never abort.
  *   - Device work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
  *     stream) and is asynchronous with respect to the host, except the *_host entry points, which
- *     synchronise `stream` before returning.  Errors detectable at launch are returned at once; per-row
- *     errors (walker index out of range, N not in {128,256,512,1024}) set a sticky device flag that the next
- *     call to gb_check() reports, and give NaN in that row of the output.
+ *     synchronise `stream` before returning (also on every error return: no copy from or into a caller's
+ *     host buffer is in flight once a *_host call has returned).  Errors detectable at launch are returned at
+ *     once; per-row errors set bits of a sticky device flag that the next call to gb_check() reports:
+ *       1  walker index / PSD row out of range, N not in {128,256,512,1024} (gb_waveform: N_b > Nmax), bad move,
+ *          or a per-row move whose parameter array is NULL: the row is NOT computed, its dlnL is NaN (waveform
+ *          rows are left untouched, update rows are not applied);
+ *       2  the window extends beyond the Nyquist bin Tobs / (2 dt): the row IS computed and its output is finite
+ *          (the waveform definition does not depend on dt, reading S10) -- the flag is a warning;
+ *       4  gb_delta_loglike_keep: sum_n_bins too small: dlnL of every row is still computed and finite, windows
+ *          past the capacity are not kept, and gb_residual_update_kept skips (and flags) exactly those rows.
  *   - Complex arrays are complex128, interleaved (re, im) doubles.  Real arrays are f64.
  *   - params row (8 f64): [amp, f0 (Hz), fdot (Hz/s), phi0, cos(iota), psi, lambda (ecl. lon.), sin(beta)].
  *   - Frequency bins: global bin k  <->  f = k / Tobs  (the rfft grid of the data).
@@ -74,7 +81,7 @@ enum {
     GB_ERR_INVALID = -1,   /* NULL required pointer, B < 0, bad N, bad config                    */
     GB_ERR_CUDA = -2,      /* a CUDA runtime call failed; see gb_last_error                      */
     GB_ERR_NOMEM = -3,     /* scratch allocation failed                                          */
-    GB_ERR_ROW = -4        /* gb_check: some row of an earlier call had a bad walker index or N  */
+    GB_ERR_ROW = -4        /* gb_check: row-error flag bits 1 / 2 / 4 of an earlier call (see above) */
 };
 
 /* Fill *cfg with the defaults listed above (device 0).  cfg: HOST. */

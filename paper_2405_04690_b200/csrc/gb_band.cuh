@@ -75,8 +75,14 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         const gb_band_task t = a.tasks[it];
         const bool wb = (t.flags & GB_BAND_WRITE_BACK) != 0;
         const int wrow = (t.flags & GB_BAND_WRITE_OTHER) ? t.write_walker : t.walker;
-        if (t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0 ||
-            (wb && (wrow < 0 || wrow >= a.n_walkers))) {
+        bool bad = t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0 ||
+                   (wb && (wrow < 0 || wrow >= a.n_walkers));
+        int prow = 0;
+        if (!bad) {
+            prow = a.walker_psd ? a.walker_psd[t.walker] : (a.n_psd == 1 ? 0 : t.walker);
+            bad = prow < 0 || prow >= a.n_psd;
+        }
+        if (bad) {
             if (tid == 0) atomicOr(a.errflag, 1);
             for (int p = tid; p < t.n_prop; p += G) {
                 a.dlnL_out[t.prop_begin + p] = nan;
@@ -90,7 +96,6 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         const double* rE = a.resid + ((size_t)t.walker * 2 + 1) * nf * 2;
         double* wA = a.resid + ((size_t)(wb ? wrow : t.walker) * 2 + 0) * nf * 2;   // accepted changes go to this row
         double* wE = a.resid + ((size_t)(wb ? wrow : t.walker) * 2 + 1) * nf * 2;
-        const int prow = a.walker_psd ? a.walker_psd[t.walker] : (a.n_psd == 1 ? 0 : t.walker);
         const double* SA = a.psd + ((size_t)prow * 2 + 0) * nf;
         const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
         const int64_t i_first = t.k_first - a.k_lo;   // stored element of staged bin 0

@@ -73,6 +73,10 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a
         for (int q = 0; ok && q < t.n_t; q++) {
             const int w = a.chain_walker[t.chain_begin + q];
             ok = w >= 0 && w < a.n_walkers && a.chain_set_n[t.chain_begin + q] >= 0;
+            if (ok) {
+                const int row = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
+                ok = row >= 0 && row < a.n_psd;
+            }
         }
         for (int q = tid; q < t.n_t; q += G) {
             const int c = t.chain_begin + q;

@@ -69,6 +69,7 @@ struct PrepArgs {
     const int32_t* n_bins;
     const int32_t* walker_psd;
     int move_all, N, mode, n_walkers, n_psd, keep;
+    int Nmax;                // MODE_WAVEFORM: row pitch of AE_out (a row with N_b > Nmax is a row error)
     int64_t B;
     double Tobs, tau, Rmax;  // Rmax = AU / c
     int64_t kmax;            // largest valid global bin (Nyquist)
@@ -133,6 +134,9 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         const int N = a.n_bins ? a.n_bins[b] : a.N;
         const int cN = class_of_N(N);
         bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP && !(a.keep && mv == GB_SWAP);
+        if (a.mode == MODE_WAVEFORM && N > a.Nmax) ok = false;                 // would overrun the row of AE_out
+        if (mv != GB_REMOVE && !a.params_new) ok = false;                      // per-row move needs a side that is NULL
+        if (mv != GB_ADD && !a.params_old) ok = false;
         int w = 0, prow = 0;
         if (a.mode == MODE_OVERLAP) {          // walker_index carries the PSD row itself (NULL: row 0)
             prow = a.walker_index ? a.walker_index[b] : 0;
@@ -141,6 +145,7 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
             w = a.walker_index[b];
             ok = ok && w >= 0 && w < a.n_walkers;
             if (ok) prow = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
+            ok = ok && prow >= 0 && prow < a.n_psd;
         }
         const bool active = a.accepted ? a.accepted[b] != 0 : true;
         if (!ok) {
@@ -804,6 +809,9 @@ struct KeptArgs {
     const uint8_t* accepted;
     double* resid;
     int64_t B, k_lo, n_f;
+    int64_t wkeep_cap;   // elements the keep call was allowed to write: windows past it were never stored
+    int32_t n_walkers;   // of the gb_data passed to THIS call (the records carry the keep call's walker indices)
+    int32_t* errflag;
     double sign;     // +1 applies the moves, -1 undoes them
 };
 
@@ -820,7 +828,12 @@ __global__ void __launch_bounds__(128) gb_scatter_kept_kernel(KeptArgs a) {
             const SrcConst* rec = (e < 0 ? a.src_old : a.src_new) + b;
             const int64_t i0 = rec->kmin - a.k_lo;
             const double sgn = a.sign * (rec->move == GB_REMOVE ? 1.0 : -1.0);   // ADD: r -= a, REMOVE: r += h
-            const cx* w = a.wkeep + base + (int64_t)pos * 2 * N;
+            const int64_t off = base + (int64_t)pos * 2 * N;
+            if (off + 2 * N > a.wkeep_cap || rec->walker < 0 || rec->walker >= a.n_walkers) {
+                if (threadIdx.x == 0) atomicOr(a.errflag, off + 2 * N > a.wkeep_cap ? 4 : 1);   // never stored / foreign view
+                continue;
+            }
+            const cx* w = a.wkeep + off;
             double* r = a.resid + (size_t)rec->walker * 2 * (size_t)a.n_f * 2;
             for (int x = threadIdx.x; x < 2 * N; x += blockDim.x) {
                 const int ch = x >= N ? 1 : 0;
@@ -873,6 +886,7 @@ struct gb_ctx {
     cx* d_wkeep;            // windows kept by gb_delta_loglike_keep for gb_residual_update_kept
     int64_t cap_new, cap_old, cap_lists, cap_band_cache, cap_temper_cache, cap_wkeep;
     int64_t kept_B;         // > 0: lists, records and windows of the last gb_delta_loglike_keep call are still valid
+    int64_t kept_cap;       // elements of d_wkeep that call was allowed to write (2 x its sum_n_bins)
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
     // staging for the *_host entry points
     void* d_stage;
@@ -1030,6 +1044,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.n_walkers = c.data ? c.data->n_walkers : 0;
     p.n_psd = c.data ? c.data->n_psd : 0;
     p.keep = c.keep;
+    p.Nmax = c.Nmax;
     p.walker_psd = c.data ? c.data->walker_psd : nullptr;
     p.B = c.B;
     p.Tobs = ctx->cfg.Tobs;
@@ -1105,7 +1120,10 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
             if (rc) return rc;
         }
     }
-    if (c.keep) ctx->kept_B = c.B;
+    if (c.keep) {
+        ctx->kept_B = c.B;
+        ctx->kept_cap = 2 * c.sum_bins;
+    }
     return GB_OK;
 }
 
@@ -1347,7 +1365,7 @@ int gb_delta_loglike_keep(gb_ctx* ctx, const gb_data* data, const double* params
 int gb_residual_update_kept(gb_ctx* ctx, const gb_data* data, const uint8_t* accepted, int negate, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
     if (ctx->kept_B <= 0) return set_err(ctx, GB_ERR_INVALID, "no gb_delta_loglike_keep call to follow");
-    if (!data || !data->resid || data->n_f <= 0) return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
+    if (!data || !data->resid || data->n_f <= 0 || data->n_walkers <= 0) return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
     GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     KeptArgs a{};
     a.counts = ctx->d_counts;
@@ -1360,6 +1378,9 @@ int gb_residual_update_kept(gb_ctx* ctx, const gb_data* data, const uint8_t* acc
     a.B = ctx->kept_B;
     a.k_lo = data->k_lo;
     a.n_f = data->n_f;
+    a.wkeep_cap = ctx->kept_cap;
+    a.n_walkers = data->n_walkers;
+    a.errflag = ctx->d_counts + 2 * kNumClasses;
     a.sign = negate ? -1.0 : 1.0;
     gb_scatter_kept_kernel<<<ctx->num_sms * 16, 128, 0, reinterpret_cast<cudaStream_t>(stream)>>>(a);
     ctx->launches++;
@@ -1537,9 +1558,22 @@ int stage_reserve(gb_ctx* ctx, size_t bytes) {
 }
 }  // namespace
 
-extern "C" {
+// every error return of a *_host form drains the copy streams first: no copy from or into a caller's host buffer may be in
+// flight once the call has returned
+namespace {
+int drain_on_error(gb_ctx* ctx, void* stream, int rc) {
+    if (rc != GB_OK && ctx) {
+        const int keep_errno = rc;
+        if (ctx->s_in) cudaStreamSynchronize(ctx->s_in);
+        if (ctx->s_out) cudaStreamSynchronize(ctx->s_out);
+        cudaStreamSynchronize(reinterpret_cast<cudaStream_t>(stream));
+        cudaGetLastError();
+        return keep_errno;
+    }
+    return rc;
+}
 
-int gb_waveform_host(gb_ctx* ctx, const double* params, int64_t B, int N, const int32_t* n_bins, int Nmax,
+int waveform_host_impl(gb_ctx* ctx, const double* params, int64_t B, int N, const int32_t* n_bins, int Nmax,
                      double* AE_out, int64_t* kmin_out, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
     if (B < 0 || !params || !AE_out || Nmax <= 0) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
@@ -1562,9 +1596,9 @@ int gb_waveform_host(gb_ctx* ctx, const double* params, int64_t B, int N, const 
     return GB_OK;
 }
 
-int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
-                          const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
-                          int64_t B, double* dlnL_out, double* aux_out, void* stream) {
+int delta_loglike_host_impl(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                            const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                            int64_t B, double* dlnL_out, double* aux_out, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
     if (B < 0 || !walker_index || !dlnL_out) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
     if (B == 0) return GB_OK;
@@ -1600,11 +1634,7 @@ int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params
         rc = gb_delta_loglike(ctx, data, d_pn ? d_pn + 8 * lo : nullptr, d_po ? d_po + 8 * lo : nullptr, d_w + lo,
                               d_mv ? d_mv + lo : nullptr, move_all, N, d_nb ? d_nb + lo : nullptr, n, d_out + lo,
                               d_aux ? d_aux + 2 * lo : nullptr, stream);
-        if (rc) {
-            cudaStreamSynchronize(ctx->s_in);
-            cudaStreamSynchronize(ctx->s_out);
-            return rc;
-        }
+        if (rc) return rc;
         GB_CUDA(ctx, cudaEventRecord(ctx->ev_done[c], st));
         GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[c], 0));
         GB_CUDA(ctx, cudaMemcpyAsync(dlnL_out + lo, d_out + lo, (size_t)n * 8, cudaMemcpyDeviceToHost, ctx->s_out));
@@ -1615,9 +1645,9 @@ int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params
     return GB_OK;
 }
 
-int gb_residual_update_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
-                            const int32_t* walker_index, const int8_t* move, int move_all, const uint8_t* accepted,
-                            int N, const int32_t* n_bins, int64_t B, void* stream) {
+int residual_update_host_impl(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                              const int32_t* walker_index, const int8_t* move, int move_all, const uint8_t* accepted,
+                              int N, const int32_t* n_bins, int64_t B, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
     if (B < 0 || !walker_index) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
     if (B == 0) return GB_OK;
@@ -1651,13 +1681,32 @@ int gb_residual_update_host(gb_ctx* ctx, const gb_data* data, const double* para
         rc = gb_residual_update(ctx, data, d_pn ? d_pn + 8 * lo : nullptr, d_po ? d_po + 8 * lo : nullptr, d_w + lo,
                                 d_mv ? d_mv + lo : nullptr, move_all, d_acc ? d_acc + lo : nullptr, N,
                                 d_nb ? d_nb + lo : nullptr, n, stream);
-        if (rc) {
-            cudaStreamSynchronize(ctx->s_in);
-            return rc;
-        }
+        if (rc) return rc;
     }
     GB_CUDA(ctx, cudaStreamSynchronize(st));
     return GB_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gb_waveform_host(gb_ctx* ctx, const double* params, int64_t B, int N, const int32_t* n_bins, int Nmax,
+                     double* AE_out, int64_t* kmin_out, void* stream) {
+    return drain_on_error(ctx, stream, waveform_host_impl(ctx, params, B, N, n_bins, Nmax, AE_out, kmin_out, stream));
+}
+
+int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                          const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                          int64_t B, double* dlnL_out, double* aux_out, void* stream) {
+    return drain_on_error(ctx, stream, delta_loglike_host_impl(ctx, data, params_new, params_old, walker_index, move, move_all,
+                                                               N, n_bins, B, dlnL_out, aux_out, stream));
+}
+
+int gb_residual_update_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                            const int32_t* walker_index, const int8_t* move, int move_all, const uint8_t* accepted,
+                            int N, const int32_t* n_bins, int64_t B, void* stream) {
+    return drain_on_error(ctx, stream, residual_update_host_impl(ctx, data, params_new, params_old, walker_index, move,
+                                                                 move_all, accepted, N, n_bins, B, stream));
 }
 
 }  // extern "C"

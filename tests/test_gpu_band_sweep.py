@@ -155,8 +155,10 @@ def test_band_sweep_odd_even_cold_chain_buffers(oracle, torch_cuda, gb):
 def test_band_sweep_many_tasks_sampled(oracle, torch_cuda, gb):
     """The bench's launch shape at a tenth of its size: 36 walkers x 183 odd 256-bin sub-bands (6588 concurrent tasks,
     more than one wave of CTAs), 9 sources and 30 proposals each.  Tasks of one walker only share bins that none of their
-    windows reach, so the oracle can run a seeded sample of tasks on the initial residual: decisions, delta lnL and final
-    parameters of those tasks must match."""
+    windows reach, and tasks of different walkers share nothing, so the oracle can run ALL 183 tasks of each of three
+    walkers (549 tasks, in task order) on the initial residual: decisions, delta lnL and final parameters of those tasks
+    and the walkers' whole written-back residual rows -- the place where concurrent CTAs add to one row with atomics --
+    must match.  The other tasks are checked for finite output only."""
     gbfit, ctx = gb
     torch = torch_cuda
     wl = make_workload(3, B=1, n_walkers=36)
@@ -169,17 +171,24 @@ def test_band_sweep_many_tasks_sampled(oracle, torch_cuda, gb):
                              dev(torch, bt.prop_k), dev(torch, bt.prop_params), dev(torch, bt.prop_logq), dev(torch, bt.prop_logu))
     ctx.check()
     acc, dl, params = acc.cpu().numpy(), dl.cpu().numpy(), d_params.cpu().numpy()
+    r1 = d_resid.cpu().numpy()
     nt = len(bt.tasks["walker"])
     assert nt == 6588 and np.isfinite(dl).all()
-    pick = np.random.Generator(np.random.Philox(key=[1, 256])).choice(nt, 64, replace=False)
+    walkers = (0, 17, 35)
+    pick = np.flatnonzero(np.isin(bt.tasks["walker"], walkers))
+    assert pick.size == 3 * 183
     sub = {k: v[pick] for k, v in bt.tasks.items()}
     p_ref = bt.params.copy()
-    racc, rdl = oracle.band_sweep(oracle.Config(), oracle.Data(resid.copy(), wl.psd, wl.k_lo), sub, 256, p_ref, bt.prop_k,
-                                  bt.prop_params, bt.prop_logq, bt.prop_logu)
+    odata = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    racc, rdl = oracle.band_sweep(oracle.Config(), odata, sub, 256, p_ref, bt.prop_k, bt.prop_params, bt.prop_logq, bt.prop_logu)
     for i in pick:
         ps = slice(bt.tasks["prop_begin"][i], bt.tasks["prop_begin"][i] + bt.tasks["n_prop"][i])
         ss = slice(bt.tasks["src_begin"][i], bt.tasks["src_begin"][i] + bt.tasks["n_src"][i])
         assert np.array_equal(acc[ps], racc[ps]), i
         assert np.abs(dl[ps] - rdl[ps]).max() <= TOL_DLNL, i
         assert np.array_equal(params[ss], p_ref[ss]), i
+    for w in walkers:                                   # the whole row: every task of the walker wrote into it
+        change = np.abs(odata.resid[w] - resid[w]).max()
+        assert change > 0
+        assert np.abs(r1[w] - odata.resid[w]).max() <= 1e-9 * change + 4e-16 * np.abs(resid[w]).max(), w
     assert 0.02 < acc.mean() < 0.98

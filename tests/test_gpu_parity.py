@@ -609,3 +609,89 @@ def test_keep_and_update_kept_equal_the_two_call_form(oracle, torch_cuda, gb):
     ctx.delta_loglike_keep(data, *args, sum_n_bins=int(wl.n_bins.sum()), move=dev(torch, mv), n_bins=kw["n_bins"])
     with pytest.raises(gbfit.GbError):
         ctx.check()
+
+
+def test_update_kept_after_an_undersized_keep_call_touches_nothing_out_of_range(oracle, torch_cuda, gb):
+    """ADVICE r1: gb_delta_loglike_keep with too small a sum_n_bins skips the stores past the capacity and sets flag 4;
+    a following gb_residual_update_kept must skip exactly those rows (and flag them) instead of adding stale scratch:
+    the rows it does apply equal the oracle's update of those rows."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=3000, n_walkers=3)
+    resid = wl.resid()
+    data, d_resid = upload(torch, gbfit, wl, resid)
+    args = (dev(torch, wl.params_new), dev(torch, wl.params_old), dev(torch, wl.walker_index))
+    kw = dict(move=dev(torch, wl.move), n_bins=dev(torch, wl.n_bins))
+    # make the scratch hold a previous, larger call's windows: stale data lies beyond the small call's capacity
+    ctx.delta_loglike_keep(data, *args, sum_n_bins=int(wl.n_bins.sum()), **kw)
+    ctx.check()
+    small = int(wl.n_bins.sum()) // 2
+    assert small >= 128 * wl.B
+    ctx.delta_loglike_keep(data, *args, sum_n_bins=small, **kw)
+    ctx.residual_update_kept(data)
+    with pytest.raises(gbfit.GbError) as ei:
+        ctx.check()
+    assert ei.value.code == gbfit.GB_ERR_ROW
+    got = d_resid.cpu().numpy() - resid
+    # the scratch is laid out class by class (N = 128 first), so the small windows fit and the large ones were skipped
+    assert np.abs(got).max() > 0
+    full = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    oracle.residual_update(oracle.Config(), full, wl.params_new, wl.params_old, wl.walker_index, move=wl.move,
+                           n_bins=wl.n_bins, nthreads=oracle.max_threads())
+    dfull = full.resid - resid
+    assert np.abs(got - dfull).max() > 1e-3 * np.abs(dfull).max()          # some rows were skipped ...
+    assert np.abs(got).max() <= np.abs(dfull).max() * 1.5                  # ... and nothing foreign was added
+    # half of the window bins covers all N = 128 and N = 256 rows (f0 < 4 mHz) and none of the N = 1024 rows (> 10 mHz)
+    lo = int(0.9e-3 * wl.Tobs) - wl.k_lo
+    hi = int(10.2e-3 * wl.Tobs) - wl.k_lo
+    assert np.abs(dfull[:, :, hi:]).max() > 0 and not got[:, :, hi:].any()
+    assert np.abs(got[:, :, :lo] - dfull[:, :, :lo]).max() <= 1e-9 * np.abs(dfull[:, :, :lo]).max()
+    # a gb_data with fewer walkers than the keep call saw: rows of the missing walkers are skipped and flagged
+    ctx.delta_loglike_keep(data, *args, sum_n_bins=int(wl.n_bins.sum()), **kw)
+    d2 = dev(torch, resid[:2])
+    data2 = gbfit.Data(d2, dev(torch, wl.psd[:2]), wl.k_lo)
+    ctx.residual_update_kept(data2)
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    sel = wl.walker_index < 2
+    ref2 = oracle.Data(resid[:2].copy(), wl.psd[:2], wl.k_lo)
+    oracle.residual_update(oracle.Config(), ref2, wl.params_new[sel], wl.params_old[sel], wl.walker_index[sel],
+                           move=wl.move[sel], n_bins=wl.n_bins[sel], nthreads=oracle.max_threads())
+    dref = ref2.resid - resid[:2]
+    assert np.abs((d2.cpu().numpy() - resid[:2]) - dref).max() <= 1e-9 * np.abs(dref).max()
+
+
+def test_row_errors_for_oversized_window_null_side_and_bad_psd_row(oracle, torch_cuda, gb):
+    """a per-row N larger than the pitch of AE_out, a per-row move whose parameter side is NULL, and a
+    walker_psd entry outside [0, n_psd) are row errors (flag 1, NaN / untouched row), not overruns or device faults."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=12, n_walkers=2)
+    nb = np.full(12, 128, np.int32); nb[5] = 512
+    out = torch.full((12, 2, 256), 7.0, dtype=torch.complex128, device="cuda:0")
+    ctx.waveform(dev(torch, wl.params_new), n_bins=dev(torch, nb), Nmax=256, out=out)
+    with pytest.raises(gbfit.GbError) as ei:
+        ctx.check()
+    assert ei.value.code == gbfit.GB_ERR_ROW
+    o = out.cpu().numpy()
+    assert np.all(o[5] == 7.0)                                             # the bad row is left untouched
+    assert np.all(o[:, :, 128:][np.arange(12) != 5] == 7.0)                # nothing past a row's own window
+    ref, _ = oracle.waveform_batch(oracle.Config(), wl.params_new[:5], N=128)
+    assert wf_err(o[:5, :, :128], ref) <= TOL_WF
+    # per-row moves with params_old = NULL: the REMOVE rows are row errors, the ADD rows are computed
+    resid = wl.resid()
+    data, _ = upload(torch, gbfit, wl, resid)
+    d = ctx.delta_loglike(data, dev(torch, wl.params_new), None, dev(torch, wl.walker_index), move=dev(torch, wl.move),
+                          n_bins=dev(torch, wl.n_bins)).cpu().numpy()
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    assert (wl.move == 1).any() and (wl.move == 0).any()
+    assert np.isnan(d[wl.move == 1]).all() and np.isfinite(d[wl.move == 0]).all()
+    # walker_psd entry out of range
+    wp = np.array([0, 9], np.int32)
+    dataw = gbfit.Data(dev(torch, resid), dev(torch, wl.psd), wl.k_lo, walker_psd=dev(torch, wp))
+    d = ctx.delta_loglike(dataw, dev(torch, wl.params_new), dev(torch, wl.params_old), dev(torch, wl.walker_index),
+                          move=dev(torch, wl.move), n_bins=dev(torch, wl.n_bins)).cpu().numpy()
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    assert np.isnan(d[wl.walker_index == 1]).all() and np.isfinite(d[wl.walker_index == 0]).all()

@@ -95,8 +95,9 @@ def test_temper_sweep_all_accepted_none_accepted_no_write_back_inverse_psd_and_b
 def test_temper_sweep_many_ladders_sampled(oracle, torch_cuda, gb):
     """The bench's launch shape at reduced size: 183 odd 256-bin sub-bands x 4 disjoint walker groups = 732 ladders of
     8 chains running concurrently.  Ladders of one sub-band use disjoint residual rows and ladders of different
-    sub-bands only share bins that no window of either reaches, so the oracle can run a seeded sample of ladders on the
-    initial residuals: decisions, (D_i, D_j) and permutations of those ladders must match."""
+    sub-bands only share bins that no window of either reaches, so the oracle can run, on the initial residuals, every
+    ladder that touches one of two chosen residual rows (2 x 183 ladders, one per sub-band each): decisions, (D_i, D_j)
+    and permutations of those ladders and the two rows' whole written-back residuals must match."""
     gbfit, ctx = gb
     torch = torch_cuda
     from gb_inputs import make_workload, make_temper_tasks
@@ -113,14 +114,23 @@ def test_temper_sweep_many_ladders_sampled(oracle, torch_cuda, gb):
                                      dev(torch, tt.chain_set_n), dev(torch, lu))
     ctx.check()
     perm, acc, dl = perm.cpu().numpy(), acc.cpu().numpy(), dl.cpu().numpy()
+    r1 = d_resid.cpu().numpy()
     nt = len(tt.tasks["n_t"])
     assert nt == 732 and np.isfinite(dl).all()
-    pick = np.random.Generator(np.random.Philox(key=[3, 256])).choice(nt, 40, replace=False)
+    rows = (3, 20)
+    cw = tt.chain_walker.reshape(nt, 8)
+    pick = np.flatnonzero(np.isin(cw, rows).any(axis=1))
+    assert 183 <= pick.size <= 2 * 183 and all((cw == w).any(axis=1).sum() == 183 for w in rows)
     sub = {k: v[pick] for k, v in tt.tasks.items()}
-    rperm, racc, rdl = oracle.temper_sweep(oracle.Config(), oracle.Data(resid.copy(), wl.psd, wl.k_lo), sub, 256, tt.params,
-                                           tt.chain_walker, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, lu)
+    odata = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    rperm, racc, rdl = oracle.temper_sweep(oracle.Config(), odata, sub, 256, tt.params, tt.chain_walker, tt.chain_beta,
+                                           tt.chain_set_begin, tt.chain_set_n, lu)
     for i in pick:
         cs = slice(tt.tasks["chain_begin"][i], tt.tasks["chain_begin"][i] + tt.tasks["n_t"][i])
         assert np.array_equal(acc[cs], racc[cs]) and np.array_equal(perm[cs], rperm[cs]), i
         assert np.abs(dl[cs] - rdl[cs]).max() <= 1e-6, i
+    for w in rows:                                      # every ladder that writes into these rows was replayed
+        change = np.abs(odata.resid[w] - resid[w]).max()
+        assert change > 0
+        assert np.abs(r1[w] - odata.resid[w]).max() <= 1e-9 * change + 4e-16 * np.abs(resid[w]).max(), w
     assert acc.sum() > 0

@@ -123,19 +123,22 @@ def test_p8_tiny_T_full_rate_rfft(oracle):
 
 
 def test_p2_full_year_rfft(oracle):
-    """Full Tobs = 1 yr sampled at dt = 15 s (M = 2^21; the pin's own cadence -- dt does not enter O1-O6,
-    reading S10), geometry frozen per sample: overlap >= 0.998, max error ~1e-2 of peak."""
-    cfg = oracle.Config(dt=15.0)
+    """SURVEY 8(c) P2 at the data's own cadence: the real signal at all M = Tobs / dt = 6 291 456 samples (dt = 5 s,
+    PAPER.md:288), geometry frozen per sample, true dt * rfft, cut to the window.  Measured here: 1 - overlap 5.0e-4,
+    max error 6.6e-3 of peak, 3.7e-4 of the energy outside the window (rectangular-window leakage aliased by the
+    N-sample FFT, inherent to the method): overlap >= 0.999, max error <= 1e-2, leakage <= 1e-3."""
+    cfg = oracle.Config()
+    assert cfg.dt == 5.0 and int(round(cfg.Tobs / cfg.dt)) == 6291456
     p = rand_params(np.random.default_rng(17), 3.1e-3)
     N = 256
     A, E, kmin = oracle.waveform(cfg, p, N)
     FA, FE, kmin_bf, fullA, fullE = td.full_rate_window(cfg, p, N)
     assert kmin == kmin_bf
-    assert _overlap(np.r_[A, E], np.r_[FA, FE]) > 0.998
-    assert relerr(np.r_[A, E], np.r_[FA, FE]) < 3e-2
+    assert _overlap(np.r_[A, E], np.r_[FA, FE]) >= 0.999
+    assert relerr(np.r_[A, E], np.r_[FA, FE]) < 1e-2
     tot = (np.abs(fullA) ** 2).sum() + (np.abs(fullE) ** 2).sum()
     inside = (np.abs(FA) ** 2).sum() + (np.abs(FE) ** 2).sum()
-    assert 1.0 - inside / tot < 3e-3
+    assert 1.0 - inside / tot < 1e-3
 
 
 # ---------------------------------------------------------------- P3: moving geometry at the coarse times
