@@ -299,6 +299,46 @@ def make_band_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_src: int,
 
 
 # ---------------------------------------------------------------------------------------------------------
+# Inputs of the in-loop proposal step of Algorithm 1 (group stretch, App. B :566-576): the stationary
+# group -- "a flattened set of all templates contained in the cold-chain in all current walkers", sorted by frequency
+# -- stands in as n_copies jittered copies of every band's initial sources (what posterior samples of the
+# same sources in other walkers look like), plus the prior box and the periodic flags of the 8 coordinates.
+@dataclass
+class StretchInputs:
+    seed: int
+    sweep: int
+    group: np.ndarray           # [n_group, 8] sorted by f0 ascending
+    n_friends: int
+    stretch_a: float
+    lo: np.ndarray              # [8] prior box
+    hi: np.ndarray
+    periodic: np.ndarray        # [8] int32
+
+
+PRIOR_LO = np.array([1e-24, 5e-5, -1e-14, 0.0, -1.0, 0.0, 0.0, -1.0])
+PRIOR_HI = np.array([1e-20, 3.1e-2, 1e-14, 2.0 * np.pi, 1.0, np.pi, 2.0 * np.pi, 1.0])
+PERIODIC = np.array([0, 0, 0, 1, 0, 1, 1, 0], np.int32)      # phi0, psi, lambda
+
+
+def make_stretch_inputs(bt: BandTasks, config: int = 3, n_copies: int = 12, n_friends: int = 24, seed: int = 0x2405,
+                        sweep: int = 1, scale: float = 1.0) -> StretchInputs:
+    g = _rng(config, 300 * _S_BAND + bt.N)
+    base = np.repeat(bt.params, n_copies, axis=0)
+    z = g.standard_normal(base.shape) * scale
+    grp = base.copy()
+    grp[:, 0] = base[:, 0] * (1.0 + 0.02 * z[:, 0])
+    grp[:, 1] = base[:, 1] + 2e-9 * z[:, 1]
+    grp[:, 2] = base[:, 2] + 2e-17 * z[:, 2]
+    grp[:, 3] = np.mod(base[:, 3] + 0.05 * z[:, 3], 2.0 * np.pi)
+    grp[:, 4] = np.clip(base[:, 4] + 0.02 * z[:, 4], -1.0, 1.0)
+    grp[:, 5] = np.mod(base[:, 5] + 0.05 * z[:, 5], np.pi)
+    grp[:, 6] = np.mod(base[:, 6] + 0.02 * z[:, 6], 2.0 * np.pi)
+    grp[:, 7] = np.clip(base[:, 7] + 0.02 * z[:, 7], -1.0, 1.0)
+    grp = np.ascontiguousarray(grp[np.argsort(grp[:, 1], kind="stable")])
+    return StretchInputs(seed, sweep, grp, n_friends, 2.0, PRIOR_LO.copy(), PRIOR_HI.copy(), PERIODIC.copy())
+
+
+# ---------------------------------------------------------------------------------------------------------
 # Temperature-swap tasks for the Algorithm-2 primitive: one task per
 # odd sub-band; a ladder of n_t chains on distinct walkers (a random permutation), inverse
 # temperatures 1.2^-t, each chain holding its own jittered copy of the band's "true" sources (hotter chains

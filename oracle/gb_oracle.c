@@ -22,7 +22,10 @@
  *
  * Pins (tests/test_oracle_pins.py, all -m "not gpu"): frozen-geometry time-domain TDI + DFT (P1),
  * decimation identity (P1'), full-rate dt*rfft (P2), moving geometry (P3), Parseval (P4),
- * monochromatic closed form (P5), delta-lnL invariants (P6), tiny-T brute force (P8).
+ * monochromatic closed form (P5), delta-lnL invariants (P6), tiny-T brute force (P8); per-channel noise rows
+ * (S_E = 4 S_A against the numpy sums); Philox4x32-10 known-answer vectors, the stretch density's closed-form CDF,
+ * friends against a numpy argsort, and the z^(D-1) factor by sampling an 8-dimensional Gaussian with the generated
+ * proposals (the proposal step of Algorithm 1).
  * "parity unpinned": physical fidelity to the LDC Sangria generator / GBGPU (neither is in this
  * container); the oracle, not those codes, defines the result.
  */
@@ -456,9 +459,113 @@ typedef struct {
     double beta;
 } gbo_band_task;
 
-int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks, int64_t n_tasks, int N,
-                   double *params, const int32_t *prop_k, const double *prop_params, const double *prop_logq,
-                   const double *prop_logu, uint8_t *accepted_out, double *dlnL_out) {
+/* ---- proposal generation inside Algorithm 1 ("k <- randint(0, g_j)", "theta'_k <- Make Proposal
+ * on theta"; group stretch of App. B; stretch move Eq. 14) --------------------
+ * The random numbers come from the counter-based generator Philox4x32-10 (Salmon et al. 2011), written out below and
+ * pinned to its published known-answer vectors.  Key = the 64-bit seed; counter = (global proposal row, 0, block, sweep):
+ * a proposal's numbers depend on nothing but (seed, sweep, its row in the proposal arrays), not on the order in which
+ * tasks are processed.  Block 0 gives k, the friend and z; block 1 gives the uniform of the accept / reject step.
+ * Readings (paper-silent points; F1-h..F1-m):
+ *   randint          k = floor(r g_j / 2^32) for a 32-bit word r
+ *   uniforms         u = (a + 1/2) 2^-52, a = the top 26 bits of two words: 0 < u < 1
+ *   stationary group rows of 8 parameters sorted by f0 ascending ("sorting this large set of templates by
+ *                    frequency"); the n_friends rows closest in f0 to the CURRENT theta_k are a run of consecutive rows
+ *                    (equal distances: the run with the lower rows); the auxiliary point is friend
+ *                    floor(r n_friends / 2^32) of that run (":576 draws uniformly")
+ *   stretch density  g(z) ~ 1/sqrt(z) on [1/a, a] (ref. [59] of the paper), z = ((a - 1) u + 1)^2 / a
+ *   move             theta' = theta_aux + z (theta_k - theta_aux) on all D = 8 coordinates of the parameter row (Eq. 14),
+ *                    proposal-density factor z^(D-1): logq = 7 ln z
+ *   periodic         coordinates flagged periodic are wrapped into [lo, hi): x - (hi - lo) floor((x - lo) / (hi - lo))
+ *   prior            uniform on the box [lo, hi] per coordinate (Eq. 13's prior ratio is 1 inside, 0 outside): a proposal
+ *                    outside the box is rejected without a likelihood evaluation (delta lnL reported as NaN)          */
+typedef struct {
+    uint64_t seed;
+    uint32_t sweep;
+    int32_t n_friends;
+    const double *group;      /* [n_group][8], sorted by f0 (column 1) ascending */
+    int64_t n_group;
+    double stretch_a;
+    double lo[8], hi[8];
+    int32_t periodic[8];
+} gbo_stretch;
+
+void gbo_philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4]) {
+    uint32_t c[4] = {ctr_in[0], ctr_in[1], ctr_in[2], ctr_in[3]};
+    uint32_t k[2] = {key_in[0], key_in[1]};
+    for (int round = 0; round < 10; round++) {
+        if (round > 0) { k[0] += 0x9E3779B9u; k[1] += 0xBB67AE85u; }      /* Weyl sequence of the key */
+        uint64_t p0 = (uint64_t)0xD2511F53u * c[0];
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c[2];
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c[1] ^ k[0], n1 = lo1, n2 = hi0 ^ c[3] ^ k[1], n3 = lo0;
+        c[0] = n0; c[1] = n1; c[2] = n2; c[3] = n3;
+    }
+    for (int i = 0; i < 4; i++) out[i] = c[i];
+}
+
+static void proposal_words(const gbo_stretch *g, int64_t row, uint32_t block, uint32_t out[4]) {
+    uint32_t ctr[4] = {(uint32_t)row, 0u, block, g->sweep};
+    uint32_t key[2] = {(uint32_t)(g->seed & 0xffffffffu), (uint32_t)(g->seed >> 32)};
+    gbo_philox4x32_10(ctr, key, out);
+}
+
+double gbo_uniform52(uint32_t w0, uint32_t w1) {                /* 0 < u < 1, 52 random bits */
+    double a = (double)(w0 >> 6) * 67108864.0 + (double)(w1 >> 6);
+    return (a + 0.5) * (1.0 / 4503599627370496.0);
+}
+
+int32_t gbo_randint(uint32_t w, int32_t n) { return (int32_t)(((uint64_t)w * (uint64_t)n) >> 32); }
+
+double gbo_stretch_z(double u, double a) {                       /* inverse CDF of g(z) ~ z^(-1/2) on [1/a, a] */
+    double t = (a - 1.0) * u + 1.0;
+    return t * t / a;
+}
+
+/* row of the j-th of the n_friends group points closest in f0 to f.  The table is sorted by f0, so the
+ * closest n_friends rows are a run of consecutive rows [s, s + n_friends): the first s at which trading row s for row
+ * s + n_friends would not bring the run closer to f, found by trying every s in turn; the j-th friend is row s + j.
+ * (Equal distances: the run with the lower rows.)                                                                       */
+int64_t gbo_friend_row(const double *group, int64_t n_group, int32_t n_friends, double f, int32_t j) {
+    int64_t nf = n_friends < n_group ? n_friends : n_group;
+    int64_t s = 0;
+    while (s < n_group - nf && f - group[8 * s + P_F0] > group[8 * (s + nf) + P_F0] - f) s++;
+    return s + j;
+}
+
+/* "theta'_k <- Make Proposal on theta" for global proposal row `row` of a band with g_j current sources
+ * theta[g_j][8].  Returns 1 if theta' lies inside the prior box, else 0.                                            */
+int gbo_make_proposal(const gbo_stretch *g, int64_t row, const double *theta, int32_t g_j, int32_t *k_out,
+                      double *theta_prop, double *logq, double *logu) {
+    uint32_t w0[4], w1[4];
+    proposal_words(g, row, 0u, w0);
+    proposal_words(g, row, 1u, w1);
+    int32_t k = gbo_randint(w0[0], g_j);                           /* k <- randint(0, g_j) */
+    const double *theta_k = theta + 8 * (size_t)k;
+    int64_t nf = g->n_friends < g->n_group ? g->n_friends : g->n_group;
+    int32_t j = gbo_randint(w0[1], (int32_t)nf);
+    const double *aux = g->group + 8 * gbo_friend_row(g->group, g->n_group, g->n_friends, theta_k[P_F0], j);
+    double z = gbo_stretch_z(gbo_uniform52(w0[2], w0[3]), g->stretch_a);
+    int inside = 1;
+    for (int cdx = 0; cdx < 8; cdx++) {
+        double x = aux[cdx] + z * (theta_k[cdx] - aux[cdx]);      /* Eq. 14 */
+        if (g->periodic[cdx]) {
+            double period = g->hi[cdx] - g->lo[cdx];
+            x = x - period * floor((x - g->lo[cdx]) / period);
+        }
+        if (!(x >= g->lo[cdx] && x <= g->hi[cdx])) inside = 0;
+        theta_prop[cdx] = x;
+    }
+    *k_out = k;
+    *logq = 7.0 * log(z);                                          /* z^(D-1), D = 8 */
+    *logu = log(gbo_uniform52(w1[0], w1[1]));
+    return inside;
+}
+
+static int band_sweep_impl(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks, int64_t n_tasks, int N,
+                           double *params, const int32_t *prop_k, const double *prop_params, const double *prop_logq,
+                           const double *prop_logu, uint8_t *accepted_out, double *dlnL_out,
+                           const gbo_stretch *gen, int32_t *k_gen, double *params_gen, double *logq_gen, double *logu_gen) {
     if (!valid_N(N)) return GBO_ERR_INVALID;
     double *h = (double *)malloc(sizeof(double) * 8 * (size_t)N);
     double *oA = h, *oE = h + 2 * (size_t)N, *aA = h + 4 * (size_t)N, *aE = h + 6 * (size_t)N;
@@ -494,13 +601,29 @@ int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks,
         memcpy(r0, rv, sizeof(double) * 4 * (size_t)n);
         for (int p = 0; p < t->n_prop && n > 0; p++) {
             int64_t ip = t->prop_begin + p;
-            int k = prop_k[ip];
+            int k;
+            const double *theta_p;
+            double lq, lu;
+            if (gen) {                             /* k <- randint(0, g_j); theta'_k <- Make Proposal */
+                if (t->n_src <= 0) { free(rv); free(r0); free(sv); free(h); return GBO_ERR_INVALID; }
+                int32_t kk;
+                int inside = gbo_make_proposal(gen, ip, params + 8 * (size_t)t->src_begin, t->n_src, &kk,
+                                               params_gen + 8 * ip, &logq_gen[ip], &logu_gen[ip]);
+                k_gen[ip] = kk;
+                if (!inside) {                     /* zero prior: rejected, no likelihood evaluation */
+                    dlnL_out[ip] = NAN;
+                    accepted_out[ip] = 0;
+                    continue;
+                }
+                k = kk; theta_p = params_gen + 8 * ip; lq = logq_gen[ip]; lu = logu_gen[ip];
+            } else {
+                k = prop_k[ip]; theta_p = prop_params + 8 * ip; lq = prop_logq[ip]; lu = prop_logu[ip];
+            }
             if (k < 0 || k >= t->n_src) { free(rv); free(r0); free(sv); free(h); return GBO_ERR_INVALID; }
             double *theta_k = params + 8 * ((size_t)t->src_begin + k);
-            const double *theta_p = prop_params + 8 * ip;
             double dl = 0.0;
             o8_row(c, &v, theta_p, theta_k, 0, GBO_SWAP, N, &dl, NULL);            /* Eq. 5 against r' */
-            int acc = t->beta * dl + prop_logq[ip] >= prop_logu[ip];
+            int acc = t->beta * dl + lq >= lu;
             dlnL_out[ip] = dl;
             accepted_out[ip] = (uint8_t)acc;
             if (acc) {
@@ -514,6 +637,7 @@ int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks,
         }
         for (int p = 0; p < t->n_prop && n <= 0; p++) {   /* nothing staged: every dlnL is 0 */
             int64_t ip = t->prop_begin + p;
+            if (gen) { free(rv); free(r0); free(sv); free(h); return GBO_ERR_INVALID; }   /* generating needs staged bins */
             int acc = prop_logq[ip] >= prop_logu[ip];
             dlnL_out[ip] = 0.0;
             accepted_out[ip] = (uint8_t)acc;
@@ -531,6 +655,24 @@ int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks,
     }
     free(h);
     return GBO_OK;
+}
+
+/* Algorithm 1 with k, theta', logq and logu given by the caller (reading F1-b) */
+int gbo_band_sweep(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks, int64_t n_tasks, int N,
+                   double *params, const int32_t *prop_k, const double *prop_params, const double *prop_logq,
+                   const double *prop_logu, uint8_t *accepted_out, double *dlnL_out) {
+    return band_sweep_impl(c, d, tasks, n_tasks, N, params, prop_k, prop_params, prop_logq, prop_logu, accepted_out,
+                           dlnL_out, NULL, NULL, NULL, NULL, NULL);
+}
+
+/* Algorithm 1 as printed: the proposal step runs inside the loop, from the CURRENT theta_k.
+ * k_out, params_out [.][8], logq_out, logu_out receive what was generated for every proposal row.            */
+int gbo_band_sweep_generate(const gbo_config *c, gbo_data *d, const gbo_band_task *tasks, int64_t n_tasks, int N,
+                            double *params, const gbo_stretch *gen, int32_t *k_out, double *params_out,
+                            double *logq_out, double *logu_out, uint8_t *accepted_out, double *dlnL_out) {
+    if (!gen || !gen->group || gen->n_group < 1 || gen->n_friends < 1 || !(gen->stretch_a > 1.0)) return GBO_ERR_INVALID;
+    return band_sweep_impl(c, d, tasks, n_tasks, N, params, NULL, NULL, NULL, NULL, accepted_out, dlnL_out,
+                           gen, k_out, params_out, logq_out, logu_out);
 }
 
 /* ---- Algorithm 2 (Eq. D2): temperature swaps of one sub-band ------------

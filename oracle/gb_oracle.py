@@ -201,11 +201,7 @@ _BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", 
                        ("flags", np.int32), ("write_walker", np.int32), ("beta", np.float64)], align=True)
 
 
-def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, prop_params, prop_logq, prop_logu):
-    """Algorithm 1 (PAPER.md:582-614), task after task, proposal after proposal.  `tasks` is a dict of equal-length
-    arrays (walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta; optional subtract_current
-    and write_walker for the odd/even buffers of PAPER.md:354-362).  `params` [n_src_total, 8]
-    and data.resid are updated in place.  Returns (accepted[n_prop_total] uint8, dlnL[n_prop_total])."""
+def _pack_band_tasks(tasks: dict) -> np.ndarray:
     n = len(tasks["walker"])
     t = np.zeros(n, _BAND_TASK)
     for key in ("walker", "n_src", "src_begin", "n_prop", "prop_begin", "n_stage", "k_first", "beta"):
@@ -217,6 +213,16 @@ def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, pro
         flags |= 4
         t["write_walker"] = tasks["write_walker"]
     t["flags"] = flags
+    return t
+
+
+def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, prop_params, prop_logq, prop_logu):
+    """Algorithm 1 (PAPER.md:582-614), task after task, proposal after proposal.  `tasks` is a dict of equal-length
+    arrays (walker, n_src, src_begin, n_prop, prop_begin, n_stage, k_first, write_back, beta; optional subtract_current
+    and write_walker for the odd/even buffers of PAPER.md:354-362).  `params` [n_src_total, 8]
+    and data.resid are updated in place.  Returns (accepted[n_prop_total] uint8, dlnL[n_prop_total])."""
+    t = _pack_band_tasks(tasks)
+    n = len(t)
     assert params.dtype == np.float64 and params.flags.c_contiguous
     pk = np.ascontiguousarray(prop_k, dtype=np.int32)
     pp, lq, lu = _f64(prop_params), _f64(prop_logq), _f64(prop_logu)
@@ -228,6 +234,89 @@ def band_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, prop_k, pro
     if rc != 0:
         raise ValueError(f"gbo_band_sweep rc={rc}")
     return acc, dl
+
+
+class _Stretch(C.Structure):
+    _fields_ = [("seed", C.c_uint64), ("sweep", C.c_uint32), ("n_friends", C.c_int32), ("group", C.c_void_p),
+                ("n_group", C.c_int64), ("stretch_a", C.c_double), ("lo", C.c_double * 8), ("hi", C.c_double * 8),
+                ("periodic", C.c_int32 * 8)]
+
+
+class Stretch:
+    """Inputs of the in-loop proposal step of Algorithm 1 (gbo_stretch): Philox seed / sweep, the stationary group
+    [n_group, 8] sorted by f0, n_friends, the stretch scale a, the prior box and the periodic flags."""
+
+    def __init__(self, seed, sweep, group, n_friends, lo, hi, periodic, stretch_a=2.0):
+        self.group = np.ascontiguousarray(group, dtype=np.float64)
+        assert self.group.ndim == 2 and self.group.shape[1] == 8
+        assert np.all(np.diff(self.group[:, 1]) >= 0), "the stationary group must be sorted by f0"
+        self.seed, self.sweep, self.n_friends, self.stretch_a = int(seed), int(sweep), int(n_friends), float(stretch_a)
+        self.lo, self.hi = np.asarray(lo, np.float64), np.asarray(hi, np.float64)
+        self.periodic = np.asarray(periodic, np.int32)
+
+    def c(self) -> _Stretch:
+        return _Stretch(self.seed, self.sweep, self.n_friends, _ptr(self.group), self.group.shape[0], self.stretch_a,
+                        (C.c_double * 8)(*self.lo), (C.c_double * 8)(*self.hi), (C.c_int32 * 8)(*self.periodic))
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) for x in key])
+    out = (C.c_uint32 * 4)()
+    lib().gbo_philox4x32_10(c, k, out)
+    return [int(x) for x in out]
+
+
+def uniform52(w0: int, w1: int) -> float:
+    f = lib().gbo_uniform52
+    f.restype = C.c_double
+    return float(f(C.c_uint32(w0), C.c_uint32(w1)))
+
+
+def randint(w: int, n: int) -> int:
+    return int(lib().gbo_randint(C.c_uint32(w), C.c_int32(n)))
+
+
+def stretch_z(u: float, a: float = 2.0) -> float:
+    f = lib().gbo_stretch_z
+    f.restype = C.c_double
+    return float(f(C.c_double(u), C.c_double(a)))
+
+
+def friend_row(group, n_friends: int, f: float, j: int) -> int:
+    g = np.ascontiguousarray(group, dtype=np.float64)
+    fn = lib().gbo_friend_row
+    fn.restype = C.c_int64
+    return int(fn(_ptr(g), C.c_int64(g.shape[0]), C.c_int32(n_friends), C.c_double(f), C.c_int32(j)))
+
+
+def make_proposal(st: Stretch, row: int, theta):
+    """One proposal for global proposal row `row` of a band whose current sources are theta [g_j, 8].
+    Returns (inside_prior, k, theta' [8], logq, logu)."""
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    k = C.c_int32(0)
+    out = np.empty(8)
+    lq, lu = C.c_double(0.0), C.c_double(0.0)
+    sc = st.c()
+    inside = lib().gbo_make_proposal(C.byref(sc), C.c_int64(row), _ptr(th), C.c_int32(th.shape[0]), C.byref(k), _ptr(out),
+                                     C.byref(lq), C.byref(lu))
+    return bool(inside), int(k.value), out, float(lq.value), float(lu.value)
+
+
+def band_sweep_generate(cfg: Config, data: Data, tasks: dict, N: int, params, st: Stretch):
+    """Algorithm 1 with the proposal step inside the loop (gbo_band_sweep_generate).  `params` and data.resid are updated
+    in place.  Returns (accepted uint8, dlnL, k int32, theta' [P, 8], logq, logu) over all proposal rows."""
+    t = _pack_band_tasks(tasks)
+    assert params.dtype == np.float64 and params.flags.c_contiguous
+    P = int((t["prop_begin"] + t["n_prop"]).max()) if len(t) else 0
+    acc, dl = np.zeros(P, np.uint8), np.zeros(P)
+    k, pp, lq, lu = np.zeros(P, np.int32), np.zeros((P, 8)), np.zeros(P), np.zeros(P)
+    cc, dd, sc = cfg.c(), data.c(), st.c()
+    rc = lib().gbo_band_sweep_generate(C.byref(cc), C.byref(dd), _ptr(t), C.c_int64(len(t)), C.c_int(N), _ptr(params),
+                                       C.byref(sc), _ptr(k), _ptr(pp), _ptr(lq), _ptr(lu), _ptr(acc), _ptr(dl))
+    if rc != 0:
+        raise ValueError(f"gbo_band_sweep_generate rc={rc}")
+    return acc, dl, k, pp, lq, lu
 
 
 _TEMPER_TASK = np.dtype([("n_t", np.int32), ("chain_begin", np.int32), ("n_stage", np.int32), ("write_back", np.int32),

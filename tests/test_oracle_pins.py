@@ -767,3 +767,196 @@ def test_oddeven_buffers_equal_the_explicit_residual_and_keep_the_odd_buffer_con
                                        move_all=oracle.REMOVE, N=N)
         assert np.abs(chk.resid[1::2] - d).max() <= 1e-12 * np.abs(buf - d[np.repeat(np.arange(len(d)), 2)]).max() \
             + 4e-16 * np.abs(d).max()
+
+
+# ------------------------------------- the proposal step inside Algorithm 1 (Eq. 14)
+def test_philox4x32_10_known_answer_vectors(oracle):
+    """The counter-based generator is fixed by its published known-answer vectors (tests/golden/philox4x32_10_kat.txt)."""
+    import os
+    rows = [ln.split() for ln in open(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt"))
+            if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        w = [int(x, 16) for x in r]
+        assert oracle.philox4x32_10(w[0:4], w[4:6]) == w[6:10]
+    # a counter-based generator: distinct counters give unrelated words, the same counter the same words
+    a = oracle.philox4x32_10([5, 0, 0, 1], [7, 9])
+    assert a == oracle.philox4x32_10([5, 0, 0, 1], [7, 9]) and a != oracle.philox4x32_10([6, 0, 0, 1], [7, 9])
+
+
+def test_uniform_randint_and_stretch_density_closed_forms(oracle):
+    # 52-bit uniforms strictly inside (0, 1), on the grid (a + 1/2) 2^-52
+    assert oracle.uniform52(0, 0) == 2.0 ** -53 and oracle.uniform52(0xffffffff, 0xffffffff) == 1.0 - 2.0 ** -53
+    assert oracle.uniform52(1 << 6, 0) == (2.0 ** 26 + 0.5) * 2.0 ** -52 and oracle.uniform52(0, 1 << 6) == 1.5 * 2.0 ** -52
+    # randint: floor(w n / 2^32), every value of [0, n) and nothing else
+    assert oracle.randint(0, 9) == 0 and oracle.randint(0xffffffff, 9) == 8
+    for n in (1, 2, 9, 30):
+        for v in range(n):
+            lo = -(-(v << 32) // n)                              # smallest word that maps to v
+            assert oracle.randint(lo, n) == v and (lo == 0 or oracle.randint(lo - 1, n) == v - 1)
+    # stretch density g(z) ~ z^(-1/2) on [1/a, a]: closed-form CDF F(z) = (sqrt z - 1/sqrt a) / (sqrt a - 1/sqrt a)
+    for a in (2.0, 3.5):
+        u = (np.arange(2000) + 0.5) / 2000
+        z = np.array([oracle.stretch_z(x, a) for x in u])
+        F = (np.sqrt(z) - 1 / np.sqrt(a)) / (np.sqrt(a) - 1 / np.sqrt(a))
+        assert np.abs(F - u).max() < 1e-14 and z.min() > 1 / a and z.max() < a
+        assert abs(oracle.stretch_z(0.0, a) - 1 / a) < 1e-16 and abs(oracle.stretch_z(1.0, a) - a) < 1e-15
+    # the symmetry the move's detailed balance rests on: g(1/z) = z g(z)  <=>  F(z) + F(1/z) ... check with the density
+    g = lambda zz, a=2.0: 1.0 / np.sqrt(zz) / (2 * (np.sqrt(a) - 1 / np.sqrt(a)))
+    zz = np.linspace(0.5, 2.0, 50)
+    assert np.abs(g(1 / zz) - zz * g(zz)).max() < 1e-15
+    # Philox-driven draws follow that CDF (Kolmogorov distance of 20 000 draws)
+    zs = np.sort([oracle.stretch_z(oracle.uniform52(*oracle.philox4x32_10([i, 0, 0, 3], [11, 12])[2:4]), 2.0)
+                  for i in range(20000)])
+    F = (np.sqrt(zs) - 1 / np.sqrt(2.0)) / (np.sqrt(2.0) - 1 / np.sqrt(2.0))
+    assert np.abs(F - (np.arange(20000) + 0.5) / 20000).max() < 1.63 / np.sqrt(20000)      # 1 % level of the KS statistic
+
+
+def test_friends_are_the_closest_in_f0_against_numpy_argsort(oracle):
+    """The n_friends rows closest in f0 against numpy: the same rows as an argsort of the distances
+    when no two distances are equal; with repeated f0 values and exact ties the same multiset of distances, a run of
+    consecutive rows, and the lower rows of two equally good runs."""
+    rng = np.random.default_rng(3)
+    grp = rng.random((57, 8))
+    grp[:, 1] = np.sort(rng.random(57))
+    for nf in (1, 5, 24, 57, 80):
+        for f in (-1.0, 0.0, 0.305, 0.5, grp[20, 1], 0.995, 2.0):
+            want = np.sort(np.argsort(np.abs(grp[:, 1] - f), kind="stable")[:min(nf, 57)])
+            got = [oracle.friend_row(grp, nf, f, j) for j in range(len(want))]
+            assert got == list(want), (nf, f)
+    tie = grp.copy()
+    tie[:, 1] = np.sort(np.round(rng.random(57) * 50) / 64)       # multiples of 1/64: repeated values, exact ties
+    for nf in (1, 2, 5, 24):
+        for f in (0.0, 20 / 64, 20.5 / 64, tie[20, 1], 0.7, 2.0):
+            got = np.array([oracle.friend_row(tie, nf, f, j) for j in range(nf)])
+            assert np.array_equal(got, got[0] + np.arange(nf)) and got[0] >= 0 and got[-1] < 57
+            dist = np.sort(np.abs(tie[:, 1] - f))
+            assert np.array_equal(np.sort(np.abs(tie[got, 1] - f)), dist[:nf])
+            if got[0] > 0:                                        # the run one row lower is strictly worse
+                assert np.abs(tie[got[0] - 1, 1] - f) > np.abs(tie[got[-1], 1] - f)
+
+
+def _toy_stretch(oracle, n_group=64, seed=99):
+    """An 8-dimensional Gaussian target of very different scales per coordinate, a stationary group drawn from it."""
+    rng = np.random.default_rng(seed)
+    mu = np.array([1e-22, 3e-3, 0.0, 3.0, 0.1, 1.5, 3.0, -0.2])
+    sig = np.array([1e-23, 1e-9, 1e-17, 0.1, 0.05, 0.1, 0.05, 0.05])
+    grp = mu + sig * rng.standard_normal((n_group, 8))
+    grp = grp[np.argsort(grp[:, 1], kind="stable")]
+    from gb_inputs.configs import PRIOR_LO, PRIOR_HI, PERIODIC
+    return mu, sig, oracle.Stretch(1234, 7, grp, n_group, PRIOR_LO, PRIOR_HI, PERIODIC)
+
+
+def test_make_proposal_is_eq14_on_the_drawn_friend(oracle):
+    """theta' = theta_aux + z (theta_k - theta_aux) (Eq. 14) rebuilt in numpy from the Philox words."""
+    mu, sig, st = _toy_stretch(oracle)
+    rng = np.random.default_rng(5)
+    theta = mu + sig * rng.standard_normal((9, 8))
+    ks = set()
+    for row in range(200):
+        inside, k, tp, lq, lu = oracle.make_proposal(st, row, theta)
+        w0 = oracle.philox4x32_10([row, 0, 0, st.sweep], [st.seed & 0xffffffff, st.seed >> 32])
+        w1 = oracle.philox4x32_10([row, 0, 1, st.sweep], [st.seed & 0xffffffff, st.seed >> 32])
+        assert k == (w0[0] * 9) >> 32
+        ks.add(k)
+        j = (w0[1] * st.n_friends) >> 32
+        aux = st.group[np.sort(np.argsort(np.abs(st.group[:, 1] - theta[k, 1]), kind="stable")[:st.n_friends])[j]]   # no ties here
+        u = ((w0[2] >> 6) * 2.0 ** 26 + (w0[3] >> 6) + 0.5) * 2.0 ** -52
+        z = (u + 1.0) ** 2 / 2.0
+        want = aux + z * (theta[k] - aux)
+        for c, per in ((3, 2 * np.pi), (5, np.pi), (6, 2 * np.pi)):
+            want[c] = want[c] - per * np.floor(want[c] / per)
+        assert np.array_equal(tp, want)
+        assert abs(lq - 7.0 * np.log(z)) <= 4e-16 * abs(lq) + 1e-300 and inside      # libm against numpy's log
+        uu = ((w1[0] >> 6) * 2.0 ** 26 + (w1[1] >> 6) + 0.5) * 2.0 ** -52
+        assert abs(lu - np.log(uu)) <= 1e-15 * abs(np.log(uu))
+    assert ks == set(range(9))
+    # outside the prior box (cos iota > 1 after the stretch): flagged, not wrapped
+    far = theta.copy()
+    far[:, 4] = 0.999
+    st2 = oracle.Stretch(st.seed, st.sweep, np.where(np.arange(8) == 4, -0.9, st.group), st.n_friends, st.lo, st.hi, st.periodic)
+    flags = [oracle.make_proposal(st2, row, far)[0] for row in range(200)]
+    assert 0 < sum(flags) < 200
+
+
+def test_stretch_proposals_with_the_z_power_sample_the_target(oracle):
+    """Detailed balance of the move: with acceptance min(1, z^(D-1) pi(theta') / pi(theta)), D = 8, a chain driven by
+    gbo_make_proposal samples the Gaussian target (mean and variance of every coordinate); with the exponent D instead
+    of D - 1 it does not (the pin has power)."""
+    mu, sig, st = _toy_stretch(oracle)
+    logpi = lambda x: -0.5 * float((((x - mu) / sig) ** 2).sum())
+
+    def chain(factor, n=30000):
+        x = mu.copy()[None, :]
+        out = np.empty((n, 8))
+        lp = logpi(x[0])
+        for i in range(n):
+            inside, k, tp, lq, lu = oracle.make_proposal(st, i, x)
+            lpn = logpi(tp)
+            if inside and (lpn - lp) + factor * lq >= lu:
+                x, lp = tp[None, :].copy(), lpn
+            out[i] = x[0]
+        return out[2000:]
+
+    good = chain(1.0)
+    m, v = good.mean(axis=0), good.var(axis=0)
+    assert np.abs((m - mu) / sig).max() < 0.15, (m - mu) / sig
+    assert np.abs(v / sig ** 2 - 1.0).max() < 0.2, v / sig ** 2
+    # measured: the mean over the coordinates of var / sigma^2 is 0.997 +- 0.003 for the exponent D - 1 = 7,
+    # 1.11 for D, 0.87 for D - 2, 0.32 without the factor
+    assert abs((v / sig ** 2).mean() - 1.0) < 0.05
+    assert (chain(8.0 / 7.0).var(axis=0) / sig ** 2).mean() > 1.07
+    assert (chain(0.0).var(axis=0) / sig ** 2).mean() < 0.5
+
+
+def _gen_case(oracle, N=128, n_bands=3, n_src=4, n_prop=14, f_lo=6e-4):
+    from gb_inputs import make_workload, make_band_tasks, make_stretch_inputs
+    wl = make_workload(3, B=1, n_walkers=2)
+    bt = make_band_tasks(wl, N, f_lo, n_bands, n_src, n_prop)
+    si = make_stretch_inputs(bt, n_copies=6, n_friends=8)
+    st = oracle.Stretch(si.seed, si.sweep, si.group, si.n_friends, si.lo, si.hi, si.periodic, si.stretch_a)
+    return wl, bt, st, wl.resid()
+
+
+def test_band_sweep_generate_proposes_from_the_current_state(oracle):
+    """Algorithm 1 as printed: the proposal of step p is made from the CURRENT theta_k.  (1) replaying the
+    loop in Python with gbo_make_proposal on the evolving parameter list gives the k, theta', logq, logu the sweep reports;
+    (2) feeding those to the inputs-only form gbo_band_sweep reproduces decisions, delta lnL, parameters and residuals;
+    (3) a source proposed again after an accepted proposal is moved from its NEW position."""
+    wl, bt, st, resid = _gen_case(oracle)
+    cfg = oracle.Config()
+    data = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params = bt.params.copy()
+    acc, dl, k, pp, lq, lu = oracle.band_sweep_generate(cfg, data, bt.tasks, bt.N, params, st)
+    assert 0 < acc.sum() < acc.size
+    t = bt.tasks
+    cur = bt.params.copy()
+    again = 0
+    for i in range(len(t["walker"])):
+        sl = slice(t["src_begin"][i], t["src_begin"][i] + t["n_src"][i])
+        moved = set()
+        for p in range(t["n_prop"][i]):
+            ip = t["prop_begin"][i] + p
+            inside, kk, tp, q, u = oracle.make_proposal(st, ip, cur[sl])
+            assert kk == k[ip] and np.array_equal(tp, pp[ip]) and q == lq[ip] and u == lu[ip]
+            assert inside or (np.isnan(dl[ip]) and not acc[ip])
+            if kk in moved:
+                again += 1
+            if acc[ip]:
+                cur[t["src_begin"][i] + kk] = tp
+                moved.add(kk)
+    assert again > 0 and np.array_equal(cur, params)
+    ok = np.isfinite(dl)
+    data2 = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    params2 = bt.params.copy()
+    acc2, dl2 = oracle.band_sweep(cfg, data2, bt.tasks, bt.N, params2, k, pp, lq, np.where(ok, lu, np.inf))
+    assert np.array_equal(acc, acc2) and np.array_equal(dl[ok], dl2[ok]) and np.array_equal(params, params2)
+    assert np.array_equal(data.resid, data2.resid)
+    # another sweep counter gives other proposals; a subset of the tasks gives the same proposals for those tasks
+    st_b = oracle.Stretch(st.seed, st.sweep + 1, st.group, st.n_friends, st.lo, st.hi, st.periodic, st.stretch_a)
+    kb = oracle.band_sweep_generate(cfg, oracle.Data(resid.copy(), wl.psd, wl.k_lo), bt.tasks, bt.N, bt.params.copy(), st_b)[2]
+    assert not np.array_equal(kb, k)
+    one = {key: v[1:2] for key, v in t.items()}
+    r1 = oracle.band_sweep_generate(cfg, oracle.Data(resid.copy(), wl.psd, wl.k_lo), one, bt.N, bt.params.copy(), st)
+    ps = slice(t["prop_begin"][1], t["prop_begin"][1] + t["n_prop"][1])
+    assert np.array_equal(r1[2][ps], k[ps]) and np.array_equal(r1[3][ps], pp[ps]) and np.array_equal(r1[0][ps], acc[ps])
