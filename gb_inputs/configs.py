@@ -250,15 +250,19 @@ class BandTasks:
 
 
 def make_band_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_src: int, n_prop: int,
-                    betas=(1.0, 0.6), stream: int = 0, amp_lo: float = 2e-23, amp_hi: float = 2e-22) -> BandTasks:
-    """n_bands odd sub-bands per walker of `wl`, starting near f_lo.  Deterministic in (wl.config, N, stream)."""
+                    betas=(1.0, 0.6), stream: int = 0, amp_lo: float = 2e-23, amp_hi: float = 2e-22,
+                    band_stride: int = 2) -> BandTasks:
+    """n_bands odd sub-bands per walker of `wl`, starting near f_lo.  Deterministic in (wl.config, N, stream).
+    band_stride = 2: every odd sub-band (the paper's schedule; bands b and b + 2 both stage sub-band b + 1);
+    band_stride = 4: every other odd sub-band, so the staged ranges of one walker's tasks are disjoint and the result of
+    a sweep does not depend on the order in which the tasks run even when proposals roam over the whole stage."""
     g = _rng(wl.config, 100 * _S_BAND + stream + N)
     T = wl.Tobs
     kb0 = int(np.ceil(f_lo * T / N)) * N                       # global bin of sub-band 0 (a multiple of N)
     nw = wl.n_walkers
     nt = nw * n_bands
     walker = np.repeat(np.arange(nw, dtype=np.int32), n_bands)
-    b = np.tile(2 * np.arange(n_bands, dtype=np.int64) + 1, nw)  # odd sub-bands
+    b = np.tile(band_stride * np.arange(n_bands, dtype=np.int64) + 1, nw)  # odd sub-bands
     tasks = {
         "walker": walker,
         "n_src": np.full(nt, n_src, np.int32),

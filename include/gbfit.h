@@ -260,6 +260,42 @@ int gb_band_sweep(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, i
                   const double *prop_logu, uint8_t *accepted_out, double *dlnL_out, void *stream);
 
 /*
+ * gb_band_sweep_generate -- Algorithm 1 exactly as printed: the proposal step runs INSIDE the sequential
+ * loop of each band, "k <- randint(0, g_j)", "theta'_k <- Make Proposal on theta", from the CURRENT
+ * theta_k -- a stretch proposal built by the caller beforehand would use a stale theta_k as soon as an earlier proposal of
+ * the same source was accepted.  The proposal is the group stretch of App. B with the stretch move of
+ * Eq. 14:
+ *   random numbers   Philox4x32-10, key = seed, counter = (proposal row, 0, block, sweep); block 0 -> k, friend, z;
+ *                    block 1 -> the uniform of the accept step.  Results do not depend on how tasks are scheduled.
+ *   k                floor(w0 g_j / 2^32);  uniforms u = (a + 1/2) 2^-52 from the top 26 bits of two words
+ *   friends          `group` is the stationary group sorted by f0 ascending; the n_friends rows closest in
+ *                    f0 to the current theta_k are a run of consecutive rows (ties: the lower rows); the auxiliary point is
+ *                    row floor(w1 n_friends / 2^32) of that run
+ *   z                g(z) ~ 1/sqrt(z) on [1/a, a]:  z = ((a - 1) u + 1)^2 / a
+ *   theta'           theta_aux + z (theta_k - theta_aux) on all 8 coordinates; logq = 7 ln z (the z^(D-1) factor)
+ *   periodic / prior coordinates flagged periodic are wrapped into [lo, hi); a proposal outside the box [lo, hi], or one
+ *                    whose window [kmin', kmin' + N) leaves the task's staged bins ("we allow samples to go halfway into
+ *                    neighboring bands"), has zero prior: rejected without a likelihood evaluation, dlnL = NaN
+ *   accept           beta * dlnL + logq >= logu with logu = ln(uniform of block 1), as gb_band_sweep
+ * Everything else (staging, Eq. 5, updates, write-back, task flags, errors) is gb_band_sweep.  A task needs n_src >= 1
+ * and n_stage >= 1.  Outputs per proposal row, all DEVICE: k_out int32, params_out [.][8], logq_out, logu_out (what was
+ * generated), accepted_out, dlnL_out.  k and theta' are reproducible bit for bit from the definition above.
+ */
+typedef struct {             /* HOST POD */
+    uint64_t seed;           /* Philox key                                                         */
+    uint32_t sweep;          /* counter word 3: a new value for every call of a run                 */
+    int32_t n_friends;       /* size of the friends run (clamped to n_group)                        */
+    const double *group;     /* DEVICE [n_group][8] parameter rows sorted by f0 (column 1) ascending */
+    int64_t n_group;
+    double stretch_a;        /* a > 1 (2 in ref. [59] of the paper)                                 */
+    double lo[8], hi[8];     /* prior box per coordinate                                            */
+    int32_t periodic[8];     /* != 0: coordinate wrapped into [lo, hi)                              */
+} gb_stretch;
+int gb_band_sweep_generate(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, int64_t n_tasks, int N,
+                           int max_stage, double *params, const gb_stretch *gen, int32_t *k_out, double *params_out,
+                           double *logq_out, double *logu_out, uint8_t *accepted_out, double *dlnL_out, void *stream);
+
+/*
  * gb_temper_sweep -- Algorithm 2 of the paper ("Galaxy Tempering algorithm") with the swap acceptance
  * of Eq. D2 for walkers that carry different residuals / PSDs.  One task = one sub-band with a ladder of
  * n_t chains (n_t <= GB_TEMPER_MAX_LADDER); chain entry c = chain_begin + t has

@@ -477,7 +477,8 @@ typedef struct {
  *                    proposal-density factor z^(D-1): logq = 7 ln z
  *   periodic         coordinates flagged periodic are wrapped into [lo, hi): x - (hi - lo) floor((x - lo) / (hi - lo))
  *   prior            uniform on the box [lo, hi] per coordinate (Eq. 13's prior ratio is 1 inside, 0 outside): a proposal
- *                    outside the box is rejected without a likelihood evaluation (delta lnL reported as NaN)          */
+ *                    outside the box is rejected without a likelihood evaluation (delta lnL reported as NaN); the same for a
+ *                    proposal whose window leaves the staged bins (applied in the sweep loop below)       */
 typedef struct {
     uint64_t seed;
     uint32_t sweep;
@@ -610,6 +611,14 @@ static int band_sweep_impl(const gbo_config *c, gbo_data *d, const gbo_band_task
                 int inside = gbo_make_proposal(gen, ip, params + 8 * (size_t)t->src_begin, t->n_src, &kk,
                                                params_gen + 8 * ip, &logq_gen[ip], &logu_gen[ip]);
                 k_gen[ip] = kk;
+                /* "We allow samples to go halfway into neighboring bands": with a window as wide as a
+                 * sub-band that is exactly the condition that the window of theta' stays on the staged sub-bands b-1, b, b+1;
+                 * beyond that the prior is zero (reading F1-n)                                                */
+                {
+                    double prod = params_gen[8 * ip + P_F0] * c->Tobs;
+                    int64_t kmin_p = (int64_t)floor(prod + 0.5) - N / 2;
+                    if (kmin_p < t->k_first || kmin_p + N > t->k_first + t->n_stage) inside = 0;
+                }
                 if (!inside) {                     /* zero prior: rejected, no likelihood evaluation */
                     dlnL_out[ip] = NAN;
                     accepted_out[ip] = 0;

@@ -34,7 +34,61 @@ struct BandArgs {
     int64_t kmax;
     int32_t* errflag;
     cx* cache;               // [gridDim.x][kBandCacheSlots][2][N] windows of the current sources of each CTA's task
+    // gb_band_sweep_generate: the proposal step runs inside the loop (gen != 0); prop_k / prop_params / prop_logq /
+    // prop_logu are then OUTPUTS (what was generated for every proposal row)
+    int32_t gen;
+    gb_stretch st;           // seed, sweep, friends table (DEVICE), stretch scale, prior box, periodic flags
+    int32_t* gen_k;
+    double* gen_params;
+    double* gen_logq;
+    double* gen_logu;
 };
+
+// ---- the proposal step of Algorithm 1 (group stretch App. B :566-576; Eq. 14 :206-212) ----------
+// Philox4x32-10 (Salmon et al. 2011): ten rounds of two 32x32 -> 64 multiplies and a key schedule by Weyl constants.
+// Key = the 64-bit seed, counter = (proposal row, 0, block, sweep): the numbers of a proposal depend only on its row.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t* out) {
+#pragma unroll
+    for (int r = 0; r < 10; r++) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0;
+        c1 = l1;
+        c2 = h0 ^ c3 ^ k1;
+        c3 = l0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0;  out[1] = c1;  out[2] = c2;  out[3] = c3;
+}
+// 52 random bits -> 0 < u < 1 (every step exact in FP64)
+__device__ __forceinline__ double uniform52(uint32_t w0, uint32_t w1) {
+    const double a = __dadd_rn(__dmul_rn((double)(w0 >> 6), 67108864.0), (double)(w1 >> 6));
+    return __dmul_rn(__dadd_rn(a, 0.5), 1.0 / 4503599627370496.0);
+}
+__device__ __forceinline__ int32_t randint32(uint32_t w, int32_t n) { return (int32_t)__umulhi(w, (uint32_t)n); }
+
+// First row s of the run of nf consecutive rows of the f0-sorted friends table that lie closest to f: the first s in
+// [0, n_group - nf] at which trading row s for row s + nf would not bring the run closer,
+//     P(s) = (f - g[s] > g[s + nf] - f)   is true below the answer and false from it on (g ascending),
+// found by a 32-ary search of one warp (each lane probes one row per step; ~5 dependent L2 round trips for 10^7 rows
+// instead of 23 for a bisection by one thread).  All 32 lanes of the warp must call it; all return the answer.
+__device__ __forceinline__ int64_t friend_run_start(const double* __restrict__ group, int64_t n_group, int64_t nf, double f,
+                                                    int lane) {
+    int64_t lo = 0, hi = n_group - nf;   // the answer lies in [lo, hi]
+    while (hi > lo) {
+        const int64_t span = hi - lo;
+        const int64_t p = lo + (span * lane) / 32;                       // lo <= p < hi, non-decreasing in lane
+        const bool pred = (f - __ldg(group + 8 * p + 1)) > (__ldg(group + 8 * (p + nf) + 1) - f);
+        const int c = __popc(__ballot_sync(0xffffffffu, pred));         // lanes [0, c) are below the answer
+        const int64_t nlo = c == 0 ? lo : lo + (span * (c - 1)) / 32 + 1;
+        const int64_t nhi = c == 32 ? hi : lo + (span * c) / 32;
+        lo = nlo;
+        hi = nhi;
+    }
+    return lo;
+}
 
 // Current-source cache: a task with at most this many sources keeps the windows of its current sources in a per-CTA
 // scratch area in global memory (8 KB per source for N = 256; all CTAs together ~150 MB, the live part ~40 MB, i.e.
@@ -66,6 +120,8 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
     __shared__ __align__(16) SrcConst s_src[2];
     __shared__ double s_red[(G / 32) * 5 + 1];
     __shared__ int s_acc;
+    __shared__ int s_gk, s_ginside;                   // generated proposal: k, inside the prior box
+    __shared__ double s_glq, s_glu;                   //                      logq, logu
     __shared__ int64_t s_kmin[kBandCacheSlots];       // window start of each cached current source
     const int tid = threadIdx.x;
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
@@ -76,7 +132,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         const bool wb = (t.flags & GB_BAND_WRITE_BACK) != 0;
         const int wrow = (t.flags & GB_BAND_WRITE_OTHER) ? t.write_walker : t.walker;
         bool bad = t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0 ||
-                   (wb && (wrow < 0 || wrow >= a.n_walkers));
+                   (wb && (wrow < 0 || wrow >= a.n_walkers)) || (a.gen && (t.n_src < 1 || t.n_stage < 1));
         int prow = 0;
         if (!bad) {
             prow = a.walker_psd ? a.walker_psd[t.walker] : (a.n_psd == 1 ? 0 : t.walker);
@@ -160,7 +216,77 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         // ---- the proposals of the band, in order
         for (int p = 0; p < t.n_prop; p++) {
             const int64_t ip = (int64_t)t.prop_begin + p;
-            const int k = a.prop_k[ip];
+            int k;
+            const double* theta_p;
+            if (a.gen) {
+                // "k <- randint(0, g_j); theta'_k <- Make Proposal on theta" by warp 0, from the CURRENT
+                // theta_k: Philox block 0 -> k, the friend, z; block 1 -> the uniform of the accept step.  Lane c < 8 owns
+                // coordinate c of theta'; every product and sum is rounded on its own (the oracle is built without FMA
+                // contraction), so k and theta' agree with it bit for bit.
+                if (tid < 32) {
+                    uint32_t w0[4], w1[4];
+                    const uint32_t key0 = (uint32_t)(a.st.seed & 0xffffffffu), key1 = (uint32_t)(a.st.seed >> 32);
+                    philox4x32_10((uint32_t)ip, 0u, 0u, a.st.sweep, key0, key1, w0);
+                    philox4x32_10((uint32_t)ip, 0u, 1u, a.st.sweep, key0, key1, w1);
+                    const int kk = randint32(w0[0], t.n_src);
+                    const double* th = a.params + 8 * ((size_t)t.src_begin + kk);
+                    const int64_t nf = a.st.n_friends < a.st.n_group ? a.st.n_friends : a.st.n_group;
+                    const int32_t jf = randint32(w0[1], (int32_t)nf);
+                    const int64_t row = friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid) + jf;
+                    const double ua = uniform52(w0[2], w0[3]);
+                    const double tz = __dadd_rn(__dmul_rn(__dadd_rn(a.st.stretch_a, -1.0), ua), 1.0);
+                    const double z = __ddiv_rn(__dmul_rn(tz, tz), a.st.stretch_a);    // g(z) ~ z^(-1/2) on [1/a, a]
+                    const int c = tid & 7;
+                    const double xa = __ldg(a.st.group + 8 * row + c);
+                    double x = __dadd_rn(xa, __dmul_rn(z, __dadd_rn(th[c], -xa)));      // Eq. 14
+                    const double lo = a.st.lo[c], hi = a.st.hi[c];
+                    if (a.st.periodic[c]) {
+                        const double period = __dadd_rn(hi, -lo);
+                        x = __dadd_rn(x, -__dmul_rn(period, floor(__ddiv_rn(__dadd_rn(x, -lo), period))));
+                    }
+                    const bool in_c = x >= lo && x <= hi;
+                    bool inside = (__ballot_sync(0xffffffffu, in_c) & 0xffu) == 0xffu;
+                    if (tid < 8) a.gen_params[8 * ip + tid] = x;
+                    double pr[8];
+#pragma unroll
+                    for (int cc = 0; cc < 8; cc++) pr[cc] = __shfl_sync(0xffffffffu, x, cc);
+                    {   // samples may go halfway into the neighbouring sub-bands: the window of theta' must
+                        // stay on the staged bins, else the prior is zero
+                        const int64_t kmin_p = (int64_t)floor(__dmul_rn(pr[1], a.Tobs) + 0.5) - N / 2;
+                        if (kmin_p < t.k_first || kmin_p + N > t.k_first + t.n_stage) inside = false;
+                    }
+                    if (tid == 0) {
+                        const double lq = 7.0 * log(z), lu = log(uniform52(w1[0], w1[1]));   // z^(D-1), D = 8
+                        a.gen_k[ip] = kk;
+                        a.gen_logq[ip] = lq;
+                        a.gen_logu[ip] = lu;
+                        s_gk = kk;
+                        s_ginside = inside ? 1 : 0;
+                        s_glq = lq;
+                        s_glu = lu;
+                        if (!inside) {          // zero prior: rejected without a likelihood evaluation
+                            a.dlnL_out[ip] = nan;
+                            a.accepted_out[ip] = 0;
+                        }
+                    }
+                    if (tid == 1 && inside) {   // step O1 of the proposed source, from registers
+                        SrcConst s;
+                        source_constants(pr, a.Tobs, a.tau, N, s);
+                        s.fast = fast_path_ok(pr, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                        if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                        s_src[1] = s;
+                    }
+                }
+                cta_sync<G>();
+                const bool inside = s_ginside != 0;
+                k = s_gk;
+                cta_sync<G>();                  // s_gk / s_ginside are rewritten by the next proposal
+                if (!inside) continue;          // uniform over the CTA
+                theta_p = a.gen_params + 8 * ip;
+            } else {
+                k = a.prop_k[ip];
+                theta_p = a.prop_params + 8 * ip;
+            }
             if (k < 0 || k >= t.n_src) {   // uniform over the CTA
                 if (tid == 0) {
                     atomicOr(a.errflag, 1);
@@ -170,8 +296,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
                 continue;
             }
             double* theta_k = a.params + 8 * ((size_t)t.src_begin + k);
-            const double* theta_p = a.prop_params + 8 * ip;
-            if (cached ? tid == 1 : tid < 2) {   // step O1 for the old (thread 0) and the proposed (thread 1) source
+            if (a.gen ? (!cached && tid == 0) : (cached ? tid == 1 : tid < 2)) {   // step O1 for the old (thread 0) and the proposed (thread 1) source
                 const double* src = tid == 0 ? theta_k : theta_p;
                 SrcConst s;
                 source_constants(src, a.Tobs, a.tau, N, s);
@@ -245,7 +370,8 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
             if (tid == 0) {
                 const double norm = 4.0 / a.Tobs;
                 const double dl = -0.5 * norm * (v[0] + v[3] - 2.0 * v[2] - 2.0 * v[1] + 2.0 * v[4]);
-                const int acc = t.beta * dl + a.prop_logq[ip] >= a.prop_logu[ip] ? 1 : 0;
+                const double lq = a.gen ? s_glq : a.prop_logq[ip], lu = a.gen ? s_glu : a.prop_logu[ip];
+                const int acc = t.beta * dl + lq >= lu ? 1 : 0;
                 a.dlnL_out[ip] = dl;
                 a.accepted_out[ip] = (uint8_t)acc;
                 s_acc = acc;

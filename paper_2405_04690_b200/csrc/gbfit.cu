@@ -1423,16 +1423,25 @@ int gb_residual_update(gb_ctx* ctx, const gb_data* data, const double* params_ne
     return run_call(ctx, c, stream);
 }
 
-int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
-                  double* params, const int32_t* prop_k, const double* prop_params, const double* prop_logq,
-                  const double* prop_logu, uint8_t* accepted_out, double* dlnL_out, void* stream) {
+static int band_sweep_call(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
+                           double* params, const int32_t* prop_k, const double* prop_params, const double* prop_logq,
+                           const double* prop_logu, const gb_stretch* gen, int32_t* k_out, double* params_out,
+                           double* logq_out, double* logu_out, uint8_t* accepted_out, double* dlnL_out, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
     if (n_tasks < 0 || n_tasks > 0x7fffffff) return set_err(ctx, GB_ERR_INVALID, "n_tasks out of range");
     if (n_tasks == 0) return GB_OK;
     if (!data || !data->resid || !data->psd || data->n_f <= 0 || data->n_walkers <= 0)
         return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
-    if (!tasks || !params || !prop_k || !prop_params || !prop_logq || !prop_logu || !accepted_out || !dlnL_out)
+    if (!tasks || !params || !accepted_out || !dlnL_out) return set_err(ctx, GB_ERR_INVALID, "NULL argument");
+    if (gen) {
+        if (!k_out || !params_out || !logq_out || !logu_out) return set_err(ctx, GB_ERR_INVALID, "NULL argument");
+        if (!gen->group || gen->n_group < 1 || gen->n_friends < 1 || !(gen->stretch_a > 1.0))
+            return set_err(ctx, GB_ERR_INVALID, "bad gb_stretch (group / n_friends / stretch_a)");
+        for (int c = 0; c < 8; c++)
+            if (!(gen->hi[c] > gen->lo[c])) return set_err(ctx, GB_ERR_INVALID, "bad gb_stretch (prior box)");
+    } else if (!prop_k || !prop_params || !prop_logq || !prop_logu) {
         return set_err(ctx, GB_ERR_INVALID, "NULL argument");
+    }
     if (!(N == 128 || N == 256 || N == 512 || N == 1024)) return set_err(ctx, GB_ERR_INVALID, "N must be 128, 256, 512 or 1024");
     if (max_stage < 1 || max_stage > GB_BAND_MAX_STAGE) return set_err(ctx, GB_ERR_INVALID, "max_stage out of range");
     GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
@@ -1444,6 +1453,14 @@ int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, i
     a.prop_params = prop_params;
     a.prop_logq = prop_logq;
     a.prop_logu = prop_logu;
+    if (gen) {
+        a.gen = 1;
+        a.st = *gen;
+        a.gen_k = k_out;
+        a.gen_params = params_out;
+        a.gen_logq = logq_out;
+        a.gen_logu = logu_out;
+    }
     a.accepted_out = accepted_out;
     a.dlnL_out = dlnL_out;
     a.orbit = ctx->d_orbit[N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3];
@@ -1469,6 +1486,21 @@ int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, i
         case 512: return launch_band<512>(ctx, a, st);
         default: return launch_band<1024>(ctx, a, st);
     }
+}
+
+int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
+                  double* params, const int32_t* prop_k, const double* prop_params, const double* prop_logq,
+                  const double* prop_logu, uint8_t* accepted_out, double* dlnL_out, void* stream) {
+    return band_sweep_call(ctx, data, tasks, n_tasks, N, max_stage, params, prop_k, prop_params, prop_logq, prop_logu, nullptr,
+                           nullptr, nullptr, nullptr, nullptr, accepted_out, dlnL_out, stream);
+}
+
+int gb_band_sweep_generate(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
+                           double* params, const gb_stretch* gen, int32_t* k_out, double* params_out, double* logq_out,
+                           double* logu_out, uint8_t* accepted_out, double* dlnL_out, void* stream) {
+    if (ctx && !gen) return set_err(ctx, GB_ERR_INVALID, "NULL gb_stretch");
+    return band_sweep_call(ctx, data, tasks, n_tasks, N, max_stage, params, nullptr, nullptr, nullptr, nullptr, gen, k_out,
+                           params_out, logq_out, logu_out, accepted_out, dlnL_out, stream);
 }
 
 int gb_temper_sweep(gb_ctx* ctx, const gb_data* data, const gb_temper_task* tasks, int64_t n_tasks, int N, int max_stage,

@@ -22,7 +22,7 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
            "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep",
-           "gb_delta_loglike_keep", "gb_residual_update_kept")
+           "gb_delta_loglike_keep", "gb_residual_update_kept", "gb_band_sweep_generate")
 
 BAND_MAX_STAGE = 3072
 # layout of gb_band_task (include/gbfit.h)
@@ -79,6 +79,31 @@ class GbData(C.Structure):
                 ("reserved", C.c_int32)]
 
 
+class GbStretch(C.Structure):   # gb_stretch (include/gbfit.h)
+    _fields_ = [("seed", C.c_uint64), ("sweep", C.c_uint32), ("n_friends", C.c_int32), ("group", C.c_void_p),
+                ("n_group", C.c_int64), ("stretch_a", C.c_double), ("lo", C.c_double * 8), ("hi", C.c_double * 8),
+                ("periodic", C.c_int32 * 8)]
+
+
+class Stretch:
+    """Inputs of the in-loop proposal step of gb_band_sweep_generate: Philox seed / sweep, the stationary group as a CUDA
+    tensor [n_group, 8] sorted by f0 ascending (the caller sorts it), n_friends, stretch scale a, prior box, periodic flags."""
+
+    def __init__(self, seed: int, sweep: int, group: torch.Tensor, n_friends: int, lo, hi, periodic, stretch_a: float = 2.0):
+        self.seed, self.sweep, self.group, self.n_friends = int(seed), int(sweep), group, int(n_friends)
+        self.lo, self.hi, self.periodic, self.stretch_a = [float(x) for x in lo], [float(x) for x in hi], \
+            [int(x) for x in periodic], float(stretch_a)
+        if len(self.lo) != 8 or len(self.hi) != 8 or len(self.periodic) != 8:
+            raise ValueError("lo, hi, periodic must have 8 entries")
+
+    def c(self, device):
+        g = _dev_ptr(self.group, torch.float64, device, "group")
+        if self.group.dim() != 2 or self.group.shape[1] != 8:
+            raise ValueError("group must be [n_group, 8]")
+        return C.byref(GbStretch(self.seed, self.sweep, self.n_friends, g, int(self.group.shape[0]), self.stretch_a,
+                                 (C.c_double * 8)(*self.lo), (C.c_double * 8)(*self.hi), (C.c_int32 * 8)(*self.periodic)))
+
+
 class GbError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"gbfit error {code}: {msg}")
@@ -123,6 +148,9 @@ def lib() -> C.CDLL:
         ru = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, vp, ci, vp, i64, vp]
         L.gb_band_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gb_band_sweep.restype = ci
+        L.gb_band_sweep_generate.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, C.POINTER(GbStretch), vp, vp, vp, vp,
+                                             vp, vp, vp]
+        L.gb_band_sweep_generate.restype = ci
         L.gb_overlap.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, ci, vp, i64, vp, vp, vp]
         L.gb_overlap.restype = ci
         L.gb_delta_loglike_keep.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, i64, vp, vp, vp]
@@ -439,6 +467,30 @@ class Context:
                                      _dev_ptr(accepted_out, torch.uint8, dev, "accepted_out"),
                                      _dev_ptr(dlnL_out, torch.float64, dev, "dlnL_out"), _stream_ptr(stream, dev)))
         return accepted_out, dlnL_out
+
+    def band_sweep_generate(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
+                            stretch: "Stretch", n_prop_total: int, stream=None):
+        """gb_band_sweep_generate (Algorithm 1 with the proposal step inside the loop): params and
+        data.resid are updated in place.  Returns CUDA tensors (accepted uint8, dlnL, k int32, theta' [P, 8], logq, logu)
+        over all P = n_prop_total proposal rows."""
+        dev = self.device
+        n_tasks = int(tasks.numel() // BAND_TASK.itemsize)
+        P = int(n_prop_total)
+        acc = torch.zeros((P,), dtype=torch.uint8, device=dev)
+        dl = torch.zeros((P,), dtype=torch.float64, device=dev)
+        k = torch.zeros((P,), dtype=torch.int32, device=dev)
+        pp = torch.zeros((P, 8), dtype=torch.float64, device=dev)
+        lq = torch.zeros((P,), dtype=torch.float64, device=dev)
+        lu = torch.zeros((P,), dtype=torch.float64, device=dev)
+        self._ok(lib().gb_band_sweep_generate(self._h, data.c(), _dev_ptr(tasks, torch.uint8, dev, "tasks"), n_tasks, int(N),
+                                              int(max_stage), _dev_ptr(params, torch.float64, dev, "params"),
+                                              stretch.c(dev), _dev_ptr(k, torch.int32, dev, "k_out"),
+                                              _dev_ptr(pp, torch.float64, dev, "params_out"),
+                                              _dev_ptr(lq, torch.float64, dev, "logq_out"),
+                                              _dev_ptr(lu, torch.float64, dev, "logu_out"),
+                                              _dev_ptr(acc, torch.uint8, dev, "accepted_out"),
+                                              _dev_ptr(dl, torch.float64, dev, "dlnL_out"), _stream_ptr(stream, dev)))
+        return acc, dl, k, pp, lq, lu
 
     # --------------------------------------------------------------------------------- host forms
     def waveform_host(self, params, N: int = 0, n_bins=None, Nmax: Optional[int] = None, out=None,

@@ -192,3 +192,156 @@ def test_band_sweep_many_tasks_sampled(oracle, torch_cuda, gb):
         assert change > 0
         assert np.abs(r1[w] - odata.resid[w]).max() <= 1e-9 * change + 4e-16 * np.abs(resid[w]).max(), w
     assert 0.02 < acc.mean() < 0.98
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# gb_band_sweep_generate: the proposal step of Algorithm 1 inside the kernel (App. B, Eq. 14)
+def _stretch_pair(oracle, gbfit, torch, si, **over):
+    f = dict(seed=si.seed, sweep=si.sweep, group=si.group, n_friends=si.n_friends, lo=si.lo, hi=si.hi, periodic=si.periodic,
+             stretch_a=si.stretch_a)
+    f.update(over)
+    so = oracle.Stretch(f["seed"], f["sweep"], f["group"], f["n_friends"], f["lo"], f["hi"], f["periodic"], f["stretch_a"])
+    sg = gbfit.Stretch(f["seed"], f["sweep"], dev(torch, f["group"]), f["n_friends"], f["lo"], f["hi"], f["periodic"],
+                       f["stretch_a"])
+    return so, sg
+
+
+def _run_generate(oracle, torch, gbfit, ctx, wl, bt, resid, so, sg, tasks=None):
+    t = bt.tasks if tasks is None else tasks
+    odata = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    p_ref = bt.params.copy()
+    ref = oracle.band_sweep_generate(oracle.Config(), odata, t, bt.N, p_ref, so)
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo)
+    d_params = dev(torch, bt.params)
+    P = int((t["prop_begin"] + t["n_prop"]).max())
+    got = ctx.band_sweep_generate(data, dev(torch, gbfit.pack_band_tasks(**t).view(np.uint8)), bt.N,
+                                  int(max(t["n_stage"].max(), 1)), d_params, sg, P)
+    ctx.check()
+    got = [x.cpu().numpy() for x in got]
+    return got, d_params.cpu().numpy(), d_resid.cpu().numpy(), ref, p_ref, odata.resid
+
+
+def _compare_generate(got, params, r1, ref, p_ref, rr1, resid, rows=None):
+    acc, dl, k, pp, lq, lu = got
+    racc, rdl, rk, rpp, rlq, rlu = ref
+    sl = slice(None) if rows is None else rows
+    assert np.array_equal(k[sl], rk[sl])                               # randint: bit-exact
+    assert np.array_equal(pp[sl], rpp[sl])                             # theta' (friend, z, Eq. 14, wrap): bit-exact
+    assert np.abs(lq[sl] - rlq[sl]).max() <= 4e-15 and np.abs(lu[sl] - rlu[sl]).max() <= 2e-14   # libm log vs CUDA log
+    assert np.array_equal(acc[sl], racc[sl]), int((acc[sl] != racc[sl]).sum())
+    assert np.array_equal(np.isnan(dl[sl]), np.isnan(rdl[sl]))
+    ok = np.isfinite(rdl[sl])
+    assert np.abs(dl[sl][ok] - rdl[sl][ok]).max() <= TOL_DLNL
+    if rows is None:
+        assert np.array_equal(params, p_ref)
+        change = np.abs(rr1 - resid).max()
+        assert np.abs(r1 - rr1).max() <= 1e-9 * change + 4e-16 * np.abs(resid).max()
+
+
+@pytest.mark.parametrize("N,f_lo,n_bands,amp", [(128, 5e-4, 6, 2e-22), (256, 2e-3, 6, 2e-22), (512, 6e-3, 4, 4e-23),
+                                                 (1024, 1.2e-2, 3, 1e-23)])
+def test_band_sweep_generate_each_window_length(oracle, torch_cuda, gb, N, f_lo, n_bands, amp):
+    """k and theta' bit-exact, decisions equal, delta lnL <= 1e-6, final parameters bit-exact, residuals <= 1e-9 of the
+    change (tasks of one walker have disjoint stages -- band_stride = 4 -- and proposals are confined to the stage, so the
+    order in which tasks run does not matter); the case contains a source that is proposed again after an accepted proposal (so theta' was built from the
+    NEW theta_k: a caller-side pre-generated proposal could not reproduce it)."""
+    from gb_inputs import make_stretch_inputs
+    gbfit, ctx = gb
+    wl = make_workload(3, B=1, n_walkers=3)
+    bt = make_band_tasks(wl, N, f_lo, n_bands, n_src=4, n_prop=16, amp_lo=0.1 * amp, amp_hi=amp, band_stride=4)
+    si = make_stretch_inputs(bt, n_copies=6, n_friends=8)
+    so, sg = _stretch_pair(oracle, gbfit, torch_cuda, si)
+    resid = wl.resid()
+    got, params, r1, ref, p_ref, rr1 = _run_generate(oracle, torch_cuda, gbfit, ctx, wl, bt, resid, so, sg)
+    racc, rk = ref[0], ref[2]
+    assert 0 < racc.sum() < racc.size
+    again = 0
+    t = bt.tasks
+    for i in range(len(t["walker"])):
+        moved = set()
+        for p in range(t["n_prop"][i]):
+            ip = t["prop_begin"][i] + p
+            again += rk[ip] in moved
+            if racc[ip]:
+                moved.add(rk[ip])
+    assert again > 0
+    _compare_generate(got, params, r1, ref, p_ref, rr1, resid)
+
+
+def test_band_sweep_generate_prior_box_wrap_small_group_and_errors(oracle, torch_cuda, gb):
+    """Proposals outside a tight prior box (NaN, rejected, no evaluation), periodic wrap, a friends table smaller than
+    n_friends, ties in f0, odd/even flags off / write_back off, and argument errors."""
+    from gb_inputs import make_stretch_inputs
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=1, n_walkers=2)
+    bt = make_band_tasks(wl, 256, 2.5e-3, 5, n_src=3, n_prop=12, stream=3, band_stride=4)
+    resid = wl.resid()
+    si = make_stretch_inputs(bt, n_copies=4, n_friends=6, scale=8.0)          # wide group: wraps and box exits happen
+    lo, hi = si.lo.copy(), si.hi.copy()
+    lo[0], hi[0] = 3e-23, 1.5e-22                                             # tight amplitude prior
+    so, sg = _stretch_pair(oracle, gbfit, torch, si, lo=lo, hi=hi)
+    got, params, r1, ref, p_ref, rr1 = _run_generate(oracle, torch, gbfit, ctx, wl, bt, resid, so, sg)
+    assert 0 < np.isnan(ref[1]).sum() < ref[1].size
+    raw = si.group[:, 3].min() < 0.3 and si.group[:, 3].max() > 5.9             # phases near both ends: wraps occur
+    assert raw
+    _compare_generate(got, params, r1, ref, p_ref, rr1, resid)
+    # table smaller than n_friends, with equal f0 values
+    grp = si.group[:5].copy()
+    grp[1, 1] = grp[2, 1]
+    so, sg = _stretch_pair(oracle, gbfit, torch, si, group=grp, n_friends=9)
+    t2 = dict(bt.tasks, write_back=np.zeros_like(bt.tasks["write_back"]))
+    got, params, r1, ref, p_ref, rr1 = _run_generate(oracle, torch, gbfit, ctx, wl, bt, resid, so, sg, tasks=t2)
+    assert np.array_equal(r1, resid)
+    _compare_generate(got, params, r1, ref, p_ref, rr1, resid + 0.0)
+    # errors: NULL table / a <= 1 are refused at the call; a task without sources is a row error
+    with pytest.raises(gbfit.GbError):
+        _run_generate(oracle, torch, gbfit, ctx, wl, bt, resid, so,
+                      gbfit.Stretch(1, 1, dev(torch, grp), 4, si.lo, si.hi, si.periodic, stretch_a=1.0))
+    bad = {k: v.copy() for k, v in bt.tasks.items()}
+    bad["n_src"][0] = 0
+    data = gbfit.Data(dev(torch, resid), dev(torch, wl.psd), wl.k_lo)
+    out = ctx.band_sweep_generate(data, dev(torch, gbfit.pack_band_tasks(**bad).view(np.uint8)), 256, 768,
+                                  dev(torch, bt.params), sg, bt.prop_k.size)
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    assert np.isnan(out[1].cpu().numpy()[:12]).all()
+
+
+def test_band_sweep_generate_many_tasks_whole_walkers(oracle, torch_cuda, gb):
+    """Launch scale (6588 tasks, more than one wave of CTAs) with a 0.7 M-row friends table: the oracle replays ALL tasks
+    of three walkers; k, theta', decisions, parameters of those tasks and the walkers' written-back residual rows match."""
+    from gb_inputs import make_stretch_inputs
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=1, n_walkers=36)
+    bt = make_band_tasks(wl, 256, 1e-3, n_bands=183, n_src=9, n_prop=30, band_stride=4)   # disjoint stages per walker
+    si = make_stretch_inputs(bt, n_copies=12, n_friends=24)
+    assert si.group.shape[0] == 36 * 183 * 9 * 12
+    so, sg = _stretch_pair(oracle, gbfit, torch, si)
+    resid = wl.resid()
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo)
+    d_params = dev(torch, bt.params)
+    got = ctx.band_sweep_generate(data, dev(torch, gbfit.pack_band_tasks(**bt.tasks).view(np.uint8)), 256, bt.max_stage,
+                                  d_params, sg, bt.prop_k.size)
+    ctx.check()
+    got = [x.cpu().numpy() for x in got]
+    params, r1 = d_params.cpu().numpy(), d_resid.cpu().numpy()
+    walkers = (0, 17, 35)
+    pick = np.flatnonzero(np.isin(bt.tasks["walker"], walkers))
+    sub = {k: v[pick] for k, v in bt.tasks.items()}
+    p_ref = bt.params.copy()
+    odata = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    ref = oracle.band_sweep_generate(oracle.Config(), odata, sub, 256, p_ref, so)
+    for i in pick:
+        ps = slice(bt.tasks["prop_begin"][i], bt.tasks["prop_begin"][i] + bt.tasks["n_prop"][i])
+        ss = slice(bt.tasks["src_begin"][i], bt.tasks["src_begin"][i] + bt.tasks["n_src"][i])
+        _compare_generate(got, None, None, ref, None, None, None, rows=ps)
+        assert np.array_equal(params[ss], p_ref[ss]), i
+    for w in walkers:
+        change = np.abs(odata.resid[w] - resid[w]).max()
+        assert change > 0
+        assert np.abs(r1[w] - odata.resid[w]).max() <= 1e-9 * change + 4e-16 * np.abs(resid[w]).max(), w
+    assert 0.02 < got[0].mean() < 0.98

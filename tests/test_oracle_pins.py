@@ -931,7 +931,7 @@ def test_band_sweep_generate_proposes_from_the_current_state(oracle):
     assert 0 < acc.sum() < acc.size
     t = bt.tasks
     cur = bt.params.copy()
-    again = 0
+    again = off_stage = 0
     for i in range(len(t["walker"])):
         sl = slice(t["src_begin"][i], t["src_begin"][i] + t["n_src"][i])
         moved = set()
@@ -939,13 +939,25 @@ def test_band_sweep_generate_proposes_from_the_current_state(oracle):
             ip = t["prop_begin"][i] + p
             inside, kk, tp, q, u = oracle.make_proposal(st, ip, cur[sl])
             assert kk == k[ip] and np.array_equal(tp, pp[ip]) and q == lq[ip] and u == lu[ip]
-            assert inside or (np.isnan(dl[ip]) and not acc[ip])
+            kmin_p = int(np.floor(tp[1] * wl.Tobs + 0.5)) - bt.N // 2        # the window stays on the stage
+            on_stage = kmin_p >= t["k_first"][i] and kmin_p + bt.N <= t["k_first"][i] + t["n_stage"][i]
+            assert np.isnan(dl[ip]) == (not (inside and on_stage)) and (acc[ip] == 0 or (inside and on_stage))
+            off_stage += inside and not on_stage
             if kk in moved:
                 again += 1
             if acc[ip]:
                 cur[t["src_begin"][i] + kk] = tp
                 moved.add(kk)
     assert again > 0 and np.array_equal(cur, params)
+    # a narrow stage: proposals whose window would leave it have zero prior (NaN, rejected) although they are inside the box
+    narrow = dict(t, n_stage=np.full_like(t["n_stage"], bt.N + 24), k_first=t["k_first"] + bt.N - 12)
+    a_n, dl_n, k_n, pp_n, _, _ = oracle.band_sweep_generate(cfg, oracle.Data(resid.copy(), wl.psd, wl.k_lo), narrow, bt.N,
+                                                            bt.params.copy(), st)
+    km = np.floor(pp_n[:, 1] * wl.Tobs + 0.5).astype(np.int64) - bt.N // 2
+    kf = np.repeat(narrow["k_first"], t["n_prop"])
+    on = (km >= kf) & (km + bt.N <= kf + bt.N + 24)
+    box = np.all((pp_n >= st.lo) & (pp_n <= st.hi), axis=1)
+    assert np.array_equal(np.isnan(dl_n), ~(on & box)) and (box & ~on).sum() > 0 and not a_n[~on].any()
     ok = np.isfinite(dl)
     data2 = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
     params2 = bt.params.copy()
