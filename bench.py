@@ -239,10 +239,28 @@ def run_ours(args):
     setup_s = time.perf_counter() - t_setup
 
     sum_nb = int(wl.n_bins.astype(np.int64).sum())
+    fused = args.update == "fused"
+    args.kept_update = args.update == "kept"
+    # the seeded 25 % "accepted" flags as uniform draws of the accept step: log u = -inf (accepted whatever delta lnL is)
+    # or +inf (rejected), so the decisions of gb_delta_loglike_accept are the workload's flags and cannot flip on a threshold
+    h_lu = pin(np.where(wl.accepted != 0, -np.inf, np.inf))
+    d_lu = h_lu.to(dev)
+    d_accout = torch.zeros(B, dtype=torch.uint8, device=dev)
+    h_accout = torch.zeros(B, dtype=torch.uint8).pin_memory()
+    store_bins = int(1.15 * wl.n_bins[wl.accepted != 0].astype(np.int64).sum()) + 1024
 
     def step_device(i, ev=None):
         if ev:
             ev[0].record(stream)
+        if fused:                    # one call: delta lnL of every row, decision, update by the accepted rows underneath
+            add = i % 2 == 0
+            ctx.delta_loglike_accept(data, d_p if add else None, None if add else d_p, d_w, d_lu,
+                                     move_all=gbfit.ADD if add else gbfit.REMOVE, n_bins=d_nb, store_bins=store_bins, apply=1,
+                                     out=d_out, accepted_out=d_accout)
+            if ev:
+                ev[1].record(stream)
+                ev[2].record(stream)
+            return
         if (not args.kept_update):   # two independent calls: the update regenerates the accepted waveforms
             ctx.delta_loglike(data, d_p, None, d_w, move_all=gbfit.ADD, n_bins=d_nb, out=d_out)
         else:                        # the sweep pair: every window is kept (42 GB of scratch) and scattered from there
@@ -259,6 +277,12 @@ def run_ours(args):
             ev[2].record(stream)
 
     def step_host(i):
+        if fused:
+            add = i % 2 == 0
+            ctx.delta_loglike_accept_host(data, h_p if add else None, None if add else h_p, h_w, h_lu,
+                                          move_all=gbfit.ADD if add else gbfit.REMOVE, n_bins=h_nb, store_bins=store_bins,
+                                          apply=1, out=h_out, accepted_out=h_accout)
+            return
         ctx.delta_loglike_host(data, h_p, None, h_w, move_all=gbfit.ADD, n_bins=h_nb, out=h_out)
         if i % 2 == 0:
             ctx.residual_update_host(data, h_p, None, h_w, move_all=gbfit.ADD, accepted=h_acc, n_bins=h_nb)
@@ -323,8 +347,37 @@ def run_ours(args):
     spot_out = d_out[:2048].cpu().numpy()
     sanity = float(h_out.numpy()[:1000].std())
     assert np.isfinite(h_out.numpy()).all() and sanity > 0
-    h2d = 2 * (h_p.numel() * 8 + h_w.numel() * 4 + h_nb.numel() * 4) + h_acc.numel()
-    d2h = h_out.numel() * 8
+    if fused:
+        assert np.array_equal(h_accout.numpy() != 0, wl.accepted != 0)
+        h2d = h_p.numel() * 8 + h_w.numel() * 4 + h_nb.numel() * 4 + h_lu.numel() * 8
+        d2h = h_out.numel() * 8 + h_accout.numel()
+    else:
+        h2d = 2 * (h_p.numel() * 8 + h_w.numel() * 4 + h_nb.numel() * 4) + h_acc.numel()
+        d2h = h_out.numel() * 8
+
+    # ---- the plain delta-lnL call on its own and the two-call form (gb_delta_loglike + gb_residual_update, which
+    #      regenerates the accepted waveforms), outside the timed step: what the fused call is compared with
+    two_call = None
+    if fused:
+        p0, p1, p2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        t_d, t_u = [], []
+        for i in range(6):
+            p0.record(stream)
+            ctx.delta_loglike(data, d_p, None, d_w, move_all=gbfit.ADD, n_bins=d_nb, out=d_out)
+            p1.record(stream)
+            if i % 2 == 0:
+                ctx.residual_update(data, d_p, None, d_w, move_all=gbfit.ADD, accepted=d_acc, n_bins=d_nb)
+            else:
+                ctx.residual_update(data, None, d_p, d_w, move_all=gbfit.REMOVE, accepted=d_acc, n_bins=d_nb)
+            p2.record(stream)
+            torch.cuda.synchronize()
+            if i >= 2:
+                t_d.append(p0.elapsed_time(p1))
+                t_u.append(p1.elapsed_time(p2))
+        ctx.check()
+        two_call = {"calls": "gb_delta_loglike + gb_residual_update", "ms_dlnl": float(np.mean(t_d)),
+                    "ms_update": float(np.mean(t_u)), "ms_per_step": float(np.mean(t_d) + np.mean(t_u)),
+                    "evals_per_s": B / ((np.mean(t_d) + np.mean(t_u)) * 1e-3)}
 
     # ---- SURVEY 8(f) row f1, outside the timed step: Algorithm 1 (gb_band_sweep) on the same residuals --
     # every odd 256-bin sub-band of 1-4 mHz of every walker, 9 sources and 30 sequential proposals per band
@@ -501,7 +554,9 @@ def run_ours(args):
     hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
     ach_tf = flops_dlnl / (ms_dlnl * 1e-3) / 1e12
     roofline = {
-        "bound": "alu", "kernel": "gb_main_kernel<N,false,true> x {1024,512,256,128} (+ gb_prep_kernel) of gb_delta_loglike",
+        "bound": "alu", "kernel": ("gb_main_kernel<N,false,true,ACC=true> x {1024,512,256,128} (+ gb_prep_kernel, gb_walker_scan_kernel) "
+                                   "of gb_delta_loglike_accept: evaluation, decision and the fused update" if fused else
+                                   "gb_main_kernel<N,false,true> x {1024,512,256,128} (+ gb_prep_kernel) of gb_delta_loglike"),
         "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tf / FP64_PEAK_TFLOPS,
         "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz (no FP64 figure in MEASURED_PEAKS.json)",
         "peak_measured_dfma": dfma_tflops, "frac_of_measured_dfma": ach_tf / dfma_tflops if dfma_tflops > 0 else None,
@@ -513,7 +568,11 @@ def run_ours(args):
         "hbm": {"achieved": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "bytes_per_launch": bytes_dlnl},
-        "update": ({"call": "gb_residual_update (regenerates the accepted waveforms)", "ms_per_launch": ms_upd,
+        "update": ({"call": "inside the same launches (gb_delta_loglike_accept, apply = 1): accepted windows are stored "
+                            "once and scattered by the delta-lnL CTAs as soon as a walker's rows are all evaluated",
+                    "bytes": 1.5 * bytes_upd, "bytes_note": "32 N written + 32 N read + 64 N read-modify-write per accepted row",
+                    "store_bytes": 32.0 * store_bins} if fused else
+                   {"call": "gb_residual_update (regenerates the accepted waveforms)", "ms_per_launch": ms_upd,
                     "flops": flops_upd, "bytes": bytes_upd,
                     "alu_frac": flops_upd / (ms_upd * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
                     "hbm_frac": bytes_upd / (ms_upd * 1e-3) / 1e9 / hbm_peak} if (not args.kept_update) else
@@ -521,9 +580,15 @@ def run_ours(args):
                     "bytes": 1.5 * bytes_upd, "bytes_note": "32 N read + 64 N read-modify-write per accepted row",
                     "hbm_frac": 1.5 * bytes_upd / (ms_upd * 1e-3) / 1e9 / hbm_peak,
                     "kept_window_store_bytes_in_dlnl_call": 32.0 * float(nb.sum())}),
-        "step_frac": (flops_dlnl + (flops_upd if (not args.kept_update) else 0.0)) / (ms_step * 1e-3) / 1e12
+        "step_frac": (flops_dlnl + (flops_upd if args.update == "regenerate" else 0.0)) / (ms_step * 1e-3) / 1e12
                      / FP64_PEAK_TFLOPS,
     }
+    if fused and two_call is not None:
+        tf = flops_dlnl / (two_call["ms_dlnl"] * 1e-3) / 1e12
+        roofline["plain_dlnl"] = {"call": "gb_delta_loglike alone (no decision, no update), timed after the step loop",
+                                  "ms_per_launch": two_call["ms_dlnl"], "achieved": tf, "frac": tf / FP64_PEAK_TFLOPS,
+                                  "frac_of_measured_dfma": tf / dfma_tflops if dfma_tflops > 0 else None}
+
 
     # ---- CPU baseline: the oracle on a bounded sample (rank 0, N = 1 only)
     cpu = None
@@ -557,14 +622,14 @@ def run_ours(args):
                        "evals_per_step_per_gpu": int(B), "n_residuals": int(wl.n_walkers), "n_f": int(wl.n_f),
                        "accepted_fraction": float(wl.accepted.mean()), "mean_N": float(nb.mean()),
                        "l2": "inputs_exceed_l2 (10.8 GB of residuals, no flush)", "psd_layout": "1/S_n rows (psd_is_inverse=1)",
-                       "update": "regenerate" if (not args.kept_update) else "kept windows (gb_delta_loglike_keep + "
-                                 "gb_residual_update_kept)",
+                       "update": {"fused": "fused (gb_delta_loglike_accept, apply = 1)", "regenerate": "regenerate (gb_delta_loglike + "
+                                  "gb_residual_update)", "kept": "kept windows (gb_delta_loglike_keep + gb_residual_update_kept)"}[args.update],
                        "parallelism": f"replicas{world}" if world > 1 else "single_gpu",
                        "ms_dlnl": ms_dlnl, "ms_update": ms_upd, "setup_s": setup_s},
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "sweep_pair_kept": pair, "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "small_configs_latency": small,
+            "two_call_form": two_call, "sweep_pair_kept": pair, "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "small_configs_latency": small,
         }
         print(json.dumps(line), flush=True)
     ctx.close()
@@ -582,9 +647,11 @@ def main(argv=None):
     ap.add_argument("--walkers", type=int, default=360, help="debug: fewer residuals (default = the full config)")
     ap.add_argument("--per-walker", type=int, default=12000, help="debug: fewer sources per walker")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kept-update", action="store_true",
-                    help="time the gb_delta_loglike_keep + gb_residual_update_kept pair (windows kept in 42 GB of scratch, "
-                         "accepted rows scattered from there) instead of gb_delta_loglike + gb_residual_update")
+    ap.add_argument("--update", default="fused", choices=["fused", "regenerate", "kept"],
+                    help="the timed step: fused = one gb_delta_loglike_accept call (decision in the epilogue, accepted windows "
+                         "kept and scattered underneath the evaluation of the remaining walkers); regenerate = "
+                         "gb_delta_loglike + gb_residual_update; kept = gb_delta_loglike_keep + gb_residual_update_kept "
+                         "(every window kept in 42 GB of scratch)")
     ap.add_argument("--no-band-sweep", action="store_true", help="skip the Algorithm-1 (gb_band_sweep) measurement")
     args = ap.parse_args(argv)
     args.warmup = max(args.warmup, 3)

@@ -31,7 +31,8 @@
  *       2  the window extends beyond the Nyquist bin Tobs / (2 dt): the row IS computed and its output is finite
  *          (the waveform definition does not depend on dt, reading S10) -- the flag is a warning;
  *       4  gb_delta_loglike_keep: sum_n_bins too small: dlnL of every row is still computed and finite, windows
- *          past the capacity are not kept, and gb_residual_update_kept skips (and flags) exactly those rows.
+ *          past the capacity are not kept, and gb_residual_update_kept skips (and flags) exactly those rows;
+ *          gb_delta_loglike_accept: store_bins too small: rows that no longer fit are reported rejected.
  *   - Complex arrays are complex128, interleaved (re, im) doubles.  Real arrays are f64.
  *   - params row (8 f64): [amp, f0 (Hz), fdot (Hz/s), phi0, cos(iota), psi, lambda (ecl. lon.), sin(beta)].
  *   - Frequency bins: global bin k  <->  f = k / Tobs  (the rfft grid of the data).
@@ -170,6 +171,16 @@ int gb_delta_loglike_host(gb_ctx *ctx, const gb_data *data, const double *params
                           const int8_t *move /*HOST*/, int move_all, int N, const int32_t *n_bins /*HOST*/,
                           int64_t B, double *dlnL_out /*HOST*/, double *aux_out /*HOST*/, void *stream);
 
+/* gb_delta_loglike_accept (below) with HOST proposal arrays and HOST outputs; batches of >= 2^18 rows flow through in
+ * chunks (each chunk is one gb_delta_loglike_accept call: the snapshot semantics hold per chunk, and a walker's rows
+ * should not straddle chunks if its accepted rows overlap).  apply = 0 runs as a single chunk. */
+int gb_delta_loglike_accept_host(gb_ctx *ctx, const gb_data *data, const double *params_new /*HOST*/,
+                                 const double *params_old /*HOST*/, const int32_t *walker_index /*HOST*/,
+                                 const int8_t *move /*HOST*/, int move_all, int N, const int32_t *n_bins /*HOST*/, int64_t B,
+                                 const double *logq /*HOST*/, const double *logu /*HOST*/, const double *beta /*HOST*/,
+                                 int64_t store_bins, int apply, double *dlnL_out /*HOST*/, double *aux_out /*HOST*/,
+                                 uint8_t *accepted_out /*HOST*/, void *stream);
+
 int gb_residual_update_host(gb_ctx *ctx, const gb_data *data, const double *params_new /*HOST*/,
                             const double *params_old /*HOST*/, const int32_t *walker_index /*HOST*/,
                             const int8_t *move /*HOST*/, int move_all, const uint8_t *accepted /*HOST*/,
@@ -192,6 +203,37 @@ int gb_delta_loglike_keep(gb_ctx *ctx, const gb_data *data, const double *params
                           const int32_t *walker_index, const int8_t *move, int move_all, int N, const int32_t *n_bins,
                           int64_t B, int64_t sum_n_bins, double *dlnL_out, double *aux_out, void *stream);
 int gb_residual_update_kept(gb_ctx *ctx, const gb_data *data, const uint8_t *accepted, int negate, void *stream);
+
+/*
+ * gb_delta_loglike_accept -- the batched sweep step with its accept / reject decision (BASELINE config 5; acceptance of
+ * Algorithm 1, with Eq. 13, in log form and the tempered likelihood of PAPER.md:674):
+ *   1. delta lnL of every ADD / REMOVE row against the same residual snapshot, exactly as gb_delta_loglike
+ *      (a SWAP row is a row error);
+ *   2. row b is accepted iff  beta[b] * dlnL[b] + logq[b] >= logu[b]  (each operation rounded on its own; logq NULL: 0,
+ *      beta NULL: 1; a NaN dlnL is rejected), written to accepted_out[b];
+ *   3. apply != 0: the accepted rows update data->resid (ADD r -= a, REMOVE r += h) -- same result as
+ *      gb_residual_update(accepted_out) after the call, to the rounding order of the atomics.
+ * Only the ACCEPTED windows are kept (context-owned scratch of 32 bytes x store_bins, plus a few per cent of reservation
+ * slack for batches of >= 2^18 rows; store_bins >= the sum of the accepted rows' window lengths, e.g. 0.3 x sum of n_bins
+ * for a 25 % acceptance rate; a row that no longer fits is reported rejected and sets row-error flag 4), so no waveform is
+ * generated twice and the scratch is a quarter of gb_delta_loglike_keep's.
+ *   apply = 0   decide and keep; gb_residual_update_kept(ctx, data, NULL, negate, stream) applies (or undoes) the
+ *               decisions later, any number of times, until the next gb_* call other than gb_check
+ *   apply = 1   fused: batches of >= 2^19 rows are worked through in up to 8 chunks of WALKERS (geometrically shrinking);
+ *               while chunk c + 1 is evaluated, the CTAs of the delta-lnL kernels move the accepted windows of chunks <= c
+ *               -- complete, and read by no row any more, because rows of other walkers never read that residual -- from
+ *               the store into the residual with bulk asynchronous copies and bulk add.f64 reductions (no thread waits
+ *               for them), so the memory-bound update runs underneath the compute-bound evaluation and the snapshot
+ *               semantics of step 1 hold exactly; a closing launch scatters what the last chunk accepted.  Smaller
+ *               batches: as apply = 2
+ *   apply = 2   the same decisions, the update as a separate launch after all evaluations
+ *   logq, logu, beta   [B] DEVICE f64 (logq, beta may be NULL);  accepted_out [B] DEVICE uint8;  dlnL_out, aux_out as
+ *               gb_delta_loglike.  Asynchronous on `stream`.
+ */
+int gb_delta_loglike_accept(gb_ctx *ctx, const gb_data *data, const double *params_new, const double *params_old,
+                            const int32_t *walker_index, const int8_t *move, int move_all, int N, const int32_t *n_bins,
+                            int64_t B, const double *logq, const double *logu, const double *beta, int64_t store_bins,
+                            int apply, double *dlnL_out, double *aux_out, uint8_t *accepted_out, void *stream);
 
 /*
  * gb_overlap -- normalised overlap of B source pairs (cataloging; the search / catalog workloads

@@ -398,6 +398,29 @@ int gbo_residual_update(const gbo_config *c, gbo_data *d, const double *params_n
     return bad ? GBO_ERR_INVALID : GBO_OK;
 }
 
+/* ---- the batched sweep step with its accept / reject decision (BASELINE config 5: "one waveform + delta lnL per source
+ * per sweep ... then scatter-add of accepted deltas"; acceptance of Algorithm 1, with Eq. 13,
+ * PAPER.md:197-202, in log form and the tempered likelihood of PAPER.md:674):
+ *   1. delta lnL of EVERY row against the same residual snapshot (O8);
+ *   2. row b is accepted iff  beta_b dlnL_b + logq_b >= logu_b   (logq NULL: 0, beta NULL: 1; a NaN dlnL is rejected);
+ *   3. if apply: the accepted rows update the residual (O9), after all of step 1.
+ * Written as exactly those three steps with the functions above. */
+int gbo_delta_loglike_accept(const gbo_config *c, gbo_data *d, const double *params_new, const double *params_old,
+                             const int32_t *walker_index, const int8_t *move, int move_all, int N, const int32_t *n_bins,
+                             int64_t B, const double *logq, const double *logu, const double *beta, double *dlnL_out,
+                             double *aux_out, uint8_t *accepted_out, int apply, int nthreads) {
+    int rc = gbo_delta_loglike(c, d, params_new, params_old, walker_index, move, move_all, N, n_bins, B, dlnL_out, aux_out,
+                               nthreads);
+    if (rc) return rc;
+    for (int64_t b = 0; b < B; b++) {
+        double lhs = (beta ? beta[b] : 1.0) * dlnL_out[b] + (logq ? logq[b] : 0.0);
+        accepted_out[b] = (uint8_t)(lhs >= logu[b] ? 1 : 0);
+    }
+    if (!apply) return GBO_OK;
+    return gbo_residual_update(c, d, params_new, params_old, walker_index, move, move_all, accepted_out, N, n_bins, B,
+                               nthreads);
+}
+
 /* <b|c> of two explicit windows against PSD row `psd_row` (exposed for pins P4-P6) */
 double gbo_inner_windows(const gbo_config *c, const gbo_data *d, int psd_row,
                          const double *bA, const double *bE, int64_t kb, int nb,

@@ -161,6 +161,29 @@ def delta_loglike(cfg: Config, data: Data, params_new, params_old, walker_index,
     return (out, aux) if want_aux else out
 
 
+def delta_loglike_accept(cfg: Config, data: Data, params_new, params_old, walker_index, logu, logq=None, beta=None,
+                         move=None, move_all=ADD, N: int = 0, n_bins=None, apply: bool = True, nthreads: int = 1):
+    """gbo_delta_loglike_accept: delta lnL of every row against one snapshot, accepted iff beta dlnL + logq >= logu, then
+    (apply) the accepted rows update data.resid in place.  Returns (dlnL[B], accepted[B] uint8)."""
+    pn = None if params_new is None else _f64(params_new).reshape(-1, 8)
+    po = None if params_old is None else _f64(params_old).reshape(-1, 8)
+    w = np.ascontiguousarray(walker_index, dtype=np.int32)
+    B = w.shape[0]
+    mv = None if move is None else np.ascontiguousarray(move, dtype=np.int8)
+    nb = None if n_bins is None else np.ascontiguousarray(n_bins, dtype=np.int32)
+    lu = _f64(logu)
+    lq = None if logq is None else _f64(logq)
+    bt = None if beta is None else _f64(beta)
+    out, acc = np.zeros(B, np.float64), np.zeros(B, np.uint8)
+    cc, dd = cfg.c(), data.c()
+    rc = lib().gbo_delta_loglike_accept(C.byref(cc), C.byref(dd), _ptr(pn), _ptr(po), _ptr(w), _ptr(mv), C.c_int(move_all),
+                                        C.c_int(N), _ptr(nb), C.c_int64(B), _ptr(lq), _ptr(lu), _ptr(bt), _ptr(out), None,
+                                        _ptr(acc), C.c_int(1 if apply else 0), C.c_int(nthreads))
+    if rc != 0:
+        raise ValueError(f"gbo_delta_loglike_accept rc={rc}")
+    return out, acc
+
+
 def residual_update(cfg: Config, data: Data, params_new, params_old, walker_index, move=None, move_all=ADD,
                     accepted=None, N: int = 0, n_bins=None, nthreads: int = 1):
     """Step O9, in place on data.resid."""

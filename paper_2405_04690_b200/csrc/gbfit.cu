@@ -79,7 +79,30 @@ struct PrepArgs {
     int32_t* counts;         // [kNumClasses]
     int32_t* errflag;
     double* dlnL_out;
+    // gb_delta_loglike_accept: per-row (beta, logq, logu) packed for the main kernels; the work lists are binned by
+    // (class, walker chunk): accept = 1 counts the rows of every bin, accept = 2 is the full pass appending at the bins' offsets
+    int accept;
+    int K;                   // walker chunks
+    int32_t chunk_first[16]; // first walker of every chunk
+    const double* logq;
+    const double* logu;
+    const double* beta;
+    double4* accpar;         // [B] (beta, logq, logu, -)
+    int32_t* bin_count;      // [kNumClasses * K] rows per bin (pass 1)
+    const int32_t* bin_off;  // [kNumClasses * K] exclusive prefix sum of bin_count
+    int32_t* bin_cursor;     // [kNumClasses * K] rows appended so far (pass 2)
+    uint8_t* accepted_out;
 };
+
+// One accepted row of gb_delta_loglike_accept: where its window sits in the store and where it goes.
+struct alignas(16) KeptEnt {
+    int64_t off;             // element offset of the window in the store: [2][N] complex128
+    int64_t kmin;            // global bin of window bin 0
+    int32_t walker;
+    int32_t N;               // 0: empty slot
+    double sgn;              // r += sgn * h   (ADD: -1, REMOVE: +1)
+};
+static_assert(sizeof(KeptEnt) == 32, "KeptEnt layout");
 
 struct MainArgs {
     const SrcConst* src_new;
@@ -111,6 +134,24 @@ struct MainArgs {
     cx* wkeep;               // gb_delta_loglike_keep: every row's window goes here (class base + list position)
     int64_t wkeep_cap;       // capacity in elements
     int32_t* errflag;
+    // gb_delta_loglike_accept (ACC instantiations): the epilogue decides beta dlnL + logq >= logu and stores the ACCEPTED
+    // windows into wkeep, one KeptEnt per accepted row in a global list; store slots and list positions are reserved a few
+    // at a time per CTA.  The rows are binned by (class, walker chunk); a launch works on one bin.
+    KeptEnt* ent;
+    int64_t ent_cap;
+    const double4* accpar;
+    uint8_t* accepted_out;
+    unsigned long long* store_cursor;   // next free element of wkeep
+    int32_t* ent_cursor;                // next free list position
+    int32_t* sc_claim;                  // fused update: pieces handed out to CTAs so far
+    const struct Piece* pieces;         // fused update: the accepted windows of EARLIER walker chunks (complete), cut up
+    const int32_t* n_pieces;            //               and how many there are (fixed during a launch)
+    const int32_t* bin_count;
+    const int32_t* bin_off;
+    int32_t* bin_ticket;
+    int K, chunk;
+    int pool_r;                         // store slots / list positions a CTA reserves at a time
+    int fuse;                           // != 0: CTAs move accepted windows of earlier chunks into the residual between items
 };
 
 // element offset of a class's region of the kept windows: the classes before it, count x 2 N each
@@ -128,12 +169,14 @@ __device__ __forceinline__ int class_of_N(int N) {
 __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int cls = -1;
+    int bin = -1;           // accept mode: cls * K + walker chunk
     bool use_old = false;   // the row's single source is the OLD one (REMOVE)
+    const bool count_only = a.accept == 1;
     if (b < a.B) {
         const int mv = a.mode == MODE_WAVEFORM ? GB_ADD : (a.move ? (int)a.move[b] : a.move_all);
         const int N = a.n_bins ? a.n_bins[b] : a.N;
         const int cN = class_of_N(N);
-        bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP && !(a.keep && mv == GB_SWAP);
+        bool ok = cN >= 0 && mv >= GB_ADD && mv <= GB_SWAP && !((a.keep || a.accept) && mv == GB_SWAP);
         if (a.mode == MODE_WAVEFORM && N > a.Nmax) ok = false;                 // would overrun the row of AE_out
         if (mv != GB_REMOVE && !a.params_new) ok = false;                      // per-row move needs a side that is NULL
         if (mv != GB_ADD && !a.params_old) ok = false;
@@ -149,34 +192,58 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         }
         const bool active = a.accepted ? a.accepted[b] != 0 : true;
         if (!ok) {
-            atomicOr(a.errflag, 1);
-            if (a.dlnL_out) a.dlnL_out[b] = __longlong_as_double(0x7ff8000000000000LL);
+            if (!count_only) {
+                atomicOr(a.errflag, 1);
+                if (a.dlnL_out) a.dlnL_out[b] = __longlong_as_double(0x7ff8000000000000LL);
+                if (a.accept) a.accepted_out[b] = 0;
+            }
         } else if (active) {
             bool fast = true;
-            if (mv != GB_REMOVE) {
-                SrcConst s;
-                source_constants(a.params_new + 8 * b, a.Tobs, a.tau, N, s);
-                s.fast = fast_path_ok(a.params_new + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                fast = fast && s.fast;
-                s.walker = w;  s.psd_row = prow;  s.move = mv;
-                if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                a.src_new[b] = s;
-            }
-            if (mv != GB_ADD) {
-                SrcConst s;
-                source_constants(a.params_old + 8 * b, a.Tobs, a.tau, N, s);
-                s.fast = fast_path_ok(a.params_old + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                fast = fast && s.fast;
-                s.walker = w;  s.psd_row = prow;  s.move = mv;
-                if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                a.src_old[b] = s;
-            }
+            if (mv != GB_REMOVE) fast = fast && fast_path_ok(a.params_new + 8 * b, a.Tobs, a.tau, a.Rmax);
+            if (mv != GB_ADD) fast = fast && fast_path_ok(a.params_old + 8 * b, a.Tobs, a.tau, a.Rmax);
             cls = 4 * cN + (fast ? 0 : 2) + (mv == GB_SWAP ? 1 : 0);
             use_old = mv == GB_REMOVE;
+            if (a.accept) {   // walker chunk: the last k with chunk_first[k] <= w
+                int k = 0;
+                while (k + 1 < a.K && a.chunk_first[k + 1] <= w) k++;
+                bin = cls * a.K + k;
+            }
+            if (!count_only) {
+                if (a.accept) a.accpar[b] = make_double4(a.beta ? a.beta[b] : 1.0, a.logq ? a.logq[b] : 0.0, a.logu[b], 0.0);
+                if (mv != GB_REMOVE) {
+                    SrcConst s;
+                    source_constants(a.params_new + 8 * b, a.Tobs, a.tau, N, s);
+                    s.fast = fast_path_ok(a.params_new + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                    s.walker = w;  s.psd_row = prow;  s.move = mv;
+                    if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                    a.src_new[b] = s;
+                }
+                if (mv != GB_ADD) {
+                    SrcConst s;
+                    source_constants(a.params_old + 8 * b, a.Tobs, a.tau, N, s);
+                    s.fast = fast_path_ok(a.params_old + 8 * b, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                    s.walker = w;  s.psd_row = prow;  s.move = mv;
+                    if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                    a.src_old[b] = s;
+                }
+            }
         }
     }
-    // warp-aggregated append: one atomic per (warp, class)
     const unsigned lane = threadIdx.x & 31;
+    if (a.accept) {   // binned lists: one atomic per (warp, bin); pass 1 counts, pass 2 appends at the bin's offset
+        const unsigned listed = __ballot_sync(0xffffffffu, bin >= 0);
+        if (bin >= 0) {
+            const unsigned m = __match_any_sync(listed, bin);
+            const int leader = __ffs(m) - 1;
+            int base = 0;
+            if ((int)lane == leader) base = atomicAdd((count_only ? a.bin_count : a.bin_cursor) + bin, __popc(m));
+            base = __shfl_sync(m, base, leader);
+            if (!count_only)
+                a.lists[a.bin_off[bin] + base + __popc(m & ((1u << lane) - 1))] = (int32_t)b | (use_old ? (int32_t)0x80000000 : 0);
+        }
+        return;
+    }
+    // warp-aggregated append: one atomic per (warp, class)
 #pragma unroll
     for (int c = 0; c < kNumClasses; c++) {
         const unsigned m = __ballot_sync(0xffffffffu, cls == c);
@@ -186,6 +253,15 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         if ((int)lane == leader) base = atomicAdd(a.counts + c, __popc(m));
         base = __shfl_sync(0xffffffffu, base, leader);
         if (cls == c) a.lists[(int64_t)c * a.B + base + __popc(m & ((1u << lane) - 1))] = (int32_t)b | (use_old ? (int32_t)0x80000000 : 0);
+    }
+}
+
+// exclusive prefix sum of the bin counts (one thread: at most 16 x 16 bins)
+__global__ void gb_bin_scan_kernel(const int32_t* __restrict__ count, int32_t* off, int n) {
+    int acc = 0;
+    for (int i = 0; i < n; i++) {
+        off[i] = acc;
+        acc += count[i];
     }
 }
 
@@ -459,6 +535,247 @@ __device__ __forceinline__ void cp_async_wait() {
 
 constexpr int kRecChunks = (int)(sizeof(SrcConst) / 16);   // 16-byte pieces of one source record
 
+// ---- fused update of gb_delta_loglike_accept -------------------------------------------------------------------
+__device__ __forceinline__ int ld_acquire_s32(const int32_t* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ int ld_relaxed_s32(const int32_t* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// entries and windows were written by other CTAs of the same launch: read them through L2 (an L1 line may predate them)
+__device__ __forceinline__ KeptEnt load_ent(const KeptEnt* p) {
+    const longlong2 a = __ldcg(reinterpret_cast<const longlong2*>(p));
+    const int4 b = __ldcg(reinterpret_cast<const int4*>(p) + 1);
+    KeptEnt e;
+    e.off = a.x;
+    e.kmin = a.y;
+    e.walker = b.x;
+    e.N = b.y;
+    e.sgn = __hiloint2double(b.w, b.z);
+    return e;
+}
+
+// r[walker] += sgn * window for one accepted row (step O9), by T threads: the window is read from the store
+// (coalesced 16-byte loads, four in flight per thread) and added with FP64 atomics resolved in L2.
+template <int T>
+__device__ __forceinline__ void scatter_entry(const KeptEnt& e, const cx* __restrict__ store, double* resid, int64_t k_lo,
+                                              int64_t n_f, int tid) {
+    const int N = e.N;
+    const cx* w = store + e.off;
+    double* r = resid + (size_t)e.walker * 2 * (size_t)n_f * 2;
+    const int64_t i0 = e.kmin - k_lo;
+    const double sgn = e.sgn;
+    const bool inband = i0 >= 0 && i0 + N <= n_f;
+    for (int x0 = tid; x0 < 2 * N; x0 += 4 * T) {
+        double2 h[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int x = x0 + u * T;
+            h[u] = x < 2 * N ? __ldcg(reinterpret_cast<const double2*>(w + x)) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; u++) {
+            const int x = x0 + u * T;
+            if (x < 2 * N) {
+                const int ch = x >= N ? 1 : 0;
+                const int64_t i = i0 + (x - ch * N);
+                if (inband || (i >= 0 && i < n_f)) {
+                    double* p = r + ((size_t)ch * (size_t)n_f + (size_t)i) * 2;
+                    atomicAdd(p, sgn * h[u].x);
+                    atomicAdd(p + 1, sgn * h[u].y);
+                }
+            }
+        }
+    }
+}
+
+// ---- bulk asynchronous copies (TMA without a tensor map) for the fused update ------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_reduce_add_f64(void* gdst, const void* smem_src, unsigned bytes) {
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f64 [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// Fused update of gb_delta_loglike_accept, one small state machine per CTA, driven by thread 0 at two checkpoints of
+// every item.  The call works through the walkers in K chunks; while the rows of chunk c+1 are evaluated, the accepted
+// windows of chunks <= c -- complete, and read by no row any more -- move from the store into the residual.  Between two
+// chunks gb_pieces_kernel cuts the new windows into PIECES of at most kPieceElems elements (one 4 KB staging buffer per
+// CTA) with their clipped destinations worked out, so that the code inside the evaluation loop is a few dozen
+// instructions: a piece goes into the staging buffer with one bulk copy (completion on an mbarrier) and from there into
+// the walker's residual row with one bulk REDUCTION per channel (cp.reduce.async.bulk ... add.f64: the adds happen in L2,
+// no thread waits for them, no register of the evaluation is involved).  Pieces are claimed four at a time.
+constexpr int kPieceElems = 256;   // complex elements of a piece = of the staging buffer
+constexpr int kScQueue = 4;
+struct alignas(16) Piece {
+    unsigned long long src;    // element offset of the piece in the store
+    unsigned long long dst;    // element offset in the residual array of the first segment's first bin
+    unsigned nload;            // bytes to copy store -> staging buffer
+    unsigned nb;               // bytes of a segment (after clipping to the stored band)
+    unsigned s0;               // byte offset of segment 0 in the staging buffer
+    unsigned s1;               // byte offset of segment 1 (the E channel of a window that fits in one piece), 0: none
+};
+static_assert(sizeof(Piece) == 32, "Piece layout");
+struct ScState {
+    unsigned long long mbar;
+    Piece q[kScQueue];     // claimed pieces
+    Piece cur;             // the piece in flight
+    int q_n, q_pos;        // pieces in q; the next one to start
+    int state;             // 0: buffer free, 1: bulk load in flight, 2: bulk reductions in flight
+    unsigned parity;       // phase of mbar the load in flight completes
+    int n_pieces;          // pieces that exist for this launch (fixed)
+    int exhausted;         // nothing left to claim
+    // this CTA's reservations for the rows it accepts
+    long long pool_off;    // next free store slot (a window of this launch's N)
+    int pool_left;
+    int ent_next, ent_left;   // next free list position
+};
+__device__ __forceinline__ void sc_init(ScState& s, int n_pieces) {
+    mbar_init(&s.mbar, 1);
+    s.q_n = s.q_pos = s.state = 0;
+    s.parity = 0;
+    s.n_pieces = n_pieces;
+    s.exhausted = n_pieces <= 0;
+    s.pool_off = 0;
+    s.pool_left = s.ent_next = s.ent_left = 0;
+}
+// first checkpoint of an item (after the slow part): a piece that has landed goes on into the residual
+__device__ __forceinline__ void sc_reduce_if_landed(const MainArgs& a, ScState& s, cx* stage) {
+    if (s.state != 1 || !mbar_test(&s.mbar, s.parity)) return;
+    s.parity ^= 1u;
+    double* dst = a.resid + 2 * s.cur.dst;
+    char* src = reinterpret_cast<char*>(stage);
+    if (s.cur.nb) {
+        bulk_reduce_add_f64(dst, src + s.cur.s0, s.cur.nb);
+        if (s.cur.s1) bulk_reduce_add_f64(dst + 2 * a.n_f, src + s.cur.s1, s.cur.nb);   // the E row follows the A row
+    }
+    bulk_commit();
+    s.state = 2;
+}
+// second checkpoint (end of the item): free the buffer, start the next piece
+__device__ __forceinline__ void sc_next_piece(const MainArgs& a, ScState& s, cx* stage) {
+    if (s.state == 1) return;            // still loading
+    if (s.state == 2) {
+        bulk_wait_read0();               // the staging buffer has been read (the adds complete on their own)
+        s.state = 0;
+    }
+    if (s.q_pos >= s.q_n) {
+        if (s.exhausted) return;
+        // a plain fetch-and-add: positions at or beyond n_pieces are taken by nobody (gb_pieces_kernel pulls the counter back)
+        const int i = atomicAdd(a.sc_claim, kScQueue);
+        if (i >= s.n_pieces) {
+            s.exhausted = 1;
+            return;
+        }
+        const int n = min(kScQueue, s.n_pieces - i);
+        for (int k = 0; k < n; k++) {
+            const uint4* p = reinterpret_cast<const uint4*>(a.pieces + i + k);
+            const uint4 lo = __ldcg(p), hi = __ldcg(p + 1);
+            reinterpret_cast<uint4*>(&s.q[k])[0] = lo;
+            reinterpret_cast<uint4*>(&s.q[k])[1] = hi;
+        }
+        s.q_n = n;
+        s.q_pos = 0;
+        fence_proxy_async();   // the windows were written with ordinary stores (by earlier launches); bulk copies read them
+    }
+    s.cur = s.q[s.q_pos++];
+    mbar_expect_tx(&s.mbar, s.cur.nload);
+    bulk_load(stage, a.wkeep + s.cur.src, s.cur.nload, &s.mbar);
+    s.state = 1;
+}
+// Between two walker chunks of gb_delta_loglike_accept: the accepted rows listed since the last time (positions
+// [*ent_done, *ent_cursor), all written by finished launches) are cut into pieces for the fused update.
+struct PiecesArgs {
+    const KeptEnt* ent;
+    Piece* pieces;
+    int64_t pieces_cap, ent_cap;
+    const int32_t* ent_cursor;
+    const int32_t* ent_done;
+    int32_t* piece_cursor;
+    int64_t k_lo, n_f;
+    int32_t n_walkers;
+};
+
+__global__ void __launch_bounds__(256) gb_pieces_kernel(PiecesArgs a) {
+    int64_t hi = *a.ent_cursor;
+    if (hi > a.ent_cap) hi = a.ent_cap;
+    for (int64_t i = *a.ent_done + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += (int64_t)gridDim.x * blockDim.x) {
+        const KeptEnt e = a.ent[i];
+        if (e.N <= 0 || e.walker < 0 || e.walker >= a.n_walkers) continue;
+        const int N = e.N;
+        const int64_t i0 = e.kmin - a.k_lo;
+        if (2 * N <= kPieceElems) {   // the whole window (A then E) is one piece
+            const int64_t jlo = max((int64_t)0, -i0), jhi = min((int64_t)N, a.n_f - i0);
+            if (jhi <= jlo) continue;
+            const int pos = atomicAdd(a.piece_cursor, 1);
+            if (pos >= a.pieces_cap) continue;
+            Piece p;
+            p.src = (unsigned long long)e.off;
+            p.dst = (unsigned long long)((int64_t)e.walker * 2 * a.n_f + i0 + jlo);
+            p.nload = 2u * N * 16u;
+            p.nb = (unsigned)(jhi - jlo) * 16u;
+            p.s0 = (unsigned)jlo * 16u;
+            p.s1 = (unsigned)(N + jlo) * 16u;
+            a.pieces[pos] = p;
+        } else {                      // pieces of kPieceElems bins of one channel
+            const int per = N / kPieceElems;
+            for (int q = 0; q < 2 * per; q++) {
+                const int ch = q / per;
+                const int64_t x0 = (int64_t)(q % per) * kPieceElems;
+                const int64_t jlo = max(x0, -i0), jhi = min(x0 + kPieceElems, a.n_f - i0);
+                if (jhi <= jlo) continue;
+                const int pos = atomicAdd(a.piece_cursor, 1);
+                if (pos >= a.pieces_cap) continue;
+                Piece p;
+                p.src = (unsigned long long)(e.off + (int64_t)ch * N + x0);
+                p.dst = (unsigned long long)(((int64_t)e.walker * 2 + ch) * a.n_f + i0 + jlo);
+                p.nload = kPieceElems * 16u;
+                p.nb = (unsigned)(jhi - jlo) * 16u;
+                p.s0 = (unsigned)(jlo - x0) * 16u;
+                p.s1 = 0;
+                a.pieces[pos] = p;
+            }
+        }
+    }
+}
+
+// ... and then published: CTAs that found nothing to claim ran the claim counter past the end; it is pulled back first
+__global__ void gb_ready_kernel(const int32_t* ent_cursor, int32_t* ent_done, const int32_t* piece_cursor, int32_t* sc_claim,
+                                int32_t* n_pieces) {
+    if (*sc_claim > *n_pieces) *sc_claim = *n_pieces;
+    *n_pieces = *piece_cursor;
+    *ent_done = *ent_cursor;
+}
+
 // Work distribution: items of a class are handed out by a global ticket counter, in list order, so the CTAs
 // that run at the same time work on neighbouring rows -- consecutive sources of one walker -- and share that
 // walker's residual in L2 (a fixed round-robin deal lets the CTAs drift apart and more than doubles the DRAM
@@ -468,7 +785,7 @@ constexpr int kRecChunks = (int)(sizeof(SrcConst) / 16);   // 16-byte pieces of 
 // before its inner products read it: no global-memory round trip is exposed between items.
 // A list entry is the row index, with bit 31 set when the row's single source is the OLD one (REMOVE);
 // -1 marks the end of the list.
-template <int N, bool SWAP, bool FAST>
+template <int N, bool SWAP, bool FAST, bool ACC>
 __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kernel(MainArgs a) {
     constexpr int G = Plan<N>::G;
     constexpr int S = N / G;
@@ -485,11 +802,42 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
 
     __shared__ int s_ent[2];
     __shared__ int s_pos[2];   // list positions of the entries in s_ent (gb_delta_loglike_keep)
+    __shared__ __align__(16) double4 s_par[2];   // (beta, logq, logu) of the item in each buffer (gb_delta_loglike_accept)
+    __shared__ long long s_off;                  // store offset of this item's window, -1: rejected
 
     const int tid = threadIdx.x;
-    const int count = a.counts[cls];
-    if (count == 0) return;
-    const int32_t* __restrict__ list = a.lists + (int64_t)cls * a.B;
+    constexpr bool accept = ACC && !SWAP;   // gb_delta_loglike_accept (its own instantiation: the plain kernels carry none of it)
+    const int bin = accept ? cls * a.K + a.chunk : cls;   // accept: the lists are binned by (class, walker chunk)
+    const int count = accept ? a.bin_count[bin] : a.counts[cls];
+    int32_t* const ticket = accept ? a.bin_ticket + bin : a.counters + cls;
+    // fused update (thread 0 only): accepted windows of earlier walker chunks travel store -> staging buffer -> residual as
+    // bulk asynchronous copies / reductions; no other thread and no register of the evaluation is involved
+    cx* stage = reinterpret_cast<cx*>(smem_raw) + 2 * PN;
+    __shared__ ScState s_scs;
+    const bool fuse = accept && a.fuse;
+    if (accept && tid == 0) sc_init(s_scs, fuse ? *a.n_pieces : 0);
+    auto finish = [&]() {   // before the CTA exits: what it claimed is finished, list positions it did not use are marked empty
+        if (accept && tid == 0) {
+            if (fuse) {
+                s_scs.exhausted = 1;
+                for (;;) {
+                    if (s_scs.state == 1) {
+                        while (!mbar_test(&s_scs.mbar, s_scs.parity)) {}
+                        sc_reduce_if_landed(a, s_scs, stage);
+                    }
+                    if (s_scs.state == 0 && s_scs.q_pos >= s_scs.q_n) break;
+                    sc_next_piece(a, s_scs, stage);
+                }
+                asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+            }
+            KeptEnt none;
+            none.off = 0;  none.kmin = 0;  none.walker = 0;  none.N = 0;  none.sgn = 0.0;
+            for (int i = 0; i < s_scs.ent_left; i++)
+                if (s_scs.ent_next + i < a.ent_cap) a.ent[s_scs.ent_next + i] = none;
+        }
+    };
+    if (!accept && count == 0) return;   // (accept: one exit at the end, so that the closing code exists once)
+    const int32_t* __restrict__ list = accept ? a.lists + a.bin_off[bin] : a.lists + (int64_t)cls * a.B;
 
     auto fetch = [&](int entry, int bufi) {
         const int64_t row = entry & 0x7fffffff;
@@ -503,12 +851,15 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         } else if (tid < kRecChunks) {
             const SrcConst* g = (entry < 0 ? a.src_old : a.src_new) + row;
             cp_async16(reinterpret_cast<char*>(&s_src[bufi][0]) + 16 * tid, reinterpret_cast<const char*>(g) + 16 * tid);
+        } else if (accept && tid < kRecChunks + 2) {
+            cp_async16(reinterpret_cast<char*>(&s_par[bufi]) + 16 * (tid - kRecChunks),
+                       reinterpret_cast<const char*>(a.accpar + row) + 16 * (tid - kRecChunks));
         }
     };
 
     int t_nx2 = 0;   // (thread 0) ticket of the item after next
     if (tid == 0) {
-        const int t = atomicAdd(a.counters + cls, 3);
+        const int t = atomicAdd(ticket, 3);
         s_ent[0] = t < count ? __ldg(list + t) : -1;
         s_ent[1] = t + 1 < count ? __ldg(list + t + 1) : -1;
         s_pos[0] = t;
@@ -518,13 +869,15 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     group_sync<G>();
     int e_cur = s_ent[0], e_nxt = s_ent[1];
     int pos_cur = s_pos[0], pos_nxt = s_pos[1];
-    const int64_t keep_base = a.wkeep ? keep_class_base(a.counts, cls) : 0;
-    if (e_cur == -1) return;
-    fetch(e_cur, 0);
-    cp_async_commit();
+    const int64_t keep_base = (a.wkeep && !accept) ? keep_class_base(a.counts, cls) : 0;
+    if (!accept && e_cur == -1) return;
     int buf = 0;
+    if (e_cur != -1) {
+        fetch(e_cur, 0);
+        cp_async_commit();
+    }
 
-    for (;;) {
+    while (e_cur != -1) {
         const bool has_nxt = e_nxt != -1;
         if (has_nxt) fetch(e_nxt, buf ^ 1);
         cp_async_commit();
@@ -544,9 +897,11 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         // register-hungry slow part, and consumed at the end of the item, behind the FFT and the epilogue
         int t_nx3 = 0, e_nx2 = -1;
         if (tid == 0) {
-            t_nx3 = atomicAdd(a.counters + cls, 1);
+            t_nx3 = atomicAdd(ticket, 1);
             if (t_nx2 < count) e_nx2 = __ldg(list + t_nx2);
         }
+        // fused update, first checkpoint of the item: move the piece in flight one stage on
+        if (fuse && tid == 0) sc_reduce_if_landed(a, s_scs, stage);
         const int64_t kmin0 = rec[0].kmin;
 
         // ---- ask L2 for the next item's residual / PSD window
@@ -645,7 +1000,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                             v[1] += wb.w[c] * (rc.re * hc.re + rc.im * hc.im);
                         }
                     }
-                    if (a.wkeep) {   // keep the window for gb_residual_update_kept: [position][channel][N]
+                    if (a.wkeep && !accept) {   // keep the window for gb_residual_update_kept: [position][channel][N]
                         const int64_t off = keep_base + (int64_t)pos_cur * 2 * N + (int64_t)ch * N + ht;
                         if (off - ht - (int64_t)ch * N + 2 * N <= a.wkeep_cap) {
 #pragma unroll
@@ -657,10 +1012,54 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     group_reduce<G, 2>(v, s_red, tid);
                     if (tid == 0) {
                         const double hh = norm * v[0], rh = norm * v[1];
-                        a.dlnL_out[b] = (mv == GB_REMOVE ? -rh : rh) - 0.5 * hh;
+                        const double dl = (mv == GB_REMOVE ? -rh : rh) - 0.5 * hh;
+                        a.dlnL_out[b] = dl;
                         if (a.aux_out) {
                             a.aux_out[2 * b] = hh;
                             a.aux_out[2 * b + 1] = rh;
+                        }
+                        if (accept) {   // Eq. 13 in log form, each operation rounded on its own (as the oracle)
+                            const double4 par = s_par[buf];
+                            bool acc = __dadd_rn(__dmul_rn(par.x, dl), par.y) >= par.z;
+                            long long off = -1;
+                            if (acc) {
+                                ScState& sc = s_scs;
+                                if (sc.pool_left == 0) {   // reserve store slots and list positions for the next few accepted rows
+                                    const int R = a.pool_r;
+                                    sc.pool_off = (long long)atomicAdd(a.store_cursor, (unsigned long long)(R * 2 * N));
+                                    sc.ent_next = atomicAdd(a.ent_cursor, R);
+                                    sc.pool_left = sc.ent_left = R;
+                                }
+                                if (sc.pool_off + 2 * N > a.wkeep_cap || sc.ent_next >= a.ent_cap) {   // store full: the row cannot be applied
+                                    atomicOr(a.errflag, 4);
+                                    acc = false;
+                                } else {
+                                    off = sc.pool_off;
+                                    KeptEnt e;
+                                    e.off = off;
+                                    e.kmin = kmin0;
+                                    e.walker = w;
+                                    e.N = N;
+                                    e.sgn = 1.0;   // the sign of the move is in the stored window
+                                    a.ent[sc.ent_next] = e;
+                                    sc.pool_off += 2 * N;
+                                    sc.pool_left--;
+                                    sc.ent_next++;
+                                    sc.ent_left--;
+                                }
+                            }
+                            a.accepted_out[b] = acc ? 1 : 0;
+                            s_off = off;
+                        }
+                    }
+                    if (accept) {
+                        group_sync<G>();
+                        const long long off = s_off;
+                        if (off >= 0) {
+                            cx* dst = a.wkeep + off + (int64_t)ch * N + ht;
+                            const double sg = mv == GB_REMOVE ? 1.0 : -1.0;   // the store holds the CHANGE of the residual
+#pragma unroll
+                            for (int m = 0; m < M; m++) dst[H * m] = {sg * h[m].re, sg * h[m].im};
                         }
                     }
                 } else {
@@ -778,6 +1177,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             t_nx2 = t_nx3;
         }
         group_sync<G>();   // the waveform buffers, s_red and this half of s_src are reused from here on
+        if (fuse && tid == 0) sc_next_piece(a, s_scs, stage);   // second checkpoint of the item
         if (!has_nxt) break;
         e_cur = e_nxt;
         e_nxt = s_ent[0];
@@ -785,14 +1185,15 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         pos_nxt = s_pos[0];
         buf ^= 1;
     }
+    finish();
 }
 
 #include "gb_band.cuh"
 #include "gb_temper.cuh"
 
-template <int N, bool SWAP>
+template <int N, bool SWAP, bool ACC = false>
 constexpr size_t main_smem_bytes() {
-    return (size_t)padded_len<N>() * sizeof(cx) * 2 * (SWAP ? 2 : 1);
+    return (size_t)padded_len<N>() * sizeof(cx) * 2 * (SWAP ? 2 : 1) + (ACC ? (size_t)kPieceElems * sizeof(cx) : 0);
 }
 
 }  // namespace
@@ -850,6 +1251,64 @@ __global__ void __launch_bounds__(128) gb_scatter_kept_kernel(KeptArgs a) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------ accepted windows
+// Scatter of the list positions [*lo, *hi) of the accepted-row list of gb_delta_loglike_accept from its store: what the
+// fused update of the call left over (the last walker chunk), the whole list for apply = 2, and gb_residual_update_kept
+// after apply = 0.  One CTA per list position at a time; unused positions (N = 0) are skipped.
+struct EntArgs {
+    const KeptEnt* ent;
+    const cx* store;
+    const int32_t* lo;        // DEVICE: first position (NULL: 0)
+    const int32_t* hi;        // DEVICE: end of the list
+    int64_t ent_cap;
+    double* resid;
+    int64_t k_lo, n_f;
+    int32_t n_walkers;        // of the gb_data passed to THIS call
+    int32_t* errflag;
+    double sign;              // +1 applies the moves, -1 undoes them
+};
+
+__global__ void __launch_bounds__(128) gb_scatter_ent_kernel(EntArgs a) {
+    const int64_t lo = a.lo ? *a.lo : 0;
+    int64_t hi = *a.hi;
+    if (hi > a.ent_cap) hi = a.ent_cap;
+    for (int64_t i = lo + blockIdx.x; i < hi; i += gridDim.x) {
+        KeptEnt e = a.ent[i];
+        if (e.N <= 0) continue;
+        if (e.walker < 0 || e.walker >= a.n_walkers) {   // a data view with fewer walkers than the accept call's
+            if (threadIdx.x == 0) atomicOr(a.errflag, 1);
+            continue;
+        }
+        e.sgn *= a.sign;
+        scatter_entry<128>(e, a.store, a.resid, a.k_lo, a.n_f, threadIdx.x);
+    }
+}
+
+// the pieces the fused update did not get to (positions [min(claim, n), n) of the piece list), by plain loads and atomics
+struct RestArgs {
+    const Piece* pieces;
+    const cx* store;
+    const int32_t* sc_claim;
+    const int32_t* n_pieces;
+    double* resid;
+    int64_t n_f;
+};
+__global__ void __launch_bounds__(128) gb_scatter_pieces_kernel(RestArgs a) {
+    const int n = *a.n_pieces;
+    const int lo = min(*a.sc_claim, n);
+    for (int i = lo + blockIdx.x; i < n; i += gridDim.x) {
+        const Piece p = a.pieces[i];
+        const int nel = (int)(p.nb / 16u);
+        for (int x = threadIdx.x; x < nel * (p.s1 ? 2 : 1); x += blockDim.x) {
+            const int seg = x >= nel ? 1 : 0, j = x - seg * nel;
+            const double2 h = __ldcg(reinterpret_cast<const double2*>(a.store + p.src) + (seg ? p.s1 : p.s0) / 16u + j);
+            double* d = a.resid + 2 * (p.dst + (seg ? (unsigned long long)a.n_f : 0ull) + (unsigned long long)j);
+            atomicAdd(d, h.x);
+            atomicAdd(d + 1, h.y);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ FP64 peak
 // 8 independent DFMA chains per thread, registers only (gb_measure_fp64_peak)
 __global__ void __launch_bounds__(128) gb_dfma_peak_kernel(double* sink, int iters, double a, double b) {
@@ -887,7 +1346,16 @@ struct gb_ctx {
     int64_t cap_new, cap_old, cap_lists, cap_band_cache, cap_temper_cache, cap_wkeep;
     int64_t kept_B;         // > 0: lists, records and windows of the last gb_delta_loglike_keep call are still valid
     int64_t kept_cap;       // elements of d_wkeep that call was allowed to write (2 x its sum_n_bins)
+    int kept_mode;          // 1: every window (gb_delta_loglike_keep), 2: accepted windows + entries (gb_delta_loglike_accept)
+    // gb_delta_loglike_accept: counters [store cursor (2 ints), list cursor, claim, ready_end, pad (3), then per bin:
+    // count, offset, append cursor, ticket], the list of accepted rows, (beta, logq, logu) per row
+    int32_t* d_wk;
+    KeptEnt* d_ent;
+    double4* d_accpar;
+    Piece* d_pieces;        // fused update: accepted windows cut into staging-buffer sized pieces
+    int64_t cap_wk, cap_ent, cap_accpar, cap_pieces;
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
+    int grid_blocks_acc[kNumClasses];   // the same for the gb_delta_loglike_accept instantiations
     // staging for the *_host entry points
     void* d_stage;
     size_t cap_stage;
@@ -936,25 +1404,25 @@ int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
     return GB_OK;
 }
 
-template <int N, bool SWAP, bool FAST>
+template <int N, bool SWAP, bool FAST, bool ACC = false>
 int setup_kernel(gb_ctx* ctx) {
     constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
-    const size_t smem = main_smem_bytes<N, SWAP>();
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP, FAST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem = main_smem_bytes<N, SWAP, ACC>();
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP, FAST, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST>, Plan<N>::G, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST, ACC>, Plan<N>::G, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_CUDA, "kernel class %d does not fit on an SM", cls);
-    ctx->grid_blocks[cls] = nb * ctx->num_sms;
+    (ACC ? ctx->grid_blocks_acc : ctx->grid_blocks)[cls] = nb * ctx->num_sms;
     return GB_OK;
 }
 
-template <int N, bool SWAP, bool FAST>
+template <int N, bool SWAP, bool FAST, bool ACC = false>
 int launch_main(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
     constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
     a.orbit = ctx->d_orbit[cls >> 2];
-    int64_t grid = ctx->grid_blocks[cls];
+    int64_t grid = (ACC ? ctx->grid_blocks_acc : ctx->grid_blocks)[cls];
     if (grid > B) grid = B;
-    gb_main_kernel<N, SWAP, FAST><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP>(), st>>>(a);
+    gb_main_kernel<N, SWAP, FAST, ACC><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP, ACC>(), st>>>(a);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -987,8 +1455,37 @@ struct Call {
     int64_t* kmin_out;
     int Nmax;
     int keep;               // gb_delta_loglike_keep
-    int64_t sum_bins;       // sum of the rows' window lengths (keep)
+    int64_t sum_bins;       // sum of the rows' window lengths (keep); accept: capacity of the store in window bins
+    int accept;             // gb_delta_loglike_accept: 1 = decide and keep, 2 = + fused update, 3 = + update by a separate launch
+    const double* logq;
+    const double* logu;
+    const double* beta;
+    uint8_t* accepted_out;
 };
+
+constexpr int kMaxChunks = 16;           // walker chunks of gb_delta_loglike_accept
+constexpr int kWkHeader = 8;             // ints before the per-bin arrays of d_wk
+constexpr int kWkInts = kWkHeader + 4 * kNumClasses * kMaxChunks;
+
+// scatter of list positions [from the claim counter (rest) or 0 (all), list cursor) of the last gb_delta_loglike_accept call
+int scatter_entries(gb_ctx* ctx, const gb_data* data, double sign, bool rest_only, cudaStream_t st) {
+    EntArgs e{};
+    e.ent = ctx->d_ent;
+    e.store = ctx->d_wkeep;
+    e.lo = rest_only ? ctx->d_wk + 5 : nullptr;   // rows listed after the last cut into pieces
+    e.hi = ctx->d_wk + 2;
+    e.ent_cap = ctx->cap_ent;
+    e.resid = data->resid;
+    e.k_lo = data->k_lo;
+    e.n_f = data->n_f;
+    e.n_walkers = data->n_walkers;
+    e.errflag = ctx->d_counts + 2 * kNumClasses;
+    e.sign = sign;
+    gb_scatter_ent_kernel<<<ctx->num_sms * 16, 128, 0, st>>>(e);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+    return GB_OK;
+}
 
 int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
@@ -1028,6 +1525,41 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
         if (c.sum_bins < 128 * c.B || c.sum_bins > 1024 * c.B) return set_err(ctx, GB_ERR_INVALID, "sum_n_bins out of range");
         if ((rc = ensure_cap(ctx, &ctx->d_wkeep, &ctx->cap_wkeep, 2 * c.sum_bins))) return rc;
     }
+    // gb_delta_loglike_accept: walker chunks (the fused update of chunk c runs under the evaluation of chunk c + 1)
+    const int nw = c.data ? c.data->n_walkers : 0;
+    int K = 1;
+    int pool_r[4] = {1, 1, 1, 1};
+    int64_t store_slack = 0, ent_slack = 0;
+    if (c.accept) {
+        if (c.sum_bins < 128 || c.sum_bins > 1024 * c.B) return set_err(ctx, GB_ERR_INVALID, "store_bins out of range");
+        if (!c.logu || !c.accepted_out) return set_err(ctx, GB_ERR_INVALID, "NULL logu / accepted_out");
+        if (c.accept == 2) {
+            K = (int)(c.B >> 18);   // ~ 2^18 rows per chunk: enough work per launch to hide its tail
+            if (K > nw) K = nw;
+            if (K > 8) K = 8;       // measured on B200 (config 5): 8 chunks 46.8 ms, 4: 47.1, 16: 47.5 (more launches, more tails)
+            if (K < 1) K = 1;
+        }
+
+        // large batches: a CTA reserves store slots and list positions a few at a time (one round trip per pool_r accepted
+        // rows) and may leave part of its last reservation unused in every launch; small batches reserve exactly
+        for (int cN = 0; cN < 4; cN++) {
+            const int Nc = 128 << cN;
+            pool_r[cN] = c.B >= (1 << 18) ? (cN == 0 ? 8 : cN == 1 ? 4 : 2) : 1;
+            const int64_t ctas = (int64_t)ctx->grid_blocks_acc[4 * cN] + ctx->grid_blocks_acc[4 * cN + 2];
+            store_slack += ctas * K * (pool_r[cN] - 1) * 2 * Nc;
+            ent_slack += ctas * K * (pool_r[cN] - 1);
+        }
+        if ((rc = ensure_cap(ctx, &ctx->d_wkeep, &ctx->cap_wkeep, 2 * c.sum_bins + store_slack))) return rc;
+        if ((rc = ensure_cap(ctx, &ctx->d_wk, &ctx->cap_wk, kWkInts))) return rc;
+        if ((rc = ensure_cap(ctx, &ctx->d_ent, &ctx->cap_ent, c.B + ent_slack))) return rc;
+        if ((rc = ensure_cap(ctx, &ctx->d_accpar, &ctx->cap_accpar, c.B))) return rc;
+        if (K > 1 && (rc = ensure_cap(ctx, &ctx->d_pieces, &ctx->cap_pieces, (2 * c.sum_bins + store_slack) / kPieceElems + 1024))) return rc;
+        GB_CUDA(ctx, cudaMemsetAsync(ctx->d_wk, 0, sizeof(int32_t) * kWkInts, st));
+    }
+    int32_t* bin_count = ctx->d_wk ? ctx->d_wk + kWkHeader : nullptr;
+    int32_t* bin_off = bin_count ? bin_count + kNumClasses * kMaxChunks : nullptr;
+    int32_t* bin_cursor = bin_count ? bin_count + 2 * kNumClasses * kMaxChunks : nullptr;
+    int32_t* bin_ticket = bin_count ? bin_count + 3 * kNumClasses * kMaxChunks : nullptr;
 
     GB_CUDA(ctx, cudaMemsetAsync(ctx->d_counts, 0, sizeof(int32_t) * 2 * kNumClasses, st));
 
@@ -1058,6 +1590,37 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.errflag = ctx->d_counts + 2 * kNumClasses;
     p.dlnL_out = (c.mode == MODE_DLNL || c.mode == MODE_OVERLAP) ? c.dlnL_out : nullptr;
     const unsigned pgrid = (unsigned)((c.B + 255) / 256);
+    if (c.accept) {   // binned work lists: count the rows of every (class, walker chunk) bin, scan, then the full pass
+        p.accept = 1;
+        p.K = K;
+        // Chunk sizes fall off geometrically (ratio 3/4): the accepted rows of chunk c are moved into the residual while
+        // chunk c + 1 is evaluated, about one 4 KB piece per evaluated row, so a chunk must not be much smaller than the
+        // one before it; and what the last chunk accepts is left to the closing launch, so the last chunk is the smallest.
+        {
+            double total = 0.0, sz = 1.0, cum = 0.0;
+            for (int k = 0; k < K; k++, sz *= 0.75) total += sz;
+            sz = 1.0;
+            for (int k = 0; k < K; k++, sz *= 0.75) {
+                int first = (int)(cum / total * nw + 0.5);
+                if (k > 0 && first <= p.chunk_first[k - 1]) first = p.chunk_first[k - 1] + 1;   // K <= n_walkers: room for all
+                p.chunk_first[k] = k == 0 ? 0 : first;
+                cum += sz;
+            }
+        }
+        p.logq = c.logq;
+        p.logu = c.logu;
+        p.beta = c.beta;
+        p.accpar = ctx->d_accpar;
+        p.bin_count = bin_count;
+        p.bin_off = bin_off;
+        p.bin_cursor = bin_cursor;
+        p.accepted_out = c.accepted_out;
+        gb_prep_kernel<<<pgrid, 256, 0, st>>>(p);
+        gb_bin_scan_kernel<<<1, 1, 0, st>>>(bin_count, bin_off, kNumClasses * K);
+        ctx->launches += 2;
+        GB_CUDA(ctx, cudaGetLastError());
+        p.accept = 2;
+    }
     gb_prep_kernel<<<pgrid, 256, 0, st>>>(p);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
@@ -1091,10 +1654,79 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     a.Nmax = c.Nmax;
     a.Tobs = ctx->cfg.Tobs;
     a.tau = p.tau;
-    a.wkeep = c.keep ? ctx->d_wkeep : nullptr;
-    a.wkeep_cap = c.keep ? 2 * c.sum_bins : 0;
+    a.wkeep = (c.keep || c.accept) ? ctx->d_wkeep : nullptr;
+    a.wkeep_cap = (c.keep || c.accept) ? 2 * c.sum_bins : 0;
     a.errflag = p.errflag;
-
+    if (c.accept) {
+        a.ent = ctx->d_ent;
+        a.ent_cap = ctx->cap_ent;
+        a.wkeep_cap = ctx->cap_wkeep < 2 * c.sum_bins + store_slack ? ctx->cap_wkeep : 2 * c.sum_bins + store_slack;
+        a.accpar = ctx->d_accpar;
+        a.accepted_out = c.accepted_out;
+        a.store_cursor = reinterpret_cast<unsigned long long*>(ctx->d_wk);
+        a.ent_cursor = ctx->d_wk + 2;
+        a.sc_claim = ctx->d_wk + 3;
+        a.n_pieces = ctx->d_wk + 4;
+        a.pieces = ctx->d_pieces;
+        a.bin_count = bin_count;
+        a.bin_off = bin_off;
+        a.bin_ticket = bin_ticket;
+        a.K = K;
+        a.fuse = c.accept == 2 && K > 1;
+        PiecesArgs pa{};
+        pa.ent = ctx->d_ent;
+        pa.pieces = ctx->d_pieces;
+        pa.pieces_cap = ctx->cap_pieces;
+        pa.ent_cap = ctx->cap_ent;
+        pa.ent_cursor = a.ent_cursor;
+        pa.ent_done = ctx->d_wk + 5;
+        pa.piece_cursor = ctx->d_wk + 6;
+        pa.k_lo = c.data->k_lo;
+        pa.n_f = c.data->n_f;
+        pa.n_walkers = c.data->n_walkers;
+        for (int chunk = 0; chunk < K; chunk++) {
+            a.chunk = chunk;
+            if (chunk > 0 && a.fuse) {   // the accepted rows of the chunks before this one are complete from here on
+                gb_pieces_kernel<<<ctx->num_sms, 256, 0, st>>>(pa);
+                gb_ready_kernel<<<1, 1, 0, st>>>(a.ent_cursor, ctx->d_wk + 5, ctx->d_wk + 6, a.sc_claim, ctx->d_wk + 4);
+                ctx->launches += 2;
+            }
+            // the rows outside the fast path first (usually none), then the fast kernels
+            for (int pass = 0; pass < 2; pass++) {
+                for (int cN = 3; cN >= 0; cN--) {
+                    const int Nc = 128 << cN;
+                    if (!c.n_bins && Nc != c.N) continue;
+                    a.pool_r = pool_r[cN];
+                    switch (Nc) {
+                        case 128: rc = pass ? launch_main<128, false, true, true>(ctx, a, c.B, st) : launch_main<128, false, false, true>(ctx, a, c.B, st); break;
+                        case 256: rc = pass ? launch_main<256, false, true, true>(ctx, a, c.B, st) : launch_main<256, false, false, true>(ctx, a, c.B, st); break;
+                        case 512: rc = pass ? launch_main<512, false, true, true>(ctx, a, c.B, st) : launch_main<512, false, false, true>(ctx, a, c.B, st); break;
+                        default: rc = pass ? launch_main<1024, false, true, true>(ctx, a, c.B, st) : launch_main<1024, false, false, true>(ctx, a, c.B, st); break;
+                    }
+                    if (rc) return rc;
+                }
+            }
+        }
+        ctx->kept_B = c.B;
+        ctx->kept_cap = a.wkeep_cap;
+        ctx->kept_mode = 2;
+        if (c.accept == 2) {   // what the fused update left: the pieces nobody took and the last chunk's rows
+            if (a.fuse) {
+                RestArgs ra{};
+                ra.pieces = ctx->d_pieces;
+                ra.store = ctx->d_wkeep;
+                ra.sc_claim = a.sc_claim;
+                ra.n_pieces = ctx->d_wk + 4;
+                ra.resid = c.data->resid;
+                ra.n_f = c.data->n_f;
+                gb_scatter_pieces_kernel<<<ctx->num_sms * 8, 128, 0, st>>>(ra);
+                ctx->launches++;
+            }
+            return scatter_entries(ctx, c.data, 1.0, a.fuse != 0, st);
+        }
+        if (c.accept == 3) return scatter_entries(ctx, c.data, 1.0, false, st);   // everything, as a separate launch
+        return GB_OK;
+    }
     // launch only the classes that can occur; largest windows first
     const bool may_swap = c.mode != MODE_WAVEFORM && (c.move ? true : c.move_all == GB_SWAP);   // MODE_OVERLAP: move_all = SWAP
     const bool may_single = c.mode == MODE_WAVEFORM || (c.move ? true : c.move_all != GB_SWAP);
@@ -1123,6 +1755,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     if (c.keep) {
         ctx->kept_B = c.B;
         ctx->kept_cap = 2 * c.sum_bins;
+        ctx->kept_mode = 1;
     }
     return GB_OK;
 }
@@ -1229,7 +1862,9 @@ int gb_create(const gb_config* cfg, gb_ctx** out) {
     if ((rc = setup_kernel<N_, false, true>(ctx))) return rc;           \
     if ((rc = setup_kernel<N_, true, true>(ctx))) return rc;            \
     if ((rc = setup_kernel<N_, false, false>(ctx))) return rc;          \
-    if ((rc = setup_kernel<N_, true, false>(ctx))) return rc;
+    if ((rc = setup_kernel<N_, true, false>(ctx))) return rc;           \
+    if ((rc = setup_kernel<N_, false, true, true>(ctx))) return rc;     \
+    if ((rc = setup_kernel<N_, false, false, true>(ctx))) return rc;
     GB_SETUP(128) GB_SETUP(256) GB_SETUP(512) GB_SETUP(1024)
 #undef GB_SETUP
     return GB_OK;
@@ -1248,6 +1883,10 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_band_cache);
     cudaFree(ctx->d_temper_cache);
     cudaFree(ctx->d_wkeep);
+    cudaFree(ctx->d_wk);
+    cudaFree(ctx->d_ent);
+    cudaFree(ctx->d_accpar);
+    cudaFree(ctx->d_pieces);
     cudaFree(ctx->d_stage);
     if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
     if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
@@ -1362,11 +2001,43 @@ int gb_delta_loglike_keep(gb_ctx* ctx, const gb_data* data, const double* params
     return run_call(ctx, c, stream);
 }
 
+int gb_delta_loglike_accept(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                            const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                            int64_t B, const double* logq, const double* logu, const double* beta, int64_t store_bins,
+                            int apply, double* dlnL_out, double* aux_out, uint8_t* accepted_out, void* stream) {
+    Call c{};
+    c.mode = MODE_DLNL;
+    c.data = data;
+    c.params_new = params_new;
+    c.params_old = params_old;
+    c.walker_index = walker_index;
+    c.move = move;
+    c.move_all = move_all;
+    c.N = N;
+    c.n_bins = n_bins;
+    c.B = B;
+    c.dlnL_out = dlnL_out;
+    c.aux_out = aux_out;
+    c.sum_bins = store_bins;
+    c.logq = logq;
+    c.logu = logu;
+    c.beta = beta;
+    c.accepted_out = accepted_out;
+    if (apply < 0 || apply > 2) return set_err(ctx, GB_ERR_INVALID, "apply must be 0, 1 or 2");
+    c.accept = apply == 0 ? 1 : apply == 1 ? 2 : 3;
+    if (!move && move_all == GB_SWAP) return set_err(ctx, GB_ERR_INVALID, "gb_delta_loglike_accept takes ADD / REMOVE rows only");
+    return run_call(ctx, c, stream);
+}
+
 int gb_residual_update_kept(gb_ctx* ctx, const gb_data* data, const uint8_t* accepted, int negate, void* stream) {
     if (!ctx) return GB_ERR_INVALID;
     if (ctx->kept_B <= 0) return set_err(ctx, GB_ERR_INVALID, "no gb_delta_loglike_keep call to follow");
     if (!data || !data->resid || data->n_f <= 0 || data->n_walkers <= 0) return set_err(ctx, GB_ERR_INVALID, "NULL / empty data view");
     GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    if (ctx->kept_mode == 2) {   // after gb_delta_loglike_accept: the accepted rows are the call's own decisions
+        if (accepted) return set_err(ctx, GB_ERR_INVALID, "after gb_delta_loglike_accept `accepted` must be NULL (the call decided)");
+        return scatter_entries(ctx, data, negate ? -1.0 : 1.0, false, reinterpret_cast<cudaStream_t>(stream));
+    }
     KeptArgs a{};
     a.counts = ctx->d_counts;
     a.lists = ctx->d_lists;
@@ -1677,6 +2348,66 @@ int delta_loglike_host_impl(gb_ctx* ctx, const gb_data* data, const double* para
     return GB_OK;
 }
 
+int delta_loglike_accept_host_impl(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                                   const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                                   int64_t B, const double* logq, const double* logu, const double* beta, int64_t store_bins,
+                                   int apply, double* dlnL_out, double* aux_out, uint8_t* accepted_out, void* stream) {
+    if (!ctx) return GB_ERR_INVALID;
+    if (B < 0 || !walker_index || !dlnL_out || !logu || !accepted_out) return set_err(ctx, GB_ERR_INVALID, "bad arguments");
+    if (B == 0) return GB_OK;
+    GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+    int rc = stage_reserve(ctx, (size_t)B * (64 + 64 + 4 + 1 + 4 + 24 + 8 + 16 + 1) + 16384);
+    if (rc) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    Stager s{ctx, st, static_cast<char*>(ctx->d_stage), 0};
+    double* d_pn = params_new ? s.put<double>(nullptr, (size_t)B * 8) : nullptr;
+    double* d_po = params_old ? s.put<double>(nullptr, (size_t)B * 8) : nullptr;
+    int32_t* d_w = s.put<int32_t>(nullptr, (size_t)B);
+    int8_t* d_mv = move ? s.put<int8_t>(nullptr, (size_t)B) : nullptr;
+    int32_t* d_nb = n_bins ? s.put<int32_t>(nullptr, (size_t)B) : nullptr;
+    double* d_lq = logq ? s.put<double>(nullptr, (size_t)B) : nullptr;
+    double* d_lu = s.put<double>(nullptr, (size_t)B);
+    double* d_bt = beta ? s.put<double>(nullptr, (size_t)B) : nullptr;
+    double* d_out = s.put<double>(nullptr, (size_t)B);
+    double* d_aux = aux_out ? s.put<double>(nullptr, (size_t)B * 2) : nullptr;
+    uint8_t* d_acc = s.put<uint8_t>(nullptr, (size_t)B);
+    // chunked as gb_delta_loglike_host; a chunk's update has finished when its last kernel ends, so the next chunk reuses
+    // the store.  apply = 0 keeps the state of ONE call for gb_residual_update_kept: a single chunk then
+    const int nch = (B >= (1 << 18) && apply != 0) ? kHostChunks : 1;
+    GB_CUDA(ctx, cudaEventRecord(ctx->ev_start, st));
+    GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ctx->ev_start, 0));
+    for (int c = 0; c < nch; c++) {
+        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        if (d_pn) GB_CUDA(ctx, cudaMemcpyAsync(d_pn + 8 * lo, params_new + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_po) GB_CUDA(ctx, cudaMemcpyAsync(d_po + 8 * lo, params_old + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaMemcpyAsync(d_w + lo, walker_index + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_mv) GB_CUDA(ctx, cudaMemcpyAsync(d_mv + lo, move + lo, (size_t)n, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_nb) GB_CUDA(ctx, cudaMemcpyAsync(d_nb + lo, n_bins + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_lq) GB_CUDA(ctx, cudaMemcpyAsync(d_lq + lo, logq + lo, (size_t)n * 8, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaMemcpyAsync(d_lu + lo, logu + lo, (size_t)n * 8, cudaMemcpyHostToDevice, ctx->s_in));
+        if (d_bt) GB_CUDA(ctx, cudaMemcpyAsync(d_bt + lo, beta + lo, (size_t)n * 8, cudaMemcpyHostToDevice, ctx->s_in));
+        GB_CUDA(ctx, cudaEventRecord(ctx->ev_in[c], ctx->s_in));
+    }
+    for (int c = 0; c < nch; c++) {
+        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        GB_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_in[c], 0));
+        rc = gb_delta_loglike_accept(ctx, data, d_pn ? d_pn + 8 * lo : nullptr, d_po ? d_po + 8 * lo : nullptr, d_w + lo,
+                                     d_mv ? d_mv + lo : nullptr, move_all, N, d_nb ? d_nb + lo : nullptr, n,
+                                     d_lq ? d_lq + lo : nullptr, d_lu + lo, d_bt ? d_bt + lo : nullptr,
+                                     store_bins < 1024 * n ? store_bins : 1024 * n, apply, d_out + lo,
+                                     d_aux ? d_aux + 2 * lo : nullptr, d_acc + lo, stream);
+        if (rc) return rc;
+        GB_CUDA(ctx, cudaEventRecord(ctx->ev_done[c], st));
+        GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[c], 0));
+        GB_CUDA(ctx, cudaMemcpyAsync(dlnL_out + lo, d_out + lo, (size_t)n * 8, cudaMemcpyDeviceToHost, ctx->s_out));
+        GB_CUDA(ctx, cudaMemcpyAsync(accepted_out + lo, d_acc + lo, (size_t)n, cudaMemcpyDeviceToHost, ctx->s_out));
+        if (aux_out) GB_CUDA(ctx, cudaMemcpyAsync(aux_out + 2 * lo, d_aux + 2 * lo, (size_t)n * 16, cudaMemcpyDeviceToHost, ctx->s_out));
+    }
+    GB_CUDA(ctx, cudaStreamSynchronize(ctx->s_out));
+    GB_CUDA(ctx, cudaStreamSynchronize(st));
+    return GB_OK;
+}
+
 int residual_update_host_impl(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
                               const int32_t* walker_index, const int8_t* move, int move_all, const uint8_t* accepted,
                               int N, const int32_t* n_bins, int64_t B, void* stream) {
@@ -1732,6 +2463,15 @@ int gb_delta_loglike_host(gb_ctx* ctx, const gb_data* data, const double* params
                           int64_t B, double* dlnL_out, double* aux_out, void* stream) {
     return drain_on_error(ctx, stream, delta_loglike_host_impl(ctx, data, params_new, params_old, walker_index, move, move_all,
                                                                N, n_bins, B, dlnL_out, aux_out, stream));
+}
+
+int gb_delta_loglike_accept_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,
+                                 const int32_t* walker_index, const int8_t* move, int move_all, int N, const int32_t* n_bins,
+                                 int64_t B, const double* logq, const double* logu, const double* beta, int64_t store_bins,
+                                 int apply, double* dlnL_out, double* aux_out, uint8_t* accepted_out, void* stream) {
+    return drain_on_error(ctx, stream, delta_loglike_accept_host_impl(ctx, data, params_new, params_old, walker_index, move,
+                                                                      move_all, N, n_bins, B, logq, logu, beta, store_bins,
+                                                                      apply, dlnL_out, aux_out, accepted_out, stream));
 }
 
 int gb_residual_update_host(gb_ctx* ctx, const gb_data* data, const double* params_new, const double* params_old,

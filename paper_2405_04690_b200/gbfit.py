@@ -22,7 +22,7 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
            "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep",
-           "gb_delta_loglike_keep", "gb_residual_update_kept", "gb_band_sweep_generate")
+           "gb_delta_loglike_keep", "gb_residual_update_kept", "gb_band_sweep_generate", "gb_delta_loglike_accept", "gb_delta_loglike_accept_host")
 
 BAND_MAX_STAGE = 3072
 # layout of gb_band_task (include/gbfit.h)
@@ -155,6 +155,11 @@ def lib() -> C.CDLL:
         L.gb_overlap.restype = ci
         L.gb_delta_loglike_keep.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, i64, vp, vp, vp]
         L.gb_delta_loglike_keep.restype = ci
+        L.gb_delta_loglike_accept.argtypes = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, ci, vp, i64, vp, vp, vp, i64, ci, vp,
+                                              vp, vp, vp]
+        L.gb_delta_loglike_accept.restype = ci
+        L.gb_delta_loglike_accept_host.argtypes = L.gb_delta_loglike_accept.argtypes
+        L.gb_delta_loglike_accept_host.restype = ci
         L.gb_residual_update_kept.argtypes = [vp, C.POINTER(GbData), vp, ci, vp]
         L.gb_residual_update_kept.restype = ci
         L.gb_temper_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -384,6 +389,35 @@ class Context:
                                              _dev_ptr(aux, torch.float64, dev, "aux"), _stream_ptr(stream, dev)))
         return out
 
+    def delta_loglike_accept(self, data: Data, params_new: Optional[torch.Tensor], params_old: Optional[torch.Tensor],
+                             walker_index: torch.Tensor, logu: torch.Tensor, logq: Optional[torch.Tensor] = None,
+                             beta: Optional[torch.Tensor] = None, move: Optional[torch.Tensor] = None, move_all: int = ADD,
+                             N: int = 0, n_bins: Optional[torch.Tensor] = None, store_bins: int = 0, apply: int = 1,
+                             out: Optional[torch.Tensor] = None, aux: Optional[torch.Tensor] = None,
+                             accepted_out: Optional[torch.Tensor] = None, stream=None):
+        """gb_delta_loglike_accept: delta lnL of every ADD / REMOVE row against one snapshot, accepted iff
+        beta dlnL + logq >= logu, then (apply 1: fused, 2: separate launch) the update by the accepted rows;
+        apply 0 keeps the accepted windows for residual_update_kept(data, None).  Returns (dlnL, accepted uint8)."""
+        dev = self.device
+        B = int(walker_index.shape[0])
+        if out is None:
+            out = torch.empty((B,), dtype=torch.float64, device=dev)
+        if accepted_out is None:
+            accepted_out = torch.zeros((B,), dtype=torch.uint8, device=dev)
+        self._ok(lib().gb_delta_loglike_accept(self._h, data.c(), _dev_ptr(params_new, torch.float64, dev, "params_new"),
+                                               _dev_ptr(params_old, torch.float64, dev, "params_old"),
+                                               _dev_ptr(walker_index, torch.int32, dev, "walker_index"),
+                                               _dev_ptr(move, torch.int8, dev, "move"), int(move_all), int(N),
+                                               _dev_ptr(n_bins, torch.int32, dev, "n_bins"), B,
+                                               _dev_ptr(logq, torch.float64, dev, "logq"),
+                                               _dev_ptr(logu, torch.float64, dev, "logu"),
+                                               _dev_ptr(beta, torch.float64, dev, "beta"), int(store_bins), int(apply),
+                                               _dev_ptr(out, torch.float64, dev, "out"),
+                                               _dev_ptr(aux, torch.float64, dev, "aux"),
+                                               _dev_ptr(accepted_out, torch.uint8, dev, "accepted_out"),
+                                               _stream_ptr(stream, dev)))
+        return out, accepted_out
+
     def residual_update_kept(self, data: Data, accepted: Optional[torch.Tensor] = None, negate: bool = False,
                              stream=None) -> None:
         """gb_residual_update_kept: scatter the accepted rows of the preceding delta_loglike_keep call."""
@@ -527,6 +561,30 @@ class Context:
         self._ok(lib().gb_delta_loglike_host(self._h, data.c(), pn, po, w, mv, int(move_all), int(N), nb, B, o, ax,
                                              _stream_ptr(stream, self.device)))
         return k5
+
+    def delta_loglike_accept_host(self, data: Data, params_new, params_old, walker_index, logu, logq=None, beta=None,
+                                  move=None, move_all: int = ADD, N: int = 0, n_bins=None, store_bins: int = 0, apply: int = 1,
+                                  out=None, accepted_out=None, stream=None):
+        """gb_delta_loglike_accept_host: HOST proposal arrays in, HOST (dlnL, accepted) out; `data` stays on the device."""
+        pn, k0 = _host_ptr(params_new, np.float64, "params_new")
+        po, k1 = _host_ptr(params_old, np.float64, "params_old")
+        w, k2 = _host_ptr(walker_index, np.int32, "walker_index")
+        B = int(k2.shape[0])
+        mv, k3 = _host_ptr(move, np.int8, "move")
+        nb, k4 = _host_ptr(n_bins, np.int32, "n_bins")
+        lu, k5 = _host_ptr(logu, np.float64, "logu")
+        lq, k6 = _host_ptr(logq, np.float64, "logq")
+        bt, k7 = _host_ptr(beta, np.float64, "beta")
+        if out is None:
+            out = np.zeros((B,), np.float64)
+        if accepted_out is None:
+            accepted_out = np.zeros((B,), np.uint8)
+        o, k8 = _host_ptr(out, np.float64, "out")
+        a, k9 = _host_ptr(accepted_out, np.uint8, "accepted_out")
+        self._ok(lib().gb_delta_loglike_accept_host(self._h, data.c(), pn, po, w, mv, int(move_all), int(N), nb, B, lq, lu, bt,
+                                                    int(store_bins), int(apply), o, None, a,
+                                                    _stream_ptr(stream, self.device)))
+        return k8, k9
 
     def residual_update_host(self, data: Data, params_new, params_old, walker_index, move=None,
                              move_all: int = ADD, accepted=None, N: int = 0, n_bins=None, stream=None) -> None:

@@ -277,6 +277,54 @@ def test_p6_swap_identities(oracle):
         oracle.residual_update(cfg, data, wl.params_old[one], new[one], wl.walker_index[one], move_all=oracle.SWAP, N=512)
 
 
+def test_delta_loglike_accept_is_snapshot_evaluation_then_update(oracle):
+    """gbo_delta_loglike_accept (the batched sweep step): (1) every row is evaluated against the SAME snapshot -- a row
+    duplicated in the batch gets the same delta lnL twice although the first copy is accepted; (2) with sources whose
+    windows do not overlap, lnL(after) - lnL(before) from the definition -1/2 <r|r> (numpy, whole band) is the sum of the
+    accepted delta lnL, and rejected rows leave no trace; (3) beta = 0 decides on logq >= logu alone, logu = -inf accepts
+    everything, +inf nothing (residual bit-identical); (4) apply = False decides but does not touch the residual."""
+    cfg = oracle.Config()
+    wl = make_workload(3, B=48, n_walkers=2)
+    data = _small_data(oracle, wl, 2)
+    before = data.resid.copy()
+    pn = wl.params_new.copy()
+    # well separated windows: one source every 3000 bins, ADD rows
+    pn[:, 1] = (wl.k_lo + 4000 + 3000 * np.arange(wl.B)) / cfg.Tobs
+    nb = np.full(wl.B, 256, np.int32)
+    w = wl.walker_index
+    g = np.random.Generator(np.random.Philox(key=[24, 5]))
+    logu = np.log(g.random(wl.B))
+    logq = 0.3 * g.standard_normal(wl.B)
+    beta = np.where(np.arange(wl.B) % 2 == 0, 1.0, 0.5)
+    d0 = oracle.delta_loglike(cfg, data, pn, None, w, move_all=oracle.ADD, n_bins=nb)
+    dl, acc = oracle.delta_loglike_accept(cfg, data, pn, None, w, logu, logq=logq, beta=beta, move_all=oracle.ADD, n_bins=nb)
+    assert np.array_equal(dl, d0) and 0 < acc.sum() < wl.B
+    for ww in range(2):
+        psd_row = wl.psd[wl.psd_row_of(ww)]
+        diff = _lnl_direct(cfg, data.resid[ww], psd_row) - _lnl_direct(cfg, before[ww], psd_row)
+        assert abs(diff - dl[(w == ww) & (acc != 0)].sum()) < 1e-6
+    # every accepted row obeys Eq. 13 in log form; flipping one term of it would change some decision below
+    for b in range(wl.B):
+        assert bool(acc[b]) == (beta[b] * dl[b] + logq[b] >= logu[b])
+    assert (acc != (dl >= logu)).any() and (acc != (dl + logq >= logu)).any()      # beta and logq both matter here
+    # (1) snapshot: duplicate rows
+    data = oracle.Data(before.copy(), wl.psd[:2], wl.k_lo)
+    dup = np.concatenate([pn[:4], pn[:4]])
+    dl2, acc2 = oracle.delta_loglike_accept(cfg, data, dup, None, np.concatenate([w[:4], w[:4]]), np.full(8, -np.inf),
+                                            move_all=oracle.ADD, n_bins=nb[:8])
+    assert np.array_equal(dl2[:4], dl2[4:]) and acc2.all()
+    ref = oracle.Data(before.copy(), wl.psd[:2], wl.k_lo)
+    oracle.residual_update(cfg, ref, dup, None, np.concatenate([w[:4], w[:4]]), move_all=oracle.ADD, n_bins=nb[:8])
+    assert np.array_equal(data.resid, ref.resid)
+    # (3), (4)
+    data = oracle.Data(before.copy(), wl.psd[:2], wl.k_lo)
+    _, a0 = oracle.delta_loglike_accept(cfg, data, pn, None, w, logu, logq=logq, beta=np.zeros(wl.B), move_all=oracle.ADD, n_bins=nb,
+                                        apply=False)
+    assert np.array_equal(a0 != 0, logq >= logu) and np.array_equal(data.resid, before)
+    _, a1 = oracle.delta_loglike_accept(cfg, data, pn, None, w, np.full(wl.B, np.inf), move_all=oracle.ADD, n_bins=nb)
+    assert not a1.any() and np.array_equal(data.resid, before)
+
+
 def test_residual_update_signs_and_band_edges(oracle):
     """ADD subtracts the waveform, REMOVE adds it; bins outside the stored band are skipped (reading S13)."""
     cfg = oracle.Config()
