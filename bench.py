@@ -140,10 +140,26 @@ def oracle_step(orc, ocfg, odata, sub, sub_w, sign_add: bool, nthreads: int):
                             n_bins=sub.n_bins, nthreads=nthreads)
 
 
-def oracle_sample(wl, n_walkers_sample: int, rows=None):
-    """Rows of the first n_walkers_sample walkers of config 5 with their residuals (host)."""
+ORACLE_WALKERS = 16          # walkers in every oracle sample: gbo_residual_update parallelises over walkers
+
+
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_sample(wl, rows_per_walker: int, rows=None, n_walkers_sample: int = ORACLE_WALKERS):
+    """The first rows_per_walker sources of each of the first n_walkers_sample walkers of config 5, with those walkers'
+    residuals (host).  Both oracle timings (cpu_baseline and --impl reference) draw their rows this way."""
+    n_walkers_sample = min(n_walkers_sample, wl.n_walkers)
     per = wl.B // wl.n_walkers
-    idx = np.arange(n_walkers_sample * per)
+    rows_per_walker = min(rows_per_walker, per)
+    idx = (np.arange(n_walkers_sample)[:, None] * per + np.arange(rows_per_walker)[None, :]).reshape(-1)
     sub = wl.subset(idx)
     resid = np.stack([wl.resid_row(w) if rows is None else rows[w] for w in range(n_walkers_sample)])
     sub_w = sub.walker_index.astype(np.int32)
@@ -161,7 +177,7 @@ def run_reference(args):
     orc.build()
     cores = orc.max_threads()
     wl = make_workload(5, n_walkers=360, per_walker=12000, B=None)
-    sub, sub_w, resid, psd_map = oracle_sample(wl, 1)
+    sub, sub_w, resid, psd_map = oracle_sample(wl, 2048)
     ocfg = orc.Config()
     odata = orc.Data(resid, wl.psd, wl.k_lo, walker_psd=psd_map)
     for i in range(args.warmup):
@@ -171,8 +187,8 @@ def run_reference(args):
         oracle_step(orc, ocfg, odata, sub, sub_w, (args.warmup + i) % 2 == 0, cores)
     dt = time.perf_counter() - t0
     value = sub.B * args.steps / dt
-    sample = (f"{sub.B} rows per step = all 12000 sources of walker 0 of config 5 (delta lnL of every row + update of "
-              f"the accepted 25 %)")
+    sample = (f"{sub.B} rows per step = the first 2048 sources of each of walkers 0..{ORACLE_WALKERS - 1} of config 5 "
+              f"(delta lnL of every row + update of the accepted 25 %); {cpu_model()}")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -212,7 +228,7 @@ def run_ours(args):
 
     # ---- residuals: generated row by row on the host (seeded), uploaded once; they live on the GPU
     d_resid = torch.empty((wl.n_walkers, 2, wl.n_f), dtype=torch.complex128, device=dev)
-    n_keep = min(4, wl.n_walkers)
+    n_keep = min(ORACLE_WALKERS, wl.n_walkers)      # host copies of the first rows: the oracle sample's residuals
     keep = {}
     stage = [torch.empty((2, wl.n_f), dtype=torch.complex128).pin_memory() for _ in range(2)]
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
@@ -419,6 +435,25 @@ def run_ours(args):
         torch.cuda.synchronize()
         ctx.check()
         ms_band_oe = b0.elapsed_time(b1) / reps
+        # row f1 as printed: the proposal step inside the kernel (Philox, randint, group stretch from a
+        # 7.1 M-row friends table, Eq. 14), from the current theta_k
+        from gb_inputs import make_stretch_inputs
+        si = make_stretch_inputs(bt, n_copies=12, n_friends=24)
+        sg = gbfit.Stretch(si.seed, si.sweep, torch.from_numpy(si.group).to(dev), si.n_friends, si.lo, si.hi, si.periodic,
+                           si.stretch_a)
+        for i in range(reps + 1):
+            d_bp.copy_(d_bp0)
+            if i == 1:
+                b0.record(stream)
+            g_out = ctx.band_sweep_generate(data, d_tasks, 256, bt.max_stage, d_bp, sg, bt.prop_k.size)
+        b1.record(stream)
+        torch.cuda.synchronize()
+        ctx.check()
+        ms_band_gen = b0.elapsed_time(b1) / reps
+        gen_eval = float(torch.isfinite(g_out[1]).float().mean().item())
+        # waveforms actually generated by a call: one per proposal plus the fill of the current-source cache (n_src per task)
+        n_wave_band = bt.prop_k.size + int(bt.tasks["n_src"].sum())
+        flops_band = n_wave_band * (711.0 * 256 + 10.0 * 256 * 8) + bt.prop_k.size * 60.0 * 256
         band = {"call": "gb_band_sweep (Algorithm 1)", "N": 256, "tasks": int(len(bt.tasks["walker"])),
                 "sources_per_band": 9, "proposals_per_band": 30, "proposals": int(bt.prop_k.size),
                 "ms_per_call": ms_band, "proposals_per_s": bt.prop_k.size / (ms_band * 1e-3),
@@ -426,11 +461,18 @@ def run_ours(args):
                 "odd_even_buffers": {"ms_per_call": ms_band_oe, "proposals_per_s": bt.prop_k.size / (ms_band_oe * 1e-3),
                                      "note": "GB_BAND_SUBTRACT_CURRENT | GB_BAND_WRITE_OTHER: residual rows needed per "
                                              "walker 2 instead of n_t (72 rows = 2.2 GB instead of 360 = 10.8 GB here)"},
-                # nominal work of a swap evaluation: 2 (711 N + 10 N log2 N) + 60 N flop
-                "alu_frac": bt.prop_k.size * (2 * (711 * 256 + 10 * 256 * 8) + 60 * 256) / (ms_band * 1e-3) / 1e12
-                            / FP64_PEAK_TFLOPS,
-                "note": "each proposal = 2 waveforms + Eq. 5 against the staged residual + accept/reject + update; "
-                        "includes the device-side reset of the 38 MB parameter array before each call"}
+                "generate": {"call": "gb_band_sweep_generate (proposal step inside the kernel: Philox4x32-10, randint, group "
+                                     "stretch from the friends table, Eq. 14, prior box)",
+                             "ms_per_call": ms_band_gen, "proposals_per_s": bt.prop_k.size / (ms_band_gen * 1e-3),
+                             "friends_table_rows": int(si.group.shape[0]), "n_friends": int(si.n_friends),
+                             "evaluated_fraction": gen_eval,
+                             "accepted_fraction_last_call": float(g_out[0].float().mean().item())},
+                # billed by the waveforms a call really generates (the current-source cache makes it one per proposal plus
+                # the fill): n_wave (711 N + 10 N log2 N) + 60 N per proposal
+                "waveforms_per_call": n_wave_band,
+                "alu_frac": flops_band / (ms_band * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                "note": "each proposal = 1 new waveform (the old one comes from the L2-resident cache) + Eq. 5 against the staged "
+                        "residual + accept/reject + update; includes the device-side reset of the 38 MB parameter array"}
 
     # ---- the same sweep as the gb_delta_loglike_keep + gb_residual_update_kept pair (outside the timed step unless
     #      --kept-update): the accepted waveforms are not generated a second time
@@ -511,6 +553,7 @@ def run_ours(args):
         tmp = {"call": "gb_temper_sweep (Algorithm 2, Eq. D2)", "N": 256, "ladders": int(len(tt.tasks["n_t"])), "chains": 10,
                "swap_proposals": n_pairs_t, "waveforms_per_call": n_wave, "ms_per_call": ms_t,
                "swap_proposals_per_s": n_pairs_t / (ms_t * 1e-3), "waveforms_per_s": n_wave / (ms_t * 1e-3),
+               "alu_frac": n_wave * (711.0 * 256 + 10.0 * 256 * 8) / (ms_t * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
                "accepted_fraction_last_call": float(t_acc.float().sum().item()) / n_pairs_t}
 
     # ---- SURVEY 8(f) row f4, outside the timed step: normalised overlaps of 1 M source pairs (gb_overlap) ----
@@ -596,20 +639,23 @@ def run_ours(args):
         from oracle import gb_oracle as orc
         orc.build()
         cores = orc.max_threads()
-        sub, sub_w, resid, psd_map = oracle_sample(wl, n_keep, keep)
+        # a 131 072-source subsample (8192 sources of each of 16 walkers), one untimed warm-up step
+        sub, sub_w, resid, psd_map = oracle_sample(wl, 8192, keep, n_keep)
         odata = orc.Data(resid, wl.psd, wl.k_lo, walker_psd=psd_map)
-        t0 = time.perf_counter()
         oracle_step(orc, orc.Config(), odata, sub, sub_w, True, cores)
+        t0 = time.perf_counter()
+        oracle_step(orc, orc.Config(), odata, sub, sub_w, False, cores)
         dt = time.perf_counter() - t0
         # spot parity of the GPU output on the sample (evaluated after the timed loops, on residuals that
         # differ from the initial ones only by the rounding of the +/- scatter pairs)
         ref = orc.delta_loglike(orc.Config(), orc.Data(np.stack([keep[w] for w in range(n_keep)]), wl.psd, wl.k_lo,
                                                        walker_psd=psd_map),
-                                sub.params_new[:2048], None, sub_w[:2048], n_bins=sub.n_bins[:2048], nthreads=cores)
+                                wl.params_new[:2048], None, wl.walker_index[:2048].astype(np.int32), n_bins=wl.n_bins[:2048],
+                                nthreads=cores)
         spot = float(np.abs(spot_out - ref).max())
-        cpu = {"value": sub.B / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{sub.B} rows = all sources of walkers 0..{n_keep - 1} of the same workload, one step "
-                         f"(delta lnL + update of accepted rows), {dt:.1f} s wall",
+        cpu = {"value": sub.B / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "cpu": cpu_model(),
+               "sample": f"{sub.B} rows = the first 8192 sources of each of walkers 0..{n_keep - 1} of the same workload, one "
+                         f"step (delta lnL + update of accepted rows) after one warm-up step, {dt:.1f} s wall",
                "spot_parity_max_abs_dlnL_err": spot}
 
     if rank == 0:

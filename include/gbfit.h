@@ -350,17 +350,30 @@ int gb_band_sweep_generate(gb_ctx *ctx, const gb_data *data, const gb_band_task 
  * D_j = lnL_j(S_i) - lnL_j(S_j) = -1/2 <delta|delta>_j + <r_j|delta>_j  (each chain's own PSD row), accepted iff
  * beta_i D_i + beta_j D_j >= logu.  Accepted: the holders are exchanged and, if write_back, r_i += delta, r_j -= delta in
  * data->resid (FP64 atomics; the paper keeps only the cold chain's residual, here every chain owns one).
- * Ladders of up to 16 chains sum each chain's set once into context-owned scratch (allocated at the first call, <= 350 MB).
+ * Ladders of up to 32 chains sum each chain's set once into context-owned scratch (allocated at the first call, <= 700 MB).
  * Outputs [n_chain]: perm_out[c] = ladder position whose INITIAL set ends in chain t; accepted_out[c]; dlnl_out[c][2] =
  * (D_i, D_j) of pair (t, t-1).  All arrays DEVICE.  N, max_stage, odd/even rule, errors and asynchrony as gb_band_sweep.
+ *
+ * Odd/even cold-chain buffers (Algorithm 2 as printed): with GB_TEMPER_ODD_EVEN the
+ * row of a chain's walker is the opposite-parity cold-chain buffer, which holds none of the band's own sources, so the
+ * kernel forms each chain's residual on chip, r_t = row(chain_walker[t]) - sum_{S_t} h over the set the chain holds
+ * (PAPER.md:626-631), and only an exchange with the cold chain (pair (1, 0)) is written: -delta into
+ * row write_walker, the cold chain's buffer of the band's own parity.  Ladders of up to GB_TEMPER_MAX_LADDER_ODD_EVEN
+ * chains (a longer one is a row error).  This is the mode that composes with gb_band_sweep's GB_BAND_SUBTRACT_CURRENT /
+ * GB_BAND_WRITE_OTHER: both then work on the 2 x n_walkers rows of the odd/even layout.
  */
 #define GB_TEMPER_MAX_LADDER 64
+#define GB_TEMPER_MAX_LADDER_ODD_EVEN 32
+#define GB_TEMPER_WRITE_BACK 1   /* accepted exchanges update data->resid                                           */
+#define GB_TEMPER_ODD_EVEN 2     /* rows hold none of the band's sources; write only the cold chain, to write_walker */
 typedef struct {
     int32_t n_t;          /* chains of the ladder                    */
     int32_t chain_begin;  /* first chain entry of the task           */
     int32_t n_stage;      /* staged bins                             */
-    int32_t write_back;   /* != 0: accepted exchanges update data->resid */
+    int32_t write_back;   /* GB_TEMPER_WRITE_BACK | GB_TEMPER_ODD_EVEN */
     int64_t k_first;      /* global bin of staged bin 0              */
+    int32_t write_walker; /* GB_TEMPER_ODD_EVEN: row that receives exchanges with the cold chain */
+    int32_t reserved;     /* set to 0                                */
 } gb_temper_task;
 int gb_temper_sweep(gb_ctx *ctx, const gb_data *data, const gb_temper_task *tasks, int64_t n_tasks, int N, int max_stage,
                     const double *params, const int32_t *chain_walker, const double *chain_beta,

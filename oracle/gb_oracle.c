@@ -721,9 +721,16 @@ int gbo_band_sweep_generate(const gbo_config *c, gbo_data *d, const gbo_band_tas
  * chain whose write_back flag is set (the paper stores only the cold chain, :652-658; here every chain owns a
  * residual), and the next pair sees the new holder of chain t-1.  Outputs per chain entry t: accepted[t] and
  * dlnl[t] = (D_i, D_j) of the pair (t, t-1) (entry 0 unused), perm[t] = the chain whose INITIAL set ends in t. */
+/* Odd/even cold-chain buffers (Algorithm 2 as printed): with bit 2 of write_back the
+ * stored row of a chain's walker holds NONE of the band's own sources (it is the opposite-parity cold-chain buffer, which
+ * carries only the leakage of the neighbours), so each chain's residual is formed first, r_t = row(p[t]) - sum_{S_t} h
+ * over the set the chain holds ("r' <- r_(0,w,b-1) + r_(0,w,b+1) - sum h"), and only an exchange with the
+ * cold chain (t - 1 = 0) is written, as -delta into row write_walker, the cold chain's buffer of the band's own parity
+ * ("if t = 1 ... update cold-chain residual").                                                        */
 typedef struct {
-    int32_t n_t, chain_begin, n_stage, write_back;
+    int32_t n_t, chain_begin, n_stage, write_back;   /* write_back: bit 1 = write accepted exchanges, bit 2 = odd/even mode */
     int64_t k_first;
+    int32_t write_walker, reserved;
 } gbo_temper_task;
 
 int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *tasks, int64_t n_tasks, int N,
@@ -738,18 +745,22 @@ int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *ta
         int64_t hi = t->k_first + t->n_stage < d->k_lo + d->n_f ? t->k_first + t->n_stage : d->k_lo + d->n_f;
         int64_t n = hi > lo ? hi - lo : 0;
         double complex *dl = (double complex *)malloc(sizeof(double complex) * 2 * (size_t)(n > 0 ? n : 1));
+        double complex *hs = (double complex *)malloc(sizeof(double complex) * 4 * (size_t)(n > 0 ? n : 1));   /* H_i, H_j */
+        const int oddeven = (t->write_back & 2) != 0;
         int *holder = (int *)malloc(sizeof(int) * (size_t)(t->n_t > 0 ? t->n_t : 1));   /* whose initial set chain t holds */
         for (int q = 0; q < t->n_t; q++) { holder[q] = q; perm_out[t->chain_begin + q] = q; accepted_out[t->chain_begin + q] = 0;
                                            dlnl_out[2 * (t->chain_begin + q)] = dlnl_out[2 * (t->chain_begin + q) + 1] = 0.0; }
         for (int q = t->n_t - 1; q >= 1; q--) {
             int ci = t->chain_begin + q, cj = ci - 1;
             int wi = chain_walker[ci], wj = chain_walker[cj];
-            if (wi < 0 || wi >= d->n_walkers || wj < 0 || wj >= d->n_walkers) { free(dl); free(holder); free(hA); return GBO_ERR_INVALID; }
+            if (wi < 0 || wi >= d->n_walkers || wj < 0 || wj >= d->n_walkers) { free(dl); free(hs); free(holder); free(hA); return GBO_ERR_INVALID; }
             /* delta = sum over the set chain i holds - sum over the set chain j holds, on the staged stored bins */
             for (int64_t x = 0; x < 2 * n; x++) dl[x] = 0.0;
+            for (int64_t x = 0; x < 4 * n; x++) hs[x] = 0.0;
             for (int side = 0; side < 2; side++) {
                 int src = t->chain_begin + holder[side == 0 ? q : q - 1];
                 double sign = side == 0 ? +1.0 : -1.0;
+                double complex *H = hs + (size_t)side * 2 * n;          /* the sum of the set this chain holds */
                 for (int sidx = 0; sidx < chain_set_n[src]; sidx++) {
                     int64_t kh;
                     gbo_waveform(c, params + 8 * ((size_t)chain_set_begin[src] + sidx), N, hA, hE, &kh);
@@ -758,6 +769,8 @@ int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *ta
                         if (k < lo || k >= hi) continue;
                         dl[k - lo] += sign * (hA[2 * jb] + I * hA[2 * jb + 1]);
                         dl[n + k - lo] += sign * (hE[2 * jb] + I * hE[2 * jb + 1]);
+                        H[k - lo] += hA[2 * jb] + I * hA[2 * jb + 1];
+                        H[n + k - lo] += hE[2 * jb] + I * hE[2 * jb + 1];
                     }
                 }
             }
@@ -770,6 +783,7 @@ int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *ta
                     const double *S = d->psd + ((size_t)row * 2 + (size_t)ch) * (size_t)d->n_f + (lo - d->k_lo);
                     for (int64_t x = 0; x < n; x++) {
                         double complex de = dl[(size_t)ch * n + x], rr = r[2 * x] + I * r[2 * x + 1];
+                        if (oddeven) rr -= hs[(size_t)side * 2 * n + (size_t)ch * n + x];   /* r_t = row - sum_{S_t} h */
                         double wgt = d->psd_is_inverse ? S[x] : 1.0 / S[x];
                         dd += wgt * creal(conj(de) * de);
                         rd += wgt * creal(conj(rr) * de);
@@ -783,7 +797,18 @@ int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *ta
             dlnl_out[2 * ci] = D[0]; dlnl_out[2 * ci + 1] = D[1];
             if (acc) {
                 int tmp = holder[q]; holder[q] = holder[q - 1]; holder[q - 1] = tmp;
-                if (t->write_back) {
+                if (oddeven) {
+                    if ((t->write_back & 1) && q - 1 == 0) {       /* the cold chain now holds S_i: its own-parity buffer -= delta */
+                        if (t->write_walker < 0 || t->write_walker >= d->n_walkers) { free(dl); free(hs); free(holder); free(hA); return GBO_ERR_INVALID; }
+                        for (int ch = 0; ch < 2; ch++) {
+                            double *rw = (double *)resid_ch(d, t->write_walker, ch) + 2 * (lo - d->k_lo);
+                            for (int64_t x = 0; x < n; x++) {
+                                double complex de = dl[(size_t)ch * n + x];
+                                rw[2 * x] -= creal(de); rw[2 * x + 1] -= cimag(de);
+                            }
+                        }
+                    }
+                } else if (t->write_back & 1) {
                     for (int ch = 0; ch < 2; ch++) {
                         double *ri = (double *)resid_ch(d, wi, ch) + 2 * (lo - d->k_lo);
                         double *rj = (double *)resid_ch(d, wj, ch) + 2 * (lo - d->k_lo);
@@ -797,7 +822,7 @@ int gbo_temper_sweep(const gbo_config *c, gbo_data *d, const gbo_temper_task *ta
             }
         }
         for (int q = 0; q < t->n_t; q++) perm_out[t->chain_begin + q] = holder[q];
-        free(dl); free(holder);
+        free(dl); free(hs); free(holder);
     }
     free(hA);
     return GBO_OK;

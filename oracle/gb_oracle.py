@@ -343,18 +343,23 @@ def band_sweep_generate(cfg: Config, data: Data, tasks: dict, N: int, params, st
 
 
 _TEMPER_TASK = np.dtype([("n_t", np.int32), ("chain_begin", np.int32), ("n_stage", np.int32), ("write_back", np.int32),
-                         ("k_first", np.int64)], align=True)
+                         ("k_first", np.int64), ("write_walker", np.int32), ("reserved", np.int32)], align=True)
 
 
 def temper_sweep(cfg: Config, data: Data, tasks: dict, N: int, params, chain_walker, chain_beta, chain_set_begin,
                  chain_set_n, chain_logu):
     """Algorithm 2 with Eq. D2, task after task.  `tasks`: dict of equal-length arrays n_t, chain_begin,
-    n_stage, write_back, k_first.  data.resid is updated in place.
+    n_stage, write_back, k_first; an optional write_walker column selects the odd/even cold-chain buffer mode (every
+    chain's residual is formed as its walker's row minus the set it holds; only exchanges with the cold chain are written,
+    into row write_walker).  data.resid is updated in place.
     Returns (perm[n_chain] int32, accepted[n_chain] uint8, dlnl[n_chain, 2])."""
     n = len(tasks["n_t"])
     t = np.zeros(n, _TEMPER_TASK)
     for key in ("n_t", "chain_begin", "n_stage", "write_back", "k_first"):
         t[key] = tasks[key]
+    if "write_walker" in tasks:          # odd/even cold-chain buffers (PAPER.md:354-362): bit 2 of write_back + the cold row
+        t["write_back"] = (np.asarray(tasks["write_back"]) != 0).astype(np.int32) | 2
+        t["write_walker"] = tasks["write_walker"]
     p = _f64(params)
     cw = np.ascontiguousarray(chain_walker, dtype=np.int32)
     sb = np.ascontiguousarray(chain_set_begin, dtype=np.int32)

@@ -72,16 +72,31 @@ __device__ __forceinline__ int32_t randint32(uint32_t w, int32_t n) { return (in
 // First row s of the run of nf consecutive rows of the f0-sorted friends table that lie closest to f: the first s in
 // [0, n_group - nf] at which trading row s for row s + nf would not bring the run closer,
 //     P(s) = (f - g[s] > g[s + nf] - f)   is true below the answer and false from it on (g ascending),
-// found by a 32-ary search of one warp (each lane probes one row per step; ~5 dependent L2 round trips for 10^7 rows
-// instead of 23 for a bisection by one thread).  All 32 lanes of the warp must call it; all return the answer.
+// found by a 32-ary search of one warp (each lane probes one row per step).  [hlo, hhi] is a HINT where the answer
+// probably lies (the friends of a band's sources sit next to each other): the first step probes both of its ends, and
+// the search leaves the hint whenever P says so, so the result is that of the full search whatever the hint was.
+// All 32 lanes of the warp must call it; all return the answer.
 __device__ __forceinline__ int64_t friend_run_start(const double* __restrict__ group, int64_t n_group, int64_t nf, double f,
-                                                    int lane) {
-    int64_t lo = 0, hi = n_group - nf;   // the answer lies in [lo, hi]
+                                                    int lane, int64_t hlo, int64_t hhi) {
+    const int64_t smax = n_group - nf;
+    auto P = [&](int64_t p) { return (f - __ldg(group + 8 * p + 1)) > (__ldg(group + 8 * (p + nf) + 1) - f); };
+    int64_t lo = 0, hi = smax;   // the answer lies in [lo, hi]
+    if (hlo > 0 || hhi < smax) {
+        const int64_t span = hhi - hlo;
+        const int64_t p = hlo + (span * lane) / 31;                     // lane 0: hlo, lane 31: hhi
+        const bool pred = p < smax ? P(p) : false;                      // (P(smax) counts as false: the answer is <= smax)
+        const int c = __popc(__ballot_sync(0xffffffffu, pred));
+        if (c == 0) hi = hlo;                                           // P(hlo) false: at or below the hint
+        else if (c == 32) lo = hhi + 1;                                 // P(hhi) true: above the hint
+        else {
+            lo = hlo + (span * (c - 1)) / 31 + 1;
+            hi = hlo + (span * c) / 31;
+        }
+    }
     while (hi > lo) {
         const int64_t span = hi - lo;
         const int64_t p = lo + (span * lane) / 32;                       // lo <= p < hi, non-decreasing in lane
-        const bool pred = (f - __ldg(group + 8 * p + 1)) > (__ldg(group + 8 * (p + nf) + 1) - f);
-        const int c = __popc(__ballot_sync(0xffffffffu, pred));         // lanes [0, c) are below the answer
+        const int c = __popc(__ballot_sync(0xffffffffu, P(p)));         // lanes [0, c) are below the answer
         const int64_t nlo = c == 0 ? lo : lo + (span * (c - 1)) / 32 + 1;
         const int64_t nhi = c == 32 ? hi : lo + (span * c) / 32;
         lo = nlo;
@@ -214,6 +229,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         }
 
         // ---- the proposals of the band, in order
+        int64_t hint_lo = 0, hint_hi = a.gen ? a.st.n_group - min((int64_t)a.st.n_friends, a.st.n_group) : 0;   // friends search hint
         for (int p = 0; p < t.n_prop; p++) {
             const int64_t ip = (int64_t)t.prop_begin + p;
             int k;
@@ -232,7 +248,10 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
                     const double* th = a.params + 8 * ((size_t)t.src_begin + kk);
                     const int64_t nf = a.st.n_friends < a.st.n_group ? a.st.n_friends : a.st.n_group;
                     const int32_t jf = randint32(w0[1], (int32_t)nf);
-                    const int64_t row = friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid) + jf;
+                    const int64_t s0 = friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid, hint_lo, hint_hi);
+                    hint_lo = max((int64_t)0, s0 - 512);                  // the next proposal of this band lands nearby
+                    hint_hi = min(a.st.n_group - nf, s0 + 512);
+                    const int64_t row = s0 + jf;
                     const double ua = uniform52(w0[2], w0[3]);
                     const double tz = __dadd_rn(__dmul_rn(__dadd_rn(a.st.stretch_a, -1.0), ua), 1.0);
                     const double z = __ddiv_rn(__dmul_rn(tz, tz), a.st.stretch_a);    // g(z) ~ z^(-1/2) on [1/a, a]

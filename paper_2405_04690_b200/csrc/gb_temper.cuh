@@ -41,7 +41,7 @@ struct TemperArgs {
 // SUM of its windows on the staged bins is ever needed.  Ladders of at most this many chains compute every chain's sum
 // once into a per-CTA scratch area in global memory (L2 / HBM) and form delta = H_i - H_j from there: 95 instead of 171
 // waveforms for a ladder of 10 chains with 9-10 sources each.
-constexpr int kTemperCacheChains = 16;
+constexpr int kTemperCacheChains = 32;
 
 template <int N>
 constexpr size_t temper_smem_bytes(int max_stage) {
@@ -69,7 +69,13 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a
 
     for (int64_t it = blockIdx.x; it < a.n_tasks; it += gridDim.x) {
         const gb_temper_task t = a.tasks[it];
+        // odd/even cold-chain buffers (Alg. 2 as printed): every chain's residual is its walker's row minus
+        // the set it holds (formed below from the set sums); only an exchange with the cold chain is written, to write_walker
+        const bool oddeven = (t.write_back & GB_TEMPER_ODD_EVEN) != 0;
+        const bool wb = (t.write_back & GB_TEMPER_WRITE_BACK) != 0;
         bool ok = t.n_t >= 0 && t.n_t <= kMaxLadder && t.n_stage >= 0 && t.n_stage <= a.max_stage;
+        if (oddeven) ok = ok && t.n_t <= kTemperCacheChains && a.cache != nullptr &&
+                          (!wb || (t.write_walker >= 0 && t.write_walker < a.n_walkers));
         for (int q = 0; ok && q < t.n_t; q++) {
             const int w = a.chain_walker[t.chain_begin + q];
             ok = w >= 0 && w < a.n_walkers && a.chain_set_n[t.chain_begin + q] >= 0;
@@ -130,7 +136,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a
             cta_sync<G>();
         };
         cx* cache = a.cache ? a.cache + (size_t)blockIdx.x * kTemperCacheChains * 2 * a.max_stage : nullptr;
-        const bool cached = cache != nullptr && t.n_t <= kTemperCacheChains && t.n_t > 2;
+        const bool cached = cache != nullptr && t.n_t <= kTemperCacheChains && (t.n_t > 2 || oddeven);
         if (cached) {   // H_c = sum of the windows of chain c's initial set
             for (int c = 0; c < t.n_t; c++) {
                 zero_delta();
@@ -173,21 +179,31 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a
             const double* SEj = a.psd + ((size_t)rowj * 2 + 1) * nf;
             const bool inv = a.psd_is_inverse != 0;
             double v[4] = {0.0, 0.0, 0.0, 0.0};   // dd_i, rd_i, dd_j, rd_j
+            const cx* Hi = cached ? cache + (size_t)s_holder[q] * 2 * a.max_stage : nullptr;       // the set sums the two
+            const cx* Hj = cached ? cache + (size_t)s_holder[q - 1] * 2 * a.max_stage : nullptr;   // chains hold
             for (int i = tid; i < t.n_stage; i += G) {
                 const int64_t e = i_first + i;
                 if (e < 0 || e >= a.n_f) continue;
                 const cx da = dA[i], de = dE[i];
                 const double na = da.re * da.re + da.im * da.im, ne = de.re * de.re + de.im * de.im;
                 {
-                    const double2 ra = __ldcg(reinterpret_cast<const double2*>(rAi + 2 * e));
-                    const double2 re = __ldcg(reinterpret_cast<const double2*>(rEi + 2 * e));
+                    double2 ra = __ldcg(reinterpret_cast<const double2*>(rAi + 2 * e));
+                    double2 re = __ldcg(reinterpret_cast<const double2*>(rEi + 2 * e));
+                    if (oddeven) {   // r_i = row - sum_{S_i} h
+                        const cx ha = Hi[i], he = Hi[a.max_stage + i];
+                        ra.x -= ha.re;  ra.y -= ha.im;  re.x -= he.re;  re.y -= he.im;
+                    }
                     const double wa = inv ? SAi[e] : 1.0 / SAi[e], we = inv ? SEi[e] : 1.0 / SEi[e];
                     v[0] += wa * na + we * ne;
                     v[1] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
                 }
                 {
-                    const double2 ra = __ldcg(reinterpret_cast<const double2*>(rAj + 2 * e));
-                    const double2 re = __ldcg(reinterpret_cast<const double2*>(rEj + 2 * e));
+                    double2 ra = __ldcg(reinterpret_cast<const double2*>(rAj + 2 * e));
+                    double2 re = __ldcg(reinterpret_cast<const double2*>(rEj + 2 * e));
+                    if (oddeven) {
+                        const cx ha = Hj[i], he = Hj[a.max_stage + i];
+                        ra.x -= ha.re;  ra.y -= ha.im;  re.x -= he.re;  re.y -= he.im;
+                    }
                     const double wa = inv ? SAj[e] : 1.0 / SAj[e], we = inv ? SEj[e] : 1.0 / SEj[e];
                     v[2] += wa * na + we * ne;
                     v[3] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
@@ -210,7 +226,21 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a
                 }
             }
             cta_sync<G>();
-            if (s_acc && t.write_back) {   // r_i += delta, r_j -= delta
+            if (s_acc && oddeven) {
+                if (wb && q == 1) {   // the cold chain now holds S_i: its buffer of the band's own parity -= delta (:652-658)
+                    double* wA = a.resid + ((size_t)t.write_walker * 2 + 0) * nf * 2;
+                    double* wE = a.resid + ((size_t)t.write_walker * 2 + 1) * nf * 2;
+                    for (int i = tid; i < t.n_stage; i += G) {
+                        const int64_t e = i_first + i;
+                        if (e < 0 || e >= a.n_f) continue;
+                        const cx da = dA[i], de = dE[i];
+                        atomicAdd(wA + 2 * e, -da.re);
+                        atomicAdd(wA + 2 * e + 1, -da.im);
+                        atomicAdd(wE + 2 * e, -de.re);
+                        atomicAdd(wE + 2 * e + 1, -de.im);
+                    }
+                }
+            } else if (s_acc && wb) {   // r_i += delta, r_j -= delta
                 for (int i = tid; i < t.n_stage; i += G) {
                     const int64_t e = i_first + i;
                     if (e < 0 || e >= a.n_f) continue;

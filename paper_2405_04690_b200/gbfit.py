@@ -35,15 +35,20 @@ BAND_WRITE_BACK, BAND_SUBTRACT_CURRENT, BAND_WRITE_OTHER = 1, 2, 4
 TEMPER_MAX_LADDER = 64
 # layout of gb_temper_task (include/gbfit.h)
 TEMPER_TASK = np.dtype([("n_t", np.int32), ("chain_begin", np.int32), ("n_stage", np.int32), ("write_back", np.int32),
-                        ("k_first", np.int64)], align=True)
+                        ("k_first", np.int64), ("write_walker", np.int32), ("reserved", np.int32)], align=True)
+TEMPER_WRITE_BACK, TEMPER_ODD_EVEN = 1, 2
 
 
-def pack_temper_tasks(n_t, chain_begin, n_stage, write_back, k_first) -> np.ndarray:
-    """Host array of gb_temper_task records from equal-length columns."""
+def pack_temper_tasks(n_t, chain_begin, n_stage, write_back, k_first, write_walker=None) -> np.ndarray:
+    """Host array of gb_temper_task records from equal-length columns.  write_walker selects the odd/even cold-chain buffer
+    mode of PAPER.md:354-362 (GB_TEMPER_ODD_EVEN): the row that receives exchanges with the cold chain."""
     t = np.zeros(len(n_t), TEMPER_TASK)
-    for key, val in (("n_t", n_t), ("chain_begin", chain_begin), ("n_stage", n_stage), ("write_back", write_back),
-                     ("k_first", k_first)):
+    for key, val in (("n_t", n_t), ("chain_begin", chain_begin), ("n_stage", n_stage), ("k_first", k_first)):
         t[key] = val
+    t["write_back"] = (np.asarray(write_back) != 0).astype(np.int32)
+    if write_walker is not None:
+        t["write_back"] |= TEMPER_ODD_EVEN
+        t["write_walker"] = write_walker
     return t
 
 

@@ -134,3 +134,51 @@ def test_temper_sweep_many_ladders_sampled(oracle, torch_cuda, gb):
         assert change > 0
         assert np.abs(r1[w] - odata.resid[w]).max() <= 1e-9 * change + 4e-16 * np.abs(resid[w]).max(), w
     assert acc.sum() > 0
+
+
+@pytest.mark.parametrize("N,f_lo,amp", [(128, 6e-4, 2e-22), (512, 6e-3, 3e-23)])
+def test_temper_sweep_odd_even_cold_chain_buffers(oracle, torch_cuda, gb, N, f_lo, amp):
+    """Row f2 on the data model of row f3 (Algorithm 2 as printed; buffers PAPER.md:354-362): ladders stage
+    from rows that hold none of the band's sources, every chain's residual is formed on chip as row - (set it holds), and
+    only exchanges with the cold chain are written, into the cold chain's own-parity row.  Decisions, permutations bit-exact,
+    (D_i, D_j) <= 1e-6, written rows <= 1e-9 of the change, the staged-from rows untouched; a 24-chain ladder (the paper's
+    temperature count) and a 33-chain one (beyond GB_TEMPER_MAX_LADDER_ODD_EVEN: row error)."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    for n_t, n_walkers, n_groups in ((4, 12, 3), (24, 24, 1)):
+        wl, tt, resid, d_rows = temper_case(oracle, N=N, f_lo=f_lo, n_bands=1, n_t=n_t, n_src=3, n_walkers=n_walkers,
+                                            amp=(0.1 * amp, amp), n_groups=n_groups, with_data=True)
+        nw = d_rows.shape[0]
+        buf = np.empty((2 * nw,) + d_rows.shape[1:], np.complex128)
+        buf[0::2] = d_rows
+        buf[1::2] = d_rows
+        cold = tt.tasks["chain_begin"]
+        for c in cold:
+            buf[2 * tt.chain_walker[c] + 1] = resid[tt.chain_walker[c]]
+        tasks = dict(tt.tasks, write_walker=(2 * tt.chain_walker[cold] + 1).astype(np.int32))
+        cw2 = (2 * tt.chain_walker).astype(np.int32)
+        wpsd = np.repeat(np.arange(nw), 2).astype(np.int32)
+        r_ref = buf.copy()
+        ref = oracle.temper_sweep(oracle.Config(), oracle.Data(r_ref, wl.psd, wl.k_lo, walker_psd=wpsd), tasks, N, tt.params, cw2,
+                                  tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)
+        assert ref[1].any()
+        d_resid = dev(torch, buf)
+        data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo, walker_psd=dev(torch, wpsd))
+        args = [dev(torch, x) for x in (tt.params, cw2, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)]
+        got = ctx.temper_sweep(data, dev(torch, gbfit.pack_temper_tasks(**tasks).view(np.uint8)), N, 3 * N, *args)
+        ctx.check()
+        perm, acc, dl = (x.cpu().numpy() for x in got)
+        assert np.array_equal(acc, ref[1]) and np.array_equal(perm, ref[0])
+        assert np.abs(dl - ref[2]).max() <= 1e-6
+        r1 = d_resid.cpu().numpy()
+        change = np.abs(r_ref - buf).max()
+        assert np.abs(r1 - r_ref).max() <= 1e-9 * change + 4e-16 * np.abs(buf).max()
+        assert np.array_equal(r1[0::2], buf[0::2])
+    # a ladder longer than the odd/even limit: row error, NaN
+    t33 = dict(tasks, n_t=np.full_like(tasks["n_t"], 33))
+    big = [np.resize(x, (40,) + x.shape[1:]) for x in (cw2, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)]
+    got = ctx.temper_sweep(data, dev(torch, gbfit.pack_temper_tasks(**t33).view(np.uint8)), N, 3 * N, dev(torch, tt.params),
+                           *[dev(torch, x) for x in big])
+    with pytest.raises(gbfit.GbError):
+        ctx.check()
+    assert np.isnan(got[2].cpu().numpy()[1:33]).all()

@@ -772,6 +772,69 @@ def test_temper_sweep_reduces_to_eq_d1_for_a_shared_likelihood_and_bubbles_when_
     assert np.array_equal(r0, resid) and not a0.any() and list(p0[:nt]) == list(range(nt))
 
 
+def _oddeven_temper_rows(wl, tt, resid, d_rows):
+    """Rows 2 w = the buffer a ladder stages from (the data of walker w: none of the band's own sets), 2 w + 1 = the cold
+    chain's buffer of the band's own parity (data minus the cold chain's set, where walker w carries a cold chain)."""
+    nw = d_rows.shape[0]
+    buf = np.empty((2 * nw,) + d_rows.shape[1:], np.complex128)
+    buf[0::2] = d_rows
+    buf[1::2] = d_rows
+    cold = tt.tasks["chain_begin"]
+    for c in cold:
+        buf[2 * tt.chain_walker[c] + 1] = resid[tt.chain_walker[c]]        # d - set of the cold chain
+    tasks = dict(tt.tasks, write_walker=(2 * tt.chain_walker[cold] + 1).astype(np.int32))
+    return buf, tasks, (2 * tt.chain_walker).astype(np.int32), np.repeat(np.arange(nw), 2).astype(np.int32)
+
+
+def test_temper_sweep_odd_even_buffers_equal_the_per_chain_residual_form(oracle):
+    """Algorithm 2 as printed on the odd/even buffers of PAPER.md:354-362: every chain forms its residual
+    as (row of its walker) - (sum of the set it holds) and only exchanges with the cold chain are written.  Pins: decisions,
+    permutations and (D_i, D_j) equal those of the per-chain-residual form on explicitly formed rows d - H_t (itself pinned
+    to the likelihood definition above); the staged-from rows are never written; afterwards the cold chain's buffer plus
+    the set the cold chain now holds gives back the data; a swapped sign of the subtraction or of the write fails."""
+    from temper_setup import temper_case
+    wl, tt, resid, d_rows = temper_case(oracle, n_bands=1, n_t=4, n_walkers=12, n_groups=3, with_data=True)
+    cfg = oracle.Config()
+    ref = oracle.temper_sweep(cfg, oracle.Data(resid.copy(), wl.psd, wl.k_lo), tt.tasks, tt.N, tt.params, tt.chain_walker,
+                              tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)
+    assert 0 < ref[1].sum() < ref[1].size
+    buf, tasks, cw2, wpsd = _oddeven_temper_rows(wl, tt, resid, d_rows)
+    r = buf.copy()
+    got = oracle.temper_sweep(cfg, oracle.Data(r, wl.psd, wl.k_lo, walker_psd=wpsd), tasks, tt.N, tt.params, cw2, tt.chain_beta,
+                              tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)
+    assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1])
+    assert np.abs(got[2] - ref[2]).max() <= 1e-9 * np.abs(ref[2]).max()
+    assert np.array_equal(r[0::2], buf[0::2])                                  # the rows staged from are only read
+    nt = int(tt.tasks["n_t"][0])
+    changed = 0
+    for it, cb in enumerate(tt.tasks["chain_begin"]):
+        w = tt.chain_walker[cb]
+        held = cb + got[0][cb]                                                 # the set the cold chain holds now
+        back = oracle.Data(r[2 * w + 1:2 * w + 2].copy(), wl.psd[w:w + 1], wl.k_lo)
+        for src in tt.params[tt.chain_set_begin[held]:tt.chain_set_begin[held] + tt.chain_set_n[held]]:
+            oracle.residual_update(cfg, back, None, src[None], np.zeros(1, np.int32), move_all=oracle.REMOVE, N=tt.N)
+        k0 = int(tt.tasks["k_first"][it] - wl.k_lo)
+        sl = slice(k0, k0 + int(tt.tasks["n_stage"][it]))
+        assert np.abs(back.resid[0][:, sl] - d_rows[w][:, sl]).max() <= 1e-10 * np.abs(d_rows[w][:, sl]).max()
+        changed += got[0][cb] != 0
+        other = [x for x in range(buf.shape[0]) if x != 2 * w + 1]
+    assert changed > 0
+    written = {2 * tt.chain_walker[cb] + 1 for cb in tt.tasks["chain_begin"]}
+    for x in range(buf.shape[0]):
+        if x not in written:
+            assert np.array_equal(r[x], buf[x])
+    # write_back = 0: same decisions, nothing written
+    r0 = buf.copy()
+    g0 = oracle.temper_sweep(cfg, oracle.Data(r0, wl.psd, wl.k_lo, walker_psd=wpsd), dict(tasks, write_back=np.zeros_like(tasks["write_back"])),
+                             tt.N, tt.params, cw2, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)
+    assert np.array_equal(g0[1], ref[1]) and np.array_equal(r0, buf)
+    # the plain form on the same rows (no subtraction of the held sets) is a different computation
+    plain = oracle.temper_sweep(cfg, oracle.Data(buf.copy(), wl.psd, wl.k_lo, walker_psd=wpsd),
+                                {k: v for k, v in tasks.items() if k != "write_walker"}, tt.N, tt.params, cw2, tt.chain_beta,
+                                tt.chain_set_begin, tt.chain_set_n, tt.chain_logu)
+    assert np.abs(plain[2] - ref[2]).max() > 1e-3 * np.abs(ref[2]).max()
+
+
 # ------------------------------------------------- odd/even cold-chain buffers (PAPER.md:354-362, Fig. 4), row f3
 def test_oddeven_buffers_equal_the_explicit_residual_and_keep_the_odd_buffer_consistent(oracle):
     from oddeven_setup import oddeven_case
