@@ -516,6 +516,9 @@ def run_ours(args):
             call = lambda: ctx.delta_loglike(dat2, a_n, a_o, a_w, move=a_m, move_all=w2.move_all, N=w2.N, n_bins=a_nb, out=o2)
             for _ in range(5):
                 call()
+            lc0 = ctx.launch_count()
+            call()
+            lpc = int(ctx.launch_count() - lc0)
             evs2 = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
             for e_a, e_b in evs2:
                 e_a.record(stream)
@@ -524,7 +527,29 @@ def run_ours(args):
             torch.cuda.synchronize()
             ctx.check()
             ms2 = float(np.median([e_a.elapsed_time(e_b) for e_a, e_b in evs2]))
-            small[w2.name] = {"rows": int(w2.B), "ms_per_call_median": ms2, "evals_per_s": w2.B / (ms2 * 1e-3)}
+            # the same call captured once into a CUDA graph and replayed: no host launch cost between its kernels
+            ms2g = None
+            try:
+                cs = torch.cuda.Stream(dev)
+                cs.wait_stream(stream)
+                gr = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gr, stream=cs):
+                    call()
+                for _ in range(3):
+                    gr.replay()
+                for e_a, e_b in evs2:
+                    e_a.record(stream)
+                    gr.replay()
+                    e_b.record(stream)
+                torch.cuda.synchronize()
+                ctx.check()
+                ms2g = float(np.median([e_a.elapsed_time(e_b) for e_a, e_b in evs2]))
+            except Exception as exc:       # capture refused: report the plain number only
+                ms2g = None
+                small.setdefault("graph_errors", []).append(f"{w2.name}: {exc}")
+            small[w2.name] = {"rows": int(w2.B), "ms_per_call_median": ms2, "evals_per_s": w2.B / (ms2 * 1e-3),
+                              "ms_per_graph_replay_median": ms2g,
+                              "launches_per_call": lpc}
 
     # ---- SURVEY 8(f) row f2, outside the timed step: Algorithm 2 (gb_temper_sweep), 10-chain ladders ------
     # every odd 256-bin sub-band of 1-4 mHz, 36 ladders per band on disjoint residuals, 9-10 sources per chain
@@ -580,6 +605,30 @@ def run_ours(args):
         ms_ov = o0.elapsed_time(o1) / 3
         ovl = {"call": "gb_overlap", "pairs": n_pairs, "ms_per_call": ms_ov, "pairs_per_s": n_pairs / (ms_ov * 1e-3),
                "mean_N": float(wl.n_bins[:n_pairs].mean()), "median_overlap": float(d_ov.median().item())}
+
+    # ---- SURVEY 8(f) row f4, second half: the search-stage batch shape of App. G: 900 sub-bands x 10
+    #      temperatures x 100 walkers, one source per walker, every row against ONE best-fit residual row
+    search = None
+    if rank == 0 and full and not args.no_band_sweep:
+        from gb_inputs import make_search_stage
+        ws = make_search_stage()
+        dat_s = gbfit.Data(d_resid[:1], torch.from_numpy(1.0 / ws.psd).to(dev), ws.k_lo, psd_is_inverse=True)
+        s_p, s_w, s_nb = (torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in (ws.params_new, ws.walker_index, ws.n_bins))
+        s_out = torch.empty(ws.B, dtype=torch.float64, device=dev)
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(6):
+            if i == 1:
+                s0.record(stream)
+            ctx.delta_loglike(dat_s, s_p, None, s_w, move_all=gbfit.ADD, n_bins=s_nb, out=s_out)
+        s1.record(stream)
+        torch.cuda.synchronize()
+        ctx.check()
+        ms_s = s0.elapsed_time(s1) / 5
+        fl_s = float(flops_eval(ws.n_bins.astype(np.float64)).sum())
+        search = {"call": "gb_delta_loglike, search-stage shape (App. G): 900 sub-bands x 10 temperatures x 100 walkers, one "
+                          "source per walker, one residual row", "rows": int(ws.B), "ms_per_call": ms_s,
+                  "evals_per_s": ws.B / (ms_s * 1e-3), "mean_N": float(ws.n_bins.mean()),
+                  "alu_frac": fl_s / (ms_s * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
 
     # ---- roofline of the delta-lnL kernels (the dominant launches) and of the scatter
     nb = wl.n_bins.astype(np.float64)
@@ -675,7 +724,7 @@ def run_ours(args):
             "e2e": {"value": evals / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "two_call_form": two_call, "sweep_pair_kept": pair, "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "small_configs_latency": small,
+            "two_call_form": two_call, "sweep_pair_kept": pair, "band_sweep": band, "temper_sweep": tmp, "overlap": ovl, "search_stage": search, "small_configs_latency": small,
         }
         print(json.dumps(line), flush=True)
     ctx.close()

@@ -6,5 +6,5 @@ PAPER.md:148-157 (Eq. 7-9) as an *input* array, and colours Gaussian noise with 
 value distributions follow BASELINE.json's five configs (recipe restated in DESIGN.md "Input recipe").
 """
 from .configs import (Workload, make_workload, band_bins, n_bins_for_f0, instrument_psd,  # noqa: F401
-                      BandTasks, make_band_tasks, TemperTasks, make_temper_tasks, StretchInputs, make_stretch_inputs,
+                      BandTasks, make_band_tasks, TemperTasks, make_temper_tasks, StretchInputs, make_stretch_inputs, make_search_stage,
                       TOBS, DT, SEED_BASE)

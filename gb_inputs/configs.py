@@ -410,3 +410,35 @@ def make_temper_tasks(wl: Workload, N: int, f_lo: float, n_bands: int, n_t: int,
     return TemperTasks(N, tasks, np.ascontiguousarray(np.concatenate(sets)), tr, np.concatenate(walkers),
                        np.tile(1.2 ** -np.arange(n_t, dtype=np.float64), ntask), np.asarray(set_begin, np.int32),
                        np.asarray(set_n, np.int32), np.log(g.random(nc)), 3 * N)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Search-stage batch shape (App. G): per-sub-band fixed-dimension parallel tempering, ~900 sub-bands x
+# ~10 temperatures x ~100 walkers, ONE source per walker, every walker of a sub-band evaluated against the same best-fit
+# residual of its band; "the priors are modified so that the initial frequency spans its assigned sub-band only" (:712).
+# Rows are band-major (all temperatures and walkers of a band are consecutive): the opposite of config 5's geometry -- many
+# rows on the same few hundred bins of ONE residual row.
+def make_search_stage(n_bands: int = 900, n_temps: int = 10, n_walkers: int = 100, f_lo: float = 3e-4, f_hi: float = 1.5e-2,
+                      snr_lo: float = 5.0, snr_hi: float = 30.0, stream: int = 0) -> Workload:
+    g = _rng(6, _S_PARAMS + stream)
+    k_lo, n_f = band_bins(0.1e-3, 30e-3)
+    psd, sc = _psd_rows(6, 1, k_lo, n_f, False)
+    # sub-bands spread log-uniformly over [f_lo, f_hi]; a band starts on a multiple of its window length
+    fb = np.sort(f_lo * (f_hi / f_lo) ** ((np.arange(n_bands) + g.random(n_bands)) / n_bands))
+    Nb = n_bins_for_f0(fb)
+    kb = (np.floor(fb * TOBS / Nb) * Nb).astype(np.int64)
+    per = n_temps * n_walkers
+    B = n_bands * per
+    p = _draw_params(g, B, 1e-3, 2e-3)
+    band = np.repeat(np.arange(n_bands), per)
+    p[:, 1] = (kb[band] + g.random(B) * Nb[band]) / TOBS               # f0 inside its sub-band only
+    f = p[:, 1]
+    # amplitude from an optimal-SNR draw in [snr_lo, snr_hi] (the search works between the SNR limits 7 -> 5, :718):
+    # rho^2 ~ 4/5 amp^2 T_obs x^2 ... is not needed exactly -- scale a reference amplitude by the noise level at f0
+    S = instrument_psd(f)
+    rho = snr_lo * (snr_hi / snr_lo) ** g.random(B)
+    x = 2.0 * np.pi * f * ARMLENGTH / 299792458.0
+    p[:, 0] = rho * np.sqrt(S / TOBS) / (np.maximum(np.abs(np.sin(x)), 1e-3) * x) * 0.22
+    nb = Nb[band].astype(np.int32)
+    return Workload(6, "search_stage", TOBS, DT, k_lo, n_f, 1, psd, None, p, None, np.zeros(B, np.int32), None, ADD, 0, nb,
+                    None, sc)

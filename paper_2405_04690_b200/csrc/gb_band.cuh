@@ -229,7 +229,16 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
         }
 
         // ---- the proposals of the band, in order
-        int64_t hint_lo = 0, hint_hi = a.gen ? a.st.n_group - min((int64_t)a.st.n_friends, a.st.n_group) : 0;   // friends search hint
+        // friends search hint: the rows of the friends table inside the staged frequency range, widened by n_friends
+        // (proposals are confined to the stage, so the run of a current source starts in there; the search checks it anyway)
+        int64_t hint_lo = 0, hint_hi = 0;
+        if (a.gen && tid < 32) {
+            const int64_t nfr = min((int64_t)a.st.n_friends, a.st.n_group);
+            const double f_lo = (double)t.k_first / a.Tobs, f_hi = (double)(t.k_first + t.n_stage) / a.Tobs;
+            hint_lo = max((int64_t)0, friend_run_start(a.st.group, a.st.n_group, 0, f_lo, tid, 0, a.st.n_group) - nfr);
+            hint_hi = min(a.st.n_group - nfr, friend_run_start(a.st.group, a.st.n_group, 0, f_hi, tid, 0, a.st.n_group));
+            if (hint_hi < hint_lo) hint_hi = hint_lo;
+        }
         for (int p = 0; p < t.n_prop; p++) {
             const int64_t ip = (int64_t)t.prop_begin + p;
             int k;
@@ -249,8 +258,6 @@ __global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
                     const int64_t nf = a.st.n_friends < a.st.n_group ? a.st.n_friends : a.st.n_group;
                     const int32_t jf = randint32(w0[1], (int32_t)nf);
                     const int64_t s0 = friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid, hint_lo, hint_hi);
-                    hint_lo = max((int64_t)0, s0 - 512);                  // the next proposal of this band lands nearby
-                    hint_hi = min(a.st.n_group - nf, s0 + 512);
                     const int64_t row = s0 + jf;
                     const double ua = uniform52(w0[2], w0[3]);
                     const double tz = __dadd_rn(__dmul_rn(__dadd_rn(a.st.stretch_a, -1.0), ua), 1.0);

@@ -149,6 +149,11 @@ struct MainArgs {
     const int32_t* bin_count;
     const int32_t* bin_off;
     int32_t* bin_ticket;
+    // DIRECT instantiations: the proposal arrays themselves (thread 0 of a CTA does step O1 of its rows)
+    const double* params_new;
+    const double* params_old;
+    double Rmax;
+    int64_t kmax;
     int K, chunk;
     int pool_r;                         // store slots / list positions a CTA reserves at a time
     int fuse;                           // != 0: CTAs move accepted windows of earlier chunks into the residual between items
@@ -785,7 +790,9 @@ __global__ void gb_ready_kernel(const int32_t* ent_cursor, int32_t* ent_done, co
 // before its inner products read it: no global-memory round trip is exposed between items.
 // A list entry is the row index, with bit 31 set when the row's single source is the OLD one (REMOVE);
 // -1 marks the end of the list.
-template <int N, bool SWAP, bool FAST, bool ACC>
+// VAR: 0 = the batched kernels; 1 = gb_delta_loglike_accept; 2 = DIRECT, the one-launch path of small uniform batches (no
+// prep kernel, no work lists: CTA c takes rows c, c + gridDim.x, ... and thread 0 works out each row's record itself)
+template <int N, bool SWAP, bool FAST, int VAR>
 __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kernel(MainArgs a) {
     constexpr int G = Plan<N>::G;
     constexpr int S = N / G;
@@ -806,10 +813,21 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     __shared__ long long s_off;                  // store offset of this item's window, -1: rejected
 
     const int tid = threadIdx.x;
-    constexpr bool accept = ACC && !SWAP;   // gb_delta_loglike_accept (its own instantiation: the plain kernels carry none of it)
+    constexpr bool accept = VAR == 1 && !SWAP;   // gb_delta_loglike_accept (its own instantiation: the plain kernels carry none of it)
+    constexpr bool direct = VAR == 2 && !SWAP;   // one-launch path of small batches
     const int bin = accept ? cls * a.K + a.chunk : cls;   // accept: the lists are binned by (class, walker chunk)
-    const int count = accept ? a.bin_count[bin] : a.counts[cls];
+    const int count = direct ? (int)((a.B - blockIdx.x + gridDim.x - 1) / gridDim.x)   // rows of THIS CTA
+                             : accept ? a.bin_count[bin] : a.counts[cls];
     int32_t* const ticket = accept ? a.bin_ticket + bin : a.counters + cls;
+    int direct_next = 0;   // (thread 0, direct) this CTA's next private ticket
+    auto take = [&](int n) {
+        if (direct) {
+            const int t = direct_next;
+            direct_next += n;
+            return t;
+        }
+        return atomicAdd(ticket, n);
+    };
     // fused update (thread 0 only): accepted windows of earlier walker chunks travel store -> staging buffer -> residual as
     // bulk asynchronous copies / reductions; no other thread and no register of the evaluation is involved
     cx* stage = reinterpret_cast<cx*>(smem_raw) + 2 * PN;
@@ -838,9 +856,38 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     };
     if (!accept && count == 0) return;   // (accept: one exit at the end, so that the closing code exists once)
     const int32_t* __restrict__ list = accept ? a.lists + a.bin_off[bin] : a.lists + (int64_t)cls * a.B;
+    // ticket -> list entry (row index, bit 31: the row's single source is the OLD one), -1 past the end
+    auto entry_of = [&](int t) -> int {
+        if (t >= count) return -1;
+        if (direct) return (int)(blockIdx.x + (int64_t)t * gridDim.x) | (a.move_all == GB_REMOVE ? (int)0x80000000 : 0);
+        return __ldg(list + t);
+    };
 
     auto fetch = [&](int entry, int bufi) {
         const int64_t row = entry & 0x7fffffff;
+        if (direct) {   // step O1 and the row checks of gb_prep_kernel, by thread 0 (move < 0 marks a row error)
+            if (tid == 0) {
+                const double* p = (entry < 0 ? a.params_old : a.params_new) + 8 * row;
+                SrcConst s;
+                source_constants(p, a.Tobs, a.tau, N, s);
+                s.fast = fast_path_ok(p, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+                s.move = a.move_all;
+                int w = 0, prow = 0;
+                bool ok = true;
+                if (a.mode != MODE_WAVEFORM) {
+                    w = a.walker_index[row];
+                    ok = w >= 0 && w < a.n_walkers;
+                    if (ok) prow = a.walker_psd ? a.walker_psd[w] : (a.n_psd == 1 ? 0 : w);
+                    ok = ok && prow >= 0 && prow < a.n_psd;
+                }
+                s.walker = w;
+                s.psd_row = prow;
+                if (!ok) s.move = -1;
+                else if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+                s_src[bufi][0] = s;
+            }
+            return;
+        }
         if (SWAP) {
             if (tid < kRecChunks)
                 cp_async16(reinterpret_cast<char*>(&s_src[bufi][0]) + 16 * tid,
@@ -859,9 +906,9 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
 
     int t_nx2 = 0;   // (thread 0) ticket of the item after next
     if (tid == 0) {
-        const int t = atomicAdd(ticket, 3);
-        s_ent[0] = t < count ? __ldg(list + t) : -1;
-        s_ent[1] = t + 1 < count ? __ldg(list + t + 1) : -1;
+        const int t = take(3);
+        s_ent[0] = entry_of(t);
+        s_ent[1] = entry_of(t + 1);
         s_pos[0] = t;
         s_pos[1] = t + 1;
         t_nx2 = t + 2;
@@ -886,9 +933,21 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         const SrcConst* rec = s_src[buf];
         const int64_t b = e_cur & 0x7fffffff;
         const int mv = rec[0].move;
+        const bool bad_row = direct && mv < 0;   // (direct) walker / PSD row out of range: NaN, nothing computed
+        if (bad_row && tid == 0) {
+            atomicOr(a.errflag, 1);
+            if (a.dlnL_out) a.dlnL_out[b] = __longlong_as_double(0x7ff8000000000000LL);
+        }
 
         // ---- waveform(s)
-        slow_part<N, G, FAST>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+        if (direct) {
+            if (!bad_row) {
+                if (rec[0].fast) slow_part<N, G, true>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+                else slow_part<N, G, false>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+            }
+        } else {
+            slow_part<N, G, FAST>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
+        }
         if (SWAP) {
             fft_store<N>(bufA0, bufE0, a.tw, tid);
             slow_part<N, G, FAST>(&rec[NS - 1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
@@ -897,8 +956,8 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         // register-hungry slow part, and consumed at the end of the item, behind the FFT and the epilogue
         int t_nx3 = 0, e_nx2 = -1;
         if (tid == 0) {
-            t_nx3 = atomicAdd(ticket, 1);
-            if (t_nx2 < count) e_nx2 = __ldg(list + t_nx2);
+            t_nx3 = take(1);
+            e_nx2 = entry_of(t_nx2);
         }
         // fused update, first checkpoint of the item: move the piece in flight one stage on
         if (fuse && tid == 0) sc_reduce_if_landed(a, s_scs, stage);
@@ -911,10 +970,12 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             const SrcConst& nx = s_src[buf ^ 1][NS - 1];
             const int64_t i0 = nx.kmin - a.k_lo;
             const size_t nf = (size_t)a.n_f;
-            const double* rAn = a.resid + ((size_t)nx.walker * 2 + 0) * nf * 2;
-            const double* rEn = a.resid + ((size_t)nx.walker * 2 + 1) * nf * 2;
-            const double* SAn = a.psd + ((size_t)nx.psd_row * 2 + 0) * nf;
-            const double* SEn = a.psd + ((size_t)nx.psd_row * 2 + 1) * nf;
+            const bool nx_bad = direct && nx.move < 0;   // (direct) a row error: its walker / PSD row are not valid indices
+            const size_t nxw = nx_bad ? 0 : (size_t)nx.walker, nxp = nx_bad ? 0 : (size_t)nx.psd_row;
+            const double* rAn = a.resid + (nxw * 2 + 0) * nf * 2;
+            const double* rEn = a.resid + (nxw * 2 + 1) * nf * 2;
+            const double* SAn = a.psd + (nxp * 2 + 0) * nf;
+            const double* SEn = a.psd + (nxp * 2 + 1) * nf;
             if (i0 >= 0 && i0 + N + 16 <= a.n_f) {           // window (plus the line it may end in) is stored
                 const double* pA = rAn + 2 * (i0 + 8 * tid);
                 const double* pE = rEn + 2 * (i0 + 8 * tid);
@@ -962,7 +1023,8 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         const int ht = tid - ch * H;
 
         // ---- epilogue
-        if (a.mode == MODE_WAVEFORM) {
+        if (bad_row) {
+        } else if (a.mode == MODE_WAVEFORM) {
             double2* outA = reinterpret_cast<double2*>(a.AE_out) + ((size_t)b * 2 + 0) * (size_t)a.Nmax;
             double2* outE = reinterpret_cast<double2*>(a.AE_out) + ((size_t)b * 2 + 1) * (size_t)a.Nmax;
 #pragma unroll
@@ -1356,6 +1418,7 @@ struct gb_ctx {
     int64_t cap_wk, cap_ent, cap_accpar, cap_pieces;
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
     int grid_blocks_acc[kNumClasses];   // the same for the gb_delta_loglike_accept instantiations
+    int grid_blocks_dir[kNumClasses];   // and for the DIRECT (one-launch) instantiations
     // staging for the *_host entry points
     void* d_stage;
     size_t cap_stage;
@@ -1404,25 +1467,25 @@ int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
     return GB_OK;
 }
 
-template <int N, bool SWAP, bool FAST, bool ACC = false>
+template <int N, bool SWAP, bool FAST, int VAR = 0>
 int setup_kernel(gb_ctx* ctx) {
     constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
-    const size_t smem = main_smem_bytes<N, SWAP, ACC>();
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP, FAST, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem = main_smem_bytes<N, SWAP, VAR == 1>();
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP, FAST, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST, ACC>, Plan<N>::G, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST, VAR>, Plan<N>::G, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_CUDA, "kernel class %d does not fit on an SM", cls);
-    (ACC ? ctx->grid_blocks_acc : ctx->grid_blocks)[cls] = nb * ctx->num_sms;
+    (VAR == 1 ? ctx->grid_blocks_acc : VAR == 2 ? ctx->grid_blocks_dir : ctx->grid_blocks)[cls] = nb * ctx->num_sms;
     return GB_OK;
 }
 
-template <int N, bool SWAP, bool FAST, bool ACC = false>
+template <int N, bool SWAP, bool FAST, int VAR = 0>
 int launch_main(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
     constexpr int cls = 4 * (N == 128 ? 0 : N == 256 ? 1 : N == 512 ? 2 : 3) + (FAST ? 0 : 2) + (SWAP ? 1 : 0);
     a.orbit = ctx->d_orbit[cls >> 2];
-    int64_t grid = (ACC ? ctx->grid_blocks_acc : ctx->grid_blocks)[cls];
+    int64_t grid = (VAR == 1 ? ctx->grid_blocks_acc : VAR == 2 ? ctx->grid_blocks_dir : ctx->grid_blocks)[cls];
     if (grid > B) grid = B;
-    gb_main_kernel<N, SWAP, FAST, ACC><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP, ACC>(), st>>>(a);
+    gb_main_kernel<N, SWAP, FAST, VAR><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP, VAR == 1>(), st>>>(a);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -1464,6 +1527,7 @@ struct Call {
 };
 
 constexpr int kMaxChunks = 16;           // walker chunks of gb_delta_loglike_accept
+constexpr int64_t kDirectMaxRows = 8192; // batches up to this size with one window length and one move type: one launch
 constexpr int kWkHeader = 8;             // ints before the per-bin arrays of d_wk
 constexpr int kWkInts = kWkHeader + 4 * kNumClasses * kMaxChunks;
 
@@ -1517,6 +1581,47 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     GB_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     int rc;
+    // Small uniform batches (one window length, one move type, no SWAP): ONE launch.  No prep kernel, no work lists, no
+    // scratch: CTA c takes rows c, c + gridDim.x, ... and its thread 0 does step O1 and the row checks (a batch of 64
+    // rows is 0.2 us of arithmetic: the call is the latency of its launches, PAPER.md:454-456 for context).
+    if (c.B <= kDirectMaxRows && !c.n_bins && !c.move && !c.keep && !c.accept && !c.accepted && c.mode != MODE_OVERLAP &&
+        (c.mode == MODE_WAVEFORM || c.move_all != GB_SWAP)) {
+        MainArgs a{};
+        a.B = c.B;
+        a.mode = c.mode;
+        a.tw = ctx->d_tw;
+        if (c.data) {
+            a.resid = c.data->resid;
+            a.psd = c.data->psd;
+            a.walker_psd = c.data->walker_psd;
+            a.k_lo = c.data->k_lo;
+            a.n_f = c.data->n_f;
+            a.n_walkers = c.data->n_walkers;
+            a.n_psd = c.data->n_psd;
+            a.psd_is_inverse = c.data->psd_is_inverse;
+        }
+        a.walker_index = c.walker_index;
+        a.move_all = c.mode == MODE_WAVEFORM ? GB_ADD : c.move_all;
+        a.dlnL_out = c.dlnL_out;
+        a.aux_out = c.aux_out;
+        a.AE_out = c.AE_out;
+        a.kmin_out = c.kmin_out;
+        a.Nmax = c.Nmax;
+        a.Tobs = ctx->cfg.Tobs;
+        a.tau = ctx->cfg.armlength / kCLight;
+        a.errflag = ctx->d_counts + 2 * kNumClasses;
+        a.params_new = c.params_new;
+        a.params_old = c.params_old;
+        a.Rmax = ctx->cfg.au / kCLight;
+        a.kmax = (int64_t)floor(ctx->cfg.Tobs / (2.0 * ctx->cfg.dt));
+        ctx->kept_B = 0;
+        switch (c.N) {
+            case 128: return launch_main<128, false, true, 2>(ctx, a, c.B, st);
+            case 256: return launch_main<256, false, true, 2>(ctx, a, c.B, st);
+            case 512: return launch_main<512, false, true, 2>(ctx, a, c.B, st);
+            default: return launch_main<1024, false, true, 2>(ctx, a, c.B, st);
+        }
+    }
     if (need_new && (rc = ensure_cap(ctx, &ctx->d_src_new, &ctx->cap_new, c.B))) return rc;
     if (need_old && (rc = ensure_cap(ctx, &ctx->d_src_old, &ctx->cap_old, c.B))) return rc;
     if ((rc = ensure_cap(ctx, &ctx->d_lists, &ctx->cap_lists, c.B * kNumClasses))) return rc;
@@ -1698,10 +1803,10 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
                     if (!c.n_bins && Nc != c.N) continue;
                     a.pool_r = pool_r[cN];
                     switch (Nc) {
-                        case 128: rc = pass ? launch_main<128, false, true, true>(ctx, a, c.B, st) : launch_main<128, false, false, true>(ctx, a, c.B, st); break;
-                        case 256: rc = pass ? launch_main<256, false, true, true>(ctx, a, c.B, st) : launch_main<256, false, false, true>(ctx, a, c.B, st); break;
-                        case 512: rc = pass ? launch_main<512, false, true, true>(ctx, a, c.B, st) : launch_main<512, false, false, true>(ctx, a, c.B, st); break;
-                        default: rc = pass ? launch_main<1024, false, true, true>(ctx, a, c.B, st) : launch_main<1024, false, false, true>(ctx, a, c.B, st); break;
+                        case 128: rc = pass ? launch_main<128, false, true, 1>(ctx, a, c.B, st) : launch_main<128, false, false, 1>(ctx, a, c.B, st); break;
+                        case 256: rc = pass ? launch_main<256, false, true, 1>(ctx, a, c.B, st) : launch_main<256, false, false, 1>(ctx, a, c.B, st); break;
+                        case 512: rc = pass ? launch_main<512, false, true, 1>(ctx, a, c.B, st) : launch_main<512, false, false, 1>(ctx, a, c.B, st); break;
+                        default: rc = pass ? launch_main<1024, false, true, 1>(ctx, a, c.B, st) : launch_main<1024, false, false, 1>(ctx, a, c.B, st); break;
                     }
                     if (rc) return rc;
                 }
@@ -1863,8 +1968,9 @@ int gb_create(const gb_config* cfg, gb_ctx** out) {
     if ((rc = setup_kernel<N_, true, true>(ctx))) return rc;            \
     if ((rc = setup_kernel<N_, false, false>(ctx))) return rc;          \
     if ((rc = setup_kernel<N_, true, false>(ctx))) return rc;           \
-    if ((rc = setup_kernel<N_, false, true, true>(ctx))) return rc;     \
-    if ((rc = setup_kernel<N_, false, false, true>(ctx))) return rc;
+    if ((rc = setup_kernel<N_, false, true, 1>(ctx))) return rc;        \
+    if ((rc = setup_kernel<N_, false, false, 1>(ctx))) return rc;       \
+    if ((rc = setup_kernel<N_, false, true, 2>(ctx))) return rc;
     GB_SETUP(128) GB_SETUP(256) GB_SETUP(512) GB_SETUP(1024)
 #undef GB_SETUP
     return GB_OK;

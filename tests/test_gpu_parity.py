@@ -695,3 +695,27 @@ def test_row_errors_for_oversized_window_null_side_and_bad_psd_row(oracle, torch
     with pytest.raises(gbfit.GbError):
         ctx.check()
     assert np.isnan(d[wl.walker_index == 1]).all() and np.isfinite(d[wl.walker_index == 0]).all()
+
+
+def test_search_stage_geometry_single_residual_many_walkers_per_band(oracle, torch_cuda, gb):
+    """App. G's batch shape: sub-bands x temperatures x walkers, one source per walker, f0 confined to
+    its sub-band, every row against the SAME residual row -- consecutive rows read the same few hundred bins (the opposite
+    of config 5, where neighbouring rows share a walker but not a frequency).  60 bands x 3 x 40 = 7200 rows, all four
+    window lengths; every row against the oracle."""
+    from gb_inputs import make_search_stage
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_search_stage(n_bands=60, n_temps=3, n_walkers=40)
+    assert set(np.unique(wl.n_bins)) == {128, 256, 512, 1024}
+    resid = wl.resid()
+    ref, raux = oracle.delta_loglike(oracle.Config(), oracle.Data(resid, wl.psd, wl.k_lo), wl.params_new, None, wl.walker_index,
+                                     n_bins=wl.n_bins, want_aux=True, nthreads=oracle.max_threads())
+    data, _ = upload(torch, gbfit, wl, resid)
+    aux = torch.zeros((wl.B, 2), dtype=torch.float64, device="cuda:0")
+    got = ctx.delta_loglike(data, dev(torch, wl.params_new), None, dev(torch, wl.walker_index), move_all=gbfit.ADD,
+                            n_bins=dev(torch, wl.n_bins), aux=aux)
+    ctx.check()
+    assert np.abs(got.cpu().numpy() - ref).max() <= TOL_DLNL
+    assert np.abs(aux.cpu().numpy() - raux).max() <= 1e-6
+    snr = np.sqrt(raux[:, 0])
+    assert 2.0 < np.median(snr) < 60.0
