@@ -39,7 +39,23 @@ WORKLOAD = "cfg5_full_ensemble_sweep_10x36x12000"
 
 # ---- algorithmic work per evaluation (frozen in BASELINE.md before optimisation) ----
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
-NCU_DRAM_BYTES_DLNL = 13.70e9                           # dram__bytes_read.sum + dram__bytes_write.sum, profiles/r1_v9
+
+
+def ncu_traffic(update: str):
+    """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the kernels of one timed step, read from the committed
+    summary of the ncu --set full capture under profiles/ (never a literal here).  Returns (bytes or None, provenance)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r2_step_traffic.csv")
+    want = {"fused": "r2_step"}.get(update)
+    try:
+        for row in csv.DictReader(open(path)):
+            if row["capture"] == want:
+                b = float(row["dram_read_bytes_per_step"]) + float(row["dram_write_bytes_per_step"])
+                return b, (f"profiles/r2_step_traffic.csv: capture {row['capture']} at commit {row['commit']}, "
+                           f"{row['launches_per_step']} launches of {row['kernels']}")
+    except (OSError, KeyError, ValueError):
+        pass
+    return None, "no committed ncu capture for this step form"
 
 
 def flops_eval(N):
@@ -645,6 +661,7 @@ def run_ours(args):
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     hbm_src = "measured" if "hbm_gbs" in peaks else "fallback"
     ach_tf = flops_dlnl / (ms_dlnl * 1e-3) / 1e12
+    traffic_bytes, traffic_src = ncu_traffic(args.update)
     roofline = {
         "bound": "alu", "kernel": ("gb_main_kernel<N,false,true,ACC=true> x {1024,512,256,128} (+ gb_prep_kernel, gb_walker_scan_kernel) "
                                    "of gb_delta_loglike_accept: evaluation, decision and the fused update" if fused else
@@ -654,9 +671,9 @@ def run_ours(args):
         "peak_measured_dfma": dfma_tflops, "frac_of_measured_dfma": ach_tf / dfma_tflops if dfma_tflops > 0 else None,
         "dfma_lanes_per_clk_sm_at_1965mhz": dfma_lanes,
         "flops_per_launch": flops_dlnl, "ms_per_launch": ms_dlnl,
-        # DRAM bytes (read + write) of the four delta-lnL kernels of one step, from the ncu --set full capture
-        # profiles/r1_v9_ncu_full_summary.csv (full workload only); algorithmic bytes are in "hbm"
-        "traffic": NCU_DRAM_BYTES_DLNL if full else None, "traffic_unit": "bytes per delta-lnL call (ncu, r1_v9)",
+        # DRAM bytes (read + write) of the kernels of one step, from the committed ncu --set full capture (full workload
+        # only); algorithmic bytes are in "hbm"
+        "traffic": traffic_bytes if full else None, "traffic_unit": "DRAM bytes per step", "traffic_source": traffic_src,
         "hbm": {"achieved": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "bytes_per_launch": bytes_dlnl},

@@ -117,8 +117,12 @@ constexpr size_t band_smem_bytes(int max_stage) {
     return (size_t)padded_len<N>() * sizeof(cx) * 4 + (size_t)max_stage * 48;
 }
 
+// resident CTAs per SM the register allocation aims at: what shared memory allows at the usual stage of 3 N bins
+template <int N>
+constexpr int band_min_blocks() { return N == 128 ? 6 : N == 256 ? 4 : N == 512 ? 2 : 1; }
+
 template <int N, int GM>
-__global__ void __launch_bounds__(Plan<N>::G * GM) gb_band_kernel(BandArgs a) {
+__global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band_kernel(BandArgs a) {
     constexpr int PG = Plan<N>::G;   // FFT group: the first PG threads
     constexpr int G = PG * GM;       // threads of the CTA
     constexpr int S = N / G;

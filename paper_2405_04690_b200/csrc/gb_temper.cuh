@@ -48,8 +48,12 @@ constexpr size_t temper_smem_bytes(int max_stage) {
     return (size_t)padded_len<N>() * sizeof(cx) * 2 + (size_t)max_stage * 32;
 }
 
+// resident CTAs per SM the register allocation aims at: what shared memory allows at the usual stage of 3 N bins
+template <int N>
+constexpr int temper_min_blocks() { return N == 128 ? 6 : N == 256 ? 6 : N == 512 ? 3 : 1; }
+
 template <int N, int GM>
-__global__ void __launch_bounds__(Plan<N>::G * GM) gb_temper_kernel(TemperArgs a) {
+__global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_temper_kernel(TemperArgs a) {
     constexpr int PG = Plan<N>::G;   // FFT group: the first PG threads
     constexpr int G = PG * GM;       // threads of the CTA
     constexpr int S = N / G;
