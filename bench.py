@@ -663,8 +663,8 @@ def run_ours(args):
     ach_tf = flops_dlnl / (ms_dlnl * 1e-3) / 1e12
     traffic_bytes, traffic_src = ncu_traffic(args.update)
     roofline = {
-        "bound": "alu", "kernel": ("gb_main_kernel<N,false,true,ACC=true> x {1024,512,256,128} (+ gb_prep_kernel, gb_walker_scan_kernel) "
-                                   "of gb_delta_loglike_accept: evaluation, decision and the fused update" if fused else
+        "bound": "alu", "kernel": ("gb_main_kernel<N,0,1,VAR=1> x {1024,512,256,128} x 8 walker chunks (+ 2 gb_prep_kernel passes, "
+                                   "gb_pieces_kernel, closing scatter) of gb_delta_loglike_accept: evaluation, decision and the fused update" if fused else
                                    "gb_main_kernel<N,false,true> x {1024,512,256,128} (+ gb_prep_kernel) of gb_delta_loglike"),
         "achieved": ach_tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": ach_tf / FP64_PEAK_TFLOPS,
         "peak_source": "derived: 148 SMs x 64 DFMA/clk x 2 x 1.965 GHz (no FP64 figure in MEASURED_PEAKS.json)",
@@ -678,7 +678,8 @@ def run_ours(args):
                 "frac": bytes_dlnl / (ms_dlnl * 1e-3) / 1e9 / hbm_peak, "peak_source": hbm_src,
                 "bytes_per_launch": bytes_dlnl},
         "update": ({"call": "inside the same launches (gb_delta_loglike_accept, apply = 1): accepted windows are stored "
-                            "once and scattered by the delta-lnL CTAs as soon as a walker's rows are all evaluated",
+                            "once; the CTAs that evaluate walker chunk c+1 move the windows of chunks <= c into the residual "
+                            "(cp.async.bulk + cp.reduce.async.bulk add.f64)",
                     "bytes": 1.5 * bytes_upd, "bytes_note": "32 N written + 32 N read + 64 N read-modify-write per accepted row",
                     "store_bytes": 32.0 * store_bins} if fused else
                    {"call": "gb_residual_update (regenerates the accepted waveforms)", "ms_per_launch": ms_upd,

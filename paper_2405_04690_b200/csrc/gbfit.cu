@@ -83,7 +83,7 @@ struct PrepArgs {
     // (class, walker chunk): accept = 1 counts the rows of every bin, accept = 2 is the full pass appending at the bins' offsets
     int accept;
     int K;                   // walker chunks
-    int32_t chunk_first[16]; // first walker of every chunk
+    const int32_t* chunk_first;   // DEVICE [K]: first walker of every chunk (gb_chunk_bounds_kernel)
     const double* logq;
     const double* logu;
     const double* beta;
@@ -258,6 +258,39 @@ __global__ void __launch_bounds__(256) gb_prep_kernel(PrepArgs a) {
         if ((int)lane == leader) base = atomicAdd(a.counts + c, __popc(m));
         base = __shfl_sync(0xffffffffu, base, leader);
         if (cls == c) a.lists[(int64_t)c * a.B + base + __popc(m & ((1u << lane) - 1))] = (int32_t)b | (use_old ? (int32_t)0x80000000 : 0);
+    }
+}
+
+// gb_delta_loglike_accept, before the binning: rows per walker of THIS batch ...
+__global__ void __launch_bounds__(256) gb_walker_hist_kernel(const int32_t* __restrict__ walker_index, int64_t B, int n_walkers,
+                                                             int32_t* hist) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = b < B ? walker_index[b] : -1;
+    const bool ok = w >= 0 && w < n_walkers;
+    const unsigned m0 = __ballot_sync(0xffffffffu, ok);
+    if (ok) {
+        const unsigned m = __match_any_sync(m0, w);
+        if ((int)(threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(hist + w, __popc(m));
+    }
+}
+// ... and the walker chunks cut from it: chunk sizes (in ROWS) fall off geometrically, ratio 3/4.  The accepted rows of
+// chunk c are moved into the residual while chunk c + 1 is evaluated, about one 4 KB piece per evaluated row, so a chunk
+// must not be much smaller than the one before it; and what the last chunk accepts is left to the closing launch, so the
+// last chunk is the smallest.  A batch that touches only some of the walkers is cut by the rows it has, not by walker index.
+__global__ void gb_chunk_bounds_kernel(const int32_t* __restrict__ hist, int n_walkers, int K, int64_t B, int32_t* chunk_first) {
+    double total = 0.0, sz = 1.0;
+    for (int k = 0; k < K; k++, sz *= 0.75) total += sz;
+    int64_t rows = 0;
+    for (int w = 0; w < n_walkers; w++) rows += hist[w];
+    double cum = 0.0;
+    sz = 1.0;
+    int w = 0;
+    int64_t seen = 0;
+    for (int k = 0; k < K; k++, sz *= 0.75) {
+        const int64_t target = (int64_t)(cum / total * (double)rows + 0.5);   // rows before chunk k
+        while (w < n_walkers && seen < target) seen += hist[w++];
+        chunk_first[k] = k == 0 ? 0 : w;
+        cum += sz;
     }
 }
 
@@ -1415,7 +1448,8 @@ struct gb_ctx {
     KeptEnt* d_ent;
     double4* d_accpar;
     Piece* d_pieces;        // fused update: accepted windows cut into staging-buffer sized pieces
-    int64_t cap_wk, cap_ent, cap_accpar, cap_pieces;
+    int32_t* d_whist;       // rows per walker of the batch (walker chunks)
+    int64_t cap_wk, cap_ent, cap_accpar, cap_pieces, cap_whist;
     int grid_blocks[kNumClasses];   // resident CTAs per SM * SMs, per class
     int grid_blocks_acc[kNumClasses];   // the same for the gb_delta_loglike_accept instantiations
     int grid_blocks_dir[kNumClasses];   // and for the DIRECT (one-launch) instantiations
@@ -1528,7 +1562,7 @@ struct Call {
 
 constexpr int kMaxChunks = 16;           // walker chunks of gb_delta_loglike_accept
 constexpr int64_t kDirectMaxRows = 8192; // batches up to this size with one window length and one move type: one launch
-constexpr int kWkHeader = 8;             // ints before the per-bin arrays of d_wk
+constexpr int kWkHeader = 8 + kMaxChunks; // ints before the per-bin arrays of d_wk (counters, then the chunks' first walkers)
 constexpr int kWkInts = kWkHeader + 4 * kNumClasses * kMaxChunks;
 
 // scatter of list positions [from the claim counter (rest) or 0 (all), list cursor) of the last gb_delta_loglike_accept call
@@ -1658,9 +1692,11 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
         if ((rc = ensure_cap(ctx, &ctx->d_wk, &ctx->cap_wk, kWkInts))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_ent, &ctx->cap_ent, c.B + ent_slack))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_accpar, &ctx->cap_accpar, c.B))) return rc;
+        if (K > 1 && (rc = ensure_cap(ctx, &ctx->d_whist, &ctx->cap_whist, nw))) return rc;
         if (K > 1 && (rc = ensure_cap(ctx, &ctx->d_pieces, &ctx->cap_pieces, (2 * c.sum_bins + store_slack) / kPieceElems + 1024))) return rc;
         GB_CUDA(ctx, cudaMemsetAsync(ctx->d_wk, 0, sizeof(int32_t) * kWkInts, st));
     }
+    int32_t* chunk_first = ctx->d_wk ? ctx->d_wk + 8 : nullptr;   // zeroed with the counters: one chunk = every walker in chunk 0
     int32_t* bin_count = ctx->d_wk ? ctx->d_wk + kWkHeader : nullptr;
     int32_t* bin_off = bin_count ? bin_count + kNumClasses * kMaxChunks : nullptr;
     int32_t* bin_cursor = bin_count ? bin_count + 2 * kNumClasses * kMaxChunks : nullptr;
@@ -1698,19 +1734,12 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     if (c.accept) {   // binned work lists: count the rows of every (class, walker chunk) bin, scan, then the full pass
         p.accept = 1;
         p.K = K;
-        // Chunk sizes fall off geometrically (ratio 3/4): the accepted rows of chunk c are moved into the residual while
-        // chunk c + 1 is evaluated, about one 4 KB piece per evaluated row, so a chunk must not be much smaller than the
-        // one before it; and what the last chunk accepts is left to the closing launch, so the last chunk is the smallest.
-        {
-            double total = 0.0, sz = 1.0, cum = 0.0;
-            for (int k = 0; k < K; k++, sz *= 0.75) total += sz;
-            sz = 1.0;
-            for (int k = 0; k < K; k++, sz *= 0.75) {
-                int first = (int)(cum / total * nw + 0.5);
-                if (k > 0 && first <= p.chunk_first[k - 1]) first = p.chunk_first[k - 1] + 1;   // K <= n_walkers: room for all
-                p.chunk_first[k] = k == 0 ? 0 : first;
-                cum += sz;
-            }
+        p.chunk_first = chunk_first;
+        if (K > 1) {
+            GB_CUDA(ctx, cudaMemsetAsync(ctx->d_whist, 0, sizeof(int32_t) * (size_t)nw, st));
+            gb_walker_hist_kernel<<<pgrid, 256, 0, st>>>(c.walker_index, c.B, nw, ctx->d_whist);
+            gb_chunk_bounds_kernel<<<1, 1, 0, st>>>(ctx->d_whist, nw, K, c.B, chunk_first);
+            ctx->launches += 2;
         }
         p.logq = c.logq;
         p.logu = c.logu;
@@ -1993,6 +2022,7 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_ent);
     cudaFree(ctx->d_accpar);
     cudaFree(ctx->d_pieces);
+    cudaFree(ctx->d_whist);
     cudaFree(ctx->d_stage);
     if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
     if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
