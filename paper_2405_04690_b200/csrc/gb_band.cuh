@@ -420,10 +420,10 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                         sRA[i] = {sRA[i].re + oa.re, sRA[i].im + oa.im};
                         sRE[i] = {sRE[i].re + oe.re, sRE[i].im + oe.im};
                         if (wb) {
-                            atomicAdd(wA + 2 * e, oa.re);
-                            atomicAdd(wA + 2 * e + 1, oa.im);
-                            atomicAdd(wE + 2 * e, oe.re);
-                            atomicAdd(wE + 2 * e + 1, oe.im);
+                            red_add_f64(wA + 2 * e, oa.re);
+                            red_add_f64(wA + 2 * e + 1, oa.im);
+                            red_add_f64(wE + 2 * e, oe.re);
+                            red_add_f64(wE + 2 * e + 1, oe.im);
                         }
                     }
                 }
@@ -438,10 +438,10 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                         sRA[i] = {sRA[i].re - ha.re, sRA[i].im - ha.im};
                         sRE[i] = {sRE[i].re - he.re, sRE[i].im - he.im};
                         if (wb) {
-                            atomicAdd(wA + 2 * e, -ha.re);
-                            atomicAdd(wA + 2 * e + 1, -ha.im);
-                            atomicAdd(wE + 2 * e, -he.re);
-                            atomicAdd(wE + 2 * e + 1, -he.im);
+                            red_add_f64(wA + 2 * e, -ha.re);
+                            red_add_f64(wA + 2 * e + 1, -ha.im);
+                            red_add_f64(wE + 2 * e, -he.re);
+                            red_add_f64(wE + 2 * e + 1, -he.im);
                         }
                     }
                 }

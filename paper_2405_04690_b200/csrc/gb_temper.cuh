@@ -238,10 +238,10 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
                         const int64_t e = i_first + i;
                         if (e < 0 || e >= a.n_f) continue;
                         const cx da = dA[i], de = dE[i];
-                        atomicAdd(wA + 2 * e, -da.re);
-                        atomicAdd(wA + 2 * e + 1, -da.im);
-                        atomicAdd(wE + 2 * e, -de.re);
-                        atomicAdd(wE + 2 * e + 1, -de.im);
+                        red_add_f64(wA + 2 * e, -da.re);
+                        red_add_f64(wA + 2 * e + 1, -da.im);
+                        red_add_f64(wE + 2 * e, -de.re);
+                        red_add_f64(wE + 2 * e + 1, -de.im);
                     }
                 }
             } else if (s_acc && wb) {   // r_i += delta, r_j -= delta
@@ -249,14 +249,14 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
                     const int64_t e = i_first + i;
                     if (e < 0 || e >= a.n_f) continue;
                     const cx da = dA[i], de = dE[i];
-                    atomicAdd(rAi + 2 * e, da.re);
-                    atomicAdd(rAi + 2 * e + 1, da.im);
-                    atomicAdd(rEi + 2 * e, de.re);
-                    atomicAdd(rEi + 2 * e + 1, de.im);
-                    atomicAdd(rAj + 2 * e, -da.re);
-                    atomicAdd(rAj + 2 * e + 1, -da.im);
-                    atomicAdd(rEj + 2 * e, -de.re);
-                    atomicAdd(rEj + 2 * e + 1, -de.im);
+                    red_add_f64(rAi + 2 * e, da.re);
+                    red_add_f64(rAi + 2 * e + 1, da.im);
+                    red_add_f64(rEi + 2 * e, de.re);
+                    red_add_f64(rEi + 2 * e + 1, de.im);
+                    red_add_f64(rAj + 2 * e, -da.re);
+                    red_add_f64(rAj + 2 * e + 1, -da.im);
+                    red_add_f64(rEj + 2 * e, -de.re);
+                    red_add_f64(rEj + 2 * e + 1, -de.im);
                 }
                 __threadfence();
             }

@@ -560,6 +560,12 @@ struct WinBatch {
         }
     }
 };
+// FP64 add into the residual, resolved in L2, no return value.  Spelled out in PTX: atomicAdd(double*) on a pointer whose
+// address space the compiler cannot prove compiles to a generic ATOM with a compare-and-swap fallback loop
+// (gb_temper_kernel<128> did), and with a fence behind it to ATOMG instead of RED.
+__device__ __forceinline__ void red_add_f64(double* p, double v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(__cvta_generic_to_global(p)), "d"(v) : "memory");
+}
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
