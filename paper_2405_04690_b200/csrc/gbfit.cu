@@ -307,13 +307,14 @@ __global__ void gb_bin_scan_kernel(const int32_t* __restrict__ count, int32_t* o
 // barrier of a group of G threads (the first G threads of the CTA, whole warps): a one-warp group only needs the
 // warp-level barrier; larger groups use named barrier 1 with a thread count, so that in the band / ladder kernels
 // (whose CTAs are wider than the FFT group) the first G threads can run the FFT while the others wait at cta_sync
+// (the SWAP kernels run two groups side by side, one per waveform: group g uses named barrier 1 + g)
 template <int G>
-__device__ __forceinline__ void group_sync() {
+__device__ __forceinline__ void group_sync(int bar = 1) {
 #if GB_WARP_SYNC
     if (G == 32) __syncwarp();
-    else asm volatile("bar.sync 1, %0;" ::"n"(G) : "memory");
+    else asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(G) : "memory");
 #else
-    asm volatile("bar.sync 1, %0;" ::"n"(G) : "memory");
+    asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(G) : "memory");
 #endif
 }
 // barrier of the whole CTA of T threads (barrier 0)
@@ -330,10 +331,10 @@ __device__ __forceinline__ void cta_sync() {
     {                                                                 \
         StageRegs<N_, R_> rg;                                         \
         fft_stage_read<N_, R_>(buf, ht, rg);                          \
-        group_sync<Plan<N_>::G>();                                    \
+        group_sync<Plan<N_>::G>(bar);                                 \
         fft_stage_compute<N_, R_, Ns_>(tw, ht, rg);                   \
         fft_stage_store<N_, R_, Ns_>(buf, ht, rg);                    \
-        group_sync<Plan<N_>::G>();                                    \
+        group_sync<Plan<N_>::G>(bar);                                 \
     }
 #define GB_STAGE_L(N_, R_, Ns_)                                       \
     {                                                                 \
@@ -343,7 +344,7 @@ __device__ __forceinline__ void cta_sync() {
         fft_last_to_bins<N_, R_>(rg, h);                              \
     }
 template <int N>
-__device__ __forceinline__ void fft_store(cx* bA, cx* bE, const cx* __restrict__ tw, int tid) {
+__device__ __forceinline__ void fft_store(cx* bA, cx* bE, const cx* __restrict__ tw, int tid, int bar = 1) {
     constexpr int H = Plan<N>::G / 2;
     cx* buf = tid < H ? bA : bE;
     const int ht = tid < H ? tid : tid - H;
@@ -354,6 +355,7 @@ __device__ __forceinline__ void fft_store(cx* bA, cx* bE, const cx* __restrict__
 }
 template <int N>
 __device__ __forceinline__ void fft_regs(cx* bA, cx* bE, const cx* __restrict__ tw, int tid, cx* h) {
+    constexpr int bar = 1;
     constexpr int H = Plan<N>::G / 2;
     cx* buf = tid < H ? bA : bE;
     const int ht = tid < H ? tid : tid - H;
@@ -408,7 +410,7 @@ struct OrbitRegs<N, false> {
 // sample j is evaluated.
 template <int N, int G, bool FAST>
 __device__ __forceinline__ void slow_part(const SrcConst* s_src, const double* __restrict__ orbit, cx* bA, cx* bE,
-                                          double Tobs, double tau, int tid) {
+                                          double Tobs, double tau, int tid, int bar = 1) {
     constexpr int S = N / G;
     const double dtN = Tobs / (double)N;
     const double scale = (tid & 1) ? -Tobs / (2.0 * N) : Tobs / (2.0 * N);   // G is even: parity of n = parity of tid
@@ -430,7 +432,7 @@ __device__ __forceinline__ void slow_part(const SrcConst* s_src, const double* _
         bA[pad_idx<N>(n)] = {As.re, As.im};
         bE[pad_idx<N>(n)] = {Es.re, Es.im};
     }
-    group_sync<G>();
+    group_sync<G>(bar);
 }
 
 // sum NV per-thread values over the group; result valid in thread 0
@@ -831,9 +833,14 @@ __global__ void gb_ready_kernel(const int32_t* ent_cursor, int32_t* ent_done, co
 // -1 marks the end of the list.
 // VAR: 0 = the batched kernels; 1 = gb_delta_loglike_accept; 2 = DIRECT, the one-launch path of small uniform batches (no
 // prep kernel, no work lists: CTA c takes rows c, c + gridDim.x, ... and thread 0 works out each row's record itself)
+// SWAP kernels: a CTA is TWO groups of G threads that compute the two waveforms of a row side by side (group 0 the old
+// source, group 1 the new one, each with its own buffers and named barrier) and share the inner products: the same
+// shared-memory footprint per CTA as one group doing them one after the other, but twice the threads, so the SM holds 16
+// warps instead of 12 and a row takes half as long.
 template <int N, bool SWAP, bool FAST, int VAR>
-__global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kernel(MainArgs a) {
+__global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>::G * (SWAP ? 2 : 1))) gb_main_kernel(MainArgs a) {
     constexpr int G = Plan<N>::G;
+    constexpr int T = SWAP ? 2 * G : G;   // threads of the CTA
     constexpr int S = N / G;
     constexpr int PN = padded_len<N>();
     constexpr int NS = SWAP ? 2 : 1;
@@ -844,7 +851,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     cx* bufA1 = bufE0 + PN;                           // SWAP: the new source; first = old
     cx* bufE1 = bufA1 + PN;
     __shared__ __align__(16) SrcConst s_src[2][NS];   // [buffer][0 = old or only, 1 = new (SWAP)]
-    __shared__ double s_red[(G / 32) * 5 + 1];
+    __shared__ double s_red[(T / 32) * 5 + 1];
 
     __shared__ int s_ent[2];
     __shared__ int s_pos[2];   // list positions of the entries in s_ent (gb_delta_loglike_keep)
@@ -852,6 +859,12 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
     __shared__ long long s_off;                  // store offset of this item's window, -1: rejected
 
     const int tid = threadIdx.x;
+    const int grp = SWAP ? tid / G : 0;      // SWAP: which waveform this thread computes
+    const int lt = SWAP ? tid - grp * G : tid;
+    auto item_sync = [&]() {                 // barrier of all threads that work on the item
+        if (SWAP) __syncthreads();
+        else group_sync<G>();
+    };
     constexpr bool accept = VAR == 1 && !SWAP;   // gb_delta_loglike_accept (its own instantiation: the plain kernels carry none of it)
     constexpr bool direct = VAR == 2 && !SWAP;   // one-launch path of small batches
     const int bin = accept ? cls * a.K + a.chunk : cls;   // accept: the lists are binned by (class, walker chunk)
@@ -952,7 +965,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         s_pos[1] = t + 1;
         t_nx2 = t + 2;
     }
-    group_sync<G>();
+    item_sync();
     int e_cur = s_ent[0], e_nxt = s_ent[1];
     int pos_cur = s_pos[0], pos_nxt = s_pos[1];
     const int64_t keep_base = (a.wkeep && !accept) ? keep_class_base(a.counts, cls) : 0;
@@ -968,7 +981,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         if (has_nxt) fetch(e_nxt, buf ^ 1);
         cp_async_commit();
         cp_async_wait<1>();            // this item's record(s) have landed (the next item's may be in flight)
-        group_sync<G>();
+        item_sync();
         const SrcConst* rec = s_src[buf];
         const int64_t b = e_cur & 0x7fffffff;
         const int mv = rec[0].move;
@@ -984,12 +997,10 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 if (rec[0].fast) slow_part<N, G, true>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
                 else slow_part<N, G, false>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
             }
+        } else if (SWAP) {   // group 0: the old source into buffers 0, group 1: the new one into buffers 1
+            slow_part<N, G, FAST>(&rec[grp ? NS - 1 : 0], a.orbit, grp ? bufA1 : bufA0, grp ? bufE1 : bufE0, a.Tobs, a.tau, lt, 1 + grp);
         } else {
             slow_part<N, G, FAST>(&rec[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-        }
-        if (SWAP) {
-            fft_store<N>(bufA0, bufE0, a.tw, tid);
-            slow_part<N, G, FAST>(&rec[NS - 1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
         }
         // (thread 0) next ticket and the list entry of the ticket taken one item ago: issued here, after the
         // register-hungry slow part, and consumed at the end of the item, behind the FFT and the epilogue
@@ -1005,7 +1016,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         // ---- ask L2 for the next item's residual / PSD window
         if (GB_L2_PREFETCH && a.mode == MODE_DLNL && has_nxt) {
             cp_async_wait<0>();
-            group_sync<G>();
+            item_sync();
             const SrcConst& nx = s_src[buf ^ 1][NS - 1];
             const int64_t i0 = nx.kmin - a.k_lo;
             const size_t nf = (size_t)a.n_f;
@@ -1019,7 +1030,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 const double* pA = rAn + 2 * (i0 + 8 * tid);
                 const double* pE = rEn + 2 * (i0 + 8 * tid);
 #pragma unroll
-                for (int l = 0; l <= N / 8; l += G) {      // 128-byte lines of the complex128 windows
+                for (int l = 0; l <= N / 8; l += T) {      // 128-byte lines of the complex128 windows
                     if (l + tid <= N / 8) {
                         prefetch_l2(pA + 16 * l);
                         prefetch_l2(pE + 16 * l);
@@ -1028,21 +1039,21 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 const double* pSA = SAn + i0 + 16 * tid;
                 const double* pSE = SEn + i0 + 16 * tid;
 #pragma unroll
-                for (int l = 0; l <= N / 16; l += G) {     // and of the f64 PSD windows
+                for (int l = 0; l <= N / 16; l += T) {     // and of the f64 PSD windows
                     if (l + tid <= N / 16) {
                         prefetch_l2(pSA + 16 * l);
                         prefetch_l2(pSE + 16 * l);
                     }
                 }
             } else {
-                for (int l = tid; l <= N / 8; l += G) {
+                for (int l = tid; l <= N / 8; l += T) {
                     const int64_t i = i0 + 8 * l;
                     if (i >= 0 && i < a.n_f) {
                         prefetch_l2(rAn + 2 * i);
                         prefetch_l2(rEn + 2 * i);
                     }
                 }
-                for (int l = tid; l <= N / 16; l += G) {
+                for (int l = tid; l <= N / 16; l += T) {
                     const int64_t i = i0 + 16 * l;
                     if (i >= 0 && i < a.n_f) {
                         prefetch_l2(SAn + i);
@@ -1056,8 +1067,12 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
         //      h[m] = bin ht + H m of this thread's channel (threads [0, H): A, [H, G): E)
         constexpr int H = G / 2, M = N / H;
         cx h[M];
-        if (SWAP) fft_store<N>(bufA1, bufE1, a.tw, tid);
-        else fft_regs<N>(bufA0, bufE0, a.tw, tid, h);
+        if (SWAP) {
+            fft_store<N>(grp ? bufA1 : bufA0, grp ? bufE1 : bufE0, a.tw, lt, 1 + grp);
+            __syncthreads();   // both windows are complete
+        } else {
+            fft_regs<N>(bufA0, bufE0, a.tw, tid, h);
+        }
         const int ch = tid >= H ? 1 : 0;
         const int ht = tid - ch * H;
 
@@ -1082,6 +1097,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                 const double* SE = a.psd + ((size_t)prow * 2 + 1) * nf;
                 const bool inv = a.psd_is_inverse != 0;
                 const double norm = 4.0 / a.Tobs;
+                constexpr int ST = N / T;                        // SWAP: bins per thread (both channels), all T threads
                 constexpr int CH = SWAP ? 2 : (S < 4 ? S : 4);   // bins per thread whose loads are in flight together
                 if (!SWAP) {
                     // this thread's channel: bins ht + H m (consecutive threads, consecutive bins)
@@ -1171,22 +1187,22 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     const bool inband1 = i1w >= 0 && i1w + N <= a.n_f;
                     double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // aa, ra, ao, oo, ro
 #pragma unroll
-                    for (int m0 = 0; m0 < S; m0 += CH) {
+                    for (int m0 = 0; m0 < ST; m0 += CH) {
                         WinBatch<CH> wn, wo;   // the new source's window and the old one's (equal when shift == 0)
                         if (a.mode == MODE_OVERLAP) {      // no residual: weights only
-                            wn.template load_weights<G>(SA, SE, i1w + tid + G * m0, a.n_f, inv);
-                            wo.template load_weights<G>(SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                            wn.template load_weights<T>(SA, SE, i1w + tid + T * m0, a.n_f, inv);
+                            wo.template load_weights<T>(SA, SE, i0w + tid + T * m0, a.n_f, inv);
                         } else if (inband0 && inband1) {
-                            wn.template load<G, false>(rA, rE, SA, SE, i1w + tid + G * m0, a.n_f, inv);
-                            if (shift != 0) wo.template load<G, false>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                            wn.template load<T, false>(rA, rE, SA, SE, i1w + tid + T * m0, a.n_f, inv);
+                            if (shift != 0) wo.template load<T, false>(rA, rE, SA, SE, i0w + tid + T * m0, a.n_f, inv);
                             else wo = wn;
                         } else {
-                            wn.template load<G, true>(rA, rE, SA, SE, i1w + tid + G * m0, a.n_f, inv);
-                            wo.template load<G, true>(rA, rE, SA, SE, i0w + tid + G * m0, a.n_f, inv);
+                            wn.template load<T, true>(rA, rE, SA, SE, i1w + tid + T * m0, a.n_f, inv);
+                            wo.template load<T, true>(rA, rE, SA, SE, i0w + tid + T * m0, a.n_f, inv);
                         }
 #pragma unroll
                         for (int c = 0; c < CH; c++) {
-                            const int j = tid + G * (m0 + c);
+                            const int j = tid + T * (m0 + c);
                             {
                                 const cx ha = bufA1[pad_idx<N>(j)], he = bufE1[pad_idx<N>(j)];
                                 const cx ra = wn.ra[c], re = wn.re[c];
@@ -1208,7 +1224,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                             }
                         }
                     }
-                    group_reduce<G, 5>(v, s_red, tid);
+                    group_reduce<T, 5>(v, s_red, tid);
                     if (tid == 0) {
                         const double aa = norm * v[0], ra = norm * v[1], ao = norm * v[2], oo = norm * v[3],
                                      ro = norm * v[4];
@@ -1249,8 +1265,8 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
                     }
                 } else
 #pragma unroll
-                for (int m = 0; m < S; m++) {
-                    const int j = tid + G * m;
+                for (int m = 0; m < N / T; m++) {
+                    const int j = tid + T * m;
                     int64_t i = kmin0 + j - a.k_lo;
                     if (i >= 0 && i < a.n_f) {
                         const cx ha = bufA0[pad_idx<N>(j)], he = bufE0[pad_idx<N>(j)];
@@ -1277,7 +1293,7 @@ __global__ void __launch_bounds__(Plan<N>::G, GB_TPSM / Plan<N>::G) gb_main_kern
             s_pos[0] = t_nx2;
             t_nx2 = t_nx3;
         }
-        group_sync<G>();   // the waveform buffers, s_red and this half of s_src are reused from here on
+        item_sync();   // the waveform buffers, s_red and this half of s_src are reused from here on
         if (fuse && tid == 0) sc_next_piece(a, s_scs, stage);   // second checkpoint of the item
         if (!has_nxt) break;
         e_cur = e_nxt;
@@ -1513,7 +1529,7 @@ int setup_kernel(gb_ctx* ctx) {
     const size_t smem = main_smem_bytes<N, SWAP, VAR == 1>();
     GB_CUDA(ctx, cudaFuncSetAttribute(gb_main_kernel<N, SWAP, FAST, VAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST, VAR>, Plan<N>::G, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_main_kernel<N, SWAP, FAST, VAR>, Plan<N>::G * (SWAP ? 2 : 1), smem));
     if (nb < 1) return set_err(ctx, GB_ERR_CUDA, "kernel class %d does not fit on an SM", cls);
     (VAR == 1 ? ctx->grid_blocks_acc : VAR == 2 ? ctx->grid_blocks_dir : ctx->grid_blocks)[cls] = nb * ctx->num_sms;
     return GB_OK;
@@ -1525,7 +1541,7 @@ int launch_main(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
     a.orbit = ctx->d_orbit[cls >> 2];
     int64_t grid = (VAR == 1 ? ctx->grid_blocks_acc : VAR == 2 ? ctx->grid_blocks_dir : ctx->grid_blocks)[cls];
     if (grid > B) grid = B;
-    gb_main_kernel<N, SWAP, FAST, VAR><<<(unsigned)grid, Plan<N>::G, main_smem_bytes<N, SWAP, VAR == 1>(), st>>>(a);
+    gb_main_kernel<N, SWAP, FAST, VAR><<<(unsigned)grid, Plan<N>::G * (SWAP ? 2 : 1), main_smem_bytes<N, SWAP, VAR == 1>(), st>>>(a);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
