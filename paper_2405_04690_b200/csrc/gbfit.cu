@@ -1479,6 +1479,8 @@ struct gb_ctx {
     void* d_stage;
     size_t cap_stage;
     // copy streams and events of the *_host forms (chunked: the copies of chunk i+1 overlap the kernels of chunk i)
+    cudaStream_t s_side[3];        // the class kernels of one call are independent: they are spread over the caller's stream
+    cudaEvent_t ev_fork, ev_join[3];   // and these three, so that the tail of one overlaps the start of the next
     cudaStream_t s_in, s_out;
     cudaEvent_t ev_start, ev_in[kHostChunks], ev_done[kHostChunks];
     int64_t launches;
@@ -1547,13 +1549,44 @@ int launch_main(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
     return GB_OK;
 }
 
+// The class kernels of one call work on disjoint rows, so they may run concurrently: they are dealt round-robin to the
+// caller's stream and three context-owned streams (fork / join with events; capturable in a CUDA graph).  Every grid is
+// persistent and fills the GPU, so in effect the CTAs of the next class start as those of the current one run out of rows:
+// the launch tails overlap, and launches that find an empty list cost nothing on the critical path.
+struct Fan {
+    gb_ctx* ctx;
+    cudaStream_t main;
+    bool on;
+    int n;
+    cudaStream_t next() {
+        if (!on) return main;
+        const int i = n++ & 3;
+        return i == 0 ? main : ctx->s_side[i - 1];
+    }
+    int begin() {
+        n = 0;
+        if (!on) return GB_OK;
+        GB_CUDA(ctx, cudaEventRecord(ctx->ev_fork, main));
+        for (int i = 0; i < 3; i++) GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_side[i], ctx->ev_fork, 0));
+        return GB_OK;
+    }
+    int end() {
+        if (!on) return GB_OK;
+        for (int i = 0; i < 3; i++) {
+            GB_CUDA(ctx, cudaEventRecord(ctx->ev_join[i], ctx->s_side[i]));
+            GB_CUDA(ctx, cudaStreamWaitEvent(main, ctx->ev_join[i], 0));
+        }
+        return GB_OK;
+    }
+};
+
 // the fast-path kernel of a class, then the general one for the rows outside its limits (usually none:
 // that launch finds an empty list and returns at once)
 template <int N, bool SWAP>
-int launch_pair(gb_ctx* ctx, MainArgs& a, int64_t B, cudaStream_t st) {
-    int rc = launch_main<N, SWAP, true>(ctx, a, B, st);
+int launch_pair(gb_ctx* ctx, MainArgs& a, int64_t B, Fan& fan) {
+    int rc = launch_main<N, SWAP, true>(ctx, a, B, fan.next());
     if (rc) return rc;
-    return launch_main<N, SWAP, false>(ctx, a, B, st);
+    return launch_main<N, SWAP, false>(ctx, a, B, fan.next());
 }
 
 struct Call {
@@ -1847,21 +1880,26 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
                 gb_ready_kernel<<<1, 1, 0, st>>>(a.ent_cursor, ctx->d_wk + 5, ctx->d_wk + 6, a.sc_claim, ctx->d_wk + 4);
                 ctx->launches += 2;
             }
-            // the rows outside the fast path first (usually none), then the fast kernels
+            // the rows outside the fast path first (usually none), then the fast kernels; the classes of a chunk side by side
+            // (only when the call is one chunk: with the fused update running, classes side by side measured 47.3 instead of
+            // 46.7 ms on config 5 -- the launches of a chunk are then kept in order)
+            Fan fan{ctx, st, c.n_bins != nullptr && K == 1, 0};
+            if ((rc = fan.begin())) return rc;
             for (int pass = 0; pass < 2; pass++) {
                 for (int cN = 3; cN >= 0; cN--) {
                     const int Nc = 128 << cN;
                     if (!c.n_bins && Nc != c.N) continue;
                     a.pool_r = pool_r[cN];
                     switch (Nc) {
-                        case 128: rc = pass ? launch_main<128, false, true, 1>(ctx, a, c.B, st) : launch_main<128, false, false, 1>(ctx, a, c.B, st); break;
-                        case 256: rc = pass ? launch_main<256, false, true, 1>(ctx, a, c.B, st) : launch_main<256, false, false, 1>(ctx, a, c.B, st); break;
-                        case 512: rc = pass ? launch_main<512, false, true, 1>(ctx, a, c.B, st) : launch_main<512, false, false, 1>(ctx, a, c.B, st); break;
-                        default: rc = pass ? launch_main<1024, false, true, 1>(ctx, a, c.B, st) : launch_main<1024, false, false, 1>(ctx, a, c.B, st); break;
+                        case 128: rc = pass ? launch_main<128, false, true, 1>(ctx, a, c.B, fan.next()) : launch_main<128, false, false, 1>(ctx, a, c.B, fan.next()); break;
+                        case 256: rc = pass ? launch_main<256, false, true, 1>(ctx, a, c.B, fan.next()) : launch_main<256, false, false, 1>(ctx, a, c.B, fan.next()); break;
+                        case 512: rc = pass ? launch_main<512, false, true, 1>(ctx, a, c.B, fan.next()) : launch_main<512, false, false, 1>(ctx, a, c.B, fan.next()); break;
+                        default: rc = pass ? launch_main<1024, false, true, 1>(ctx, a, c.B, fan.next()) : launch_main<1024, false, false, 1>(ctx, a, c.B, fan.next()); break;
                     }
                     if (rc) return rc;
                 }
             }
+            if ((rc = fan.end())) return rc;
         }
         ctx->kept_B = c.B;
         ctx->kept_cap = a.wkeep_cap;
@@ -1886,28 +1924,31 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     // launch only the classes that can occur; largest windows first
     const bool may_swap = c.mode != MODE_WAVEFORM && (c.move ? true : c.move_all == GB_SWAP);   // MODE_OVERLAP: move_all = SWAP
     const bool may_single = c.mode == MODE_WAVEFORM || (c.move ? true : c.move_all != GB_SWAP);
+    Fan fan{ctx, st, c.n_bins != nullptr || (may_swap && may_single), 0};
+    if ((rc = fan.begin())) return rc;
     for (int cN = 3; cN >= 0; cN--) {
         const int Nc = 128 << cN;
         if (!c.n_bins && Nc != c.N) continue;
         if (may_swap) {
             switch (Nc) {
-                case 128: rc = launch_pair<128, true>(ctx, a, c.B, st); break;
-                case 256: rc = launch_pair<256, true>(ctx, a, c.B, st); break;
-                case 512: rc = launch_pair<512, true>(ctx, a, c.B, st); break;
-                default: rc = launch_pair<1024, true>(ctx, a, c.B, st); break;
+                case 128: rc = launch_pair<128, true>(ctx, a, c.B, fan); break;
+                case 256: rc = launch_pair<256, true>(ctx, a, c.B, fan); break;
+                case 512: rc = launch_pair<512, true>(ctx, a, c.B, fan); break;
+                default: rc = launch_pair<1024, true>(ctx, a, c.B, fan); break;
             }
             if (rc) return rc;
         }
         if (may_single) {
             switch (Nc) {
-                case 128: rc = launch_pair<128, false>(ctx, a, c.B, st); break;
-                case 256: rc = launch_pair<256, false>(ctx, a, c.B, st); break;
-                case 512: rc = launch_pair<512, false>(ctx, a, c.B, st); break;
-                default: rc = launch_pair<1024, false>(ctx, a, c.B, st); break;
+                case 128: rc = launch_pair<128, false>(ctx, a, c.B, fan); break;
+                case 256: rc = launch_pair<256, false>(ctx, a, c.B, fan); break;
+                case 512: rc = launch_pair<512, false>(ctx, a, c.B, fan); break;
+                default: rc = launch_pair<1024, false>(ctx, a, c.B, fan); break;
             }
             if (rc) return rc;
         }
     }
+    if ((rc = fan.end())) return rc;
     if (c.keep) {
         ctx->kept_B = c.B;
         ctx->kept_cap = 2 * c.sum_bins;
@@ -2006,6 +2047,11 @@ int gb_create(const gb_config* cfg, gb_ctx** out) {
     GB_CUDA(ctx, cudaMemcpy(ctx->d_tw, tw.data(), tw.size() * sizeof(double), cudaMemcpyHostToDevice));
     GB_CUDA(ctx, cudaMalloc(reinterpret_cast<void**>(&ctx->d_counts), sizeof(int32_t) * (2 * kNumClasses + 1)));
     GB_CUDA(ctx, cudaMemset(ctx->d_counts, 0, sizeof(int32_t) * (2 * kNumClasses + 1)));
+    for (int i = 0; i < 3; i++) {
+        GB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_side[i], cudaStreamNonBlocking));
+        GB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming));
+    }
+    GB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
     GB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking));
     GB_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking));
     GB_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming));
@@ -2046,6 +2092,11 @@ void gb_destroy(gb_ctx* ctx) {
     cudaFree(ctx->d_pieces);
     cudaFree(ctx->d_whist);
     cudaFree(ctx->d_stage);
+    for (int i = 0; i < 3; i++) {
+        if (ctx->s_side[i]) cudaStreamDestroy(ctx->s_side[i]);
+        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
     if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
     if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
