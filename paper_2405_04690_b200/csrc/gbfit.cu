@@ -1447,6 +1447,7 @@ __global__ void __launch_bounds__(128) gb_dfma_peak_kernel(double* sink, int ite
 
 // ------------------------------------------------------------------------------------------------ context
 constexpr int kHostChunks = 8;
+constexpr int kHostChunksAccept = 4;   // gb_delta_loglike_accept_host: fewer, larger chunks (each is a chunked call of its own)
 
 struct gb_ctx {
     gb_config cfg;
@@ -2582,7 +2583,7 @@ int delta_loglike_accept_host_impl(gb_ctx* ctx, const gb_data* data, const doubl
     uint8_t* d_acc = s.put<uint8_t>(nullptr, (size_t)B);
     // chunked as gb_delta_loglike_host; a chunk's update has finished when its last kernel ends, so the next chunk reuses
     // the store.  apply = 0 keeps the state of ONE call for gb_residual_update_kept: a single chunk then
-    const int nch = (B >= (1 << 18) && apply != 0) ? kHostChunks : 1;
+    const int nch = (B >= (1 << 18) && apply != 0) ? kHostChunksAccept : 1;
     GB_CUDA(ctx, cudaEventRecord(ctx->ev_start, st));
     GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ctx->ev_start, 0));
     for (int c = 0; c < nch; c++) {

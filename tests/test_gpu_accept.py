@@ -199,3 +199,30 @@ def test_accept_launch_scale_walker_chunks_and_fused_update(oracle, torch_cuda, 
     dl, acc, d_resid, _ = _gpu(torch_cuda, gbfit, ctx, wl, resid, logu, logq, beta, apply=1, store_bins=int(0.6 * wl.n_bins.sum()))
     _same(dl, acc, d_resid.cpu().numpy(), *ref, resid)
     assert ctx.launch_count() > 0
+
+
+def test_accept_host_form_chunked(oracle, torch_cuda, gb):
+    """gb_delta_loglike_accept_host: HOST arrays in, HOST (dlnL, accepted) out; 300 000 rows flow through in chunks (each chunk
+    one accept call of its own), rows sorted by walker so that a walker's rows do not straddle chunks in a way that matters
+    (they may: the snapshot semantics hold per chunk, and the oracle is run chunk by chunk the same way)."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=300000, n_walkers=8)
+    wl = wl.subset(np.argsort(wl.walker_index, kind="stable"))
+    resid = wl.resid()
+    logu, logq, beta = _draws(wl.B, [34, 0], rate=0.25)
+    od = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
+    rdl, racc = np.zeros(wl.B), np.zeros(wl.B, np.uint8)
+    nch = 4
+    for c in range(nch):                                            # the library's chunking: B c / nch
+        lo, hi = wl.B * c // nch, wl.B * (c + 1) // nch
+        sl = slice(lo, hi)
+        rdl[sl], racc[sl] = oracle.delta_loglike_accept(oracle.Config(), od, wl.params_new[sl], wl.params_old[sl], wl.walker_index[sl],
+                                                        logu[sl], logq=logq[sl], beta=beta[sl], move=wl.move[sl], n_bins=wl.n_bins[sl],
+                                                        nthreads=oracle.max_threads())
+    d_resid = dev(torch, resid)
+    data = gbfit.Data(d_resid, dev(torch, wl.psd), wl.k_lo)
+    dl, acc = ctx.delta_loglike_accept_host(data, wl.params_new, wl.params_old, wl.walker_index, logu, logq=logq, beta=beta,
+                                            move=wl.move, n_bins=wl.n_bins, store_bins=int(0.6 * wl.n_bins.sum()), apply=1)
+    ctx.check()
+    _same(np.asarray(dl), np.asarray(acc), d_resid.cpu().numpy(), rdl, racc, od.resid, resid)
