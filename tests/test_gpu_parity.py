@@ -511,6 +511,22 @@ def test_config5_full_size_sampled(oracle, torch_cuda, gb):
         dgot = d_resid[w].cpu().numpy() - keep[w]
         assert np.abs(dref).max() > 0
         assert np.abs(dgot - dref).max() <= 1e-9 * np.abs(dref).max(), w
+    # (c) the call bench.py times: the same step as ONE gb_delta_loglike_accept call (8 walker chunks, fused update).  The
+    #     residuals go back first (REMOVE of the same rows: equal to the initial ones to rounding); the seeded flags enter as
+    #     log u = -inf / +inf, so the decisions must reproduce them exactly
+    ctx.residual_update(data, None, d_p, d_w, move_all=gbfit.REMOVE, accepted=dev(torch, wl.accepted), n_bins=d_nb)
+    logu = np.where(wl.accepted != 0, -np.inf, np.inf)
+    store_bins = int(1.15 * wl.n_bins[wl.accepted != 0].astype(np.int64).sum()) + 1024
+    dl2, acc2 = ctx.delta_loglike_accept(data, d_p, None, d_w, dev(torch, logu), move_all=gbfit.ADD, n_bins=d_nb,
+                                         store_bins=store_bins, apply=1)
+    ctx.check()
+    assert np.array_equal(acc2.cpu().numpy() != 0, wl.accepted != 0)
+    dl2 = dl2.cpu().numpy()
+    assert np.abs(dl2[sample] - ref).max() <= TOL_DLNL and np.abs(dl2 - got).max() <= 1e-6
+    for i, w in enumerate(check_walkers):
+        dref = od.resid[i] - keep[w]
+        dgot = d_resid[w].cpu().numpy() - keep[w]
+        assert np.abs(dgot - dref).max() <= 1e-9 * np.abs(dref).max(), w
 
 
 # ------------------------------------------------------------------- row f4: normalised overlap of source pairs
