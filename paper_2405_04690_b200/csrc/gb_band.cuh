@@ -142,6 +142,9 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
     __shared__ int s_gk, s_ginside;                   // generated proposal: k, inside the prior box
     __shared__ double s_glq, s_glu;                   //                      logq, logu
     __shared__ int64_t s_kmin[kBandCacheSlots];       // window start of each cached current source
+    __shared__ double s_theta[kBandCacheSlots][8];    // generate mode: the band's CURRENT parameter rows ...
+    __shared__ int64_t s_run[kBandCacheSlots];        // ... and where each one's run of friends starts in the table
+    __shared__ int s_redo;                            // source whose run has to be searched again (it was just accepted)
     const int tid = threadIdx.x;
     const double nan = __longlong_as_double(0x7ff8000000000000LL);
     cx* cache = a.cache ? a.cache + (size_t)blockIdx.x * kBandCacheSlots * 2 * N : nullptr;
@@ -236,12 +239,27 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
         // friends search hint: the rows of the friends table inside the staged frequency range, widened by n_friends
         // (proposals are confined to the stage, so the run of a current source starts in there; the search checks it anyway)
         int64_t hint_lo = 0, hint_hi = 0;
-        if (a.gen && tid < 32) {
+        // bands of up to kBandCacheSlots sources keep their current parameter rows and the start of each source's run of
+        // friends on chip: the search (4-5 dependent table probes) then leaves the per-proposal chain -- it is done once
+        // per source here, all warps taking sources in turn, and again only for a source whose proposal was accepted
+        const bool gen_cached = a.gen && t.n_src <= kBandCacheSlots;
+        if (a.gen) {
+            const int lane = tid & 31;
             const int64_t nfr = min((int64_t)a.st.n_friends, a.st.n_group);
             const double f_lo = (double)t.k_first / a.Tobs, f_hi = (double)(t.k_first + t.n_stage) / a.Tobs;
-            hint_lo = max((int64_t)0, friend_run_start(a.st.group, a.st.n_group, 0, f_lo, tid, 0, a.st.n_group) - nfr);
-            hint_hi = min(a.st.n_group - nfr, friend_run_start(a.st.group, a.st.n_group, 0, f_hi, tid, 0, a.st.n_group));
+            hint_lo = max((int64_t)0, friend_run_start(a.st.group, a.st.n_group, 0, f_lo, lane, 0, a.st.n_group) - nfr);
+            hint_hi = min(a.st.n_group - nfr, friend_run_start(a.st.group, a.st.n_group, 0, f_hi, lane, 0, a.st.n_group));
             if (hint_hi < hint_lo) hint_hi = hint_lo;
+            if (gen_cached) {
+                for (int i = tid; i < 8 * t.n_src; i += G) s_theta[i >> 3][i & 7] = a.params[8 * (size_t)t.src_begin + i];
+                if (tid == 0) s_redo = -1;
+                cta_sync<G>();
+                for (int kk = tid >> 5; kk < t.n_src; kk += G / 32) {
+                    const int64_t s0 = friend_run_start(a.st.group, a.st.n_group, nfr, s_theta[kk][1], lane, hint_lo, hint_hi);
+                    if (lane == 0) s_run[kk] = s0;
+                }
+                cta_sync<G>();
+            }
         }
         for (int p = 0; p < t.n_prop; p++) {
             const int64_t ip = (int64_t)t.prop_begin + p;
@@ -258,10 +276,21 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                     philox4x32_10((uint32_t)ip, 0u, 0u, a.st.sweep, key0, key1, w0);
                     philox4x32_10((uint32_t)ip, 0u, 1u, a.st.sweep, key0, key1, w1);
                     const int kk = randint32(w0[0], t.n_src);
-                    const double* th = a.params + 8 * ((size_t)t.src_begin + kk);
+                    const double* th = gen_cached ? s_theta[kk] : a.params + 8 * ((size_t)t.src_begin + kk);
                     const int64_t nf = a.st.n_friends < a.st.n_group ? a.st.n_friends : a.st.n_group;
                     const int32_t jf = randint32(w0[1], (int32_t)nf);
-                    const int64_t s0 = friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid, hint_lo, hint_hi);
+                    if (gen_cached && s_redo >= 0) {   // the source accepted last has moved: its run of friends again
+                        const int kr = s_redo;
+                        const int64_t sr = friend_run_start(a.st.group, a.st.n_group, nf, s_theta[kr][1], tid, hint_lo, hint_hi);
+                        __syncwarp();
+                        if (tid == 0) {
+                            s_run[kr] = sr;
+                            s_redo = -1;
+                        }
+                        __syncwarp();
+                    }
+                    const int64_t s0 = gen_cached ? s_run[kk]
+                                                  : friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid, hint_lo, hint_hi);
                     const int64_t row = s0 + jf;
                     const double ua = uniform52(w0[2], w0[3]);
                     const double tz = __dadd_rn(__dmul_rn(__dadd_rn(a.st.stretch_a, -1.0), ua), 1.0);
@@ -445,7 +474,12 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                         }
                     }
                 }
-                if (tid < 8) theta_k[tid] = theta_p[tid];   // theta_j[k] <- theta'_k
+                if (tid < 8) {                              // theta_j[k] <- theta'_k
+                    const double v = theta_p[tid];
+                    theta_k[tid] = v;
+                    if (gen_cached) s_theta[k][tid] = v;
+                }
+                if (gen_cached && tid == 0) s_redo = k;
                 if (cached) {                               // and its window replaces the cached one
                     if (tid == 0) s_kmin[k] = s_src[1].kmin;
 #pragma unroll
