@@ -40,8 +40,10 @@
  *   - Residual semantic r = d - H: ADD subtracts the waveform, REMOVE adds it, SWAP adds old, subtracts new.
  *   - Window bins outside the stored band [k_lo, k_lo + n_f) contribute nothing to any inner product and
  *     are not scattered.
- *   - Tempering, priors and proposal densities (Eq. 13) are not applied: the caller does
- *     accept/reject.  Rows of one call are evaluated independently against the same residual snapshot.
+ *   - gb_waveform / gb_delta_loglike / gb_residual_update apply no tempering, prior or proposal density (Eq. 13,
+ *     PAPER.md:197): the caller does accept/reject.  gb_delta_loglike_accept, gb_band_sweep(_generate) and gb_temper_sweep
+ *     take the decision themselves (inverse temperatures, log q and the uniform draws are inputs, or generated in the
+ *     kernel).  Rows of one batched call are evaluated independently against the same residual snapshot.
  *   - A gb_ctx may be used from one host thread at a time.
  */
 #ifndef GBFIT_H
