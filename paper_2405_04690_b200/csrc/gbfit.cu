@@ -658,9 +658,14 @@ __device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned pari
         : "memory");
     return ok != 0;
 }
+// (the stored windows are read exactly once: L2 evict-first, so that they do not push out the residual lines the
+// evaluation shares between neighbouring rows)
 __device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
-                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(pol)
                  : "memory");
 }
 __device__ __forceinline__ void bulk_reduce_add_f64(void* gdst, const void* smem_src, unsigned bytes) {
@@ -1176,7 +1181,8 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
                             cx* dst = a.wkeep + off + (int64_t)ch * N + ht;
                             const double sg = mv == GB_REMOVE ? 1.0 : -1.0;   // the store holds the CHANGE of the residual
 #pragma unroll
-                            for (int m = 0; m < M; m++) dst[H * m] = {sg * h[m].re, sg * h[m].im};
+                            for (int m = 0; m < M; m++)   // streaming stores: read back once, much later -- not worth L2 lines
+                                __stcs(reinterpret_cast<double2*>(dst + H * m), make_double2(sg * h[m].re, sg * h[m].im));
                         }
                     }
                 } else {
