@@ -317,6 +317,13 @@ __device__ __forceinline__ void group_sync(int bar = 1) {
     asm volatile("bar.sync %0, %1;" ::"r"(bar), "n"(G) : "memory");
 #endif
 }
+// barrier of the H threads that transform ONE channel (the FFT stages of A and E never touch each other's buffer): a
+// warp-level barrier when the channel is one warp or less (N <= 512), else a named barrier of its own
+template <int H>
+__device__ __forceinline__ void chan_sync(int id) {
+    if (H <= 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(H) : "memory");
+}
 // barrier of the whole CTA of T threads (barrier 0)
 template <int T>
 __device__ __forceinline__ void cta_sync() {
@@ -331,10 +338,10 @@ __device__ __forceinline__ void cta_sync() {
     {                                                                 \
         StageRegs<N_, R_> rg;                                         \
         fft_stage_read<N_, R_>(buf, ht, rg);                          \
-        group_sync<Plan<N_>::G>(bar);                                 \
+        chan_sync<Plan<N_>::G / 2>(cbar);                             \
         fft_stage_compute<N_, R_, Ns_>(tw, ht, rg);                   \
         fft_stage_store<N_, R_, Ns_>(buf, ht, rg);                    \
-        group_sync<Plan<N_>::G>(bar);                                 \
+        chan_sync<Plan<N_>::G / 2>(cbar);                             \
     }
 #define GB_STAGE_L(N_, R_, Ns_)                                       \
     {                                                                 \
@@ -348,6 +355,7 @@ __device__ __forceinline__ void fft_store(cx* bA, cx* bE, const cx* __restrict__
     constexpr int H = Plan<N>::G / 2;
     cx* buf = tid < H ? bA : bE;
     const int ht = tid < H ? tid : tid - H;
+    const int cbar = 3 + 2 * (bar - 1) + (tid < H ? 0 : 1);   // named barrier of this group's channel (ids 3 .. 6)
     if constexpr (N == 128) { GB_FFT_PLAN_128(GB_STAGE_X, GB_STAGE_X) }
     if constexpr (N == 256) { GB_FFT_PLAN_256(GB_STAGE_X, GB_STAGE_X) }
     if constexpr (N == 512) { GB_FFT_PLAN_512(GB_STAGE_X, GB_STAGE_X) }
@@ -355,10 +363,10 @@ __device__ __forceinline__ void fft_store(cx* bA, cx* bE, const cx* __restrict__
 }
 template <int N>
 __device__ __forceinline__ void fft_regs(cx* bA, cx* bE, const cx* __restrict__ tw, int tid, cx* h) {
-    constexpr int bar = 1;
     constexpr int H = Plan<N>::G / 2;
     cx* buf = tid < H ? bA : bE;
     const int ht = tid < H ? tid : tid - H;
+    const int cbar = 3 + (tid < H ? 0 : 1);
     if constexpr (N == 128) { GB_FFT_PLAN_128(GB_STAGE_X, GB_STAGE_L) }
     if constexpr (N == 256) { GB_FFT_PLAN_256(GB_STAGE_X, GB_STAGE_L) }
     if constexpr (N == 512) { GB_FFT_PLAN_512(GB_STAGE_X, GB_STAGE_L) }
