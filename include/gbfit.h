@@ -229,6 +229,9 @@ int gb_residual_update_kept(gb_ctx *ctx, const gb_data *data, const uint8_t *acc
  *               semantics of step 1 hold exactly; a closing launch scatters what the last chunk accepted.  Smaller
  *               batches: as apply = 2
  *   apply = 2   the same decisions, the update as a separate launch after all evaluations
+ *               (after apply = 1 or 2 the accepted windows stay in the context like after apply = 0:
+ *               gb_residual_update_kept(ctx, data, NULL, 1, stream) undoes the call's update, e.g. for a step that the
+ *               caller rejects as a whole; with negate = 0 it would apply the rows a second time)
  *   logq, logu, beta   [B] DEVICE f64 (logq, beta may be NULL);  accepted_out [B] DEVICE uint8;  dlnL_out, aux_out as
  *               gb_delta_loglike.  Asynchronous on `stream`.
  */

@@ -1758,6 +1758,8 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
             store_slack += ctas * K * (pool_r[cN] - 1) * 2 * Nc;
             ent_slack += ctas * K * (pool_r[cN] - 1);
         }
+        if (K > 1 && (2 * c.sum_bins + store_slack) / kPieceElems + 1024 > 0x7fffffff)
+            return set_err(ctx, GB_ERR_INVALID, "store_bins too large for the fused update (piece positions are 32-bit)");
         if ((rc = ensure_cap(ctx, &ctx->d_wkeep, &ctx->cap_wkeep, 2 * c.sum_bins + store_slack))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_wk, &ctx->cap_wk, kWkInts))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_ent, &ctx->cap_ent, c.B + ent_slack))) return rc;

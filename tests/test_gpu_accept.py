@@ -87,8 +87,12 @@ def test_accept_fused_and_separate_update_match_the_oracle(oracle, torch_cuda, g
     logu, logq, beta = _draws(wl.B, [31, apply])
     ref = _oracle(oracle, wl, resid, logu, logq, beta)
     assert 0.2 < ref[1].mean() < 0.6
-    dl, acc, d_resid, _ = _gpu(torch_cuda, gbfit, ctx, wl, resid, logu, logq, beta, apply)
+    dl, acc, d_resid, data_acc = _gpu(torch_cuda, gbfit, ctx, wl, resid, logu, logq, beta, apply)
     _same(dl, acc, d_resid.cpu().numpy(), *ref, resid)
+    # the accepted windows stay in the context: negate = 1 undoes the call's update
+    ctx.residual_update_kept(data_acc, negate=True)
+    ctx.check()
+    assert np.abs(d_resid.cpu().numpy() - resid).max() <= 4e-16 * max(np.abs(resid).max(), np.abs(ref[2] - resid).max())
     # the same bits of delta lnL as the plain call
     data = gbfit.Data(dev(torch_cuda, resid), dev(torch_cuda, wl.psd), wl.k_lo)
     plain = ctx.delta_loglike(data, dev(torch_cuda, wl.params_new), dev(torch_cuda, wl.params_old),
