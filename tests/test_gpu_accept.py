@@ -230,3 +230,25 @@ def test_accept_host_form_chunked(oracle, torch_cuda, gb):
                                             move=wl.move, n_bins=wl.n_bins, store_bins=int(0.6 * wl.n_bins.sum()), apply=1)
     ctx.check()
     _same(np.asarray(dl), np.asarray(acc), d_resid.cpu().numpy(), rdl, racc, od.resid, resid)
+
+
+def test_accept_repeated_calls_agree(oracle, torch_cuda, gb):
+    """Race check without a sanitizer: the fused call repeated on fresh copies of the residual gives bit-identical delta lnL
+    and decisions every time, and final residuals that agree to the rounding order of the adds (400 000 rows, 2 walker
+    chunks, so the in-loop update, the piece kernel and the closing scatter all run)."""
+    gbfit, ctx = gb
+    torch = torch_cuda
+    wl = make_workload(3, B=400000, n_walkers=12)
+    resid = wl.resid()
+    logu, logq, beta = _draws(wl.B, [35, 0], rate=0.25)
+    first = None
+    for rep in range(3):
+        dl, acc, d_resid, _ = _gpu(torch, gbfit, ctx, wl, resid, logu, logq, beta, apply=1, store_bins=int(0.6 * wl.n_bins.sum()))
+        r1 = d_resid.cpu().numpy()
+        if first is None:
+            first = (dl, acc, r1)
+            assert 0.2 < acc.mean() < 0.6
+        else:
+            assert np.array_equal(dl, first[0]) and np.array_equal(acc, first[1])
+            change = np.abs(first[2] - resid).max()
+            assert np.abs(r1 - first[2]).max() <= 1e-12 * change + 4e-16 * np.abs(resid).max()
