@@ -307,6 +307,29 @@ int gb_band_sweep(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, i
                   const double *prop_logu, uint8_t *accepted_out, double *dlnL_out, void *stream);
 
 /*
+ * gb_band_sweep_static -- gb_band_sweep (Algorithm 1) for callers that cannot allocate device memory
+ * around the call: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same arguments,
+ * same kernel, same results as gb_band_sweep; the only scratch of that kernel, the per-CTA cache of the current sources'
+ * windows, lives in a file-scope device array of GB_STATIC_SCRATCH_BYTES (32 MiB) that every GPU which loads the library
+ * holds until exit, and the call performs no cudaMalloc, no cudaFree and no allocating library call (gb_create, the
+ * set-up, resolves the array's device address once per device).
+ *   limit     n_tasks * N <= GB_STATIC_MAX_TASK_BINS (256 tasks of N = 128 ... 32 of N = 1024: one resident CTA and one
+ *             32-window cache per task); a larger call returns GB_ERR_INVALID with the limit in gb_last_error and does
+ *             nothing -- use gb_band_sweep
+ *   sharing   every call on a device -- of every context -- uses the same array.  Nothing in it has to start at zero (a
+ *             CTA writes a cache slot before it reads it, so the contents an earlier call left are never read) and
+ *             nothing is cleared.  Calls that may OVERLAP on the GPU (different streams, or different contexts on one
+ *             device) race on it: issue them on one stream or order them with events.
+ * Asynchronous on `stream`; errors, flags and outputs as gb_band_sweep.
+ */
+#define GB_STATIC_SCRATCH_BYTES (32 * 1024 * 1024)
+#define GB_STATIC_MAX_TASK_BINS 32768
+int gb_band_sweep_static(gb_ctx *ctx, const gb_data *data, const gb_band_task *tasks, int64_t n_tasks, int N,
+                         int max_stage, double *params, const int32_t *prop_k, const double *prop_params,
+                         const double *prop_logq, const double *prop_logu, uint8_t *accepted_out, double *dlnL_out,
+                         void *stream);
+
+/*
  * gb_band_sweep_generate -- Algorithm 1 exactly as printed: the proposal step runs INSIDE the sequential
  * loop of each band, "k <- randint(0, g_j)", "theta'_k <- Make Proposal on theta", from the CURRENT
  * theta_k -- a stretch proposal built by the caller beforehand would use a stale theta_k as soon as an earlier proposal of

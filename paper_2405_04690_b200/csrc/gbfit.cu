@@ -20,6 +20,7 @@
 #include <stdarg.h>
 #include <stdio.h>
 #include <string.h>
+#include <mutex>
 
 #include <vector>
 
@@ -1499,6 +1500,7 @@ struct gb_ctx {
     cudaStream_t s_in, s_out;
     cudaEvent_t ev_start, ev_in[kHostChunks], ev_done[kHostChunks];
     int64_t launches;
+    cx* d_static;           // device address of g_static_scratch on cfg.device (gb_band_sweep_static)
     char err[512];
 };
 
@@ -1976,6 +1978,59 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------ static scratch
+// Scratch of gb_band_sweep_static, the entry point that allocates nothing: a file-scope array in device memory that every
+// GPU which loads this library holds until exit.  In HOST code the name g_static_scratch is only a stand-in for the symbol,
+// not a device address: a kernel handed &g_static_scratch[0] from the host would fault (or, where the GPU can reach host
+// memory, silently use the wrong memory).  The device address is resolved once per device by cudaGetSymbolAddress, with
+// that device current (static_scratch_setup, called by gb_create), and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char g_static_scratch[GB_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[kMaxDevices];   // [device] -> device address of g_static_scratch there (0: not resolved yet)
+
+// requires: cfg.device is the current device
+int static_scratch_setup(gb_ctx* ctx) {
+    const int d = ctx->cfg.device;
+    if (d < 0 || d >= kMaxDevices) return GB_OK;   // such a device gets no static scratch: gb_band_sweep_static says so
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[d]) {
+        void* p = nullptr;
+        GB_CUDA(ctx, cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255) != 0)
+            return set_err(ctx, GB_ERR_CUDA, "static scratch resolved to a bad address %p on device %d", p, d);
+        g_static_ptr[d] = p;
+    }
+    ctx->d_static = reinterpret_cast<cx*>(g_static_ptr[d]);
+    return GB_OK;
+}
+
+// gb_band_kernel with the current-source cache of its CTAs in the static array: the grid is one CTA per task (callers
+// check n_tasks * N <= GB_STATIC_MAX_TASK_BINS), no allocation, no free
+template <int N>
+int launch_band_static(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
+    static_assert((size_t)kBandCacheSlots * 2 * sizeof(cx) * GB_STATIC_MAX_TASK_BINS <= (size_t)GB_STATIC_SCRATCH_BYTES,
+                  "the static scratch must hold the caches of GB_STATIC_MAX_TASK_BINS / N CTAs");
+    const size_t smem = band_smem_bytes<N>(a.max_stage);
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N, GB_BAND_GM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int nb = 0;
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N, GB_BAND_GM>, Plan<N>::G * GB_BAND_GM, smem));
+    if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
+    int64_t grid = (int64_t)nb * ctx->num_sms;
+    if (grid > a.n_tasks) grid = a.n_tasks;
+    if ((size_t)grid * kBandCacheSlots * 2 * N * sizeof(cx) > (size_t)GB_STATIC_SCRATCH_BYTES)
+        return set_err(ctx, GB_ERR_INVALID, "static scratch too small for %lld CTAs of N = %d", (long long)grid, N);
+    BandArgs b = a;
+    b.cache = ctx->d_static;
+    gb_band_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
+    ctx->launches++;
+    GB_CUDA(ctx, cudaGetLastError());
+    return GB_OK;
+}
+}  // namespace
+
 namespace {
 template <int N>
 int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
@@ -2050,6 +2105,10 @@ int gb_create(const gb_config* cfg, gb_ctx** out) {
         return set_err(ctx, GB_ERR_CUDA, "device %d is sm_%d%d; this library is built for sm_100a only", cfg->device,
                        prop.major, prop.minor);
     ctx->num_sms = prop.multiProcessorCount;
+    {
+        const int rc_static = static_scratch_setup(ctx);
+        if (rc_static) return rc_static;
+    }
     OrbitParams op{cfg->Tobs, cfg->armlength, cfg->au, cfg->year, cfg->kappa, cfg->lambda0};
     for (int i = 0; i < 4; i++) {
         const int N = 128 << i;
@@ -2323,7 +2382,8 @@ int gb_residual_update(gb_ctx* ctx, const gb_data* data, const double* params_ne
 static int band_sweep_call(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
                            double* params, const int32_t* prop_k, const double* prop_params, const double* prop_logq,
                            const double* prop_logu, const gb_stretch* gen, int32_t* k_out, double* params_out,
-                           double* logq_out, double* logu_out, uint8_t* accepted_out, double* dlnL_out, void* stream) {
+                           double* logq_out, double* logu_out, uint8_t* accepted_out, double* dlnL_out, void* stream,
+                           bool static_scratch = false) {
     if (!ctx) return GB_ERR_INVALID;
     if (n_tasks < 0 || n_tasks > 0x7fffffff) return set_err(ctx, GB_ERR_INVALID, "n_tasks out of range");
     if (n_tasks == 0) return GB_OK;
@@ -2377,6 +2437,23 @@ static int band_sweep_call(gb_ctx* ctx, const gb_data* data, const gb_band_task*
     a.kmax = (int64_t)floor(ctx->cfg.Tobs / (2.0 * ctx->cfg.dt));
     a.errflag = ctx->d_counts + 2 * kNumClasses;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    if (static_scratch) {
+        if (!ctx->d_static)
+            return set_err(ctx, GB_ERR_INVALID, "gb_band_sweep_static: no static scratch on device %d (device index >= %d)",
+                           ctx->cfg.device, kMaxDevices);
+        if (n_tasks * N > GB_STATIC_MAX_TASK_BINS)
+            return set_err(ctx, GB_ERR_INVALID,
+                           "gb_band_sweep_static: n_tasks * N = %lld exceeds GB_STATIC_MAX_TASK_BINS = %d (the static scratch "
+                           "of %d bytes holds the caches of at most %d tasks of N = %d); use gb_band_sweep",
+                           (long long)(n_tasks * N), GB_STATIC_MAX_TASK_BINS, GB_STATIC_SCRATCH_BYTES,
+                           GB_STATIC_MAX_TASK_BINS / N, N);
+        switch (N) {
+            case 128: return launch_band_static<128>(ctx, a, st);
+            case 256: return launch_band_static<256>(ctx, a, st);
+            case 512: return launch_band_static<512>(ctx, a, st);
+            default: return launch_band_static<1024>(ctx, a, st);
+        }
+    }
     switch (N) {
         case 128: return launch_band<128>(ctx, a, st);
         case 256: return launch_band<256>(ctx, a, st);
@@ -2390,6 +2467,13 @@ int gb_band_sweep(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, i
                   const double* prop_logu, uint8_t* accepted_out, double* dlnL_out, void* stream) {
     return band_sweep_call(ctx, data, tasks, n_tasks, N, max_stage, params, prop_k, prop_params, prop_logq, prop_logu, nullptr,
                            nullptr, nullptr, nullptr, nullptr, accepted_out, dlnL_out, stream);
+}
+
+int gb_band_sweep_static(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,
+                         double* params, const int32_t* prop_k, const double* prop_params, const double* prop_logq,
+                         const double* prop_logu, uint8_t* accepted_out, double* dlnL_out, void* stream) {
+    return band_sweep_call(ctx, data, tasks, n_tasks, N, max_stage, params, prop_k, prop_params, prop_logq, prop_logu, nullptr,
+                           nullptr, nullptr, nullptr, nullptr, accepted_out, dlnL_out, stream, true);
 }
 
 int gb_band_sweep_generate(gb_ctx* ctx, const gb_data* data, const gb_band_task* tasks, int64_t n_tasks, int N, int max_stage,

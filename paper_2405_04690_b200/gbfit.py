@@ -22,9 +22,12 @@ GB_OK, GB_ERR_INVALID, GB_ERR_CUDA, GB_ERR_NOMEM, GB_ERR_ROW = 0, -1, -2, -3, -4
 EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_check", "gb_version",
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
            "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep",
-           "gb_delta_loglike_keep", "gb_residual_update_kept", "gb_band_sweep_generate", "gb_delta_loglike_accept", "gb_delta_loglike_accept_host")
+           "gb_delta_loglike_keep", "gb_residual_update_kept", "gb_band_sweep_generate", "gb_delta_loglike_accept", "gb_delta_loglike_accept_host",
+           "gb_band_sweep_static")
 
 BAND_MAX_STAGE = 3072
+STATIC_SCRATCH_BYTES = 32 * 1024 * 1024   # GB_STATIC_SCRATCH_BYTES
+STATIC_MAX_TASK_BINS = 32768             # GB_STATIC_MAX_TASK_BINS: gb_band_sweep_static takes n_tasks * N up to this
 # layout of gb_band_task (include/gbfit.h)
 BAND_TASK = np.dtype([("walker", np.int32), ("n_src", np.int32), ("src_begin", np.int32), ("n_prop", np.int32),
                       ("prop_begin", np.int32), ("n_stage", np.int32), ("k_first", np.int64),
@@ -153,6 +156,8 @@ def lib() -> C.CDLL:
         ru = [vp, C.POINTER(GbData), vp, vp, vp, vp, ci, vp, ci, vp, i64, vp]
         L.gb_band_sweep.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, vp, vp, vp, vp, vp, vp, vp]
         L.gb_band_sweep.restype = ci
+        L.gb_band_sweep_static.argtypes = L.gb_band_sweep.argtypes
+        L.gb_band_sweep_static.restype = ci
         L.gb_band_sweep_generate.argtypes = [vp, C.POINTER(GbData), vp, i64, ci, ci, vp, C.POINTER(GbStretch), vp, vp, vp, vp,
                                              vp, vp, vp]
         L.gb_band_sweep_generate.restype = ci
@@ -505,6 +510,24 @@ class Context:
                                      _dev_ptr(prop_logu, torch.float64, dev, "prop_logu"),
                                      _dev_ptr(accepted_out, torch.uint8, dev, "accepted_out"),
                                      _dev_ptr(dlnL_out, torch.float64, dev, "dlnL_out"), _stream_ptr(stream, dev)))
+        return accepted_out, dlnL_out
+
+    def band_sweep_static(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
+                          prop_k: torch.Tensor, prop_params: torch.Tensor, prop_logq: torch.Tensor, prop_logu: torch.Tensor,
+                          accepted_out: torch.Tensor, dlnL_out: torch.Tensor, stream=None):
+        """gb_band_sweep_static: gb_band_sweep with the kernel's scratch in the library's static device array; the call
+        allocates nothing (the caller passes both outputs), n_tasks * N <= STATIC_MAX_TASK_BINS, and calls that overlap on
+        the GPU race on the shared array.  Returns (accepted_out, dlnL_out)."""
+        dev = self.device
+        n_tasks = int(tasks.numel() // BAND_TASK.itemsize)
+        self._ok(lib().gb_band_sweep_static(self._h, data.c(), _dev_ptr(tasks, torch.uint8, dev, "tasks"), n_tasks, int(N),
+                                            int(max_stage), _dev_ptr(params, torch.float64, dev, "params"),
+                                            _dev_ptr(prop_k, torch.int32, dev, "prop_k"),
+                                            _dev_ptr(prop_params, torch.float64, dev, "prop_params"),
+                                            _dev_ptr(prop_logq, torch.float64, dev, "prop_logq"),
+                                            _dev_ptr(prop_logu, torch.float64, dev, "prop_logu"),
+                                            _dev_ptr(accepted_out, torch.uint8, dev, "accepted_out"),
+                                            _dev_ptr(dlnL_out, torch.float64, dev, "dlnL_out"), _stream_ptr(stream, dev)))
         return accepted_out, dlnL_out
 
     def band_sweep_generate(self, data: Data, tasks: torch.Tensor, N: int, max_stage: int, params: torch.Tensor,
