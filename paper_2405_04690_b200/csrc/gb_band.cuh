@@ -210,9 +210,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                     s_src[0] = s;
                 }
                 cta_sync<G>();
-                if (s_src[0].fast) slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                else slow_part<N, G, false>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
+                seq_window<N, G, PG>(&s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
                 cta_sync<G>();
                 const int64_t j0 = s_src[0].kmin - t.k_first;
                 if (cached && tid == 0) s_kmin[sidx] = s_src[0].kmin;
@@ -375,24 +373,13 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
             }
             cta_sync<G>();
             if (cached) {
-                if (s_src[1].fast) slow_part<N, G, true>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
-                else slow_part<N, G, false>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA1, bufE1, a.tw, tid);
+                seq_window<N, G, PG>(&s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
                 cp_async_wait<0>();
                 cta_sync<G>();
-            } else if (s_src[0].fast && s_src[1].fast) {
-                slow_part<N, G, true>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
-                cta_sync<G>();
-                slow_part<N, G, true>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA1, bufE1, a.tw, tid);
-                cta_sync<G>();
             } else {
-                slow_part<N, G, false>(&s_src[0], a.orbit, bufA0, bufE0, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA0, bufE0, a.tw, tid);
+                seq_window<N, G, PG>(&s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
                 cta_sync<G>();
-                slow_part<N, G, false>(&s_src[1], a.orbit, bufA1, bufE1, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA1, bufE1, a.tw, tid);
+                seq_window<N, G, PG>(&s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
                 cta_sync<G>();
             }
             // ---- the five sums of Eq. 5 against the staged r' (buffers: 0 = old o, 1 = new a)

@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
     cx* bufE = bufA + PN;
     cx* dA = bufE + PN;                 // delta on the staged bins
     cx* dE = dA + a.max_stage;
-    __shared__ __align__(16) SrcConst s_src;
+    __shared__ __align__(16) SrcConst s_src[2];   // the source being generated and the next one (step O1 runs one source ahead)
     __shared__ double s_red[(G / 32) * 4 + 1];
     __shared__ int s_holder[kMaxLadder];
     __shared__ int s_acc;
@@ -101,24 +101,34 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
         }
         cta_sync<G>();
         const int64_t i_first = t.k_first - a.k_lo;
-        // dA, dE += sign * (sum of the windows of the set held at chain entry `src`), on the staged bins
-        auto add_set = [&](int src, double sign) {
+        // dA, dE += sign * (sum of the windows of the set held at chain entry `src`), on the staged bins.
+        // Step O1 (one thread, ~1500 cycles) runs one source ahead: while the first PG threads transform source s, thread PG
+        // -- idle otherwise -- works out the record of source s + 1 (the next source of the set, else `next_first`: the first
+        // source of the set that the caller sums next) into the other half of s_src.
+        constexpr bool kAhead = GM > 1;
+        int slot = 0;
+        bool have = false;   // s_src[slot] already holds the record of the next source (uniform over the CTA)
+        auto o1 = [&](const double* theta, SrcConst& dst) {
+            SrcConst s;
+            source_constants(theta, a.Tobs, a.tau, N, s);
+            s.fast = fast_path_ok(theta, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
+            if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
+            dst = s;
+        };
+        auto add_set = [&](int src, double sign, const double* next_first) {
             const int n_set = a.chain_set_n[src];
             const double* set = a.params + 8 * (size_t)a.chain_set_begin[src];
             for (int sidx = 0; sidx < n_set; sidx++) {
-                if (tid == 0) {
-                    SrcConst s;
-                    source_constants(set + 8 * sidx, a.Tobs, a.tau, N, s);
-                    s.fast = fast_path_ok(set + 8 * sidx, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                    if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                    s_src = s;
+                if (!have) {
+                    if (tid == 0) o1(set + 8 * sidx, s_src[slot]);
+                    cta_sync<G>();
                 }
+                const SrcConst* cur = &s_src[slot];
+                const double* nxt = !kAhead ? nullptr : sidx + 1 < n_set ? set + 8 * (sidx + 1) : next_first;
+                seq_window<N, G, PG>(cur, a.orbit, a.tw, bufA, bufE, a.Tobs, a.tau, tid);
+                if (tid == PG && nxt) o1(nxt, s_src[slot ^ 1]);
                 cta_sync<G>();
-                if (s_src.fast) slow_part<N, G, true>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
-                else slow_part<N, G, false>(&s_src, a.orbit, bufA, bufE, a.Tobs, a.tau, tid);
-                if (tid < PG) fft_store<N>(bufA, bufE, a.tw, tid);
-                cta_sync<G>();
-                const int64_t j0 = s_src.kmin - t.k_first;
+                const int64_t j0 = cur->kmin - t.k_first;
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -130,7 +140,15 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
                     }
                 }
                 cta_sync<G>();
+                have = nxt != nullptr;
+                slot ^= 1;
             }
+        };
+        // first source of the first non-empty set among chain entries [c, c_end), or NULL
+        auto first_source = [&](int c, int c_end) -> const double* {
+            for (; c < c_end; c++)
+                if (a.chain_set_n[c] > 0) return a.params + 8 * (size_t)a.chain_set_begin[c];
+            return nullptr;
         };
         auto zero_delta = [&]() {
             for (int i = tid; i < t.n_stage; i += G) {
@@ -144,7 +162,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
         if (cached) {   // H_c = sum of the windows of chain c's initial set
             for (int c = 0; c < t.n_t; c++) {
                 zero_delta();
-                add_set(t.chain_begin + c, 1.0);
+                add_set(t.chain_begin + c, 1.0, first_source(t.chain_begin + c + 1, t.chain_begin + t.n_t));
                 for (int i = tid; i < t.n_stage; i += G) {
                     cache[((size_t)c * 2 + 0) * a.max_stage + i] = dA[i];
                     cache[((size_t)c * 2 + 1) * a.max_stage + i] = dE[i];
@@ -166,8 +184,8 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
                 cta_sync<G>();
             } else {
                 zero_delta();
-                add_set(t.chain_begin + s_holder[q], 1.0);
-                add_set(t.chain_begin + s_holder[q - 1], -1.0);
+                add_set(t.chain_begin + s_holder[q], 1.0, first_source(t.chain_begin + s_holder[q - 1], t.chain_begin + s_holder[q - 1] + 1));
+                add_set(t.chain_begin + s_holder[q - 1], -1.0, nullptr);
             }
             // ---- <delta|delta> and <r|delta> for both chains, stored bins only
             const int wi = a.chain_walker[ci], wj = a.chain_walker[cj];

@@ -1320,6 +1320,18 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
     finish();
 }
 
+// One waveform of the band / ladder kernels: slow part by all G threads of the CTA, FFT (every stage written back) by the
+// first PG.  Deliberately NOT inlined: those kernels generate waveforms at several places (cache fill, old and new source,
+// fast and general slow part) and their hot loops are bound by instruction fetch (17 % of the warp samples wait for
+// instructions, ncu); one copy of this code, at one address, serves every call site of a kernel.
+template <int N, int G, int PG>
+__device__ __noinline__ void seq_window(const SrcConst* rec, const double* __restrict__ orbit, const cx* __restrict__ tw,
+                                        cx* bA, cx* bE, double Tobs, double tau, int tid) {
+    if (rec->fast) slow_part<N, G, true>(rec, orbit, bA, bE, Tobs, tau, tid);
+    else slow_part<N, G, false>(rec, orbit, bA, bE, Tobs, tau, tid);
+    if (tid < PG) fft_store<N>(bA, bE, tw, tid);
+}
+
 #include "gb_band.cuh"
 #include "gb_temper.cuh"
 
