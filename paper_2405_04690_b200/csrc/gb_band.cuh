@@ -136,6 +136,9 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
     cx* sRE = sRA + a.max_stage;
     double* sWA = reinterpret_cast<double*>(sRE + a.max_stage);
     double* sWE = sWA + a.max_stage;
+    // records (step O1).  Window cache in use: the new source's record alternates between the two (step O1 runs one waveform
+    // ahead) and the old source is known by its window start s_kmin[k] alone; else 0 = the old source, 1 = the new one.
+    // (Static shared memory is full: 4 CTAs of N = 256 with a stage of 768 bins fill the SM to the byte.)
     __shared__ __align__(16) SrcConst s_src[2];
     __shared__ double s_red[(G / 32) * 5 + 1];
     __shared__ int s_acc;
@@ -199,21 +202,34 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
         // ---- odd/even buffers: the staged row holds none of the band's own sources; subtract them
         const bool cached = cache != nullptr && t.n_src <= kBandCacheSlots;
         const bool subtract = (t.flags & GB_BAND_SUBTRACT_CURRENT) != 0;
+        // Step O1 (one thread, ~1500 cycles) runs one waveform ahead wherever the next parameter row is known: while the
+        // first PG threads transform a waveform, thread PG -- idle otherwise -- works out the record of the next one (the
+        // band's next current source; with proposals given as inputs, the next proposal) into the other half of s_src.
+        constexpr bool kAhead = GM > 1;
+        int ns = 1;          // s_src slot of the next new-source record (toggles only with the window cache in use)
+        bool have = false;   // s_src[ns] already holds it (uniform over the CTA)
+        auto o1 = [&](const double* theta, SrcConst& dst) { seq_o1<N>(theta, a.Tobs, a.tau, a.Rmax, a.kmax, a.errflag, &dst); };
+        // proposal p of the task can have its record made ahead: inputs-only form, window cache in use, k in range
+        auto ahead_ok = [&](int p) -> bool {
+            if (!kAhead || a.gen || !cached || p >= t.n_prop) return false;
+            const int kn = a.prop_k[(int64_t)t.prop_begin + p];
+            return kn >= 0 && kn < t.n_src;
+        };
         if (subtract || cached) {
             for (int sidx = 0; sidx < t.n_src; sidx++) {
                 const double* theta = a.params + 8 * ((size_t)t.src_begin + sidx);
-                if (tid == 0) {
-                    SrcConst s;
-                    source_constants(theta, a.Tobs, a.tau, N, s);
-                    s.fast = fast_path_ok(theta, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                    if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                    s_src[0] = s;
+                if (!have) {
+                    if (tid == 0) o1(theta, s_src[ns]);
+                    cta_sync<G>();
                 }
+                const SrcConst* cur = &s_src[ns];
+                const double* nxt = !kAhead || !cached ? nullptr : sidx + 1 < t.n_src ? theta + 8
+                                              : ahead_ok(0) ? a.prop_params + 8 * (int64_t)t.prop_begin : nullptr;
+                seq_window<N, G, PG>(cur, a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
+                if (tid == PG && nxt) o1(nxt, s_src[ns ^ 1]);
                 cta_sync<G>();
-                seq_window<N, G, PG>(&s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
-                cta_sync<G>();
-                const int64_t j0 = s_src[0].kmin - t.k_first;
-                if (cached && tid == 0) s_kmin[sidx] = s_src[0].kmin;
+                const int64_t j0 = cur->kmin - t.k_first;
+                if (cached && tid == 0) s_kmin[sidx] = cur->kmin;
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -230,6 +246,8 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                     }
                 }
                 cta_sync<G>();
+                have = nxt != nullptr;
+                if (cached) ns ^= 1;
             }
         }
 
@@ -326,13 +344,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                             a.accepted_out[ip] = 0;
                         }
                     }
-                    if (tid == 1 && inside) {   // step O1 of the proposed source, from registers
-                        SrcConst s;
-                        source_constants(pr, a.Tobs, a.tau, N, s);
-                        s.fast = fast_path_ok(pr, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                        if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                        s_src[1] = s;
-                    }
+                    if (tid == 1 && inside) o1(pr, s_src[ns]);   // step O1 of the proposed source, from registers
                 }
                 cta_sync<G>();
                 const bool inside = s_ginside != 0;
@@ -353,16 +365,12 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                 continue;
             }
             double* theta_k = a.params + 8 * ((size_t)t.src_begin + k);
-            if (a.gen ? (!cached && tid == 0) : (cached ? tid == 1 : tid < 2)) {   // step O1 for the old (thread 0) and the proposed (thread 1) source
-                const double* src = tid == 0 ? theta_k : theta_p;
-                SrcConst s;
-                source_constants(src, a.Tobs, a.tau, N, s);
-                s.fast = fast_path_ok(src, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-                if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-                s_src[tid] = s;
+            const int nw = ns;   // slot of this proposal's record
+            const bool nxt_ok = ahead_ok(p + 1);
+            if (!have) {   // step O1 for the old (thread 0) and the proposed (thread 1) source, as far as they are still missing
+                if (a.gen ? (!cached && tid == 0) : (cached ? tid == 1 : tid < 2)) o1(tid == 0 ? theta_k : theta_p, s_src[tid == 0 ? 0 : nw]);
             }
             if (cached) {   // the old window comes from the cache while the new one is generated
-                if (tid == 0) s_src[0].kmin = s_kmin[k];
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -372,20 +380,21 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                 cp_async_commit();
             }
             cta_sync<G>();
-            if (cached) {
-                seq_window<N, G, PG>(&s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
-                cp_async_wait<0>();
-                cta_sync<G>();
-            } else {
+            if (!cached) {
                 seq_window<N, G, PG>(&s_src[0], a.orbit, a.tw, bufA0, bufE0, a.Tobs, a.tau, tid);
                 cta_sync<G>();
-                seq_window<N, G, PG>(&s_src[1], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
-                cta_sync<G>();
             }
+            seq_window<N, G, PG>(&s_src[nw], a.orbit, a.tw, bufA1, bufE1, a.Tobs, a.tau, tid);
+            if (tid == PG && nxt_ok) o1(theta_p + 8, s_src[nw ^ 1]);   // the next proposal's record, one ahead
+            cp_async_wait<0>();
+            cta_sync<G>();
+            have = nxt_ok;
+            if (cached) ns ^= 1;
             // ---- the five sums of Eq. 5 against the staged r' (buffers: 0 = old o, 1 = new a)
-            const int64_t j0o = s_src[0].kmin - t.k_first;   // staged bin of window bin 0, old and new
-            const int64_t j0a = s_src[1].kmin - t.k_first;
-            const int64_t shift = s_src[1].kmin - s_src[0].kmin;
+            const int64_t kmin_o = cached ? s_kmin[k] : s_src[0].kmin;
+            const int64_t j0o = kmin_o - t.k_first;   // staged bin of window bin 0, old and new
+            const int64_t j0a = s_src[nw].kmin - t.k_first;
+            const int64_t shift = s_src[nw].kmin - kmin_o;
             double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};   // aa, ra, ao, oo, ro
 #pragma unroll
             for (int m = 0; m < S; m++) {
@@ -468,7 +477,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                 }
                 if (gen_cached && tid == 0) s_redo = k;
                 if (cached) {                               // and its window replaces the cached one
-                    if (tid == 0) s_kmin[k] = s_src[1].kmin;
+                    if (tid == 0) s_kmin[k] = s_src[nw].kmin;
 #pragma unroll
                     for (int m = 0; m < S; m++) {
                         const int j = tid + G * m;

@@ -108,13 +108,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
         constexpr bool kAhead = GM > 1;
         int slot = 0;
         bool have = false;   // s_src[slot] already holds the record of the next source (uniform over the CTA)
-        auto o1 = [&](const double* theta, SrcConst& dst) {
-            SrcConst s;
-            source_constants(theta, a.Tobs, a.tau, N, s);
-            s.fast = fast_path_ok(theta, a.Tobs, a.tau, a.Rmax) ? 1 : 0;
-            if (s.kmin + N - 1 > a.kmax) atomicOr(a.errflag, 2);
-            dst = s;
-        };
+        auto o1 = [&](const double* theta, SrcConst& dst) { seq_o1<N>(theta, a.Tobs, a.tau, a.Rmax, a.kmax, a.errflag, &dst); };
         auto add_set = [&](int src, double sign, const double* next_first) {
             const int n_set = a.chain_set_n[src];
             const double* set = a.params + 8 * (size_t)a.chain_set_begin[src];

@@ -1332,6 +1332,17 @@ __device__ __noinline__ void seq_window(const SrcConst* rec, const double* __res
     if (tid < PG) fft_store<N>(bA, bE, tw, tid);
 }
 
+// Step O1 of one source by the calling thread (band / ladder kernels), out of line for the same reason
+template <int N>
+__device__ __noinline__ void seq_o1(const double* theta, double Tobs, double tau, double Rmax, int64_t kmax, int32_t* errflag,
+                                    SrcConst* dst) {
+    SrcConst s;
+    source_constants(theta, Tobs, tau, N, s);
+    s.fast = fast_path_ok(theta, Tobs, tau, Rmax) ? 1 : 0;
+    if (s.kmin + N - 1 > kmax) atomicOr(errflag, 2);
+    *dst = s;
+}
+
 #include "gb_band.cuh"
 #include "gb_temper.cuh"
 
