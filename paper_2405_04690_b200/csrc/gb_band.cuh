@@ -121,7 +121,9 @@ constexpr size_t band_smem_bytes(int max_stage) {
 template <int N>
 constexpr int band_min_blocks() { return N == 128 ? 6 : N == 256 ? 4 : N == 512 ? 2 : 1; }
 
-template <int N, int GM>
+// GEN: the proposal step runs inside the loop (gb_band_sweep_generate).  A template parameter rather than a flag: the loops
+// of these kernels wait for instructions (ncu: 8-17 % of the warp samples), and each form is faster without the other's code.
+template <int N, int GM, bool GEN>
 __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band_kernel(BandArgs a) {
     constexpr int PG = Plan<N>::G;   // FFT group: the first PG threads
     constexpr int G = PG * GM;       // threads of the CTA
@@ -137,14 +139,14 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
     double* sWA = reinterpret_cast<double*>(sRE + a.max_stage);
     double* sWE = sWA + a.max_stage;
     // records (step O1).  Window cache in use: the new source's record alternates between the two (step O1 runs one waveform
-    // ahead) and the old source is known by its window start s_kmin[k] alone; else 0 = the old source, 1 = the new one.
+    // ahead) and the old source is known by its window start s_koff[k] alone; else 0 = the old source, 1 = the new one.
     // (Static shared memory is full: 4 CTAs of N = 256 with a stage of 768 bins fill the SM to the byte.)
     __shared__ __align__(16) SrcConst s_src[2];
     __shared__ double s_red[(G / 32) * 5 + 1];
     __shared__ int s_acc;
-    __shared__ int s_gk, s_ginside;                   // generated proposal: k, inside the prior box
-    __shared__ double s_glq, s_glu;                   //                      logq, logu
-    __shared__ int64_t s_kmin[kBandCacheSlots];       // window start of each cached current source
+    __shared__ int s_gk[2], s_ginside[2];             // generated proposal (per record slot): k, inside the prior box
+    __shared__ double s_glq[2], s_glu[2];             //                                       logq, logu
+    __shared__ int32_t s_koff[kBandCacheSlots];       // window start of each cached current source, relative to t.k_first
     __shared__ double s_theta[kBandCacheSlots][8];    // generate mode: the band's CURRENT parameter rows ...
     __shared__ int64_t s_run[kBandCacheSlots];        // ... and where each one's run of friends starts in the table
     __shared__ int s_redo;                            // source whose run has to be searched again (it was just accepted)
@@ -157,7 +159,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
         const bool wb = (t.flags & GB_BAND_WRITE_BACK) != 0;
         const int wrow = (t.flags & GB_BAND_WRITE_OTHER) ? t.write_walker : t.walker;
         bool bad = t.walker < 0 || t.walker >= a.n_walkers || t.n_stage < 0 || t.n_stage > a.max_stage || t.n_src < 0 ||
-                   (wb && (wrow < 0 || wrow >= a.n_walkers)) || (a.gen && (t.n_src < 1 || t.n_stage < 1));
+                   (wb && (wrow < 0 || wrow >= a.n_walkers)) || (GEN && (t.n_src < 1 || t.n_stage < 1));
         int prow = 0;
         if (!bad) {
             prow = a.walker_psd ? a.walker_psd[t.walker] : (a.n_psd == 1 ? 0 : t.walker);
@@ -211,7 +213,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
         auto o1 = [&](const double* theta, SrcConst& dst) { seq_o1<N>(theta, a.Tobs, a.tau, a.Rmax, a.kmax, a.errflag, &dst); };
         // proposal p of the task can have its record made ahead: inputs-only form, window cache in use, k in range
         auto ahead_ok = [&](int p) -> bool {
-            if (!kAhead || a.gen || !cached || p >= t.n_prop) return false;
+            if (!kAhead || GEN || !cached || p >= t.n_prop) return false;
             const int kn = a.prop_k[(int64_t)t.prop_begin + p];
             return kn >= 0 && kn < t.n_src;
         };
@@ -229,7 +231,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                 if (tid == PG && nxt) o1(nxt, s_src[ns ^ 1]);
                 cta_sync<G>();
                 const int64_t j0 = cur->kmin - t.k_first;
-                if (cached && tid == 0) s_kmin[sidx] = cur->kmin;
+                if (cached && tid == 0) s_koff[sidx] = (int32_t)(cur->kmin - t.k_first);
 #pragma unroll
                 for (int m = 0; m < S; m++) {
                     const int j = tid + G * m;
@@ -258,8 +260,8 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
         // bands of up to kBandCacheSlots sources keep their current parameter rows and the start of each source's run of
         // friends on chip: the search (4-5 dependent table probes) then leaves the per-proposal chain -- it is done once
         // per source here, all warps taking sources in turn, and again only for a source whose proposal was accepted
-        const bool gen_cached = a.gen && t.n_src <= kBandCacheSlots;
-        if (a.gen) {
+        const bool gen_cached = GEN && t.n_src <= kBandCacheSlots;
+        if (GEN) {
             const int lane = tid & 31;
             const int64_t nfr = min((int64_t)a.st.n_friends, a.st.n_group);
             const double f_lo = (double)t.k_first / a.Tobs, f_hi = (double)(t.k_first + t.n_stage) / a.Tobs;
@@ -277,80 +279,85 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                 cta_sync<G>();
             }
         }
+        // "k <- randint(0, g_j); theta'_k <- Make Proposal on theta" of proposal row ipx by ONE warp (lane =
+        // 0 .. 31), from the CURRENT theta_k: Philox block 0 -> k, the friend, z; block 1 -> the uniform of the accept step.
+        // Lane c < 8 owns coordinate c of theta'; every product and sum is rounded on its own (the oracle is built without
+        // FMA contraction), so k and theta' agree with it bit for bit.  Results: record slot `slot` of s_src / s_g*, and the
+        // proposal's rows of the gen_* outputs.
+        auto generate = [&](int64_t ipx, int slot, int lane) {
+            uint32_t w0[4], w1[4];
+            const uint32_t key0 = (uint32_t)(a.st.seed & 0xffffffffu), key1 = (uint32_t)(a.st.seed >> 32);
+            philox4x32_10((uint32_t)ipx, 0u, 0u, a.st.sweep, key0, key1, w0);
+            philox4x32_10((uint32_t)ipx, 0u, 1u, a.st.sweep, key0, key1, w1);
+            const int kk = randint32(w0[0], t.n_src);
+            const double* th = gen_cached ? s_theta[kk] : a.params + 8 * ((size_t)t.src_begin + kk);
+            const int64_t nf = a.st.n_friends < a.st.n_group ? a.st.n_friends : a.st.n_group;
+            const int32_t jf = randint32(w0[1], (int32_t)nf);
+            if (gen_cached && s_redo >= 0) {   // the source accepted last has moved: its run of friends again
+                const int kr = s_redo;
+                const int64_t sr = friend_run_start(a.st.group, a.st.n_group, nf, s_theta[kr][1], lane, hint_lo, hint_hi);
+                __syncwarp();
+                if (lane == 0) {
+                    s_run[kr] = sr;
+                    s_redo = -1;
+                }
+                __syncwarp();
+            }
+            const int64_t s0 = gen_cached ? s_run[kk]
+                                          : friend_run_start(a.st.group, a.st.n_group, nf, th[1], lane, hint_lo, hint_hi);
+            const int64_t row = s0 + jf;
+            const double ua = uniform52(w0[2], w0[3]);
+            const double tz = __dadd_rn(__dmul_rn(__dadd_rn(a.st.stretch_a, -1.0), ua), 1.0);
+            const double z = __ddiv_rn(__dmul_rn(tz, tz), a.st.stretch_a);    // g(z) ~ z^(-1/2) on [1/a, a]
+            const int c = lane & 7;
+            const double xa = __ldg(a.st.group + 8 * row + c);
+            double x = __dadd_rn(xa, __dmul_rn(z, __dadd_rn(th[c], -xa)));      // Eq. 14
+            const double lo = a.st.lo[c], hi = a.st.hi[c];
+            if (a.st.periodic[c]) {
+                const double period = __dadd_rn(hi, -lo);
+                x = __dadd_rn(x, -__dmul_rn(period, floor(__ddiv_rn(__dadd_rn(x, -lo), period))));
+            }
+            const bool in_c = x >= lo && x <= hi;
+            bool inside = (__ballot_sync(0xffffffffu, in_c) & 0xffu) == 0xffu;
+            if (lane < 8) a.gen_params[8 * ipx + lane] = x;
+            double pr[8];
+#pragma unroll
+            for (int cc = 0; cc < 8; cc++) pr[cc] = __shfl_sync(0xffffffffu, x, cc);
+            {   // samples may go halfway into the neighbouring sub-bands: the window of theta' must
+                // stay on the staged bins, else the prior is zero
+                const int64_t kmin_p = (int64_t)floor(__dmul_rn(pr[1], a.Tobs) + 0.5) - N / 2;
+                if (kmin_p < t.k_first || kmin_p + N > t.k_first + t.n_stage) inside = false;
+            }
+            if (lane == 0) {
+                const double lq = 7.0 * log(z), lu = log(uniform52(w1[0], w1[1]));   // z^(D-1), D = 8
+                a.gen_k[ipx] = kk;
+                a.gen_logq[ipx] = lq;
+                a.gen_logu[ipx] = lu;
+                s_gk[slot] = kk;
+                s_ginside[slot] = inside ? 1 : 0;
+                s_glq[slot] = lq;
+                s_glu[slot] = lu;
+                if (!inside) {          // zero prior: rejected without a likelihood evaluation
+                    a.dlnL_out[ipx] = nan;
+                    a.accepted_out[ipx] = 0;
+                }
+            }
+            if (lane == 1 && inside) o1(pr, s_src[slot]);   // step O1 of the proposed source, from registers
+        };
         for (int p = 0; p < t.n_prop; p++) {
             const int64_t ip = (int64_t)t.prop_begin + p;
             int k;
             const double* theta_p;
-            if (a.gen) {
-                // "k <- randint(0, g_j); theta'_k <- Make Proposal on theta" by warp 0, from the CURRENT
-                // theta_k: Philox block 0 -> k, the friend, z; block 1 -> the uniform of the accept step.  Lane c < 8 owns
-                // coordinate c of theta'; every product and sum is rounded on its own (the oracle is built without FMA
-                // contraction), so k and theta' agree with it bit for bit.
-                if (tid < 32) {
-                    uint32_t w0[4], w1[4];
-                    const uint32_t key0 = (uint32_t)(a.st.seed & 0xffffffffu), key1 = (uint32_t)(a.st.seed >> 32);
-                    philox4x32_10((uint32_t)ip, 0u, 0u, a.st.sweep, key0, key1, w0);
-                    philox4x32_10((uint32_t)ip, 0u, 1u, a.st.sweep, key0, key1, w1);
-                    const int kk = randint32(w0[0], t.n_src);
-                    const double* th = gen_cached ? s_theta[kk] : a.params + 8 * ((size_t)t.src_begin + kk);
-                    const int64_t nf = a.st.n_friends < a.st.n_group ? a.st.n_friends : a.st.n_group;
-                    const int32_t jf = randint32(w0[1], (int32_t)nf);
-                    if (gen_cached && s_redo >= 0) {   // the source accepted last has moved: its run of friends again
-                        const int kr = s_redo;
-                        const int64_t sr = friend_run_start(a.st.group, a.st.n_group, nf, s_theta[kr][1], tid, hint_lo, hint_hi);
-                        __syncwarp();
-                        if (tid == 0) {
-                            s_run[kr] = sr;
-                            s_redo = -1;
-                        }
-                        __syncwarp();
-                    }
-                    const int64_t s0 = gen_cached ? s_run[kk]
-                                                  : friend_run_start(a.st.group, a.st.n_group, nf, th[1], tid, hint_lo, hint_hi);
-                    const int64_t row = s0 + jf;
-                    const double ua = uniform52(w0[2], w0[3]);
-                    const double tz = __dadd_rn(__dmul_rn(__dadd_rn(a.st.stretch_a, -1.0), ua), 1.0);
-                    const double z = __ddiv_rn(__dmul_rn(tz, tz), a.st.stretch_a);    // g(z) ~ z^(-1/2) on [1/a, a]
-                    const int c = tid & 7;
-                    const double xa = __ldg(a.st.group + 8 * row + c);
-                    double x = __dadd_rn(xa, __dmul_rn(z, __dadd_rn(th[c], -xa)));      // Eq. 14
-                    const double lo = a.st.lo[c], hi = a.st.hi[c];
-                    if (a.st.periodic[c]) {
-                        const double period = __dadd_rn(hi, -lo);
-                        x = __dadd_rn(x, -__dmul_rn(period, floor(__ddiv_rn(__dadd_rn(x, -lo), period))));
-                    }
-                    const bool in_c = x >= lo && x <= hi;
-                    bool inside = (__ballot_sync(0xffffffffu, in_c) & 0xffu) == 0xffu;
-                    if (tid < 8) a.gen_params[8 * ip + tid] = x;
-                    double pr[8];
-#pragma unroll
-                    for (int cc = 0; cc < 8; cc++) pr[cc] = __shfl_sync(0xffffffffu, x, cc);
-                    {   // samples may go halfway into the neighbouring sub-bands: the window of theta' must
-                        // stay on the staged bins, else the prior is zero
-                        const int64_t kmin_p = (int64_t)floor(__dmul_rn(pr[1], a.Tobs) + 0.5) - N / 2;
-                        if (kmin_p < t.k_first || kmin_p + N > t.k_first + t.n_stage) inside = false;
-                    }
-                    if (tid == 0) {
-                        const double lq = 7.0 * log(z), lu = log(uniform52(w1[0], w1[1]));   // z^(D-1), D = 8
-                        a.gen_k[ip] = kk;
-                        a.gen_logq[ip] = lq;
-                        a.gen_logu[ip] = lu;
-                        s_gk = kk;
-                        s_ginside = inside ? 1 : 0;
-                        s_glq = lq;
-                        s_glu = lu;
-                        if (!inside) {          // zero prior: rejected without a likelihood evaluation
-                            a.dlnL_out[ip] = nan;
-                            a.accepted_out[ip] = 0;
-                        }
-                    }
-                    if (tid == 1 && inside) o1(pr, s_src[ns]);   // step O1 of the proposed source, from registers
-                }
+            if (GEN) {
+                if (tid < 32) generate(ip, ns, tid);
                 cta_sync<G>();
-                const bool inside = s_ginside != 0;
-                k = s_gk;
-                cta_sync<G>();                  // s_gk / s_ginside are rewritten by the next proposal
-                if (!inside) continue;          // uniform over the CTA
+                const bool inside = s_ginside[ns] != 0;
+                k = s_gk[ns];
+                if (!inside) {                  // uniform over the CTA
+                    cta_sync<G>();              // slot ns is rewritten by the next proposal
+                    have = false;
+                    continue;
+                }
                 theta_p = a.gen_params + 8 * ip;
             } else {
                 k = a.prop_k[ip];
@@ -368,7 +375,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
             const int nw = ns;   // slot of this proposal's record
             const bool nxt_ok = ahead_ok(p + 1);
             if (!have) {   // step O1 for the old (thread 0) and the proposed (thread 1) source, as far as they are still missing
-                if (a.gen ? (!cached && tid == 0) : (cached ? tid == 1 : tid < 2)) o1(tid == 0 ? theta_k : theta_p, s_src[tid == 0 ? 0 : nw]);
+                if (GEN ? (!cached && tid == 0) : (cached ? tid == 1 : tid < 2)) o1(tid == 0 ? theta_k : theta_p, s_src[tid == 0 ? 0 : nw]);
             }
             if (cached) {   // the old window comes from the cache while the new one is generated
 #pragma unroll
@@ -391,7 +398,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
             have = nxt_ok;
             if (cached) ns ^= 1;
             // ---- the five sums of Eq. 5 against the staged r' (buffers: 0 = old o, 1 = new a)
-            const int64_t kmin_o = cached ? s_kmin[k] : s_src[0].kmin;
+            const int64_t kmin_o = cached ? t.k_first + s_koff[k] : s_src[0].kmin;
             const int64_t j0o = kmin_o - t.k_first;   // staged bin of window bin 0, old and new
             const int64_t j0a = s_src[nw].kmin - t.k_first;
             const int64_t shift = s_src[nw].kmin - kmin_o;
@@ -425,7 +432,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
             if (tid == 0) {
                 const double norm = 4.0 / a.Tobs;
                 const double dl = -0.5 * norm * (v[0] + v[3] - 2.0 * v[2] - 2.0 * v[1] + 2.0 * v[4]);
-                const double lq = a.gen ? s_glq : a.prop_logq[ip], lu = a.gen ? s_glu : a.prop_logu[ip];
+                const double lq = GEN ? s_glq[nw] : a.prop_logq[ip], lu = GEN ? s_glu[nw] : a.prop_logu[ip];
                 const int acc = t.beta * dl + lq >= lu ? 1 : 0;
                 a.dlnL_out[ip] = dl;
                 a.accepted_out[ip] = (uint8_t)acc;
@@ -477,7 +484,7 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, band_min_blocks<N>()) gb_band
                 }
                 if (gen_cached && tid == 0) s_redo = k;
                 if (cached) {                               // and its window replaces the cached one
-                    if (tid == 0) s_kmin[k] = s_src[nw].kmin;
+                    if (tid == 0) s_koff[k] = (int32_t)(s_src[nw].kmin - t.k_first);
 #pragma unroll
                     for (int m = 0; m < S; m++) {
                         const int j = tid + G * m;

@@ -2032,14 +2032,14 @@ int static_scratch_setup(gb_ctx* ctx) {
 
 // gb_band_kernel with the current-source cache of its CTAs in the static array: the grid is one CTA per task (callers
 // check n_tasks * N <= GB_STATIC_MAX_TASK_BINS), no allocation, no free
-template <int N>
+template <int N, bool GEN = false>
 int launch_band_static(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
     static_assert((size_t)kBandCacheSlots * 2 * sizeof(cx) * GB_STATIC_MAX_TASK_BINS <= (size_t)GB_STATIC_SCRATCH_BYTES,
                   "the static scratch must hold the caches of GB_STATIC_MAX_TASK_BINS / N CTAs");
     const size_t smem = band_smem_bytes<N>(a.max_stage);
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N, GB_BAND_GM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N, GB_BAND_GM, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N, GB_BAND_GM>, Plan<N>::G * GB_BAND_GM, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N, GB_BAND_GM, GEN>, Plan<N>::G * GB_BAND_GM, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
     int64_t grid = (int64_t)nb * ctx->num_sms;
     if (grid > a.n_tasks) grid = a.n_tasks;
@@ -2047,7 +2047,7 @@ int launch_band_static(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
         return set_err(ctx, GB_ERR_INVALID, "static scratch too small for %lld CTAs of N = %d", (long long)grid, N);
     BandArgs b = a;
     b.cache = ctx->d_static;
-    gb_band_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
+    gb_band_kernel<N, GB_BAND_GM, GEN><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -2055,12 +2055,12 @@ int launch_band_static(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
 }  // namespace
 
 namespace {
-template <int N>
+template <int N, bool GEN>
 int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
     const size_t smem = band_smem_bytes<N>(a.max_stage);
-    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N, GB_BAND_GM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    GB_CUDA(ctx, cudaFuncSetAttribute(gb_band_kernel<N, GB_BAND_GM, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int nb = 0;
-    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N, GB_BAND_GM>, Plan<N>::G * GB_BAND_GM, smem));
+    GB_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, gb_band_kernel<N, GB_BAND_GM, GEN>, Plan<N>::G * GB_BAND_GM, smem));
     if (nb < 1) return set_err(ctx, GB_ERR_INVALID, "max_stage %d does not fit in shared memory for N = %d", a.max_stage, N);
     int64_t grid = (int64_t)nb * ctx->num_sms;
     if (grid > a.n_tasks) grid = a.n_tasks;
@@ -2068,7 +2068,7 @@ int launch_band(gb_ctx* ctx, const BandArgs& a, cudaStream_t st) {
     int rc = ensure_cap(ctx, &ctx->d_band_cache, &ctx->cap_band_cache, grid * kBandCacheSlots * 2 * N);
     if (rc) return rc;
     b.cache = ctx->d_band_cache;
-    gb_band_kernel<N, GB_BAND_GM><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
+    gb_band_kernel<N, GB_BAND_GM, GEN><<<(unsigned)grid, Plan<N>::G * GB_BAND_GM, smem, st>>>(b);
     ctx->launches++;
     GB_CUDA(ctx, cudaGetLastError());
     return GB_OK;
@@ -2477,11 +2477,19 @@ static int band_sweep_call(gb_ctx* ctx, const gb_data* data, const gb_band_task*
             default: return launch_band_static<1024>(ctx, a, st);
         }
     }
+    if (a.gen) {
+        switch (N) {
+            case 128: return launch_band<128, true>(ctx, a, st);
+            case 256: return launch_band<256, true>(ctx, a, st);
+            case 512: return launch_band<512, true>(ctx, a, st);
+            default: return launch_band<1024, true>(ctx, a, st);
+        }
+    }
     switch (N) {
-        case 128: return launch_band<128>(ctx, a, st);
-        case 256: return launch_band<256>(ctx, a, st);
-        case 512: return launch_band<512>(ctx, a, st);
-        default: return launch_band<1024>(ctx, a, st);
+        case 128: return launch_band<128, false>(ctx, a, st);
+        case 256: return launch_band<256, false>(ctx, a, st);
+        case 512: return launch_band<512, false>(ctx, a, st);
+        default: return launch_band<1024, false>(ctx, a, st);
     }
 }
 
