@@ -170,10 +170,25 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
             if (cached) {
                 const cx* Hi = cache + (size_t)s_holder[q] * 2 * a.max_stage;
                 const cx* Hj = cache + (size_t)s_holder[q - 1] * 2 * a.max_stage;
-                for (int i = tid; i < t.n_stage; i += G) {
-                    const cx ai = Hi[i], ei = Hi[a.max_stage + i], aj = Hj[i], ej = Hj[a.max_stage + i];
-                    dA[i] = {ai.re - aj.re, ai.im - aj.im};
-                    dE[i] = {ei.re - ej.re, ei.im - ej.im};
+                // (four bins per thread in flight: the set sums come from L2 / HBM and a round trip per bin is the whole loop)
+                for (int i0 = tid; i0 < t.n_stage; i0 += 4 * G) {
+                    cx ai[4], ei[4], aj[4], ej[4];
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const int i = min(i0 + u * G, t.n_stage - 1);
+                        ai[u] = Hi[i];
+                        ei[u] = Hi[a.max_stage + i];
+                        aj[u] = Hj[i];
+                        ej[u] = Hj[a.max_stage + i];
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const int i = i0 + u * G;
+                        if (i < t.n_stage) {
+                            dA[i] = {ai[u].re - aj[u].re, ai[u].im - aj[u].im};
+                            dE[i] = {ei[u].re - ej[u].re, ei[u].im - ej[u].im};
+                        }
+                    }
                 }
                 cta_sync<G>();
             } else {
@@ -197,32 +212,52 @@ __global__ void __launch_bounds__(Plan<N>::G * GM, temper_min_blocks<N>()) gb_te
             double v[4] = {0.0, 0.0, 0.0, 0.0};   // dd_i, rd_i, dd_j, rd_j
             const cx* Hi = cached ? cache + (size_t)s_holder[q] * 2 * a.max_stage : nullptr;       // the set sums the two
             const cx* Hj = cached ? cache + (size_t)s_holder[q - 1] * 2 * a.max_stage : nullptr;   // chains hold
-            for (int i = tid; i < t.n_stage; i += G) {
-                const int64_t e = i_first + i;
-                if (e < 0 || e >= a.n_f) continue;
-                const cx da = dA[i], de = dE[i];
-                const double na = da.re * da.re + da.im * da.im, ne = de.re * de.re + de.im * de.im;
-                {
-                    double2 ra = __ldcg(reinterpret_cast<const double2*>(rAi + 2 * e));
-                    double2 re = __ldcg(reinterpret_cast<const double2*>(rEi + 2 * e));
-                    if (oddeven) {   // r_i = row - sum_{S_i} h
-                        const cx ha = Hi[i], he = Hi[a.max_stage + i];
-                        ra.x -= ha.re;  ra.y -= ha.im;  re.x -= he.re;  re.y -= he.im;
-                    }
-                    const double wa = inv ? SAi[e] : 1.0 / SAi[e], we = inv ? SEi[e] : 1.0 / SEi[e];
-                    v[0] += wa * na + we * ne;
-                    v[1] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
+            // two bins per thread in flight (residual rows, weights and -- odd/even -- the set sums come from L2 / HBM)
+            for (int i0 = tid; i0 < t.n_stage; i0 += 2 * G) {
+                double2 rai[2], rei[2], raj[2], rej[2];
+                double wai[2], wei[2], waj[2], wej[2];
+                bool okb[2];
+#pragma unroll
+                for (int u = 0; u < 2; u++) {
+                    const int i = i0 + u * G;
+                    const int64_t e = i_first + i;
+                    okb[u] = i < t.n_stage && e >= 0 && e < a.n_f;
+                    const int64_t ec = okb[u] ? e : (i_first < 0 ? 0 : i_first >= a.n_f ? a.n_f - 1 : i_first);
+                    rai[u] = __ldcg(reinterpret_cast<const double2*>(rAi + 2 * ec));
+                    rei[u] = __ldcg(reinterpret_cast<const double2*>(rEi + 2 * ec));
+                    raj[u] = __ldcg(reinterpret_cast<const double2*>(rAj + 2 * ec));
+                    rej[u] = __ldcg(reinterpret_cast<const double2*>(rEj + 2 * ec));
+                    wai[u] = SAi[ec];
+                    wei[u] = SEi[ec];
+                    waj[u] = SAj[ec];
+                    wej[u] = SEj[ec];
                 }
-                {
-                    double2 ra = __ldcg(reinterpret_cast<const double2*>(rAj + 2 * e));
-                    double2 re = __ldcg(reinterpret_cast<const double2*>(rEj + 2 * e));
-                    if (oddeven) {
-                        const cx ha = Hj[i], he = Hj[a.max_stage + i];
-                        ra.x -= ha.re;  ra.y -= ha.im;  re.x -= he.re;  re.y -= he.im;
+#pragma unroll
+                for (int u = 0; u < 2; u++) {
+                    if (!okb[u]) continue;
+                    const int i = i0 + u * G;
+                    const cx da = dA[i], de = dE[i];
+                    const double na = da.re * da.re + da.im * da.im, ne = de.re * de.re + de.im * de.im;
+                    {
+                        double2 ra = rai[u], re = rei[u];
+                        if (oddeven) {   // r_i = row - sum_{S_i} h
+                            const cx ha = Hi[i], he = Hi[a.max_stage + i];
+                            ra.x -= ha.re;  ra.y -= ha.im;  re.x -= he.re;  re.y -= he.im;
+                        }
+                        const double wa = inv ? wai[u] : 1.0 / wai[u], we = inv ? wei[u] : 1.0 / wei[u];
+                        v[0] += wa * na + we * ne;
+                        v[1] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
                     }
-                    const double wa = inv ? SAj[e] : 1.0 / SAj[e], we = inv ? SEj[e] : 1.0 / SEj[e];
-                    v[2] += wa * na + we * ne;
-                    v[3] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
+                    {
+                        double2 ra = raj[u], re = rej[u];
+                        if (oddeven) {
+                            const cx ha = Hj[i], he = Hj[a.max_stage + i];
+                            ra.x -= ha.re;  ra.y -= ha.im;  re.x -= he.re;  re.y -= he.im;
+                        }
+                        const double wa = inv ? waj[u] : 1.0 / waj[u], we = inv ? wej[u] : 1.0 / wej[u];
+                        v[2] += wa * na + we * ne;
+                        v[3] += wa * (ra.x * da.re + ra.y * da.im) + we * (re.x * de.re + re.y * de.im);
+                    }
                 }
             }
             group_reduce<G, 4>(v, s_red, tid);
