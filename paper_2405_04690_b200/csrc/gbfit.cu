@@ -44,6 +44,12 @@ namespace {
 #ifndef GB_L2_PREFETCH
 #define GB_L2_PREFETCH 1      // delta lnL: request the next item's residual / PSD window into L2
 #endif
+#ifndef GB_EPI_BATCH
+#define GB_EPI_BATCH 8        // delta-lnL epilogue: window bins per thread whose loads are in flight together
+#endif
+#ifndef GB_L1_PREFETCH
+#define GB_L1_PREFETCH 0      // delta lnL: request THIS item's window into L1 before its FFT; the epilogue then loads through L1
+#endif
 #ifndef GB_STREAM_LOADS
 #define GB_STREAM_LOADS 1     // window loads bypass L1 allocation
 #endif
@@ -485,7 +491,10 @@ struct WinBatch1 {
             const int64_t i = i_first + H * c;
             ok[c] = CHECK ? (i >= 0 && i < n_f) : true;   // !CHECK: the whole window lies inside the stored band
             const int64_t ic = ok[c] ? i : 0;
-#if GB_STREAM_LOADS
+#if GB_L1_PREFETCH
+            const double2 a2 = __ldca(reinterpret_cast<const double2*>(rC + 2 * ic));
+            w[c] = __ldca(SC + ic);
+#elif GB_STREAM_LOADS
             const double2 a2 = __ldcg(reinterpret_cast<const double2*>(rC + 2 * ic));
             w[c] = __ldcg(SC + ic);
 #else
@@ -578,6 +587,7 @@ __device__ __forceinline__ void red_add_f64(double* p, double v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(__cvta_generic_to_global(p)), "d"(v) : "memory");
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
@@ -1077,6 +1087,32 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
             }
         }
 
+        // ---- and L1 for this item's own window, which the epilogue reads right after the FFT
+        if (GB_L1_PREFETCH && !SWAP && a.mode == MODE_DLNL && !bad_row) {
+            const int64_t i0 = kmin0 - a.k_lo;
+            const size_t nf = (size_t)a.n_f;
+            if (i0 >= 0 && i0 + N + 16 <= a.n_f) {
+                const double* pA = a.resid + ((size_t)rec[0].walker * 2 + 0) * nf * 2 + 2 * (i0 + 8 * tid);
+                const double* pE = a.resid + ((size_t)rec[0].walker * 2 + 1) * nf * 2 + 2 * (i0 + 8 * tid);
+#pragma unroll
+                for (int l = 0; l <= N / 8; l += T) {
+                    if (l + tid <= N / 8) {
+                        prefetch_l1(pA + 16 * l);
+                        prefetch_l1(pE + 16 * l);
+                    }
+                }
+                const double* pSA = a.psd + ((size_t)rec[0].psd_row * 2 + 0) * nf + i0 + 16 * tid;
+                const double* pSE = a.psd + ((size_t)rec[0].psd_row * 2 + 1) * nf + i0 + 16 * tid;
+#pragma unroll
+                for (int l = 0; l <= N / 16; l += T) {
+                    if (l + tid <= N / 16) {
+                        prefetch_l1(pSA + 16 * l);
+                        prefetch_l1(pSE + 16 * l);
+                    }
+                }
+            }
+        }
+
         // ---- FFT: SWAP keeps both windows in shared memory; otherwise the last stage stays in registers,
         //      h[m] = bin ht + H m of this thread's channel (threads [0, H): A, [H, G): E)
         constexpr int H = G / 2, M = N / H;
@@ -1117,7 +1153,7 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
                     // this thread's channel: bins ht + H m (consecutive threads, consecutive bins)
                     const double* rC = ch ? rE : rA;
                     const double* SC = ch ? SE : SA;
-                    constexpr int CH1 = 4;      // bins per thread whose loads are in flight together
+                    constexpr int CH1 = GB_EPI_BATCH < M ? GB_EPI_BATCH : M;      // bins per thread whose loads are in flight together
                     double v[2] = {0.0, 0.0};   // <h|h>, <r|h>
 #pragma unroll
                     for (int m0 = 0; m0 < M; m0 += CH1) {
