@@ -279,7 +279,8 @@ def run_ours(args):
     d_lu = h_lu.to(dev)
     d_accout = torch.zeros(B, dtype=torch.uint8, device=dev)
     h_accout = torch.zeros(B, dtype=torch.uint8).pin_memory()
-    store_bins = int(1.15 * wl.n_bins[wl.accepted != 0].astype(np.int64).sum()) + 1024
+    # store of the accepted windows: 3 % above what this step's decisions need (the library adds its own reservation slack)
+    store_bins = int(1.03 * wl.n_bins[wl.accepted != 0].astype(np.int64).sum()) + 1024
 
     def step_device(i, ev=None):
         if ev:
@@ -349,6 +350,7 @@ def run_ours(args):
     barrier()
     tw1 = time.perf_counter()
     launches = ctx.launch_count() - l0
+    scratch_step = ctx.scratch_bytes()   # device scratch of the context after the timed steps (before any other measurement)
     clocks = clk.stop(tw0, tw1) if rank == 0 else None
     ctx.check()
     ms_total = e0.elapsed_time(e1)
@@ -681,7 +683,10 @@ def run_ours(args):
                             "once; the CTAs that evaluate walker chunk c+1 move the windows of chunks <= c into the residual "
                             "(cp.async.bulk + cp.reduce.async.bulk add.f64)",
                     "bytes": 1.5 * bytes_upd, "bytes_note": "32 N written + 32 N read + 64 N read-modify-write per accepted row",
-                    "store_bytes": 32.0 * store_bins} if fused else
+                    "store_bytes": 32.0 * store_bins,
+                    "scratch_bytes_ctx": scratch_step,
+                    "scratch_note": "gb_scratch_bytes after the timed steps: window store incl. reservation slack, source "
+                                    "records (192 B/row), work lists, (beta, logq, logu) rows, accepted-row list, pieces"} if fused else
                    {"call": "gb_residual_update (regenerates the accepted waveforms)", "ms_per_launch": ms_upd,
                     "flops": flops_upd, "bytes": bytes_upd,
                     "alu_frac": flops_upd / (ms_upd * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,

@@ -109,6 +109,10 @@ const char *gb_version(void);
 /* Number of kernels launched by this context since creation (bench.py's gpu_launches counter). */
 int64_t gb_launch_count(const gb_ctx *ctx);
 
+/* Bytes of device scratch the context holds right now (work lists, source records, window stores, caches, staging of the
+ * *_host forms; grown on demand by the calls, freed by gb_destroy).  Tables (orbit, twiddles) are not counted. */
+int64_t gb_scratch_bytes(const gb_ctx *ctx);
+
 /*
  * gb_measure_fp64_peak -- diagnostic, not on the hot path: times a register-only stream of independent DFMAs
  * (8 chains per thread, 512 threads per SM, every SM) on the context's device and returns the sustained rate.

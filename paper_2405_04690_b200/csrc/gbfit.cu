@@ -284,7 +284,9 @@ __global__ void __launch_bounds__(256) gb_walker_hist_kernel(const int32_t* __re
 // chunk c are moved into the residual while chunk c + 1 is evaluated, about one 4 KB piece per evaluated row, so a chunk
 // must not be much smaller than the one before it; and what the last chunk accepts is left to the closing launch, so the
 // last chunk is the smallest.  A batch that touches only some of the walkers is cut by the rows it has, not by walker index.
-__global__ void gb_chunk_bounds_kernel(const int32_t* __restrict__ hist, int n_walkers, int K, int64_t B, int32_t* chunk_first) {
+// row_start[k] = rows of the batch in the chunks before k (the binned lists of chunk k start there, see run_call)
+__global__ void gb_chunk_bounds_kernel(const int32_t* __restrict__ hist, int n_walkers, int K, int64_t B, int32_t* chunk_first,
+                                       int32_t* row_start) {
     double total = 0.0, sz = 1.0;
     for (int k = 0; k < K; k++, sz *= 0.75) total += sz;
     int64_t rows = 0;
@@ -297,8 +299,16 @@ __global__ void gb_chunk_bounds_kernel(const int32_t* __restrict__ hist, int n_w
         const int64_t target = (int64_t)(cum / total * (double)rows + 0.5);   // rows before chunk k
         while (w < n_walkers && seen < target) seen += hist[w++];
         chunk_first[k] = k == 0 ? 0 : w;
+        row_start[k] = (int32_t)seen;
         cum += sz;
     }
+}
+
+// One-pass binning: the list of bin (class, chunk k) may hold every row of chunk k, so it starts at class * B + row_start[k]
+// and no counting pass is needed (the lists have room for B rows per class)
+__global__ void gb_bin_off_kernel(const int32_t* __restrict__ row_start, int64_t B, int K, int32_t* off) {
+    const int i = threadIdx.x;
+    if (i < kNumClasses * K) off[i] = (int32_t)((i / K) * B + (row_start ? row_start[i % K] : 0));
 }
 
 // exclusive prefix sum of the bin counts (one thread: at most 16 x 16 bins)
@@ -1584,7 +1594,7 @@ int set_err(gb_ctx* ctx, int code, const char* fmt, ...) {
     } while (0)
 
 template <typename T>
-int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
+int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need, bool exact = false) {
     if (need <= *cap) return GB_OK;
     if (*ptr) {
         GB_CUDA(ctx, cudaDeviceSynchronize());
@@ -1592,7 +1602,7 @@ int ensure_cap(gb_ctx* ctx, T** ptr, int64_t* cap, int64_t need) {
         *ptr = nullptr;
         *cap = 0;
     }
-    const int64_t want = need + need / 8;
+    const int64_t want = exact ? need : need + need / 8;   // (exact: the multi-GB window stores, sized by the caller)
     if (cudaMalloc(reinterpret_cast<void**>(ptr), (size_t)want * sizeof(T)) != cudaSuccess) {
         cudaGetLastError();
         return set_err(ctx, GB_ERR_NOMEM, "scratch allocation of %lld bytes failed", (long long)(want * sizeof(T)));
@@ -1815,13 +1825,13 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
         for (int cN = 0; cN < 4; cN++) {
             const int Nc = 128 << cN;
             pool_r[cN] = c.B >= (1 << 18) ? (cN == 0 ? 8 : cN == 1 ? 4 : 2) : 1;
-            const int64_t ctas = (int64_t)ctx->grid_blocks_acc[4 * cN] + ctx->grid_blocks_acc[4 * cN + 2];
+            const int64_t ctas = (int64_t)ctx->grid_blocks_acc[4 * cN];   // (the general-path kernels reserve one at a time)
             store_slack += ctas * K * (pool_r[cN] - 1) * 2 * Nc;
             ent_slack += ctas * K * (pool_r[cN] - 1);
         }
         if (K > 1 && (2 * c.sum_bins + store_slack) / kPieceElems + 1024 > 0x7fffffff)
             return set_err(ctx, GB_ERR_INVALID, "store_bins too large for the fused update (piece positions are 32-bit)");
-        if ((rc = ensure_cap(ctx, &ctx->d_wkeep, &ctx->cap_wkeep, 2 * c.sum_bins + store_slack))) return rc;
+        if ((rc = ensure_cap(ctx, &ctx->d_wkeep, &ctx->cap_wkeep, 2 * c.sum_bins + store_slack, true))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_wk, &ctx->cap_wk, kWkInts))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_ent, &ctx->cap_ent, c.B + ent_slack))) return rc;
         if ((rc = ensure_cap(ctx, &ctx->d_accpar, &ctx->cap_accpar, c.B))) return rc;
@@ -1864,14 +1874,18 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
     p.errflag = ctx->d_counts + 2 * kNumClasses;
     p.dlnL_out = (c.mode == MODE_DLNL || c.mode == MODE_OVERLAP) ? c.dlnL_out : nullptr;
     const unsigned pgrid = (unsigned)((c.B + 255) / 256);
-    if (c.accept) {   // binned work lists: count the rows of every (class, walker chunk) bin, scan, then the full pass
+    // binned work lists of gb_delta_loglike_accept.  Up to 2^27 rows: ONE pass -- a bin's list starts where its walker chunk
+    // starts among the rows of its class (room for every row of the chunk), its length is the final append cursor.  Beyond
+    // that (32-bit list offsets): count the rows of every (class, walker chunk) bin, scan, then the full pass.
+    const bool one_pass = c.accept && c.B <= ((int64_t)1 << 27);
+    if (c.accept) {
         p.accept = 1;
         p.K = K;
         p.chunk_first = chunk_first;
         if (K > 1) {
             GB_CUDA(ctx, cudaMemsetAsync(ctx->d_whist, 0, sizeof(int32_t) * (size_t)nw, st));
             gb_walker_hist_kernel<<<pgrid, 256, 0, st>>>(c.walker_index, c.B, nw, ctx->d_whist);
-            gb_chunk_bounds_kernel<<<1, 1, 0, st>>>(ctx->d_whist, nw, K, c.B, chunk_first);
+            gb_chunk_bounds_kernel<<<1, 1, 0, st>>>(ctx->d_whist, nw, K, c.B, chunk_first, chunk_first + 8);   // (K <= 8)
             ctx->launches += 2;
         }
         p.logq = c.logq;
@@ -1882,9 +1896,14 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
         p.bin_off = bin_off;
         p.bin_cursor = bin_cursor;
         p.accepted_out = c.accepted_out;
-        gb_prep_kernel<<<pgrid, 256, 0, st>>>(p);
-        gb_bin_scan_kernel<<<1, 1, 0, st>>>(bin_count, bin_off, kNumClasses * K);
-        ctx->launches += 2;
+        if (one_pass) {
+            gb_bin_off_kernel<<<1, kNumClasses * kMaxChunks, 0, st>>>(K > 1 ? chunk_first + 8 : nullptr, c.B, K, bin_off);
+            ctx->launches++;
+        } else {
+            gb_prep_kernel<<<pgrid, 256, 0, st>>>(p);
+            gb_bin_scan_kernel<<<1, 1, 0, st>>>(bin_count, bin_off, kNumClasses * K);
+            ctx->launches += 2;
+        }
         GB_CUDA(ctx, cudaGetLastError());
         p.accept = 2;
     }
@@ -1935,7 +1954,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
         a.sc_claim = ctx->d_wk + 3;
         a.n_pieces = ctx->d_wk + 4;
         a.pieces = ctx->d_pieces;
-        a.bin_count = bin_count;
+        a.bin_count = one_pass ? bin_cursor : bin_count;
         a.bin_off = bin_off;
         a.bin_ticket = bin_ticket;
         a.K = K;
@@ -1967,7 +1986,7 @@ int run_call(gb_ctx* ctx, const Call& c, void* stream) {
                 for (int cN = 3; cN >= 0; cN--) {
                     const int Nc = 128 << cN;
                     if (!c.n_bins && Nc != c.N) continue;
-                    a.pool_r = pool_r[cN];
+                    a.pool_r = pass ? pool_r[cN] : 1;
                     switch (Nc) {
                         case 128: rc = pass ? launch_main<128, false, true, 1>(ctx, a, c.B, fan.next()) : launch_main<128, false, false, 1>(ctx, a, c.B, fan.next()); break;
                         case 256: rc = pass ? launch_main<256, false, true, 1>(ctx, a, c.B, fan.next()) : launch_main<256, false, false, 1>(ctx, a, c.B, fan.next()); break;
@@ -2245,6 +2264,15 @@ void gb_destroy(gb_ctx* ctx) {
 const char* gb_last_error(const gb_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
 
 int64_t gb_launch_count(const gb_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int64_t gb_scratch_bytes(const gb_ctx* ctx) {
+    if (!ctx) return 0;
+    return ctx->cap_new * (int64_t)sizeof(SrcConst) + ctx->cap_old * (int64_t)sizeof(SrcConst) + ctx->cap_lists * 4 +
+           ctx->cap_band_cache * (int64_t)sizeof(cx) + ctx->cap_temper_cache * (int64_t)sizeof(cx) +
+           ctx->cap_wkeep * (int64_t)sizeof(cx) + ctx->cap_wk * 4 + ctx->cap_ent * (int64_t)sizeof(KeptEnt) +
+           ctx->cap_accpar * (int64_t)sizeof(double4) + ctx->cap_pieces * (int64_t)sizeof(Piece) + ctx->cap_whist * 4 +
+           (int64_t)ctx->cap_stage;
+}
 
 int gb_measure_fp64_peak(gb_ctx* ctx, double* tflops_out, double* dfma_per_clk_sm_out, double clock_mhz, void* stream) {
     if (!ctx || !tflops_out) return GB_ERR_INVALID;

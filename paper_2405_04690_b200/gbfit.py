@@ -23,7 +23,7 @@ EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_
            "gb_launch_count", "gb_measure_fp64_peak", "gb_waveform", "gb_delta_loglike", "gb_residual_update",
            "gb_waveform_host", "gb_delta_loglike_host", "gb_residual_update_host", "gb_band_sweep", "gb_overlap", "gb_temper_sweep",
            "gb_delta_loglike_keep", "gb_residual_update_kept", "gb_band_sweep_generate", "gb_delta_loglike_accept", "gb_delta_loglike_accept_host",
-           "gb_band_sweep_static")
+           "gb_band_sweep_static", "gb_scratch_bytes")
 
 BAND_MAX_STAGE = 3072
 STATIC_SCRATCH_BYTES = 32 * 1024 * 1024   # GB_STATIC_SCRATCH_BYTES
@@ -149,6 +149,8 @@ def lib() -> C.CDLL:
         L.gb_version.restype = C.c_char_p
         L.gb_launch_count.argtypes = [vp]
         L.gb_launch_count.restype = i64
+        L.gb_scratch_bytes.argtypes = [vp]
+        L.gb_scratch_bytes.restype = i64
         L.gb_measure_fp64_peak.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, vp]
         L.gb_measure_fp64_peak.restype = ci
         wf = [vp, vp, i64, ci, vp, ci, vp, vp, vp]
@@ -330,6 +332,10 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().gb_launch_count(self._h))
+
+    def scratch_bytes(self) -> int:
+        """gb_scratch_bytes: device scratch the context holds right now."""
+        return int(lib().gb_scratch_bytes(self._h))
 
     def measure_fp64_peak(self, clock_mhz: float = 0.0, stream=None):
         """Diagnostic: sustained DFMA rate of the device -> (TFLOP/s, DFMA lanes per SM per clock at clock_mhz)."""
