@@ -44,6 +44,9 @@ namespace {
 #ifndef GB_L2_PREFETCH
 #define GB_L2_PREFETCH 1      // delta lnL: request the next item's residual / PSD window into L2
 #endif
+#ifndef GB_SWAP_BATCH
+#define GB_SWAP_BATCH 4       // SWAP / overlap epilogue: window bins per thread whose loads are in flight together
+#endif
 #ifndef GB_EPI_BATCH
 #define GB_EPI_BATCH 8        // delta-lnL epilogue: window bins per thread whose loads are in flight together
 #endif
@@ -1158,7 +1161,7 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
                 const bool inv = a.psd_is_inverse != 0;
                 const double norm = 4.0 / a.Tobs;
                 constexpr int ST = N / T;                        // SWAP: bins per thread (both channels), all T threads
-                constexpr int CH = SWAP ? 2 : (S < 4 ? S : 4);   // bins per thread whose loads are in flight together
+                constexpr int CH = SWAP ? (ST < GB_SWAP_BATCH ? ST : GB_SWAP_BATCH) : (S < 4 ? S : 4);   // bins per thread whose loads are in flight together
                 if (!SWAP) {
                     // this thread's channel: bins ht + H m (consecutive threads, consecutive bins)
                     const double* rC = ch ? rE : rA;
