@@ -1267,20 +1267,26 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
 #pragma unroll
                         for (int c = 0; c < CH; c++) {
                             const int j = tid + T * (m0 + c);
+                            const cx oa = bufA0[pad_idx<N>(j)], oe = bufE0[pad_idx<N>(j)];   // the old window at bin j
                             {
                                 const cx ha = bufA1[pad_idx<N>(j)], he = bufE1[pad_idx<N>(j)];
                                 const cx ra = wn.ra[c], re = wn.re[c];
                                 const double wa = wn.wa[c], we = wn.we[c];
                                 v[0] += wa * (ha.re * ha.re + ha.im * ha.im) + we * (he.re * he.re + he.im * he.im);
                                 v[1] += wa * (ra.re * ha.re + ra.im * ha.im) + we * (re.re * he.re + re.im * he.im);
-                                const int64_t jo = j + shift;
-                                if (jo >= 0 && jo < N) {
-                                    const cx oa = bufA0[pad_idx<N>((int)jo)], oe = bufE0[pad_idx<N>((int)jo)];
-                                    v[2] += wa * (ha.re * oa.re + ha.im * oa.im) + we * (he.re * oe.re + he.im * oe.im);
+                                cx sa = oa, se = oe;   // ... and at the bin under a's bin j (the same one when the windows coincide)
+                                bool in = true;
+                                if (shift != 0) {      // uniform over the CTA
+                                    const int64_t jo = j + shift;
+                                    in = jo >= 0 && jo < N;
+                                    if (in) {
+                                        sa = bufA0[pad_idx<N>((int)jo)];
+                                        se = bufE0[pad_idx<N>((int)jo)];
+                                    }
                                 }
+                                if (in) v[2] += wa * (ha.re * sa.re + ha.im * sa.im) + we * (he.re * se.re + he.im * se.im);
                             }
                             {
-                                const cx oa = bufA0[pad_idx<N>(j)], oe = bufE0[pad_idx<N>(j)];
                                 const cx ra = wo.ra[c], re = wo.re[c];
                                 const double wa = wo.wa[c], we = wo.we[c];
                                 v[3] += wa * (oa.re * oa.re + oa.im * oa.im) + we * (oe.re * oe.re + oe.im * oe.im);
