@@ -178,8 +178,11 @@ int gb_delta_loglike_host(gb_ctx *ctx, const gb_data *data, const double *params
                           int64_t B, double *dlnL_out /*HOST*/, double *aux_out /*HOST*/, void *stream);
 
 /* gb_delta_loglike_accept (below) with HOST proposal arrays and HOST outputs; batches of >= 2^18 rows flow through in
- * chunks (each chunk is one gb_delta_loglike_accept call: the snapshot semantics hold per chunk, and a walker's rows
- * should not straddle chunks if its accepted rows overlap).  apply = 0 runs as a single chunk. */
+ * 4 chunks, rows [B a_c / 24, B a_(c+1) / 24) with a = 0, 2, 9, 16, 24 (GB_HOST_ACCEPT_CUTS; the first chunk is the small one
+ * because its copy is the only one no kernel hides).  Each chunk is one gb_delta_loglike_accept call: the snapshot
+ * semantics hold per chunk, and a walker's rows should not straddle chunks if its accepted rows overlap.  apply = 0 runs
+ * as a single chunk. */
+#define GB_HOST_ACCEPT_CUTS {0, 2, 9, 16, 24}
 int gb_delta_loglike_accept_host(gb_ctx *ctx, const gb_data *data, const double *params_new /*HOST*/,
                                  const double *params_old /*HOST*/, const int32_t *walker_index /*HOST*/,
                                  const int8_t *move /*HOST*/, int move_all, int N, const int32_t *n_bins /*HOST*/, int64_t B,

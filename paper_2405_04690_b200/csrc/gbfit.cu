@@ -2788,10 +2788,14 @@ int delta_loglike_accept_host_impl(gb_ctx* ctx, const gb_data* data, const doubl
     // chunked as gb_delta_loglike_host; a chunk's update has finished when its last kernel ends, so the next chunk reuses
     // the store.  apply = 0 keeps the state of ONE call for gb_residual_update_kept: a single chunk then
     const int nch = (B >= (1 << 18) && apply != 0) ? kHostChunksAccept : 1;
+    // the first chunk is the small one: its copy is the only one no kernel hides (cuts at 2/24, 9/24, 16/24 of the rows)
+    static_assert(kHostChunksAccept == 4, "chunk cuts below");
+    const int cut24[kHostChunksAccept + 1] = GB_HOST_ACCEPT_CUTS;
+    auto cut = [&](int c) -> int64_t { return nch == 1 ? (c ? B : 0) : B * cut24[c] / 24; };
     GB_CUDA(ctx, cudaEventRecord(ctx->ev_start, st));
     GB_CUDA(ctx, cudaStreamWaitEvent(ctx->s_in, ctx->ev_start, 0));
     for (int c = 0; c < nch; c++) {
-        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        const int64_t lo = cut(c), n = cut(c + 1) - lo;
         if (d_pn) GB_CUDA(ctx, cudaMemcpyAsync(d_pn + 8 * lo, params_new + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
         if (d_po) GB_CUDA(ctx, cudaMemcpyAsync(d_po + 8 * lo, params_old + 8 * lo, (size_t)n * 64, cudaMemcpyHostToDevice, ctx->s_in));
         GB_CUDA(ctx, cudaMemcpyAsync(d_w + lo, walker_index + lo, (size_t)n * 4, cudaMemcpyHostToDevice, ctx->s_in));
@@ -2803,7 +2807,7 @@ int delta_loglike_accept_host_impl(gb_ctx* ctx, const gb_data* data, const doubl
         GB_CUDA(ctx, cudaEventRecord(ctx->ev_in[c], ctx->s_in));
     }
     for (int c = 0; c < nch; c++) {
-        const int64_t lo = B * c / nch, n = B * (c + 1) / nch - lo;
+        const int64_t lo = cut(c), n = cut(c + 1) - lo;
         GB_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_in[c], 0));
         rc = gb_delta_loglike_accept(ctx, data, d_pn ? d_pn + 8 * lo : nullptr, d_po ? d_po + 8 * lo : nullptr, d_w + lo,
                                      d_mv ? d_mv + lo : nullptr, move_all, N, d_nb ? d_nb + lo : nullptr, n,

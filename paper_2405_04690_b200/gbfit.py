@@ -26,6 +26,7 @@ EXPORTS = ("gb_default_config", "gb_create", "gb_destroy", "gb_last_error", "gb_
            "gb_band_sweep_static", "gb_scratch_bytes")
 
 BAND_MAX_STAGE = 3072
+HOST_ACCEPT_CUTS = (0, 2, 9, 16, 24)    # GB_HOST_ACCEPT_CUTS: chunk c of delta_loglike_accept_host = rows [B a_c / 24, B a_(c+1) / 24)
 STATIC_SCRATCH_BYTES = 32 * 1024 * 1024   # GB_STATIC_SCRATCH_BYTES
 STATIC_MAX_TASK_BINS = 32768             # GB_STATIC_MAX_TASK_BINS: gb_band_sweep_static takes n_tasks * N up to this
 # layout of gb_band_task (include/gbfit.h)

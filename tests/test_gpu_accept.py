@@ -217,9 +217,9 @@ def test_accept_host_form_chunked(oracle, torch_cuda, gb):
     logu, logq, beta = _draws(wl.B, [34, 0], rate=0.25)
     od = oracle.Data(resid.copy(), wl.psd, wl.k_lo)
     rdl, racc = np.zeros(wl.B), np.zeros(wl.B, np.uint8)
-    nch = 4
-    for c in range(nch):                                            # the library's chunking: B c / nch
-        lo, hi = wl.B * c // nch, wl.B * (c + 1) // nch
+    cuts = gbfit.HOST_ACCEPT_CUTS                                   # the library's chunking (include/gbfit.h)
+    for c in range(len(cuts) - 1):
+        lo, hi = wl.B * cuts[c] // 24, wl.B * cuts[c + 1] // 24
         sl = slice(lo, hi)
         rdl[sl], racc[sl] = oracle.delta_loglike_accept(oracle.Config(), od, wl.params_new[sl], wl.params_old[sl], wl.walker_index[sl],
                                                         logu[sl], logq=logq[sl], beta=beta[sl], move=wl.move[sl], n_bins=wl.n_bins[sl],
