@@ -50,9 +50,6 @@ namespace {
 #ifndef GB_EPI_BATCH
 #define GB_EPI_BATCH 8        // delta-lnL epilogue: window bins per thread whose loads are in flight together
 #endif
-#ifndef GB_L1_PREFETCH
-#define GB_L1_PREFETCH 0      // delta lnL: request THIS item's window into L1 before its FFT; the epilogue then loads through L1
-#endif
 #ifndef GB_STREAM_LOADS
 #define GB_STREAM_LOADS 1     // window loads bypass L1 allocation
 #endif
@@ -504,10 +501,7 @@ struct WinBatch1 {
             const int64_t i = i_first + H * c;
             ok[c] = CHECK ? (i >= 0 && i < n_f) : true;   // !CHECK: the whole window lies inside the stored band
             const int64_t ic = ok[c] ? i : 0;
-#if GB_L1_PREFETCH
-            const double2 a2 = __ldca(reinterpret_cast<const double2*>(rC + 2 * ic));
-            w[c] = __ldca(SC + ic);
-#elif GB_STREAM_LOADS
+#if GB_STREAM_LOADS
             const double2 a2 = __ldcg(reinterpret_cast<const double2*>(rC + 2 * ic));
             w[c] = __ldcg(SC + ic);
 #else
@@ -600,7 +594,6 @@ __device__ __forceinline__ void red_add_f64(double* p, double v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(__cvta_generic_to_global(p)), "d"(v) : "memory");
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
@@ -1095,32 +1088,6 @@ __global__ void __launch_bounds__(Plan<N>::G*(SWAP ? 2 : 1), GB_TPSM / (Plan<N>:
                     if (i >= 0 && i < a.n_f) {
                         prefetch_l2(SAn + i);
                         prefetch_l2(SEn + i);
-                    }
-                }
-            }
-        }
-
-        // ---- and L1 for this item's own window, which the epilogue reads right after the FFT
-        if (GB_L1_PREFETCH && !SWAP && a.mode == MODE_DLNL && !bad_row) {
-            const int64_t i0 = kmin0 - a.k_lo;
-            const size_t nf = (size_t)a.n_f;
-            if (i0 >= 0 && i0 + N + 16 <= a.n_f) {
-                const double* pA = a.resid + ((size_t)rec[0].walker * 2 + 0) * nf * 2 + 2 * (i0 + 8 * tid);
-                const double* pE = a.resid + ((size_t)rec[0].walker * 2 + 1) * nf * 2 + 2 * (i0 + 8 * tid);
-#pragma unroll
-                for (int l = 0; l <= N / 8; l += T) {
-                    if (l + tid <= N / 8) {
-                        prefetch_l1(pA + 16 * l);
-                        prefetch_l1(pE + 16 * l);
-                    }
-                }
-                const double* pSA = a.psd + ((size_t)rec[0].psd_row * 2 + 0) * nf + i0 + 16 * tid;
-                const double* pSE = a.psd + ((size_t)rec[0].psd_row * 2 + 1) * nf + i0 + 16 * tid;
-#pragma unroll
-                for (int l = 0; l <= N / 16; l += T) {
-                    if (l + tid <= N / 16) {
-                        prefetch_l1(pSA + 16 * l);
-                        prefetch_l1(pSE + 16 * l);
                     }
                 }
             }
