@@ -57,6 +57,7 @@ def test_calls_without_gpu_fail_with_status_not_crash(libpath):
     assert h.value is not None and len(L.gb_last_error(h)) > 0
     L.gb_destroy(h)
     assert L.gb_create(None, ctypes.byref(h)) == gbfit.GB_ERR_INVALID
+    assert L.gb_scratch_bytes(None) == 0 and L.gb_launch_count(None) == 0
     with pytest.raises(gbfit.GbError):
         gbfit.Context(0)
 

@@ -252,3 +252,5 @@ def test_accept_repeated_calls_agree(oracle, torch_cuda, gb):
             assert np.array_equal(dl, first[0]) and np.array_equal(acc, first[1])
             change = np.abs(first[2] - resid).max()
             assert np.abs(r1 - first[2]).max() <= 1e-12 * change + 4e-16 * np.abs(resid).max()
+    # gb_scratch_bytes: at least the window store (32 bytes per store bin) and the source records (192 bytes per row)
+    assert ctx.scratch_bytes() >= 32 * int(0.6 * wl.n_bins.sum()) + 192 * wl.B
