@@ -41,6 +41,20 @@ WORKLOAD = "cfg5_full_ensemble_sweep_10x36x12000"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
 
 
+def median_ms(torch, stream, fn, reps: int = 3, warm: int = 1) -> float:
+    """Median over `reps` timed calls of fn() (CUDA events on `stream`, one pair per call) after `warm` untimed ones: the
+    side measurements outside the timed step use it so that one disturbed call does not shift the reported figure."""
+    for _ in range(warm):
+        fn()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for a, b in evs:
+        a.record(stream)
+        fn()
+        b.record(stream)
+    torch.cuda.synchronize()
+    return float(np.median([a.elapsed_time(b) for a, b in evs]))
+
+
 def ncu_traffic(update: str):
     """DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the kernels of one timed step, read from the committed
     summary of the ncu --set full capture under profiles/ (never a literal here).  Returns (bytes or None, provenance)."""
@@ -427,47 +441,33 @@ def run_ours(args):
         d_lq, d_lu = torch.from_numpy(bt.prop_logq).to(dev), torch.from_numpy(bt.prop_logu).to(dev)
         d_acc_b = torch.zeros(bt.prop_k.size, dtype=torch.uint8, device=dev)
         d_dl_b = torch.zeros(bt.prop_k.size, dtype=torch.float64, device=dev)
-        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = 3
-        for i in range(reps + 1):          # first call warms up; every call starts from the same parameters
+        def band_call(tasks_dev):            # every call starts from the same parameters (the reset is inside the timing)
             d_bp.copy_(d_bp0)
-            if i == 1:
-                b0.record(stream)
-            ctx.band_sweep(data, d_tasks, 256, bt.max_stage, d_bp, d_bk, d_bq, d_lq, d_lu, d_acc_b, d_dl_b)
-        b1.record(stream)
-        torch.cuda.synchronize()
+            ctx.band_sweep(data, tasks_dev, 256, bt.max_stage, d_bp, d_bk, d_bq, d_lq, d_lu, d_acc_b, d_dl_b)
+        ms_band = median_ms(torch, stream, lambda: band_call(d_tasks))
         ctx.check()
-        ms_band = b0.elapsed_time(b1) / reps
         # row f3: the same tasks in the odd/even cold-chain buffer mode: residual rows 2w / 2w+1 stand for
         # the even / odd buffer of "walker" w, r' is formed on chip (9 extra waveforms per task), write-back to the odd row
         wv = bt.tasks["walker"]
         packed_oe = gbfit.pack_band_tasks(**dict(bt.tasks, walker=(wv // 2) * 2), subtract_current=np.ones_like(wv),
                                           write_walker=(wv // 2) * 2 + 1)
         d_tasks_oe = torch.from_numpy(packed_oe.view(np.uint8)).to(dev)
-        for i in range(reps + 1):
-            d_bp.copy_(d_bp0)
-            if i == 1:
-                b0.record(stream)
-            ctx.band_sweep(data, d_tasks_oe, 256, bt.max_stage, d_bp, d_bk, d_bq, d_lq, d_lu, d_acc_b, d_dl_b)
-        b1.record(stream)
-        torch.cuda.synchronize()
+        ms_band_oe = median_ms(torch, stream, lambda: band_call(d_tasks_oe))
         ctx.check()
-        ms_band_oe = b0.elapsed_time(b1) / reps
         # row f1 as printed: the proposal step inside the kernel (Philox, randint, group stretch from a
         # 7.1 M-row friends table, Eq. 14), from the current theta_k
         from gb_inputs import make_stretch_inputs
         si = make_stretch_inputs(bt, n_copies=12, n_friends=24)
         sg = gbfit.Stretch(si.seed, si.sweep, torch.from_numpy(si.group).to(dev), si.n_friends, si.lo, si.hi, si.periodic,
                            si.stretch_a)
-        for i in range(reps + 1):
+        g_box = {}
+
+        def gen_call():
             d_bp.copy_(d_bp0)
-            if i == 1:
-                b0.record(stream)
-            g_out = ctx.band_sweep_generate(data, d_tasks, 256, bt.max_stage, d_bp, sg, bt.prop_k.size)
-        b1.record(stream)
-        torch.cuda.synchronize()
+            g_box["out"] = ctx.band_sweep_generate(data, d_tasks, 256, bt.max_stage, d_bp, sg, bt.prop_k.size)
+        ms_band_gen = median_ms(torch, stream, gen_call)
         ctx.check()
-        ms_band_gen = b0.elapsed_time(b1) / reps
+        g_out = g_box["out"]
         gen_eval = float(torch.isfinite(g_out[1]).float().mean().item())
         # waveforms actually generated by a call: one per proposal plus the fill of the current-source cache (n_src per task)
         n_wave_band = bt.prop_k.size + int(bt.tasks["n_src"].sum())
@@ -582,15 +582,13 @@ def run_ours(args):
         lu[np.random.Generator(np.random.Philox(key=[5, 77])).random(lu.size) < 0.25] = -np.inf
         targs = [torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in
                  (tt.params, tt.chain_walker, tt.chain_beta, tt.chain_set_begin, tt.chain_set_n, lu)]
-        t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for i in range(4):
-            if i == 1:
-                t0e.record(stream)
-            t_perm, t_acc, t_dl = ctx.temper_sweep(data, d_tt, 256, tt.max_stage, *targs)
-        t1e.record(stream)
-        torch.cuda.synchronize()
+        t_box = {}
+
+        def temper_call():
+            t_box["out"] = ctx.temper_sweep(data, d_tt, 256, tt.max_stage, *targs)
+        ms_t = median_ms(torch, stream, temper_call)
         ctx.check()
-        ms_t = t0e.elapsed_time(t1e) / 3
+        t_perm, t_acc, t_dl = t_box["out"]
         n_pairs_t = int((tt.tasks["n_t"] - 1).sum())
         n_wave = int(tt.chain_set_n.sum())          # every chain's set is summed once (set-sum cache of gb_temper.cuh)
         tmp = {"call": "gb_temper_sweep (Algorithm 2, Eq. D2)", "N": 256, "ladders": int(len(tt.tasks["n_t"])), "chains": 10,
@@ -610,17 +608,10 @@ def run_ours(args):
         d_pc = d_pa + jit
         d_rows = (torch.arange(n_pairs, device=dev, dtype=torch.int32) % wl.psd.shape[0]).contiguous()
         d_ov = torch.empty(n_pairs, dtype=torch.float64, device=dev)
-        o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         view = gbfit.Data.psd_only(d_psd, wl.k_lo, psd_is_inverse=True)
         nb_pairs = d_nb[:n_pairs].contiguous()
-        for i in range(4):
-            if i == 1:
-                o0.record(stream)
-            ctx.overlap(view, d_pa, d_pc, psd_row=d_rows, n_bins=nb_pairs, out=d_ov)
-        o1.record(stream)
-        torch.cuda.synchronize()
+        ms_ov = median_ms(torch, stream, lambda: ctx.overlap(view, d_pa, d_pc, psd_row=d_rows, n_bins=nb_pairs, out=d_ov))
         ctx.check()
-        ms_ov = o0.elapsed_time(o1) / 3
         ovl = {"call": "gb_overlap", "pairs": n_pairs, "ms_per_call": ms_ov, "pairs_per_s": n_pairs / (ms_ov * 1e-3),
                "mean_N": float(wl.n_bins[:n_pairs].mean()), "median_overlap": float(d_ov.median().item())}
 
@@ -633,15 +624,9 @@ def run_ours(args):
         dat_s = gbfit.Data(d_resid[:1], torch.from_numpy(1.0 / ws.psd).to(dev), ws.k_lo, psd_is_inverse=True)
         s_p, s_w, s_nb = (torch.from_numpy(np.ascontiguousarray(x)).to(dev) for x in (ws.params_new, ws.walker_index, ws.n_bins))
         s_out = torch.empty(ws.B, dtype=torch.float64, device=dev)
-        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for i in range(6):
-            if i == 1:
-                s0.record(stream)
-            ctx.delta_loglike(dat_s, s_p, None, s_w, move_all=gbfit.ADD, n_bins=s_nb, out=s_out)
-        s1.record(stream)
-        torch.cuda.synchronize()
+        ms_s = median_ms(torch, stream, lambda: ctx.delta_loglike(dat_s, s_p, None, s_w, move_all=gbfit.ADD, n_bins=s_nb,
+                                                                  out=s_out), reps=5)
         ctx.check()
-        ms_s = s0.elapsed_time(s1) / 5
         fl_s = float(flops_eval(ws.n_bins.astype(np.float64)).sum())
         search = {"call": "gb_delta_loglike, search-stage shape (App. G): 900 sub-bands x 10 temperatures x 100 walkers, one "
                           "source per walker, one residual row", "rows": int(ws.B), "ms_per_call": ms_s,
